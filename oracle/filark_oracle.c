@@ -1,0 +1,210 @@
+/*
+ * filark_oracle.c -- TEST INFRASTRUCTURE, NOT PRODUCT CODE.
+ *
+ * Plain, slow, float64 CPU oracle for the one hot path this repository builds:
+ * stateful chunked temporal filtering of a channel x time DAS stream =
+ * per-channel cascaded second-order-section (SOS) IIR filter with state carried
+ * across chunk boundaries, followed by a recursive STA/LTA characteristic
+ * function (CF) with its own carried state.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may build, load or call this file.  It shares no code,
+ * header, table or constant with paper_2605_20132_b200/csrc (the CUDA path).
+ *
+ * What it follows (PAPER.md = /root/reference/PAPER.md):
+ *  - PAPER.md:109 (section 3.4): IIR operators are "stateful-compatible",
+ *    "causal, sample-wise real-time variants" that "accept incremental data
+ *    chunks and return outputs of matching length while maintaining correct
+ *    state propagation internally".
+ *  - PAPER.md:121 (Table 1): "IIR (offline & realtime second-order sections, SOS)".
+ *  - PAPER.md:255 (section 6.2): state "is carried forward exactly"; the first
+ *    chunk after initialisation carries a transient "determined by the filter
+ *    order and the initial condition" -> reading R6: zero initial state.
+ *  - PAPER.md:130 (section 3.4): monitors such as a "threshold-based energy
+ *    detector" consume the stream; the paper never defines STA/LTA, so the CF
+ *    follows BASELINE.json north_star ("recursive STA/LTA characteristic
+ *    function (also with carried state)") with readings R8-R13 of SURVEY.md 8(c).
+ *
+ * The method reaches exactly (up to rounding order) a result with a plain
+ * definition -- a causal LTI cascade and two exponential averages -- so the
+ * oracle is that definition written out, sample by sample, in double:
+ *
+ *   for each channel c (independent), state zero at create/reset:
+ *     for each sample n (g = samples since create/reset, counted across pushes):
+ *       v = (double) x[c][n]
+ *       for k = 0 .. n_sec-1 (given order; b*,a* divided by a0_k once):   (R1,R4,R5)
+ *           y     = b0_k*v + z1[k]               transposed direct form II
+ *           z1[k] = b1_k*v - a1_k*y + z2[k]
+ *           z2[k] = b2_k*v - a2_k*y
+ *           v = y
+ *       filt[c][n] = (float) v                   round to nearest           (R18)
+ *       e   = v*v                                unrounded double v         (R9)
+ *       sta = sta + (e - sta)/sta_len            both use current sample    (R8,R13)
+ *       lta = lta + (e - lta)/lta_len
+ *       cf[c][n] = (g >= lta_len && lta > 1e-30) ? (float)(sta/lta) : 0     (R10,R11)
+ *
+ * No blocking, fusion or reordering.  Compile WITHOUT -ffast-math and with
+ * -ffp-contract=off so that every operation is an IEEE double operation in the
+ * order written (chunked == whole must be bit-identical).
+ *
+ * Pins (tests/test_oracle_pins.py): closed-form biquad impulse response, zero
+ * gain at DC and Nyquist, |H|^2 = 1/2 at the band edges, linearity,
+ * bit-identical chunk invariance, brute-force expanded difference equation,
+ * scipy.signal.sosfilt / lfilter special cases, STA/LTA closed forms, CF bound
+ * and scale invariance.  The composition SOS -> y^2 -> STA/LTA -> ratio has no
+ * closed form of its own: it is pinned through its parts.
+ */
+#include <stdlib.h>
+#include <string.h>
+
+#define FILARK_ORACLE_LTA_TINY 1e-30
+
+typedef struct filark_oracle {
+    int n_ch;
+    int n_sec;
+    int sta_len;
+    int lta_len;
+    double *coef;   /* [n_sec][5] = b0 b1 b2 a1 a2, already divided by a0 */
+    double *z;      /* [n_ch][n_sec][2]  DF2T state z1, z2                */
+    double *sta;    /* [n_ch]                                            */
+    double *lta;    /* [n_ch]                                            */
+    long long g;    /* samples pushed since create/reset                 */
+} filark_oracle_t;
+
+/* sos: row-major [n_sec][6] = b0 b1 b2 a0 a1 a2 (scipy convention). */
+filark_oracle_t *filark_oracle_create(int n_ch, const double *sos, int n_sec,
+                                      int sta_len, int lta_len)
+{
+    if (n_ch <= 0 || n_sec <= 0 || !sos || sta_len < 1 || lta_len < sta_len) return NULL;
+    for (int k = 0; k < n_sec; ++k)
+        if (sos[6 * k + 3] == 0.0) return NULL;
+    filark_oracle_t *o = (filark_oracle_t *)calloc(1, sizeof(*o));
+    if (!o) return NULL;
+    o->n_ch = n_ch; o->n_sec = n_sec; o->sta_len = sta_len; o->lta_len = lta_len;
+    o->coef = (double *)malloc(sizeof(double) * 5 * (size_t)n_sec);
+    o->z    = (double *)calloc((size_t)n_ch * (size_t)n_sec * 2, sizeof(double));
+    o->sta  = (double *)calloc((size_t)n_ch, sizeof(double));
+    o->lta  = (double *)calloc((size_t)n_ch, sizeof(double));
+    if (!o->coef || !o->z || !o->sta || !o->lta) {
+        free(o->coef); free(o->z); free(o->sta); free(o->lta); free(o);
+        return NULL;
+    }
+    for (int k = 0; k < n_sec; ++k) {
+        const double a0 = sos[6 * k + 3];
+        o->coef[5 * k + 0] = sos[6 * k + 0] / a0;
+        o->coef[5 * k + 1] = sos[6 * k + 1] / a0;
+        o->coef[5 * k + 2] = sos[6 * k + 2] / a0;
+        o->coef[5 * k + 3] = sos[6 * k + 4] / a0;
+        o->coef[5 * k + 4] = sos[6 * k + 5] / a0;
+    }
+    o->g = 0;
+    return o;
+}
+
+void filark_oracle_reset(filark_oracle_t *o)
+{
+    if (!o) return;
+    memset(o->z, 0, sizeof(double) * (size_t)o->n_ch * (size_t)o->n_sec * 2);
+    memset(o->sta, 0, sizeof(double) * (size_t)o->n_ch);
+    memset(o->lta, 0, sizeof(double) * (size_t)o->n_ch);
+    o->g = 0;
+}
+
+void filark_oracle_destroy(filark_oracle_t *o)
+{
+    if (!o) return;
+    free(o->coef); free(o->z); free(o->sta); free(o->lta); free(o);
+}
+
+long long filark_oracle_samples_seen(const filark_oracle_t *o) { return o ? o->g : -1; }
+
+/*
+ * Process channels [ch_begin, ch_end) of one chunk of n_t samples WITHOUT
+ * advancing the sample counter (so that a caller may split the channel range
+ * over threads; channels are independent).  Element (c, n) of x / filt / cf
+ * lives at index c*stride_c + n*stride_n (in elements): channel-major dense
+ * chunk = (n_t, 1), time-major dense chunk = (1, n_ch).  filt or cf may be NULL.
+ */
+int filark_oracle_push_range(filark_oracle_t *o, const float *x, long long n_t,
+                             long long stride_c, long long stride_n,
+                             float *filt, float *cf, int ch_begin, int ch_end)
+{
+    if (!o || !x || n_t < 0 || ch_begin < 0 || ch_end > o->n_ch || ch_begin > ch_end) return 1;
+    const int n_sec = o->n_sec;
+    const double sta_len = (double)o->sta_len;
+    const double lta_len = (double)o->lta_len;
+    for (int c = ch_begin; c < ch_end; ++c) {
+        double *z = o->z + (size_t)c * (size_t)n_sec * 2;
+        double sta = o->sta[c];
+        double lta = o->lta[c];
+        long long g = o->g;
+        for (long long n = 0; n < n_t; ++n) {
+            const long long idx = (long long)c * stride_c + n * stride_n;
+            double v = (double)x[idx];
+            for (int k = 0; k < n_sec; ++k) {
+                const double *q = o->coef + 5 * k;     /* b0 b1 b2 a1 a2 */
+                const double y = q[0] * v + z[2 * k];
+                z[2 * k]     = q[1] * v - q[3] * y + z[2 * k + 1];
+                z[2 * k + 1] = q[2] * v - q[4] * y;
+                v = y;
+            }
+            if (filt) filt[idx] = (float)v;
+            const double e = v * v;
+            sta = sta + (e - sta) / sta_len;
+            lta = lta + (e - lta) / lta_len;
+            if (cf)
+                cf[idx] = (g >= (long long)o->lta_len && lta > FILARK_ORACLE_LTA_TINY)
+                              ? (float)(sta / lta) : 0.0f;
+            g += 1;
+        }
+        o->sta[c] = sta;
+        o->lta[c] = lta;
+    }
+    return 0;
+}
+
+/* Advance the sample counter once every channel range of the chunk is done. */
+void filark_oracle_advance(filark_oracle_t *o, long long n_t)
+{
+    if (o && n_t > 0) o->g += n_t;
+}
+
+/* One whole push: all channels, then advance the counter. */
+int filark_oracle_push(filark_oracle_t *o, const float *x, long long n_t,
+                       long long stride_c, long long stride_n, float *filt, float *cf)
+{
+    if (!o) return 1;
+    const int rc = filark_oracle_push_range(o, x, n_t, stride_c, stride_n, filt, cf, 0, o->n_ch);
+    if (rc == 0) filark_oracle_advance(o, n_t);
+    return rc;
+}
+
+/* Expose the float64 intermediates for pins that need them unrounded:
+ * runs ONE channel of double input through the cascade + averages and returns
+ * y (double), sta, lta per sample.  Same statements as above. */
+int filark_oracle_trace_f64(filark_oracle_t *o, int c, const double *x, long long n_t,
+                            double *y_out, double *sta_out, double *lta_out)
+{
+    if (!o || !x || c < 0 || c >= o->n_ch || n_t < 0) return 1;
+    const int n_sec = o->n_sec;
+    double *z = o->z + (size_t)c * (size_t)n_sec * 2;
+    double sta = o->sta[c], lta = o->lta[c];
+    for (long long n = 0; n < n_t; ++n) {
+        double v = x[n];
+        for (int k = 0; k < n_sec; ++k) {
+            const double *q = o->coef + 5 * k;
+            const double y = q[0] * v + z[2 * k];
+            z[2 * k]     = q[1] * v - q[3] * y + z[2 * k + 1];
+            z[2 * k + 1] = q[2] * v - q[4] * y;
+            v = y;
+        }
+        const double e = v * v;
+        sta = sta + (e - sta) / (double)o->sta_len;
+        lta = lta + (e - lta) / (double)o->lta_len;
+        if (y_out) y_out[n] = v;
+        if (sta_out) sta_out[n] = sta;
+        if (lta_out) lta_out[n] = lta;
+    }
+    o->sta[c] = sta; o->lta[c] = lta;
+    return 0;
+}

@@ -1,0 +1,146 @@
+"""ctypes wrapper around oracle/filark_oracle.c (TEST INFRASTRUCTURE, not product code).
+
+The arithmetic lives in the C file, which states the definition it follows
+(SURVEY.md 8(c) readings R1-R18).  This module only builds
+the shared object with gcc, marshals numpy arrays, and -- for the timed cpu_baseline
+run -- splits the independent channels over host threads (ctypes drops the GIL).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+import threading
+from concurrent.futures import ThreadPoolExecutor
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "filark_oracle.c")
+_LIB = os.path.join(_HERE, "libfilark_oracle.so")
+_lock = threading.Lock()
+_lib = None
+
+CHANNEL_MAJOR = 0  # chunk is [n_ch][n_t], time contiguous
+TIME_MAJOR = 1     # chunk is [n_t][n_ch], channel contiguous
+
+
+def oracle_lib_path() -> str:
+    return _LIB
+
+
+def build_oracle(force: bool = False) -> str:
+    """Compile the oracle with gcc: no fast-math, no FMA contraction, plain -O2."""
+    with _lock:
+        if (not force and os.path.exists(_LIB)
+                and os.path.getmtime(_LIB) >= os.path.getmtime(_SRC)):
+            return _LIB
+        cmd = ["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-ffp-contract=off",
+               "-fno-fast-math", "-o", _LIB, _SRC]
+        subprocess.run(cmd, check=True, capture_output=True)
+        return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    build_oracle()
+    lib = ctypes.CDLL(_LIB)
+    vp, ll, ci = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int
+    lib.filark_oracle_create.restype = vp
+    lib.filark_oracle_create.argtypes = [ci, vp, ci, ci, ci]
+    lib.filark_oracle_reset.restype = None
+    lib.filark_oracle_reset.argtypes = [vp]
+    lib.filark_oracle_destroy.restype = None
+    lib.filark_oracle_destroy.argtypes = [vp]
+    lib.filark_oracle_samples_seen.restype = ll
+    lib.filark_oracle_samples_seen.argtypes = [vp]
+    lib.filark_oracle_push_range.restype = ci
+    lib.filark_oracle_push_range.argtypes = [vp, vp, ll, ll, ll, vp, vp, ci, ci]
+    lib.filark_oracle_advance.restype = None
+    lib.filark_oracle_advance.argtypes = [vp, ll]
+    lib.filark_oracle_push.restype = ci
+    lib.filark_oracle_push.argtypes = [vp, vp, ll, ll, ll, vp, vp]
+    lib.filark_oracle_trace_f64.restype = ci
+    lib.filark_oracle_trace_f64.argtypes = [vp, ci, vp, ll, vp, vp, vp]
+    _lib = lib
+    return lib
+
+
+class Oracle:
+    """Stateful float64 oracle stream: create -> push* -> reset, like the C ABI under test."""
+
+    def __init__(self, n_ch: int, sos, sta_len: int, lta_len: int, layout: int = CHANNEL_MAJOR):
+        lib = _load()
+        sos = np.ascontiguousarray(np.asarray(sos, dtype=np.float64))
+        if sos.ndim != 2 or sos.shape[1] != 6:
+            raise ValueError("sos must be [n_sec][6]")
+        self._lib = lib
+        self.n_ch, self.n_sec = int(n_ch), int(sos.shape[0])
+        self.sta_len, self.lta_len, self.layout = int(sta_len), int(lta_len), int(layout)
+        self._h = lib.filark_oracle_create(self.n_ch, sos.ctypes.data, self.n_sec,
+                                           self.sta_len, self.lta_len)
+        if not self._h:
+            raise ValueError("filark_oracle_create rejected its arguments")
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.filark_oracle_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def reset(self):
+        self._lib.filark_oracle_reset(self._h)
+
+    @property
+    def samples_seen(self) -> int:
+        return int(self._lib.filark_oracle_samples_seen(self._h))
+
+    def _strides(self, n_t):
+        return (n_t, 1) if self.layout == CHANNEL_MAJOR else (1, self.n_ch)
+
+    def push(self, x: np.ndarray, want_filt=True, want_cf=True, threads: int = 1):
+        """x: float32 dense chunk, [n_ch][n_t] (channel-major) or [n_t][n_ch] (time-major).
+        Returns (filt, cf) float32 arrays of the same shape (None where not wanted)."""
+        x = np.ascontiguousarray(x, dtype=np.float32)
+        if x.ndim != 2:
+            raise ValueError("chunk must be 2-D")
+        n_t = x.shape[1] if self.layout == CHANNEL_MAJOR else x.shape[0]
+        n_c = x.shape[0] if self.layout == CHANNEL_MAJOR else x.shape[1]
+        if n_c != self.n_ch:
+            raise ValueError("chunk channel count does not match the stream")
+        filt = np.empty_like(x) if want_filt else None
+        cf = np.empty_like(x) if want_cf else None
+        sc, sn = self._strides(n_t)
+        fp = filt.ctypes.data if filt is not None else None
+        cp = cf.ctypes.data if cf is not None else None
+        threads = max(1, min(int(threads), self.n_ch))
+        if threads == 1:
+            rc = self._lib.filark_oracle_push_range(self._h, x.ctypes.data, n_t, sc, sn, fp, cp,
+                                                    0, self.n_ch)
+            if rc:
+                raise RuntimeError("oracle push failed")
+        else:
+            bounds = np.linspace(0, self.n_ch, threads + 1).astype(int)
+
+            def work(i):
+                return self._lib.filark_oracle_push_range(self._h, x.ctypes.data, n_t, sc, sn,
+                                                          fp, cp, int(bounds[i]), int(bounds[i + 1]))
+            with ThreadPoolExecutor(max_workers=threads) as ex:
+                if any(ex.map(work, range(threads))):
+                    raise RuntimeError("oracle push failed")
+        self._lib.filark_oracle_advance(self._h, n_t)
+        return filt, cf
+
+    def trace_f64(self, x: np.ndarray, channel: int = 0):
+        """Double-precision input, one channel: returns (y, sta, lta) as float64 (for pins).
+        Does not advance the warm-up counter."""
+        x = np.ascontiguousarray(x, dtype=np.float64)
+        y = np.empty_like(x); s = np.empty_like(x); l = np.empty_like(x)
+        rc = self._lib.filark_oracle_trace_f64(self._h, int(channel), x.ctypes.data, x.size,
+                                               y.ctypes.data, s.ctypes.data, l.ctypes.data)
+        if rc:
+            raise RuntimeError("oracle trace failed")
+        return y, s, l
