@@ -1,0 +1,38 @@
+/*
+ * filark_debug.h -- host-only introspection of the preparation stage (no CUDA calls).
+ *
+ * Used by the CPU test-suite to check the host logic of the library against numpy: the
+ * per-section state-space rewrite (s[n] = A s[n-1] + B x[n], y[n] = C s[n-1] + D x[n]) of the
+ * SOS operator of PAPER.md:109/121, the float64 block powers the scan relies on, and the
+ * tiling of a push of n_t samples.  Return values are filark_status_t codes as int.
+ */
+#ifndef FILARK_DEBUG_H
+#define FILARK_DEBUG_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/*
+ * sos    [host, in]  [n_sec][6] doubles (b0 b1 b2 a0 a1 a2).
+ * kinds  [host, out] n_sec ints: 0 = transposed direct form II, 1 = normal (coupled) form. May be NULL.
+ * coefs  [host, out] n_sec x 9 doubles: A row-major (4), B (2), C (2), D.  May be NULL.
+ * gain   [host, out] product of the b0 factors moved in front of the cascade.  May be NULL.
+ * The cascade equals gain * (sections in state-space form applied in order).
+ */
+int filark_debug_design(const double *sos, int n_sec, int *kinds, double *coefs, double *gain);
+
+/*
+ * Tiling of one channel-major push of n_t samples: n_full tiles of 1024 samples, then a tail
+ * tile whose lanes hold `len` samples each: `nfull` full lanes, one partial lane with `part`
+ * samples (0 = none); `jl` = lane whose end state is carried out (-1 if there is no tail).
+ */
+int filark_debug_tail_geometry(long long n_t, int *n_full, int *len, int *nfull, int *part, int *jl);
+
+/* out4 (row-major 2x2) = A^e for the state-space form chosen for one section (6 doubles). */
+int filark_debug_block_power(const double *sos6, long long e, double *out4);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FILARK_DEBUG_H */

@@ -1,0 +1,166 @@
+/*
+ * filark_stream.h -- C ABI of the B200-native fused SOS + STA/LTA stream path.
+ *
+ * What the path computes (one "push" of a chunk of n_t samples on n_ch channels):
+ *
+ *   S0  load the chunk once from HBM (4 B/sample)
+ *   S1  per SOS section, per time sub-block: zero-state local response      \
+ *   S2  combine the sub-block transfer operators (warp-shuffle scan)         | stateful causal
+ *   S3  fix-up with the carried state; new carried state kept in the handle /  SOS IIR filter
+ *   S4  e = y^2
+ *   S5  two exponential averages of e (STA, LTA) by the same local/scan/fix-up pattern
+ *   S6  cf = sta/lta, 0 during the LTA warm-up and on dead channels
+ *   S7  store filt and cf once (4 B + 4 B per sample)
+ *
+ * Source passages (PAPER.md = text of arxiv 2605.20132, "FiLark"):
+ *   - PAPER.md:109 (sec. 3.4): IIR operators are "stateful-compatible", with "causal,
+ *     sample-wise real-time variants (iir_filter_time_rt ...)" that "accept incremental
+ *     data chunks and return outputs of matching length while maintaining correct state
+ *     propagation internally".
+ *   - PAPER.md:121 (Table 1): "IIR (offline & realtime second-order sections, SOS)".
+ *   - PAPER.md:255 (sec. 6.2): state "is carried forward exactly"; only the first chunk
+ *     after initialisation carries a transient.
+ *   - PAPER.md:169 (sec. 3.5): state must propagate across file (= chunk) boundaries.
+ *   - PAPER.md:83 (sec. 3.2): the filter leaves the underlying recording unchanged.
+ *   - PAPER.md:130, 132 (sec. 3.4): the filtered stream feeds a streaming monitor such as a
+ *     threshold-based energy detector.  The paper never defines STA/LTA; the characteristic
+ *     function follows BASELINE.json `north_star` and the readings R8-R13 in DESIGN.md.
+ *
+ * Contract: concatenating the outputs of ANY sequence of pushes equals pushing the
+ * concatenated input once (within the fp32 tolerance stated in DESIGN.md).
+ *
+ * All pointers named d_* are DEVICE pointers; everything else is a HOST pointer.
+ * No exceptions cross this boundary, nothing aborts, nothing prints: every call returns a
+ * filark_status_t.  A handle is bound to the CUDA device that was current at create and is
+ * not thread-safe; pushes on one handle must be stream-ordered with respect to each other.
+ */
+#ifndef FILARK_STREAM_H
+#define FILARK_STREAM_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* Forward declaration so that this header needs no CUDA include. */
+#ifndef __DRIVER_TYPES_H__
+typedef struct CUstream_st *cudaStream_t;
+#endif
+
+typedef struct filark_stream filark_stream_t;   /* opaque; owns device state and tables */
+
+typedef enum filark_status {
+    FILARK_OK = 0,
+    FILARK_ERR_INVALID_ARG = 1,     /* null pointer, non-positive size, bad layout/flags, aliasing */
+    FILARK_ERR_UNSTABLE = 2,        /* a section has a pole with radius >= 1                       */
+    FILARK_ERR_ALLOC = 3,           /* host or device allocation failed                            */
+    FILARK_ERR_CUDA = 4,            /* a CUDA call failed; see filark_last_cuda_error              */
+    FILARK_ERR_DEVICE_MISMATCH = 5, /* current device differs from the handle's device             */
+    FILARK_ERR_ALIGNMENT = 6        /* a device pointer is not 4-byte aligned                      */
+} filark_status_t;
+
+/* Memory order of a chunk (reading R14/R15 in DESIGN.md). */
+#define FILARK_LAYOUT_CHANNEL_MAJOR 0   /* [n_ch][n_t]: time contiguous (BASELINE.json configs[0]) */
+#define FILARK_LAYOUT_TIME_MAJOR    1   /* [n_t][n_ch]: channel contiguous (PAPER.md:160 'nt_nc')  */
+
+/* create_ex flags */
+#define FILARK_FLAG_NONE        0u
+#define FILARK_FLAG_SERIAL_SCAN 1u  /* diagnostic kernel: one thread per channel, serial in time,
+                                       same state-space arithmetic, no blocked scan             */
+
+#define FILARK_MAX_SECTIONS 16
+
+/*
+ * filark_stream_create -- build a stream for n_ch channels.
+ *   out      [host, out]  receives the handle; untouched on error.
+ *   n_ch     channels, >= 1.
+ *   sos      [host, in]   row-major [n_sec][6] = b0 b1 b2 a0 a1 a2 per section, DOUBLE: fp32
+ *                         coefficients alone break the tolerance for poles near z = 1
+ *                         (DESIGN.md 4).  Sections are applied in the order given; each row is
+ *                         divided by its a0.  Copied; the caller keeps ownership.
+ *   n_sec    sections, 1 .. FILARK_MAX_SECTIONS.
+ *   sta_len, lta_len  averaging lengths in SAMPLES, 1 <= sta_len <= lta_len (readings R8, R12).
+ * Layout is channel-major, flags none.  Initial condition: zero state (reading R6).
+ * Errors: INVALID_ARG (null, sizes, a0 == 0, non-finite coefficient), UNSTABLE, ALLOC, CUDA.
+ * The handle owns n_ch*(2*n_sec+2) floats of device state plus a few KB of tables, allocated
+ * on the current device.
+ */
+filark_status_t filark_stream_create(filark_stream_t **out, int n_ch, const double *sos, int n_sec,
+                                     int sta_len, int lta_len);
+
+/* Same, with the chunk layout (FILARK_LAYOUT_*) and flags (FILARK_FLAG_*). */
+filark_status_t filark_stream_create_ex(filark_stream_t **out, int n_ch, const double *sos,
+                                        int n_sec, int sta_len, int lta_len, int layout,
+                                        unsigned flags);
+
+/*
+ * filark_stream_push -- filter one dense chunk and advance the carried state
+ * ("accept incremental data chunks and return outputs of matching length";
+ *  PAPER.md:255 state "carried forward exactly").
+ *   d_in    [device, in]  n_ch*n_t floats in the handle's layout; never written.
+ *   n_t     samples per channel in this chunk, >= 0; 0 is a no-op returning FILARK_OK.
+ *   d_filt  [device, out] band-passed samples, same shape/layout as d_in; may be NULL.
+ *   d_cf    [device, out] STA/LTA characteristic function, same shape/layout; may be NULL.
+ *                         cf = 0 while fewer than lta_len samples have been seen since
+ *                         create/reset, and where lta <= 1e-30 (readings R10, R11).
+ *   stream  CUDA stream the work is enqueued on.
+ * Asynchronous: enqueues exactly one kernel on `stream`, performs no host synchronisation and
+ * no allocation, and may be captured into a CUDA graph.  The caller owns all three buffers and
+ * keeps them alive until the stream reaches the push.  Outputs must not alias the input or
+ * each other (in-place is rejected).
+ * Errors: INVALID_ARG (null handle/d_in, n_t < 0, both outputs NULL, aliasing), ALIGNMENT,
+ * DEVICE_MISMATCH, CUDA (launch failure).
+ */
+filark_status_t filark_stream_push(filark_stream_t *h, const float *d_in, long long n_t,
+                                   float *d_filt, float *d_cf, cudaStream_t stream);
+
+/*
+ * filark_stream_push_pitched -- as push, for a sub-view of a larger record: consecutive
+ * rows of the chunk (rows = channels if channel-major, time samples if time-major) are
+ * in_pitch / out_pitch ELEMENTS apart (>= the row length).  Both outputs share out_pitch.
+ */
+filark_status_t filark_stream_push_pitched(filark_stream_t *h, const float *d_in, long long n_t,
+                                           long long in_pitch, float *d_filt, float *d_cf,
+                                           long long out_pitch, cudaStream_t stream);
+
+/*
+ * filark_stream_push_host -- end-to-end variant for callers whose chunk lives in HOST memory
+ * (the paper's pipeline executor hands the operator host arrays): copies the
+ * dense chunk host->device into staging buffers owned by the handle, runs push, and copies
+ * the requested outputs device->host, all asynchronously on `stream`.  h_in / h_filt / h_cf
+ * are HOST pointers (pinned memory for true asynchrony), n_ch*n_t floats each in the handle's
+ * layout; h_filt or h_cf may be NULL.  The staging buffers grow on demand: a push larger than
+ * any before it synchronises `stream` and allocates (the only allocation in the push family).
+ * The caller synchronises `stream` before reading the outputs.
+ * Errors: as push, plus ALLOC.
+ */
+filark_status_t filark_stream_push_host(filark_stream_t *h, const float *h_in, long long n_t,
+                                        float *h_filt, float *h_cf, cudaStream_t stream);
+
+/*
+ * filark_stream_reset -- return the handle to the just-created state (zero filter state, zero
+ * sta/lta, sample counter 0), ordered on `stream` (the transient belongs to
+ * "the first chunk processed after the filter is initialized").
+ */
+filark_status_t filark_stream_reset(filark_stream_t *h, cudaStream_t stream);
+
+/* Free the handle and its device memory.  NULL is accepted.  Synchronises the device. */
+filark_status_t filark_stream_destroy(filark_stream_t *h);
+
+/* Static description of a status code; never NULL. */
+const char *filark_status_string(filark_status_t s);
+
+/* The cudaError_t (as int) of the last failing CUDA call on this handle, 0 if none. */
+int filark_last_cuda_error(const filark_stream_t *h);
+
+/*
+ * Introspection used by the harness: number of kernels launched so far through this handle
+ * (bench.py reports it as gpu_launches) and the number of samples per channel pushed since
+ * create/reset as tracked on the host.
+ */
+long long filark_stream_launch_count(const filark_stream_t *h);
+long long filark_stream_samples_pushed(const filark_stream_t *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* FILARK_STREAM_H */

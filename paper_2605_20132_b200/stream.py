@@ -1,0 +1,218 @@
+"""Thin ctypes binding of include/filark_stream.h -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of csrc/; there is no CPU fallback: if
+libfilark_stream.so is missing or fails to load, importing this module's functions raises.
+torch is used for device memory and streams only.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import numpy as np
+
+from .build import LIB_PATH
+from .workloads import CHANNEL_MAJOR, TIME_MAJOR
+
+FLAG_NONE = 0
+FLAG_SERIAL_SCAN = 1
+MAX_SECTIONS = 16
+
+STATUS_NAMES = {0: "FILARK_OK", 1: "FILARK_ERR_INVALID_ARG", 2: "FILARK_ERR_UNSTABLE",
+                3: "FILARK_ERR_ALLOC", 4: "FILARK_ERR_CUDA", 5: "FILARK_ERR_DEVICE_MISMATCH",
+                6: "FILARK_ERR_ALIGNMENT"}
+
+_lib = None
+
+
+class FilarkError(RuntimeError):
+    def __init__(self, status: int, where: str, detail: str = ""):
+        self.status = int(status)
+        super().__init__(f"{where}: {STATUS_NAMES.get(self.status, self.status)} {detail}".strip())
+
+
+def library_path() -> str:
+    return LIB_PATH
+
+
+def load_library():
+    """Load the C-ABI library; fails loudly if it has not been built (no fallback)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise FileNotFoundError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2605_20132_b200.build` "
+            "(there is no CPU fallback for the filark stream path)")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, ll, ci, cu = ctypes.c_void_p, ctypes.c_longlong, ctypes.c_int, ctypes.c_uint
+    lib.filark_stream_create.restype = ci
+    lib.filark_stream_create.argtypes = [ctypes.POINTER(vp), ci, vp, ci, ci, ci]
+    lib.filark_stream_create_ex.restype = ci
+    lib.filark_stream_create_ex.argtypes = [ctypes.POINTER(vp), ci, vp, ci, ci, ci, ci, cu]
+    lib.filark_stream_push.restype = ci
+    lib.filark_stream_push.argtypes = [vp, vp, ll, vp, vp, vp]
+    lib.filark_stream_push_pitched.restype = ci
+    lib.filark_stream_push_pitched.argtypes = [vp, vp, ll, ll, vp, vp, ll, vp]
+    lib.filark_stream_push_host.restype = ci
+    lib.filark_stream_push_host.argtypes = [vp, vp, ll, vp, vp, vp]
+    lib.filark_stream_reset.restype = ci
+    lib.filark_stream_reset.argtypes = [vp, vp]
+    lib.filark_stream_destroy.restype = ci
+    lib.filark_stream_destroy.argtypes = [vp]
+    lib.filark_status_string.restype = ctypes.c_char_p
+    lib.filark_status_string.argtypes = [ci]
+    lib.filark_last_cuda_error.restype = ci
+    lib.filark_last_cuda_error.argtypes = [vp]
+    lib.filark_stream_launch_count.restype = ll
+    lib.filark_stream_launch_count.argtypes = [vp]
+    lib.filark_stream_samples_pushed.restype = ll
+    lib.filark_stream_samples_pushed.argtypes = [vp]
+    lib.filark_debug_design.restype = ci
+    lib.filark_debug_design.argtypes = [vp, ci, vp, vp, vp]
+    lib.filark_debug_tail_geometry.restype = ci
+    lib.filark_debug_tail_geometry.argtypes = [ll, vp, vp, vp, vp, vp]
+    lib.filark_debug_block_power.restype = ci
+    lib.filark_debug_block_power.argtypes = [vp, ll, vp]
+    _lib = lib
+    return lib
+
+
+def _ptr(t) -> Optional[int]:
+    return None if t is None else int(t.data_ptr())
+
+
+def _cur_stream() -> int:
+    import torch
+    return int(torch.cuda.current_stream().cuda_stream)
+
+
+class FilarkStream:
+    """filark_stream_create / push / reset / destroy with torch CUDA tensors as buffers."""
+
+    def __init__(self, n_ch: int, sos, sta_len: int, lta_len: int, layout: int = CHANNEL_MAJOR,
+                 flags: int = FLAG_NONE):
+        lib = load_library()
+        sos = np.ascontiguousarray(np.asarray(sos, dtype=np.float64))
+        if sos.ndim != 2 or sos.shape[1] != 6:
+            raise ValueError("sos must be [n_sec][6]")
+        self._lib = lib
+        self._h = ctypes.c_void_p()
+        self.n_ch, self.n_sec, self.layout = int(n_ch), int(sos.shape[0]), int(layout)
+        st = lib.filark_stream_create_ex(ctypes.byref(self._h), self.n_ch, sos.ctypes.data,
+                                         self.n_sec, int(sta_len), int(lta_len), self.layout,
+                                         int(flags))
+        if st != 0:
+            self._h = ctypes.c_void_p()
+            raise FilarkError(st, "filark_stream_create_ex")
+
+    # -- helpers
+    def _check(self, st: int, where: str):
+        if st != 0:
+            detail = ""
+            if st == 4:
+                detail = f"(cudaError {self._lib.filark_last_cuda_error(self._h)})"
+            raise FilarkError(st, where, detail)
+
+    def _n_t(self, x) -> int:
+        if x.dim() != 2:
+            raise ValueError("chunk must be 2-D")
+        n_c, n_t = (x.shape[0], x.shape[1]) if self.layout == CHANNEL_MAJOR else (x.shape[1], x.shape[0])
+        if n_c != self.n_ch:
+            raise ValueError("chunk channel count does not match the stream")
+        return int(n_t)
+
+    # -- C ABI mirrors
+    def push(self, d_in, d_filt=None, d_cf=None, stream: Optional[int] = None):
+        """d_in/d_filt/d_cf: contiguous float32 CUDA tensors of identical 2-D shape."""
+        import torch
+        for t in (d_in, d_filt, d_cf):
+            if t is not None and (not t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous()):
+                raise ValueError("buffers must be contiguous float32 CUDA tensors")
+        n_t = self._n_t(d_in)
+        st = self._lib.filark_stream_push(self._h, _ptr(d_in), n_t, _ptr(d_filt), _ptr(d_cf),
+                                          _cur_stream() if stream is None else stream)
+        self._check(st, "filark_stream_push")
+
+    def push_pitched(self, d_in, n_t: int, in_pitch: int, d_filt, d_cf, out_pitch: int,
+                     in_offset: int = 0, out_offset: int = 0, stream: Optional[int] = None):
+        """Sub-view push: pointers are tensor base + offset (elements); pitches in elements."""
+        pin = _ptr(d_in) + 4 * in_offset
+        pf = None if d_filt is None else _ptr(d_filt) + 4 * out_offset
+        pc = None if d_cf is None else _ptr(d_cf) + 4 * out_offset
+        st = self._lib.filark_stream_push_pitched(self._h, pin, int(n_t), int(in_pitch), pf, pc,
+                                                  int(out_pitch),
+                                                  _cur_stream() if stream is None else stream)
+        self._check(st, "filark_stream_push_pitched")
+
+    def push_host(self, h_in, h_filt=None, h_cf=None, stream: Optional[int] = None):
+        """Host (ideally pinned) float32 tensors/arrays; asynchronous on the stream."""
+        n_t = self._n_t(h_in)
+        st = self._lib.filark_stream_push_host(self._h, _ptr(h_in), n_t, _ptr(h_filt), _ptr(h_cf),
+                                               _cur_stream() if stream is None else stream)
+        self._check(st, "filark_stream_push_host")
+
+    def reset(self, stream: Optional[int] = None):
+        self._check(self._lib.filark_stream_reset(self._h, _cur_stream() if stream is None else stream),
+                    "filark_stream_reset")
+
+    def destroy(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            self._lib.filark_stream_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    close = destroy
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    @property
+    def launch_count(self) -> int:
+        return int(self._lib.filark_stream_launch_count(self._h))
+
+    @property
+    def samples_pushed(self) -> int:
+        return int(self._lib.filark_stream_samples_pushed(self._h))
+
+
+def push_host(stream_obj: FilarkStream, h_in, h_filt=None, h_cf=None):
+    """Module-level alias of FilarkStream.push_host (the end-to-end call bench.py times)."""
+    stream_obj.push_host(h_in, h_filt, h_cf)
+
+
+# ---- host-only introspection (include/filark_debug.h) ----------------------------------------
+def debug_design(sos):
+    lib = load_library()
+    sos = np.ascontiguousarray(np.asarray(sos, dtype=np.float64))
+    n = sos.shape[0]
+    kinds = np.zeros(n, dtype=np.int32)
+    coefs = np.zeros((n, 9), dtype=np.float64)
+    gain = ctypes.c_double(0.0)
+    st = lib.filark_debug_design(sos.ctypes.data, n, kinds.ctypes.data, coefs.ctypes.data,
+                                 ctypes.addressof(gain))
+    if st != 0:
+        raise FilarkError(st, "filark_debug_design")
+    return kinds, coefs, float(gain.value)
+
+
+def debug_tail_geometry(n_t: int):
+    lib = load_library()
+    v = [ctypes.c_int(0) for _ in range(5)]
+    st = lib.filark_debug_tail_geometry(int(n_t), *[ctypes.addressof(x) for x in v])
+    if st != 0:
+        raise FilarkError(st, "filark_debug_tail_geometry")
+    return tuple(int(x.value) for x in v)
+
+
+def debug_block_power(sos6, e: int):
+    lib = load_library()
+    sos6 = np.ascontiguousarray(np.asarray(sos6, dtype=np.float64))
+    out = np.zeros(4, dtype=np.float64)
+    st = lib.filark_debug_block_power(sos6.ctypes.data, int(e), out.ctypes.data)
+    if st != 0:
+        raise FilarkError(st, "filark_debug_block_power")
+    return out.reshape(2, 2)

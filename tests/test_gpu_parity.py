@@ -1,0 +1,234 @@
+"""GPU parity: the CUDA path (through the C ABI) against the float64 oracle, element by element,
+on the same seeded inputs.  Tolerance: BASELINE.json north_star (tests/_util.py)."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2605_20132_b200.workloads import (CHANNEL_MAJOR, TIME_MAJOR, CONFIGS, design_sos,
+                                              generate, push_schedule)
+from tests._util import as_cm, assert_parity, channel_errors, run_gpu, run_oracle, split
+
+pytestmark = pytest.mark.gpu
+
+
+def _stream(w, layout=CHANNEL_MAJOR, flags=0):
+    from paper_2605_20132_b200.stream import FilarkStream
+    return FilarkStream(w.n_ch, design_sos(w), w.sta_len, w.lta_len, layout, flags)
+
+
+def _case(w, cuda_device, layout):
+    x_cm = generate(w, device="cpu", layout=CHANNEL_MAJOR)
+    ref_f, ref_c = run_oracle(x_cm.numpy(), design_sos(w), w.sta_len, w.lta_len)
+    x_dev = (x_cm if layout == CHANNEL_MAJOR else x_cm.t().contiguous()).to(cuda_device)
+    return x_dev, ref_f, ref_c
+
+
+def _check(filt, cf, ref_f, ref_c, layout, what):
+    r1 = assert_parity(as_cm(filt.cpu().numpy(), layout), ref_f, what + " filt")
+    r2 = assert_parity(as_cm(cf.cpu().numpy(), layout), ref_c, what + " cf")
+    return r1, r2
+
+
+# ------------------------------------------------------------------ configs[0]: full size
+@pytest.mark.parametrize("layout", [CHANNEL_MAJOR, TIME_MAJOR])
+def test_cfg1_whole_and_chunked(cuda_device, layout):
+    w = CONFIGS["cfg1"]
+    x_dev, ref_f, ref_c = _case(w, cuda_device, layout)
+    s = _stream(w, layout)
+    f, c = run_gpu(s, x_dev, layout, [(0, w.n_t)])
+    _check(f, c, ref_f, ref_c, layout, "cfg1 whole")
+    s.reset()
+    f2, c2 = run_gpu(s, x_dev, layout, split(w.n_t, [w.chunk]))
+    _check(f2, c2, ref_f, ref_c, layout, "cfg1 chunked")
+    # chunked vs whole on the GPU itself, same tolerance
+    assert_parity(as_cm(f2.cpu().numpy(), layout), as_cm(f.cpu().numpy(), layout), "gpu chunked vs whole filt")
+    assert_parity(as_cm(c2.cpu().numpy(), layout), as_cm(c.cpu().numpy(), layout), "gpu chunked vs whole cf")
+    s.destroy()
+
+
+# ------------------------------------------------------------------ configs[1..4]: scaled shapes
+SCALED = [("cfg2", 96, 60_000), ("cfg3", 64, 90_000), ("cfg4", 80, 100_000), ("cfg5", 40, 300_000)]
+
+
+@pytest.mark.parametrize("name,n_ch,n_t", SCALED)
+def test_scaled_configs_channel_major(cuda_device, name, n_ch, n_t):
+    w = CONFIGS[name].scaled(n_ch=n_ch, n_t=n_t)
+    x_dev, ref_f, ref_c = _case(w, cuda_device, CHANNEL_MAJOR)
+    s = _stream(w)
+    f, c = run_gpu(s, x_dev, CHANNEL_MAJOR, [(0, n_t)])
+    _check(f, c, ref_f, ref_c, CHANNEL_MAJOR, f"{name} whole")
+    s.reset()
+    sched = push_schedule(w)
+    bounds = split(n_t, sched)
+    f, c = run_gpu(s, x_dev, CHANNEL_MAJOR, bounds)
+    _check(f, c, ref_f, ref_c, CHANNEL_MAJOR, f"{name} in {len(bounds)} pushes")
+    s.destroy()
+
+
+@pytest.mark.parametrize("name,n_ch,n_t", [("cfg3", 48, 30_000), ("cfg5", 33, 60_000)])
+def test_scaled_configs_time_major(cuda_device, name, n_ch, n_t):
+    w = CONFIGS[name].scaled(n_ch=n_ch, n_t=n_t)
+    x_dev, ref_f, ref_c = _case(w, cuda_device, TIME_MAJOR)
+    s = _stream(w, TIME_MAJOR)
+    f, c = run_gpu(s, x_dev, TIME_MAJOR, split(n_t, push_schedule(w)))
+    _check(f, c, ref_f, ref_c, TIME_MAJOR, f"{name} time-major")
+    s.destroy()
+
+
+# ------------------------------------------------------------------ chunking fuzz / ragged tails
+FUZZ = [[1], [2, 3], [31, 32, 33], [1, 2, 3, 31, 32, 33, 97, 499, 1021, 1024, 1025, 2047, 4099],
+        [7919], [1023, 1], [4096, 5], "random"]
+
+
+@pytest.mark.parametrize("sizes", FUZZ, ids=[str(s) for s in FUZZ])
+def test_chunking_fuzz(cuda_device, sizes):
+    w = CONFIGS["cfg3"].scaled(n_ch=9, n_t=13_007 if sizes != [1] else 700)
+    if sizes == "random":
+        sizes = np.random.default_rng(99).integers(1, 3000, size=64).tolist()
+    x_dev, ref_f, ref_c = _case(w, cuda_device, CHANNEL_MAJOR)
+    s = _stream(w)
+    f, c = run_gpu(s, x_dev, CHANNEL_MAJOR, split(w.n_t, sizes))
+    _check(f, c, ref_f, ref_c, CHANNEL_MAJOR, f"fuzz {sizes[:6]}")
+    s.destroy()
+
+
+def test_serial_diagnostic_kernel(cuda_device):
+    w = CONFIGS["cfg2"].scaled(n_ch=40, n_t=20_000)
+    x_dev, ref_f, ref_c = _case(w, cuda_device, CHANNEL_MAJOR)
+    s = _stream(w, CHANNEL_MAJOR, flags=1)
+    f, c = run_gpu(s, x_dev, CHANNEL_MAJOR, split(w.n_t, [999]))
+    _check(f, c, ref_f, ref_c, CHANNEL_MAJOR, "serial kernel")
+    s.destroy()
+
+
+# ------------------------------------------------------------------ degenerate inputs
+def test_dead_channel_dc_offset_and_spike(cuda_device):
+    w = CONFIGS["cfg1"].scaled(n_ch=6, n_t=9000)
+    x = generate(w).numpy().copy()
+    x[0] = 0.0                       # dead channel -> filt = cf = 0 exactly
+    x[1] += 1000.0                   # DC offset (fp32 dynamic range)
+    x[2, 4000] += 1e4                # single huge spike
+    x[3] *= 1e-12                    # tiny amplitudes
+    ref_f, ref_c = run_oracle(x, design_sos(w), w.sta_len, w.lta_len)
+    s = _stream(w)
+    f, c = run_gpu(s, torch.from_numpy(x).to(cuda_device), CHANNEL_MAJOR, split(w.n_t, [1000]))
+    f, c = f.cpu().numpy(), c.cpu().numpy()
+    assert np.all(f[0] == 0) and np.all(c[0] == 0)
+    for ch in (2, 3, 4, 5):
+        assert_parity(f[ch:ch + 1], ref_f[ch:ch + 1], f"ch{ch} filt")
+        assert_parity(c[ch:ch + 1], ref_c[ch:ch + 1], f"ch{ch} cf")
+    # DC offset 1000: absolute error ~ 6e-8 * 1000 on an O(1) band-passed signal after the transient
+    rel, _ = channel_errors(f[1:2], ref_f[1:2])
+    assert rel < 1e-3
+    assert np.all(c >= 0) and c.max() <= w.lta_len / w.sta_len * (1 + 1e-5)
+    s.destroy()
+
+
+def test_warmup_and_reset(cuda_device):
+    w = CONFIGS["cfg1"].scaled(n_ch=4, n_t=3000)
+    x_dev, ref_f, ref_c = _case(w, cuda_device, CHANNEL_MAJOR)
+    s = _stream(w)
+    f, c = run_gpu(s, x_dev, CHANNEL_MAJOR, split(w.n_t, [300]))
+    c_np = c.cpu().numpy()
+    assert np.all(c_np[:, :w.lta_len] == 0) and np.all(c_np[:, w.lta_len] > 0)
+    assert s.samples_pushed == w.n_t
+    s.reset()
+    f2, c2 = run_gpu(s, x_dev, CHANNEL_MAJOR, split(w.n_t, [300]))
+    assert torch.equal(f, f2) and torch.equal(c, c2)      # same launches -> bit-identical
+    s.destroy()
+
+
+def test_optional_outputs_and_empty_push(cuda_device):
+    w = CONFIGS["cfg2"].scaled(n_ch=5, n_t=5000)
+    x_dev, ref_f, ref_c = _case(w, cuda_device, CHANNEL_MAJOR)
+    s = _stream(w)
+    bounds = split(w.n_t, [1234])
+    f, _ = run_gpu(s, x_dev, CHANNEL_MAJOR, bounds, want_cf=False)
+    s.reset()
+    s.push(x_dev[:, :0].contiguous(), torch.empty((5, 0), device=cuda_device),
+           torch.empty((5, 0), device=cuda_device))          # n_t = 0: no-op
+    assert s.samples_pushed == 0
+    _, c = run_gpu(s, x_dev, CHANNEL_MAJOR, bounds, want_filt=False)
+    assert_parity(f.cpu().numpy(), ref_f, "filt only")
+    assert_parity(c.cpu().numpy(), ref_c, "cf only (state still advances without filt)")
+    s.destroy()
+
+
+def test_pitched_push_on_subviews(cuda_device):
+    """Push column windows of a whole channel-major record without packing them."""
+    w = CONFIGS["cfg4"].scaled(n_ch=12, n_t=7000)
+    x_dev, ref_f, ref_c = _case(w, cuda_device, CHANNEL_MAJOR)
+    s = _stream(w)
+    filt = torch.zeros_like(x_dev); cf = torch.zeros_like(x_dev)
+    for a, b in split(w.n_t, [1000, 333]):
+        s.push_pitched(x_dev, b - a, w.n_t, filt, cf, w.n_t, in_offset=a, out_offset=a)
+    torch.cuda.synchronize()
+    _check(filt, cf, ref_f, ref_c, CHANNEL_MAJOR, "pitched")
+    s.destroy()
+
+
+def test_error_codes(cuda_device):
+    from paper_2605_20132_b200.stream import FilarkError, FilarkStream
+    w = CONFIGS["cfg1"].scaled(n_ch=4, n_t=64)
+    sos = design_sos(w)
+    for bad in [dict(n_ch=0), dict(sta_len=0), dict(lta_len=10, sta_len=20), dict(layout=7), dict(flags=8)]:
+        kw = dict(n_ch=4, sos=sos, sta_len=5, lta_len=50, layout=0, flags=0); kw.update(bad)
+        with pytest.raises(FilarkError) as e:
+            FilarkStream(**kw)
+        assert e.value.status == 1
+    with pytest.raises(FilarkError) as e:
+        FilarkStream(4, np.array([[1.0, 0, 0, 1.0, -2.1, 1.1]]), 5, 50)
+    assert e.value.status == 2
+    s = FilarkStream(4, sos, 5, 50)
+    x = torch.zeros((4, 64), device=cuda_device)
+    with pytest.raises(FilarkError) as e:
+        s.push(x, None, None)                         # both outputs NULL
+    assert e.value.status == 1
+    with pytest.raises(FilarkError) as e:
+        s.push(x, x, None)                            # in-place rejected
+    assert e.value.status == 1
+    big = torch.zeros((4 * 64 + 1,), device=cuda_device)
+    with pytest.raises(FilarkError) as e:             # misaligned pointer (2 bytes off)
+        s._check(s._lib.filark_stream_push(s._h, big.data_ptr() + 2, 64, x.data_ptr(), None, None), "push")
+    assert e.value.status == 6
+    s.destroy()
+
+
+def test_cuda_graph_capture_replays_with_carried_state(cuda_device):
+    """A captured push has no host-side mutable arguments: replaying it streams the record."""
+    w = CONFIGS["cfg1"].scaled(n_ch=8, n_t=6000)
+    x_dev, ref_f, ref_c = _case(w, cuda_device, CHANNEL_MAJOR)
+    s = _stream(w)
+    chunk = 1000
+    xin = torch.empty((8, chunk), device=cuda_device); f = torch.empty_like(xin); c = torch.empty_like(xin)
+    side = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        xin.copy_(x_dev[:, :chunk]); s.push(xin, f, c); s.reset()      # warm-up outside capture
+        torch.cuda.synchronize()
+        with torch.cuda.graph(g, stream=side):
+            s.push(xin, f, c)
+    outs_f, outs_c = [], []
+    for a, b in split(w.n_t, [chunk]):
+        xin.copy_(x_dev[:, a:b]); g.replay()
+        outs_f.append(f.clone()); outs_c.append(c.clone())
+    torch.cuda.synchronize()
+    _check(torch.cat(outs_f, 1), torch.cat(outs_c, 1), ref_f, ref_c, CHANNEL_MAJOR, "graph replay")
+    s.destroy()
+
+
+def test_push_host_end_to_end(cuda_device):
+    w = CONFIGS["cfg2"].scaled(n_ch=16, n_t=8000)
+    x = generate(w)
+    ref_f, ref_c = run_oracle(x.numpy(), design_sos(w), w.sta_len, w.lta_len)
+    s = _stream(w)
+    fs, cs = [], []
+    for a, b in split(w.n_t, [2000]):
+        hin = x[:, a:b].contiguous().pin_memory()
+        hf = torch.empty_like(hin).pin_memory(); hc = torch.empty_like(hin).pin_memory()
+        s.push_host(hin, hf, hc)
+        torch.cuda.synchronize()
+        fs.append(hf.clone()); cs.append(hc.clone())
+    assert_parity(torch.cat(fs, 1).numpy(), ref_f, "push_host filt")
+    assert_parity(torch.cat(cs, 1).numpy(), ref_c, "push_host cf")
+    s.destroy()
