@@ -15,7 +15,8 @@ extern "C" {
 
 /*
  * sos    [host, in]  [n_sec][6] doubles (b0 b1 b2 a0 a1 a2).
- * kinds  [host, out] n_sec ints: 0 = transposed direct form II, 1 = normal (coupled) form. May be NULL.
+ * kinds  [host, out] n_sec ints: 0 direct form II, 1 direct form II with explicit b0, 2 delta form,
+ *                    3 delta form without a zero at z = 1, 4 normal (coupled) form.  May be NULL.
  * coefs  [host, out] n_sec x 9 doubles: A row-major (4), B (2), C (2), D.  May be NULL.
  * gain   [host, out] product of the b0 factors moved in front of the cascade.  May be NULL.
  * The cascade equals gain * (sections in state-space form applied in order).
@@ -23,11 +24,14 @@ extern "C" {
 int filark_debug_design(const double *sos, int n_sec, int *kinds, double *coefs, double *gain);
 
 /*
- * Tiling of one channel-major push of n_t samples: n_full tiles of 1024 samples, then a tail
- * tile whose lanes hold `len` samples each: `nfull` full lanes, one partial lane with `part`
- * samples (0 = none); `jl` = lane whose end state is carried out (-1 if there is no tail).
+ * Slot geometry of one channel-major push of n_t >= 1 samples (csrc/filark_kernels.cuh): the time
+ * axis is cut into slots of L samples aligned to the END of the push; a tile is 64 slots (lane l
+ * owns slots 2l, 2l+1).  force_L = 0 lets the library choose L among its compiled variants
+ * (8, 16, 24, 32, 48), otherwise L = force_L.  out7 = { L, n_tiles, lead (idle slots in front),
+ * r (samples in the first, possibly short, slot), pad0 (zeros in front of sample 0),
+ * last_lane, last_half (position in the last tile of the slot holding the last sample) }.
  */
-int filark_debug_tail_geometry(long long n_t, int *n_full, int *len, int *nfull, int *part, int *jl);
+int filark_debug_push_geometry(long long n_t, int force_L, int *out7);
 
 /* out4 (row-major 2x2) = A^e for the state-space form chosen for one section (6 doubles). */
 int filark_debug_block_power(const double *sos6, long long e, double *out4);

@@ -67,6 +67,10 @@ typedef enum filark_status {
 #define FILARK_FLAG_SERIAL_SCAN 1u  /* diagnostic kernel: one thread per channel, serial in time,
                                        same state-space arithmetic, no blocked scan             */
 
+#define FILARK_FLAG_FORCE_L(L) ((unsigned)(L) << 8)  /* tuning/testing: use the kernel variant with
+                                       sub-block length L (8, 16, 24, 32 or 48) for every push
+                                       instead of the one chosen from n_t                        */
+
 #define FILARK_MAX_SECTIONS 16
 
 /*

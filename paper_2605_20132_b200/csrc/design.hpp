@@ -3,30 +3,35 @@
 // Every section (b0 b1 b2 a0 a1 a2) of the stateful SOS IIR operator is
 // rewritten as a 2-state linear system
 //        s[n] = A s[n-1] + B x[n],      y[n] = C s[n-1] + D x[n]
-// in one of two coordinate systems, chosen for fp32 conditioning:
+// in a coordinate system chosen for fp32 conditioning and instruction count.
+// With the numerator normalised to 1 + n1 z^-1 + n2 z^-2 (b0 moves into one global gain):
 //
-//   KIND_T  transposed direct form II:  A = [[-a1, 1], [-a2, 0]],  B = (b1 - a1 b0, b2 - a2 b0),
-//           C = (1, 0), D = b0.  5 FMA-class ops per sample.  Used when both poles are far
-//           from z = +-1 (coefficient rounding then moves the response by < 1e-6).
-//   KIND_R  normal ("coupled") form for a complex pole pair sigma +- i omega:
-//           A = [[sigma, omega], [-omega, sigma]], B = (1, 0), C = (c1, c2), D = 1, with the
-//           section's b0 factored out into one global gain.  6 ops per sample.  The state
-//           coordinates are orthogonal, so rounding noise injected into the carried state is
-//           not amplified by the long memory of poles next to z = 1.
+//   KIND_DF2    direct form II:  w = x - a1 w1 - a2 w2,  y = w + n1 w1 + n2 w2,  s = (w1, w2).
+//               4 FMA per sample.  Used when both poles are far from z = +-1.
+//   KIND_DF2G   the same with an explicit b0 (sections whose b0 is 0):  y = b0 w + b1 w1 + b2 w2.
+//   KIND_DELTA  delta (difference) form for poles next to z = +1, s = (u, w), u = w[n] - w[n-1]:
+//                    u' = p u - q w + x,   w' = w + u',   y = u' - n2 u  (+ m w),
+//               p = a2, q = 1 + a1 + a2, m = 1 + n1 + n2.  The large, slowly varying state w is
+//               only ever multiplied by the tiny q, and q = |1 - pole|^2 keeps full relative
+//               precision in fp32 -- the two things direct forms lose next to z = 1.
+//               4 FMA per sample when the section has a zero at z = 1 (m = 0), else 5
+//               (KIND_DELTAG).
+//   KIND_NORMAL normal ("coupled") form for a complex pole pair sigma +- i omega next to
+//               z = -1:  A = [[sigma, omega], [-omega, sigma]], B = e1, C = (c1, c2), D = 1.
+//               6 FMA per sample.
 //
-// The blocked scan needs, per section: the fix-up rows C A^i (i < L), the block powers
-// A^(len 2^d) for the warp-shuffle scan, and A^len / A^part for the carry-out.  All are computed
-// here in float64 from the unrounded A and rounded to fp32 last.
+// The blocked scan needs, per section and per sub-block length L: the fix-up rows C A^i (i < L),
+// the powers A^r (r <= L) for the carry across a (possibly short) sub-block, and A^(2L 2^d) for
+// the warp-shuffle scan over lane pairs.  All are computed here in float64 from the unrounded A
+// and rounded to fp32 last.
 #pragma once
 #include <cmath>
 #include <cstring>
 
 namespace filark {
 
-enum { KIND_T = 0, KIND_R = 1 };
-constexpr int kSubBlock = 32;      // samples per lane in a full tile (L)
-constexpr int kScanSteps = 5;      // log2(32 lanes)
-constexpr double kUseNormalFormBelow = 0.05;   // |1 -+ p|^2 threshold, see DESIGN.md 4
+enum { KIND_DF2 = 0, KIND_DF2G = 1, KIND_DELTA = 2, KIND_DELTAG = 3, KIND_NORMAL = 4 };
+constexpr double kNearUnitCircle = 0.05;   // |1 -+ pole|^2 threshold, see DESIGN.md 4
 
 struct Mat2 { double a, b, c, d; };             // [[a, b], [c, d]]
 inline Mat2 mul(const Mat2& x, const Mat2& y) {
@@ -39,15 +44,18 @@ inline Mat2 mpow(Mat2 m, long long e) {
     while (e > 0) { if (e & 1) r = mul(r, m); m = mul(m, m); e >>= 1; }
     return r;
 }
+inline double norm1(const Mat2& m) {
+    return std::fmax(std::fabs(m.a) + std::fabs(m.c), std::fabs(m.b) + std::fabs(m.d));
+}
 
 struct Section {
     int kind;
     Mat2 A;
     double B[2], C[2], D;
-    double gain;          // factor moved into the global input gain (1 for KIND_T)
+    double gain;          // factor moved into the global input gain (1 for KIND_DF2G)
     double coef[6];       // what the local pass multiplies with (meaning depends on kind)
     double pole_radius;
-    double dist2;         // min(|1-p|^2, |1+p|^2)
+    double dist_p1, dist_m1;     // |1 - p|^2 = 1 + a1 + a2,  |1 + p|^2 = 1 - a1 + a2
 };
 
 enum DesignStatus { DESIGN_OK = 0, DESIGN_INVALID = 1, DESIGN_UNSTABLE = 2 };
@@ -64,34 +72,51 @@ inline DesignStatus design_section(const double* sos6, Section* out)
     if (!(std::fabs(a2) < 1.0 && std::fabs(a1) < 1.0 + a2)) return DESIGN_UNSTABLE;
     const double disc = a1 * a1 - 4.0 * a2;
     Section s{};
-    s.dist2 = std::fmin(1.0 + a1 + a2, 1.0 - a1 + a2);
+    s.dist_p1 = 1.0 + a1 + a2;
+    s.dist_m1 = 1.0 - a1 + a2;
     s.gain = 1.0;
     if (disc < 0.0) s.pole_radius = std::sqrt(a2);
     else s.pole_radius = std::fmax(std::fabs((-a1 + std::sqrt(disc)) / 2), std::fabs((-a1 - std::sqrt(disc)) / 2));
     const double omega = disc < 0.0 ? 0.5 * std::sqrt(-disc) : 0.0;
-    const bool normal_form = disc < 0.0 && b0 != 0.0 && omega > 1e-7 && s.dist2 < kUseNormalFormBelow;
-    if (!normal_form) {
-        s.kind = KIND_T;
-        s.A = { -a1, 1.0, -a2, 0.0 };
-        s.B[0] = b1 - a1 * b0; s.B[1] = b2 - a2 * b0;
-        s.C[0] = 1.0; s.C[1] = 0.0; s.D = b0;
-        s.coef[0] = b0; s.coef[1] = b1; s.coef[2] = b2; s.coef[3] = -a1; s.coef[4] = -a2; s.coef[5] = 0;
-    } else {
-        // Normalise the numerator by b0 (D = 1); b0 goes to the global gain.
-        const double n1 = b1 / b0, n2 = b2 / b0;
+    if (b0 == 0.0) {
+        s.kind = KIND_DF2G;
+        s.A = { -a1, -a2, 1.0, 0.0 };
+        s.B[0] = 1.0; s.B[1] = 0.0;
+        s.C[0] = b1; s.C[1] = b2; s.D = 0.0;
+        s.coef[0] = -a1; s.coef[1] = -a2; s.coef[2] = b1; s.coef[3] = b2; s.coef[4] = 0.0;
+        *out = s;
+        return DESIGN_OK;
+    }
+    const double n1 = b1 / b0, n2 = b2 / b0;       // numerator 1 + n1 z^-1 + n2 z^-2, gain b0
+    s.gain = b0;
+    s.D = 1.0;
+    if (s.dist_p1 < kNearUnitCircle) {
+        const double p = a2, q = s.dist_p1;
+        double m = 1.0 + n1 + n2;
+        if (std::fabs(m) < 1e-13 * (1.0 + std::fabs(n1) + std::fabs(n2))) m = 0.0;   // zero at z = 1
+        s.kind = m == 0.0 ? KIND_DELTA : KIND_DELTAG;
+        s.A = { p, -q, p, 1.0 - q };
+        s.B[0] = 1.0; s.B[1] = 1.0;
+        s.C[0] = p - n2; s.C[1] = m - q;
+        s.coef[0] = p; s.coef[1] = -q; s.coef[2] = -n2; s.coef[3] = m;
+    } else if (s.dist_m1 < kNearUnitCircle && disc < 0.0 && omega > 1e-7) {
         const double B1 = n1 - a1, B2 = n2 - a2;                 // DF2T input vector, D = 1
         const double sigma = -0.5 * a1;
         // T = [Re v, Im v], v = (1, -sigma + i omega): T^-1 A T = [[sigma, omega], [-omega, sigma]],
-        // T^-1 B = (B1, (sigma B1 + B2)/omega), C T = (1, 0).
+        // T^-1 B = (B1, (sigma B1 + B2)/omega), C T = (1, 0).  M = [[Bp1, -Bp2], [Bp2, Bp1]] maps
+        // e1 -> B' and commutes with A': B'' = e1, C'' = C' M.
         const double Bp1 = B1, Bp2 = (sigma * B1 + B2) / omega;
-        // M = [[Bp1, -Bp2], [Bp2, Bp1]] maps e1 -> B' and commutes with A': B'' = e1, C'' = C' M.
-        s.kind = KIND_R;
+        s.kind = KIND_NORMAL;
         s.A = { sigma, omega, -omega, sigma };
         s.B[0] = 1.0; s.B[1] = 0.0;
-        s.C[0] = Bp1; s.C[1] = -Bp2; s.D = 1.0;
-        s.gain = b0;
+        s.C[0] = Bp1; s.C[1] = -Bp2;
         s.coef[0] = sigma; s.coef[1] = omega; s.coef[2] = s.C[0]; s.coef[3] = s.C[1];
-        s.coef[4] = 0; s.coef[5] = 0;
+    } else {
+        s.kind = KIND_DF2;
+        s.A = { -a1, -a2, 1.0, 0.0 };
+        s.B[0] = 1.0; s.B[1] = 0.0;
+        s.C[0] = n1 - a1; s.C[1] = n2 - a2;
+        s.coef[0] = -a1; s.coef[1] = -a2; s.coef[2] = n1; s.coef[3] = n2;
     }
     *out = s;
     return DESIGN_OK;
@@ -108,11 +133,12 @@ inline void fixup_rows(const Section& s, int n, double* out)
     }
 }
 
-// Block powers for the scan over sub-blocks of `len` samples: P[d] = A^(len 2^d).
-inline void scan_powers(const Section& s, int len, Mat2* P /* [kScanSteps] */)
+// 1 - (1-c)^e, accurate for tiny c (the averages' block decay in the "v += u - beta u" form).
+inline double one_minus_pow(double c, double e)
 {
-    Mat2 m = mpow(s.A, len);
-    for (int d = 0; d < kScanSteps; ++d) { P[d] = m; m = mul(m, m); }
+    if (e <= 0.0) return 0.0;
+    if (c >= 1.0) return 1.0;
+    return -std::expm1(e * std::log1p(-c));
 }
 
 }  // namespace filark

@@ -19,21 +19,25 @@
 
 using namespace filark;
 
+// Sub-block lengths compiled as kernel variants; a push picks the cheapest for its n_t.
+static const int kVariantL[] = {8, 16, 24, 32, 48};
+constexpr int kNumVariants = 5;
+
+struct Geometry { int L, n_tiles, lead, r, pad0, last_lane, last_half; };
+
 struct filark_stream {
     int device;
     int n_ch, n_sec, sta_len, lta_len, layout;
     unsigned flags;
     Section sec[kMaxSec];
     double gain;
-    float* d_tab;
+    float* d_tab[kNumVariants];
+    size_t tab_floats[kNumVariants];
     float* d_state;
     Counter* d_ctr;
-    size_t tab_floats, state_floats;
+    size_t state_floats;
     int last_cuda_error;
     long long launches, samples;
-    long long cached_tail_rem;      // n_t % kTile the cached TailTab was built for (-1: none)
-    TailTab tail;
-    int tail_len, tail_nfull, tail_part, tail_jl, tail_magic;
     // staging for push_host
     float* d_stage[3];
     size_t stage_elems;
@@ -50,65 +54,136 @@ static void put_mat(float* dst, const Mat2& m)
     dst[0] = (float)m.a; dst[1] = (float)m.b; dst[2] = (float)m.c; dst[3] = (float)m.d;
 }
 
-// Static table for full tiles (layout documented in filark_kernels.cuh).
-static void build_static_table(const filark_stream* h, float* tab)
+template <int L> static size_t variant_floats(int n_sec)
 {
-    std::memset(tab, 0, sizeof(float) * h->tab_floats);
+    return (size_t)n_sec * SecTab<L>::stride + AvgTab<L>::size;
+}
+
+// Device table of sub-block length L (layout documented in filark_kernels.cuh).
+template <int L> static void build_variant_table(const filark_stream* h, float* tab)
+{
+    using ST = SecTab<L>;
+    using AT = AvgTab<L>;
+    std::memset(tab, 0, sizeof(float) * variant_floats<L>(h->n_sec));
     for (int k = 0; k < h->n_sec; ++k) {
         const Section& s = h->sec[k];
-        float* T = tab + k * kSecStride;
-        const int kind = s.kind == KIND_R ? kKindR : kKindT;
-        std::memcpy(&T[0], &kind, sizeof(int));
+        float* T = tab + (size_t)k * ST::stride;
+        std::memcpy(&T[kOffKind], &s.kind, sizeof(int));
         for (int i = 0; i < 5; ++i) T[kOffCoef + i] = (float)s.coef[i];
-        Mat2 P[kSteps];
-        scan_powers(s, kL, P);
-        for (int d = 0; d < kSteps; ++d) put_mat(T + kOffP + 4 * d, P[d]);
-        double g[2 * kL];
-        fixup_rows(s, kL, g);
-        for (int i = 0; i < 2 * kL; ++i) T[kOffG + i] = (float)g[i];
+        put_mat(T + kOffP, mpow(s.A, L));
+        Mat2 q = mpow(s.A, 2 * L);
+        int nsteps = kSteps;
+        for (int d = 0; d < kSteps; ++d) {
+            put_mat(T + kOffQ + 4 * d, q);
+            if (nsteps == kSteps && norm1(q) < 1e-10) nsteps = d;      // this and later steps add < 1e-10
+            q = mul(q, q);
+        }
+        std::memcpy(&T[kOffNSteps], &nsteps, sizeof(int));
+        Mat2 ap = ident();
+        for (int r = 0; r <= L; ++r) { put_mat(T + ST::apow + 4 * r, ap); ap = mul(ap, s.A); }
+        double g[2 * L];
+        fixup_rows(s, L, g);
+        for (int i = 0; i < L; ++i) {
+            T[ST::g0 + 2 * (L + i)] = (float)g[2 * i];         T[ST::g0 + 2 * (L + i) + 1] = (float)g[2 * i + 1];
+            T[ST::g1 + 2 * (L + i + 1)] = (float)g[2 * i];     T[ST::g1 + 2 * (L + i + 1) + 1] = (float)g[2 * i + 1];
+        }
+        // (row 2L of G1 would be g[L-1] shifted out of the table: it lands in the 4-float pad)
     }
-    float* AV = tab + h->n_sec * kSecStride;
+    float* AV = tab + (size_t)h->n_sec * ST::stride;
     const double cs = 1.0 / h->sta_len, cl = 1.0 / h->lta_len;
-    const double as = 1.0 - cs, al = 1.0 - cl;
-    AV[0] = (float)as; AV[1] = (float)al; AV[2] = (float)cs; AV[3] = (float)cl;
+    AV[0] = (float)(1.0 - cs); AV[1] = (float)(1.0 - cl);
+    AV[AT::beta_l] = (float)one_minus_pow(cs, L); AV[AT::beta_l + 1] = (float)one_minus_pow(cl, L);
     for (int d = 0; d < kSteps; ++d) {
-        const double e = (double)kL * (double)(1 << d);
-        AV[4 + d] = (float)(-std::expm1(e * std::log1p(-cs)));   // 1 - as^e without cancellation
-        AV[9 + d] = (float)(-std::expm1(e * std::log1p(-cl)));
+        const double e = 2.0 * L * (double)(1 << d);
+        AV[AT::beta_q + 2 * d] = (float)one_minus_pow(cs, e);
+        AV[AT::beta_q + 2 * d + 1] = (float)one_minus_pow(cl, e);
+    }
+    AV[14] = (float)cs; AV[15] = (float)cl;
+    for (int r = 0; r <= L; ++r) {
+        AV[AT::beta_r + 2 * r] = (float)one_minus_pow(cs, r);
+        AV[AT::beta_r + 2 * r + 1] = (float)one_minus_pow(cl, r);
+    }
+    for (int sh = 0; sh < L; ++sh) {
+        // alpha^-sh; alpha = 0 (length-1 average) keeps no memory, any finite factor will do
+        AV[AT::inv + 2 * sh] = cs >= 1.0 ? (sh == 0 ? 1.0f : 0.0f) : (float)std::exp(-(double)sh * std::log1p(-cs));
+        AV[AT::inv + 2 * sh + 1] = cl >= 1.0 ? (sh == 0 ? 1.0f : 0.0f) : (float)std::exp(-(double)sh * std::log1p(-cl));
     }
 }
 
-static double one_minus_pow(double c, double e)      // 1 - (1-c)^e, accurate for tiny c
+static size_t variant_floats_rt(int v, int n_sec)
 {
-    if (c >= 1.0) return e > 0 ? 1.0 : 0.0;
-    return -std::expm1(e * std::log1p(-c));
+    switch (kVariantL[v]) {
+        case 8: return variant_floats<8>(n_sec);
+        case 16: return variant_floats<16>(n_sec);
+        case 24: return variant_floats<24>(n_sec);
+        case 32: return variant_floats<32>(n_sec);
+        default: return variant_floats<48>(n_sec);
+    }
+}
+static void build_variant_rt(int v, const filark_stream* h, float* tab)
+{
+    switch (kVariantL[v]) {
+        case 8: build_variant_table<8>(h, tab); break;
+        case 16: build_variant_table<16>(h, tab); break;
+        case 24: build_variant_table<24>(h, tab); break;
+        case 32: build_variant_table<32>(h, tab); break;
+        default: build_variant_table<48>(h, tab); break;
+    }
+}
+static int sec_stride_rt(int v)
+{
+    switch (kVariantL[v]) {
+        case 8: return SecTab<8>::stride;
+        case 16: return SecTab<16>::stride;
+        case 24: return SecTab<24>::stride;
+        case 32: return SecTab<32>::stride;
+        default: return SecTab<48>::stride;
+    }
 }
 
-// Geometry + table of the ragged tail tile for rem = n_t % kTile samples (rem >= 1).
-static void build_tail(filark_stream* h, int rem)
+// Slot geometry of a push of n_t >= 1 samples with sub-block length L: slots are aligned to the
+// end of the push; a short first slot (r < L) sits behind one idle slot (high half of lane 0).
+static Geometry geometry_for(long long n_t, int L)
 {
-    if (h->cached_tail_rem == rem) return;
-    const int len = (rem + 31) / 32;
-    const int nfull = rem / len, part = rem % len;
-    h->tail_len = len; h->tail_nfull = nfull; h->tail_part = part;
-    h->tail_jl = part > 0 ? nfull : nfull - 1;
-    h->tail_magic = (65536 + len - 1) / len;
-    const int end_len = part > 0 ? part : len;
-    std::memset(&h->tail, 0, sizeof(TailTab));
-    for (int k = 0; k < h->n_sec; ++k) {
-        Mat2 P[kSteps];
-        scan_powers(h->sec[k], len, P);
-        for (int d = 0; d < kSteps; ++d) put_mat(&h->tail.P[k][d][0], P[d]);
-        put_mat(&h->tail.Aend[k][0], mpow(h->sec[k].A, end_len));
+    Geometry g{};
+    g.L = L;
+    const long long U = (n_t + L - 1) / L;                 // slots holding samples
+    g.r = (int)(n_t - (U - 1) * L);
+    g.lead = g.r < L ? 1 : 0;
+    g.pad0 = g.lead * L + (L - g.r);
+    const long long slots = U + g.lead;
+    g.n_tiles = (int)((slots + 63) / 64);
+    const int s_last = (int)((slots - 1) % 64);
+    g.last_lane = s_last >> 1; g.last_half = s_last & 1;
+    return g;
+}
+
+// Cheapest variant: a tile costs its L samples per lane-half plus a fixed part (scans, staging).
+static int choose_variant(long long n_t)
+{
+    int best = 0; double best_cost = 1e300;
+    for (int v = 0; v < kNumVariants; ++v) {
+        const Geometry g = geometry_for(n_t, kVariantL[v]);
+        const double cost = (double)g.n_tiles * (kVariantL[v] + 10.0);
+        if (cost < best_cost) { best_cost = cost; best = v; }
     }
-    const double cs = 1.0 / h->sta_len, cl = 1.0 / h->lta_len;
-    for (int d = 0; d < kSteps; ++d) {
-        h->tail.beta_s[d] = (float)one_minus_pow(cs, (double)len * (1 << d));
-        h->tail.beta_l[d] = (float)one_minus_pow(cl, (double)len * (1 << d));
+    return best;
+}
+
+template <int L>
+static cudaError_t launch_cm(const PushParams& p, int n_sec, cudaStream_t stream)
+{
+    const int ns = 2 * n_sec + 2, st_floats = (ns + 3) & ~3;
+    const size_t smem = sizeof(float) * (variant_floats<L>(n_sec) + (size_t)kWarps * (Geo<L>::buf_floats + st_floats));
+    static bool attr_done = false;           // per variant (template instance); idempotent
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(filark_push_cm_kernel<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
     }
-    h->tail.beta_end_s = (float)one_minus_pow(cs, end_len);
-    h->tail.beta_end_l = (float)one_minus_pow(cl, end_len);
-    h->cached_tail_rem = rem;
+    const int grid = (p.n_ch + kWarps - 1) / kWarps;
+    filark_push_cm_kernel<L><<<grid, kWarps * 32, smem, stream>>>(p);
+    return cudaGetLastError();
 }
 
 extern "C" {
@@ -151,7 +226,12 @@ static filark_status_t check_create_args(const void* out, int n_ch, const double
     if (!out || !sos || n_ch <= 0 || n_sec <= 0 || n_sec > FILARK_MAX_SECTIONS) return FILARK_ERR_INVALID_ARG;
     if (sta_len < 1 || lta_len < sta_len) return FILARK_ERR_INVALID_ARG;
     if (layout != FILARK_LAYOUT_CHANNEL_MAJOR && layout != FILARK_LAYOUT_TIME_MAJOR) return FILARK_ERR_INVALID_ARG;
-    if (flags & ~FILARK_FLAG_SERIAL_SCAN) return FILARK_ERR_INVALID_ARG;
+    if (flags & ~(FILARK_FLAG_SERIAL_SCAN | 0xFF00u)) return FILARK_ERR_INVALID_ARG;
+    if (flags & 0xFF00u) {
+        bool ok = false;
+        for (int v = 0; v < kNumVariants; ++v) ok = ok || kVariantL[v] == (int)((flags >> 8) & 0xFF);
+        if (!ok) return FILARK_ERR_INVALID_ARG;
+    }
     return FILARK_OK;
 }
 
@@ -166,26 +246,28 @@ filark_status_t filark_stream_create_ex(filark_stream_t** out, int n_ch, const d
     st = design_all(sos, n_sec, h->sec, &h->gain);
     if (st != FILARK_OK) { delete h; return st; }
     h->n_ch = n_ch; h->n_sec = n_sec; h->sta_len = sta_len; h->lta_len = lta_len;
-    h->layout = layout; h->flags = flags; h->cached_tail_rem = -1;
-    h->tab_floats = (size_t)n_sec * kSecStride + kAvgFloats;
+    h->layout = layout; h->flags = flags;
     h->state_floats = (size_t)n_ch * (size_t)(2 * n_sec + 2);
     cudaError_t e = cudaGetDevice(&h->device);
-    float* tab = nullptr;
-    if (e == cudaSuccess) {
-        tab = (float*)std::malloc(sizeof(float) * h->tab_floats);
-        if (!tab) { delete h; return FILARK_ERR_ALLOC; }
-        build_static_table(h, tab);
-    }
-    if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_tab, sizeof(float) * h->tab_floats);
     if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_state, sizeof(float) * h->state_floats);
     if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_ctr, sizeof(Counter));
-    if (e == cudaSuccess) e = cudaMemcpy(h->d_tab, tab, sizeof(float) * h->tab_floats, cudaMemcpyHostToDevice);
     if (e == cudaSuccess) e = cudaMemset(h->d_state, 0, sizeof(float) * h->state_floats);
     if (e == cudaSuccess) e = cudaMemset(h->d_ctr, 0, sizeof(Counter));
-    std::free(tab);
-    if (e != cudaSuccess) {
-        const bool oom = e == cudaErrorMemoryAllocation;
-        cudaFree(h->d_tab); cudaFree(h->d_state); cudaFree(h->d_ctr);
+    bool host_oom = false;
+    for (int v = 0; v < kNumVariants && e == cudaSuccess && !host_oom; ++v) {
+        h->tab_floats[v] = variant_floats_rt(v, n_sec);
+        float* tab = (float*)std::malloc(sizeof(float) * h->tab_floats[v]);
+        if (!tab) { host_oom = true; break; }
+        build_variant_rt(v, h, tab);
+        e = cudaMalloc((void**)&h->d_tab[v], sizeof(float) * h->tab_floats[v]);
+        if (e == cudaSuccess)
+            e = cudaMemcpy(h->d_tab[v], tab, sizeof(float) * h->tab_floats[v], cudaMemcpyHostToDevice);
+        std::free(tab);
+    }
+    if (e != cudaSuccess || host_oom) {
+        const bool oom = host_oom || e == cudaErrorMemoryAllocation;
+        for (int v = 0; v < kNumVariants; ++v) cudaFree(h->d_tab[v]);
+        cudaFree(h->d_state); cudaFree(h->d_ctr);
         delete h;
         cudaGetLastError();
         return oom ? FILARK_ERR_ALLOC : FILARK_ERR_CUDA;
@@ -205,7 +287,8 @@ filark_status_t filark_stream_destroy(filark_stream_t* h)
 {
     if (!h) return FILARK_OK;
     cudaDeviceSynchronize();
-    cudaFree(h->d_tab); cudaFree(h->d_state); cudaFree(h->d_ctr);
+    for (int v = 0; v < kNumVariants; ++v) cudaFree(h->d_tab[v]);
+    cudaFree(h->d_state); cudaFree(h->d_ctr);
     for (int i = 0; i < 3; ++i) cudaFree(h->d_stage[i]);
     delete h;
     return FILARK_OK;
@@ -256,14 +339,13 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
 
     PushParams p{};
     p.in = d_in; p.filt = d_filt; p.cf = d_cf;
-    p.tab = h->d_tab; p.state = h->d_state; p.ctr = h->d_ctr;
+    p.state = h->d_state; p.ctr = h->d_ctr;
     p.n_t = n_t; p.in_pitch = in_pitch; p.out_pitch = out_pitch;
     p.n_ch = h->n_ch; p.n_sec = h->n_sec;
     p.lta_len = h->lta_len;
     p.gain = (float)h->gain;
     p.ratio = (float)((double)h->lta_len / (double)h->sta_len);
     p.lta_thr = (float)(1e-30 * (double)h->lta_len);      // lta <= 1e-30  <=>  lta~ <= 1e-30 N_l
-    const size_t tab_bytes = sizeof(float) * ((h->tab_floats + 3) & ~(size_t)3);
     const int ns = 2 * h->n_sec + 2;
 
     if ((h->flags & FILARK_FLAG_SERIAL_SCAN) || !cm) {
@@ -273,24 +355,27 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
         const long long sc_out = cm ? out_pitch : 1, st_out = cm ? 1 : out_pitch;
         const long long state_sc = cm ? ns : 1, state_sk = cm ? 1 : h->n_ch;
         const int block = 128, grid = (h->n_ch + block - 1) / block;
-        filark_push_serial_kernel<<<grid, block, tab_bytes, stream>>>(p, sc_in, st_in, sc_out, st_out,
-                                                                      state_sc, state_sk);
+        p.tab = h->d_tab[0];
+        filark_push_serial_kernel<<<grid, block, 0, stream>>>(p, sec_stride_rt(0), sc_in, st_in, sc_out,
+                                                              st_out, state_sc, state_sk);
+        e = cudaGetLastError();
     } else {
-        p.n_full = (int)(n_t / kTile);
-        const int rem = (int)(n_t % kTile);
-        if (rem > 0) {
-            build_tail(h, rem);
-            p.tail_len = h->tail_len; p.tail_nfull = h->tail_nfull; p.tail_part = h->tail_part;
-            p.tail_jl = h->tail_jl; p.tail_magic = h->tail_magic;
-        }
+        int v = choose_variant(n_t);
+        for (int i = 0; i < kNumVariants; ++i) if (kVariantL[i] == (int)((h->flags >> 8) & 0xFF)) v = i;
+        const Geometry g = geometry_for(n_t, kVariantL[v]);
+        p.tab = h->d_tab[v];
+        p.n_tiles = g.n_tiles; p.lead = g.lead; p.r = g.r; p.pad0 = g.pad0;
+        p.last_lane = g.last_lane; p.last_half = g.last_half;
         const uintptr_t all = (uintptr_t)d_in | (uintptr_t)d_filt | (uintptr_t)d_cf;
-        p.vec4 = ((all & 15u) == 0 && (in_pitch & 3) == 0 && (out_pitch & 3) == 0) ? 1 : 0;
-        const int st_floats = (ns + 3) & ~3;
-        const size_t smem = tab_bytes + sizeof(float) * (size_t)kWarps * (32 * kPitch + st_floats);
-        const int grid = (h->n_ch + kWarps - 1) / kWarps;
-        filark_push_cm_kernel<<<grid, kWarps * 32, smem, stream>>>(p, h->tail);
+        p.vec4 = ((all & 15u) == 0 && (in_pitch & 3) == 0 && (out_pitch & 3) == 0 && (n_t & 3) == 0) ? 1 : 0;
+        switch (g.L) {
+            case 8: e = launch_cm<8>(p, h->n_sec, stream); break;
+            case 16: e = launch_cm<16>(p, h->n_sec, stream); break;
+            case 24: e = launch_cm<24>(p, h->n_sec, stream); break;
+            case 32: e = launch_cm<32>(p, h->n_sec, stream); break;
+            default: e = launch_cm<48>(p, h->n_sec, stream); break;
+        }
     }
-    e = cudaGetLastError();
     if (e != cudaSuccess) return cuda_fail(h, e);
     h->launches += 1;
     h->samples += n_t;
@@ -360,17 +445,16 @@ int filark_debug_design(const double* sos, int n_sec, int* kinds, double* coefs,
     return (int)FILARK_OK;
 }
 
-int filark_debug_tail_geometry(long long n_t, int* n_full, int* len, int* nfull, int* part, int* jl)
+int filark_debug_push_geometry(long long n_t, int force_L, int* out7)
 {
-    if (n_t < 0) return (int)FILARK_ERR_INVALID_ARG;
-    const int rem = (int)(n_t % kTile);
-    if (n_full) *n_full = (int)(n_t / kTile);
-    int l = 0, nf = 0, pt = 0, j = -1;
-    if (rem > 0) { l = (rem + 31) / 32; nf = rem / l; pt = rem % l; j = pt > 0 ? nf : nf - 1; }
-    if (len) *len = l;
-    if (nfull) *nfull = nf;
-    if (part) *part = pt;
-    if (jl) *jl = j;
+    if (n_t < 1 || !out7) return (int)FILARK_ERR_INVALID_ARG;
+    int L = 0;
+    if (force_L == 0) L = kVariantL[choose_variant(n_t)];
+    else for (int v = 0; v < kNumVariants; ++v) if (kVariantL[v] == force_L) L = force_L;
+    if (L == 0) return (int)FILARK_ERR_INVALID_ARG;
+    const Geometry g = geometry_for(n_t, L);
+    out7[0] = g.L; out7[1] = g.n_tiles; out7[2] = g.lead; out7[3] = g.r; out7[4] = g.pad0;
+    out7[5] = g.last_lane; out7[6] = g.last_half;
     return (int)FILARK_OK;
 }
 

@@ -71,8 +71,8 @@ def load_library():
     lib.filark_stream_samples_pushed.argtypes = [vp]
     lib.filark_debug_design.restype = ci
     lib.filark_debug_design.argtypes = [vp, ci, vp, vp, vp]
-    lib.filark_debug_tail_geometry.restype = ci
-    lib.filark_debug_tail_geometry.argtypes = [ll, vp, vp, vp, vp, vp]
+    lib.filark_debug_push_geometry.restype = ci
+    lib.filark_debug_push_geometry.argtypes = [ll, ci, vp]
     lib.filark_debug_block_power.restype = ci
     lib.filark_debug_block_power.argtypes = [vp, ll, vp]
     _lib = lib
@@ -199,13 +199,14 @@ def debug_design(sos):
     return kinds, coefs, float(gain.value)
 
 
-def debug_tail_geometry(n_t: int):
+def debug_push_geometry(n_t: int, force_L: int = 0):
+    """dict(L, n_tiles, lead, r, pad0, last_lane, last_half) of a channel-major push of n_t samples."""
     lib = load_library()
-    v = [ctypes.c_int(0) for _ in range(5)]
-    st = lib.filark_debug_tail_geometry(int(n_t), *[ctypes.addressof(x) for x in v])
+    out = np.zeros(7, dtype=np.int32)
+    st = lib.filark_debug_push_geometry(int(n_t), int(force_L), out.ctypes.data)
     if st != 0:
-        raise FilarkError(st, "filark_debug_tail_geometry")
-    return tuple(int(x.value) for x in v)
+        raise FilarkError(st, "filark_debug_push_geometry")
+    return dict(zip(("L", "n_tiles", "lead", "r", "pad0", "last_lane", "last_half"), map(int, out)))
 
 
 def debug_block_power(sos6, e: int):

@@ -92,6 +92,18 @@ def test_chunking_fuzz(cuda_device, sizes):
     s.destroy()
 
 
+@pytest.mark.parametrize("L", [8, 16, 24, 32, 48])
+@pytest.mark.parametrize("n_t", [13_007, 6_144, 1_500, 777])
+def test_every_kernel_variant(cuda_device, L, n_t):
+    """Each compiled sub-block length on ragged and exact pushes (flags force the variant)."""
+    w = CONFIGS["cfg5"].scaled(n_ch=7, n_t=n_t)
+    x_dev, ref_f, ref_c = _case(w, cuda_device, CHANNEL_MAJOR)
+    s = _stream(w, CHANNEL_MAJOR, flags=L << 8)
+    f, c = run_gpu(s, x_dev, CHANNEL_MAJOR, split(w.n_t, [2048, 1500, 64 * L, 64 * L - 1, 64 * L + 1, 5, 1, 3001]))
+    _check(f, c, ref_f, ref_c, CHANNEL_MAJOR, f"L={L} n_t={n_t}")
+    s.destroy()
+
+
 def test_serial_diagnostic_kernel(cuda_device):
     w = CONFIGS["cfg2"].scaled(n_ch=40, n_t=20_000)
     x_dev, ref_f, ref_c = _case(w, cuda_device, CHANNEL_MAJOR)
@@ -171,7 +183,7 @@ def test_error_codes(cuda_device):
     from paper_2605_20132_b200.stream import FilarkError, FilarkStream
     w = CONFIGS["cfg1"].scaled(n_ch=4, n_t=64)
     sos = design_sos(w)
-    for bad in [dict(n_ch=0), dict(sta_len=0), dict(lta_len=10, sta_len=20), dict(layout=7), dict(flags=8)]:
+    for bad in [dict(n_ch=0), dict(sta_len=0), dict(lta_len=10, sta_len=20), dict(layout=7), dict(flags=8), dict(flags=7 << 8)]:
         kw = dict(n_ch=4, sos=sos, sta_len=5, lta_len=50, layout=0, flags=0); kw.update(bad)
         with pytest.raises(FilarkError) as e:
             FilarkStream(**kw)

@@ -67,18 +67,22 @@ def test_state_space_rewrite_equals_sosfilt(lib, name):
     ref = signal.sosfilt(sos, x)
     got = _simulate(kinds, coefs, gain, x)
     assert np.max(np.abs(got - ref)) < 1e-9 * np.max(np.abs(ref))
-    # poles next to z = 1 must be in the normal form, the rest in DF2T
+    # poles next to z = 1 must be in the delta form (all these designs have zeros at z = 1 there),
+    # the rest in direct form II
     for k, s in enumerate(sos):
-        d2 = min(1 + s[4] / s[3] + s[5] / s[3], 1 - s[4] / s[3] + s[5] / s[3])
-        assert kinds[k] == (1 if d2 < 0.05 else 0)
+        assert kinds[k] == (2 if 1 + s[4] / s[3] + s[5] / s[3] < 0.05 else 0)
 
 
 def test_rewrite_handles_odd_sections(lib):
     sos = np.array([[0.0, 1.0, 0.0, 1.0, -1.9, 0.9025 + 1e-4],     # b0 = 0, complex poles near z=1
                     [2.0, 0.5, 0.0, 2.0, -1.0, 0.0],               # first order, a0 != 1
                     [1.0, 0.0, 0.0, 1.0, 0.0, 0.0],                # identity
-                    [0.3, 0.1, 0.2, 1.0, -1.6, 0.64]])             # double real pole 0.8
+                    [0.3, 0.1, 0.2, 1.0, -1.6, 0.64],              # double real pole 0.8 (near z = 1, no zero there)
+                    [1.0, 2.0, 1.0, 1.0, -1.95, 0.9512],           # complex poles near z = 1, zeros at z = -1
+                    [1.0, -1.0, 0.0, 1.0, -0.999, 0.0],            # first-order high-pass, real pole near z = 1
+                    [0.5, 0.3, 0.5, 1.0, 1.9, 0.9125]])            # complex poles near z = -1
     kinds, coefs, gain = lib.debug_design(sos)
+    assert list(kinds) == [1, 0, 0, 3, 3, 2, 4]
     x = np.random.default_rng(4).standard_normal(400)
     ref = signal.sosfilt(sos / sos[:, 3:4], x)       # scipy wants a0 == 1
     got = _simulate(kinds, coefs, gain, x)
@@ -111,17 +115,28 @@ def test_block_powers_match_numpy(lib, e):
         assert np.max(np.abs(got - ref)) < 1e-9 * max(1.0, np.abs(ref).max())
 
 
-def test_tail_geometry_covers_every_sample_once(lib):
-    lens = set(range(0, 70)) | {1000, 1023, 1024, 1025, 1500, 2047, 2048, 6000, 90000, 99991}
+def test_push_geometry_covers_every_sample_once(lib):
+    lens = set(range(1, 70)) | {1000, 1023, 1024, 1025, 1500, 1530, 2047, 2048, 6000, 90000, 99991, 900000}
     lens |= set(push_schedule(CONFIGS["cfg5"])[:50])
     for n_t in sorted(lens):
-        n_full, ln, nfull, part, jl = lib.debug_tail_geometry(n_t)
-        assert n_full * 1024 + nfull * ln + part == n_t
-        if n_t % 1024 == 0:
-            assert ln == 0 and jl == -1
-        else:
-            assert 1 <= ln <= 32 and 0 <= part < ln and nfull + (part > 0) <= 32
-            assert jl == (nfull if part else nfull - 1) and 0 <= jl <= 31
+        for force in (0, 8, 16, 24, 32, 48):
+            g = lib.debug_push_geometry(n_t, force)
+            L = g["L"]
+            assert L in (8, 16, 24, 32, 48) and (force == 0 or L == force)
+            assert 1 <= g["r"] <= L and g["lead"] == (1 if g["r"] < L else 0)
+            assert g["pad0"] == g["lead"] * L + (L - g["r"])
+            # slots are aligned to the end of the push: the last sample ends the slot (last_lane, last_half)
+            end = n_t + g["pad0"]
+            assert end % L == 0
+            s_last = end // L - 1
+            assert g["n_tiles"] == s_last // 64 + 1
+            assert (g["last_lane"], g["last_half"]) == ((s_last % 64) // 2, (s_last % 64) % 2)
+            # a short first slot sits in the high half of lane 0 behind one idle slot
+            if g["r"] < L:
+                assert g["pad0"] // L == 1
+    # the cheapest variant for the configs' chunk lengths puts the whole chunk in one tile
+    assert lib.debug_push_geometry(1500)["L"] == 24 and lib.debug_push_geometry(1500)["n_tiles"] == 1
+    assert lib.debug_push_geometry(1000)["L"] == 16 and lib.debug_push_geometry(1000)["n_tiles"] == 1
 
 
 def test_missing_library_fails_loudly(monkeypatch, tmp_path):
