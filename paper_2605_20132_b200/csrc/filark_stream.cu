@@ -34,8 +34,9 @@ struct filark_stream {
     float* d_tab[kNumVariants];
     size_t tab_floats[kNumVariants];
     float* d_state;
-    Counter* d_ctr;
     size_t state_floats;
+    int n_sm;
+    size_t smem_optin;
     int last_cuda_error;
     long long launches, samples;
     // staging for push_host
@@ -56,14 +57,13 @@ static void put_mat(float* dst, const Mat2& m)
 
 template <int L> static size_t variant_floats(int n_sec)
 {
-    return (size_t)n_sec * SecTab<L>::stride + AvgTab<L>::size;
+    return (size_t)n_sec * SecTab<L>::stride + kAvgFloats;
 }
 
 // Device table of sub-block length L (layout documented in filark_kernels.cuh).
 template <int L> static void build_variant_table(const filark_stream* h, float* tab)
 {
     using ST = SecTab<L>;
-    using AT = AvgTab<L>;
     std::memset(tab, 0, sizeof(float) * variant_floats<L>(h->n_sec));
     for (int k = 0; k < h->n_sec; ++k) {
         const Section& s = h->sec[k];
@@ -79,8 +79,6 @@ template <int L> static void build_variant_table(const filark_stream* h, float* 
             q = mul(q, q);
         }
         std::memcpy(&T[kOffNSteps], &nsteps, sizeof(int));
-        Mat2 ap = ident();
-        for (int r = 0; r <= L; ++r) { put_mat(T + ST::apow + 4 * r, ap); ap = mul(ap, s.A); }
         double g[2 * L];
         fixup_rows(s, L, g);
         for (int i = 0; i < L; ++i) {
@@ -92,22 +90,25 @@ template <int L> static void build_variant_table(const filark_stream* h, float* 
     float* AV = tab + (size_t)h->n_sec * ST::stride;
     const double cs = 1.0 / h->sta_len, cl = 1.0 / h->lta_len;
     AV[0] = (float)(1.0 - cs); AV[1] = (float)(1.0 - cl);
-    AV[AT::beta_l] = (float)one_minus_pow(cs, L); AV[AT::beta_l + 1] = (float)one_minus_pow(cl, L);
+    AV[kAvgBetaL] = (float)one_minus_pow(cs, L); AV[kAvgBetaL + 1] = (float)one_minus_pow(cl, L);
     for (int d = 0; d < kSteps; ++d) {
         const double e = 2.0 * L * (double)(1 << d);
-        AV[AT::beta_q + 2 * d] = (float)one_minus_pow(cs, e);
-        AV[AT::beta_q + 2 * d + 1] = (float)one_minus_pow(cl, e);
+        AV[kAvgBetaQ + 2 * d] = (float)one_minus_pow(cs, e);
+        AV[kAvgBetaQ + 2 * d + 1] = (float)one_minus_pow(cl, e);
     }
-    AV[14] = (float)cs; AV[15] = (float)cl;
-    for (int r = 0; r <= L; ++r) {
-        AV[AT::beta_r + 2 * r] = (float)one_minus_pow(cs, r);
-        AV[AT::beta_r + 2 * r + 1] = (float)one_minus_pow(cl, r);
-    }
-    for (int sh = 0; sh < L; ++sh) {
-        // alpha^-sh; alpha = 0 (length-1 average) keeps no memory, any finite factor will do
-        AV[AT::inv + 2 * sh] = cs >= 1.0 ? (sh == 0 ? 1.0f : 0.0f) : (float)std::exp(-(double)sh * std::log1p(-cs));
-        AV[AT::inv + 2 * sh + 1] = cl >= 1.0 ? (sh == 0 ? 1.0f : 0.0f) : (float)std::exp(-(double)sh * std::log1p(-cl));
-    }
+    AV[kAvgInvN] = (float)cs; AV[kAvgInvN + 1] = (float)cl;
+}
+
+// What a push needs beyond the table: powers for its first (possibly short) slot of r samples.
+static void fill_first_slot_params(const filark_stream* h, int L, int r, PushParams* p)
+{
+    const double cs = 1.0 / h->sta_len, cl = 1.0 / h->lta_len;
+    const int sh = L - r;
+    p->beta_r[0] = (float)one_minus_pow(cs, r); p->beta_r[1] = (float)one_minus_pow(cl, r);
+    // alpha^-sh; alpha = 0 (length-1 average) keeps no memory, any finite factor will do
+    p->inv_sh[0] = cs >= 1.0 ? (sh == 0 ? 1.0f : 0.0f) : (float)std::exp(-(double)sh * std::log1p(-cs));
+    p->inv_sh[1] = cl >= 1.0 ? (sh == 0 ? 1.0f : 0.0f) : (float)std::exp(-(double)sh * std::log1p(-cl));
+    for (int k = 0; k < h->n_sec; ++k) put_mat(&p->apow_r[k][0], mpow(h->sec[k].A, r));
 }
 
 static size_t variant_floats_rt(int v, int n_sec)
@@ -170,19 +171,30 @@ static int choose_variant(long long n_t)
     return best;
 }
 
+// One CTA per SM; W warps per CTA as far as registers and shared memory allow; fewer, on more
+// SMs, when there are few channels.
 template <int L>
-static cudaError_t launch_cm(const PushParams& p, int n_sec, cudaStream_t stream)
+static cudaError_t launch_cm(const filark_stream* h, const PushParams& p, cudaStream_t stream)
 {
-    const int ns = 2 * n_sec + 2, st_floats = (ns + 3) & ~3;
-    const size_t smem = sizeof(float) * (variant_floats<L>(n_sec) + (size_t)kWarps * (Geo<L>::buf_floats + st_floats));
+    const size_t tab_bytes = sizeof(float) * variant_floats<L>(p.n_sec);
+    const size_t warp_bytes = sizeof(float) * (size_t)warp_smem_floats<L>();
+    int W = cm_max_warps<L>();
+    const int fit = (int)((h->smem_optin - tab_bytes) / warp_bytes);
+    if (fit < W) W = fit;
+    const int want = (p.n_ch + h->n_sm - 1) / h->n_sm;
+    if (want < W) W = want;
+    if (W < 1) return cudaErrorInvalidConfiguration;
+    const size_t smem = tab_bytes + (size_t)W * warp_bytes;
     static bool attr_done = false;           // per variant (template instance); idempotent
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(filark_push_cm_kernel<L>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024);
+        cudaError_t e = cudaFuncSetAttribute(filark_push_cm_kernel<L>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)h->smem_optin);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    const int grid = (p.n_ch + kWarps - 1) / kWarps;
-    filark_push_cm_kernel<L><<<grid, kWarps * 32, smem, stream>>>(p);
+    int grid = (p.n_ch + W - 1) / W;
+    if (grid > h->n_sm) grid = h->n_sm;
+    filark_push_cm_kernel<L><<<grid, W * 32, smem, stream>>>(p);
     return cudaGetLastError();
 }
 
@@ -247,12 +259,14 @@ filark_status_t filark_stream_create_ex(filark_stream_t** out, int n_ch, const d
     if (st != FILARK_OK) { delete h; return st; }
     h->n_ch = n_ch; h->n_sec = n_sec; h->sta_len = sta_len; h->lta_len = lta_len;
     h->layout = layout; h->flags = flags;
-    h->state_floats = (size_t)n_ch * (size_t)(2 * n_sec + 2);
+    h->state_floats = (size_t)n_ch * (size_t)state_floats(n_sec);
     cudaError_t e = cudaGetDevice(&h->device);
+    int optin = 0;
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, h->device);
+    h->smem_optin = (size_t)optin;
     if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_state, sizeof(float) * h->state_floats);
-    if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_ctr, sizeof(Counter));
     if (e == cudaSuccess) e = cudaMemset(h->d_state, 0, sizeof(float) * h->state_floats);
-    if (e == cudaSuccess) e = cudaMemset(h->d_ctr, 0, sizeof(Counter));
     bool host_oom = false;
     for (int v = 0; v < kNumVariants && e == cudaSuccess && !host_oom; ++v) {
         h->tab_floats[v] = variant_floats_rt(v, n_sec);
@@ -267,7 +281,7 @@ filark_status_t filark_stream_create_ex(filark_stream_t** out, int n_ch, const d
     if (e != cudaSuccess || host_oom) {
         const bool oom = host_oom || e == cudaErrorMemoryAllocation;
         for (int v = 0; v < kNumVariants; ++v) cudaFree(h->d_tab[v]);
-        cudaFree(h->d_state); cudaFree(h->d_ctr);
+        cudaFree(h->d_state);
         delete h;
         cudaGetLastError();
         return oom ? FILARK_ERR_ALLOC : FILARK_ERR_CUDA;
@@ -288,7 +302,7 @@ filark_status_t filark_stream_destroy(filark_stream_t* h)
     if (!h) return FILARK_OK;
     cudaDeviceSynchronize();
     for (int v = 0; v < kNumVariants; ++v) cudaFree(h->d_tab[v]);
-    cudaFree(h->d_state); cudaFree(h->d_ctr);
+    cudaFree(h->d_state);
     for (int i = 0; i < 3; ++i) cudaFree(h->d_stage[i]);
     delete h;
     return FILARK_OK;
@@ -302,7 +316,6 @@ filark_status_t filark_stream_reset(filark_stream_t* h, cudaStream_t stream)
     if (e != cudaSuccess) return cuda_fail(h, e);
     if (dev != h->device) return FILARK_ERR_DEVICE_MISMATCH;
     e = cudaMemsetAsync(h->d_state, 0, sizeof(float) * h->state_floats, stream);
-    if (e == cudaSuccess) e = cudaMemsetAsync(h->d_ctr, 0, sizeof(Counter), stream);
     if (e != cudaSuccess) return cuda_fail(h, e);
     h->samples = 0;
     return FILARK_OK;
@@ -339,14 +352,14 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
 
     PushParams p{};
     p.in = d_in; p.filt = d_filt; p.cf = d_cf;
-    p.state = h->d_state; p.ctr = h->d_ctr;
+    p.state = h->d_state;
     p.n_t = n_t; p.in_pitch = in_pitch; p.out_pitch = out_pitch;
     p.n_ch = h->n_ch; p.n_sec = h->n_sec;
     p.lta_len = h->lta_len;
     p.gain = (float)h->gain;
     p.ratio = (float)((double)h->lta_len / (double)h->sta_len);
     p.lta_thr = (float)(1e-30 * (double)h->lta_len);      // lta <= 1e-30  <=>  lta~ <= 1e-30 N_l
-    const int ns = 2 * h->n_sec + 2;
+    const int ns = state_floats(h->n_sec);
 
     if ((h->flags & FILARK_FLAG_SERIAL_SCAN) || !cm) {
         // Serial diagnostic kernel; also the time-major path until the blocked time-major
@@ -366,14 +379,15 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
         p.tab = h->d_tab[v];
         p.n_tiles = g.n_tiles; p.lead = g.lead; p.r = g.r; p.pad0 = g.pad0;
         p.last_lane = g.last_lane; p.last_half = g.last_half;
+        fill_first_slot_params(h, g.L, g.r, &p);
         const uintptr_t all = (uintptr_t)d_in | (uintptr_t)d_filt | (uintptr_t)d_cf;
         p.vec4 = ((all & 15u) == 0 && (in_pitch & 3) == 0 && (out_pitch & 3) == 0 && (n_t & 3) == 0) ? 1 : 0;
         switch (g.L) {
-            case 8: e = launch_cm<8>(p, h->n_sec, stream); break;
-            case 16: e = launch_cm<16>(p, h->n_sec, stream); break;
-            case 24: e = launch_cm<24>(p, h->n_sec, stream); break;
-            case 32: e = launch_cm<32>(p, h->n_sec, stream); break;
-            default: e = launch_cm<48>(p, h->n_sec, stream); break;
+            case 8: e = launch_cm<8>(h, p, stream); break;
+            case 16: e = launch_cm<16>(h, p, stream); break;
+            case 24: e = launch_cm<24>(h, p, stream); break;
+            case 32: e = launch_cm<32>(h, p, stream); break;
+            default: e = launch_cm<48>(h, p, stream); break;
         }
     }
     if (e != cudaSuccess) return cuda_fail(h, e);
