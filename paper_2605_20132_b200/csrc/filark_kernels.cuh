@@ -110,6 +110,10 @@ template <int L> struct Geo {
     static constexpr int chunks = L / 2;           // 16-byte chunks per lane region
 };
 
+// All dynamic shared memory, addressed by float offsets so that every access is provably a
+// shared-memory access (32-bit addresses, LDS/STS instead of generic LD/ST).
+extern __shared__ __align__(16) float fk_smem[];
+
 // Shared memory of one warp: two tile buffers (input of tile k / staging of its outputs, and the
 // prefetched input of tile k+1) and two copies of the channel state.
 constexpr int kStateSmem = 40;                     // >= state_floats(kMaxSec), multiple of 4
@@ -120,70 +124,73 @@ template <int L> __host__ __device__ constexpr int warp_smem_floats() { return 2
 // `wst`.  t0 = time index (within the push) of the tile's position 0; samples outside [0, n_t)
 // are zero-filled.
 template <int L>
-__device__ __forceinline__ void issue_tile_load(const PushParams& p, int ch, int tile, float* buf, float* wst,
+__device__ __forceinline__ void issue_tile_load(const PushParams& p, int ch, int tile, int buf, int wst,
                                                 int lane, bool with_state)
 {
+    const int t0 = tile * Geo<L>::tile - p.pad0;
+    const int n_t = (int)p.n_t;
     const float* __restrict__ src = p.in + (long long)ch * p.in_pitch;
-    const long long t0 = (long long)tile * Geo<L>::tile - p.pad0;
     if (p.vec4) {
         // valid 16-byte chunks of this tile: [c_lo, c_hi)
-        const long long hi = p.n_t - t0;
-        const int c_lo = t0 < 0 ? (int)(-t0 >> 2) : 0;
-        const int c_hi = hi >= Geo<L>::tile ? Geo<L>::tile / 4 : (int)(hi >> 2);
+        const int c_lo = t0 < 0 ? (-t0 >> 2) : 0;
+        const int c_hi = min(Geo<L>::tile, n_t - t0) >> 2;
+        const unsigned span = (unsigned)(c_hi - c_lo);
+        const float* __restrict__ srct = src + t0;
 #pragma unroll
         for (int m = 0; m < Geo<L>::chunks; ++m) {
             const int c = 32 * m + lane;
-            const bool ok = c >= c_lo && c < c_hi;
-            cp_async16(buf + 4 * c + 4 * (c / Geo<L>::chunks), ok ? src + (t0 + 4 * c) : src, ok ? 16 : 0);
+            const bool ok = (unsigned)(c - c_lo) < span;
+            cp_async16(&fk_smem[buf + 4 * c + 4 * (c / Geo<L>::chunks)], ok ? srct + 4 * c : src, ok ? 16 : 0);
         }
     } else {
 #pragma unroll 8
         for (int m = 0; m < 2 * L; ++m) {
             const int e = 32 * m + lane;
-            const long long t = t0 + e;
-            const bool ok = t >= 0 && t < p.n_t;
-            cp_async4(buf + e + 4 * (e / (2 * L)), ok ? src + t : src, ok ? 4 : 0);
+            const int t = t0 + e;
+            const bool ok = (unsigned)t < (unsigned)n_t;
+            cp_async4(&fk_smem[buf + e + 4 * (e / (2 * L))], ok ? src + t : src, ok ? 4 : 0);
         }
     }
     if (with_state) {
         const int ns = state_floats(p.n_sec);
         const float* gst = p.state + (long long)ch * ns;
-        if (lane < ns) cp_async4(wst + lane, gst + lane, 4);
-        if (lane + 32 < ns) cp_async4(wst + lane + 32, gst + lane + 32, 4);
+        if (lane < ns) cp_async4(&fk_smem[wst + lane], gst + lane, 4);
+        if (lane + 32 < ns) cp_async4(&fk_smem[wst + lane + 32], gst + lane + 32, 4);
     }
     cp_async_commit();
 }
 
 // S7: the lane regions of `buf` -> one output array (coalesced 16-byte stores).
 template <int L>
-__device__ __forceinline__ void store_tile(const PushParams& p, float* __restrict__ dst, const float* buf,
-                                           int lane, long long t0)
+__device__ __forceinline__ void store_tile(const PushParams& p, float* __restrict__ dst, int buf, int lane, int t0)
 {
+    const int n_t = (int)p.n_t;
     if (p.vec4) {
-        const long long hi = p.n_t - t0;
-        const int c_lo = t0 < 0 ? (int)(-t0 >> 2) : 0;
-        const int c_hi = hi >= Geo<L>::tile ? Geo<L>::tile / 4 : (int)(hi >> 2);
+        const int c_lo = t0 < 0 ? (-t0 >> 2) : 0;
+        const int c_hi = min(Geo<L>::tile, n_t - t0) >> 2;
+        const unsigned span = (unsigned)(c_hi - c_lo);
+        float* __restrict__ dstt = dst + t0;
 #pragma unroll
         for (int m = 0; m < Geo<L>::chunks; ++m) {
             const int c = 32 * m + lane;
-            const float4 v = *reinterpret_cast<const float4*>(buf + 4 * c + 4 * (c / Geo<L>::chunks));
-            if (c >= c_lo && c < c_hi) st_stream4(dst + (t0 + 4 * c), v);
+            const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + 4 * c + 4 * (c / Geo<L>::chunks)]);
+            if ((unsigned)(c - c_lo) < span) st_stream4(dstt + 4 * c, v);
         }
     } else {
 #pragma unroll 8
         for (int m = 0; m < 2 * L; ++m) {
             const int e = 32 * m + lane;
-            const long long t = t0 + e;
-            const float v = buf[e + 4 * (e / (2 * L))];
-            if (t >= 0 && t < p.n_t) st_stream(dst + t, v);
+            const int t = t0 + e;
+            const float v = fk_smem[buf + e + 4 * (e / (2 * L))];
+            if ((unsigned)t < (unsigned)n_t) st_stream(dst + t, v);
         }
     }
 }
 
 template <int L>
-__device__ __forceinline__ void regs_to_buf(const float (&lo)[L], const float (&hi)[L], float* buf, int lane)
+__device__ __forceinline__ void regs_to_buf(const float (&lo)[L], const float (&hi)[L], int buf, int lane)
 {
-    float4* d = reinterpret_cast<float4*>(buf + lane * Geo<L>::pitch);
+    float4* d = reinterpret_cast<float4*>(&fk_smem[buf + lane * Geo<L>::pitch]);
 #pragma unroll
     for (int q = 0; q < L / 4; ++q) {
         d[q] = make_float4(lo[4 * q], lo[4 * q + 1], lo[4 * q + 2], lo[4 * q + 3]);
@@ -193,9 +200,10 @@ __device__ __forceinline__ void regs_to_buf(const float (&lo)[L], const float (&
 
 // S1: zero-state response of one section on the lane's two slots; returns their end states.
 template <int L, int KIND>
-__device__ __forceinline__ void local_pass(float (&lo)[L], float (&hi)[L], const float* __restrict__ T,
+__device__ __forceinline__ void local_pass(float (&lo)[L], float (&hi)[L], int Toff,
                                            float& a1, float& a2, float& b1, float& b2)
 {
+    const float* T = &fk_smem[Toff];
     const float c0 = T[kOffCoef], c1 = T[kOffCoef + 1], c2 = T[kOffCoef + 2], c3 = T[kOffCoef + 3];
     a1 = a2 = b1 = b2 = 0.0f;                       // (a1, a2): state of the lo slot, (b1, b2): hi slot
     if (KIND == kKindDF2) {
@@ -250,82 +258,73 @@ __device__ __forceinline__ void local_pass(float (&lo)[L], float (&hi)[L], const
     }
 }
 
-// Geometry of one tile, uniform over the warp.
-struct TileGeo {
-    bool inj_hi;      // the carried state enters the hi slot of lane 0 (tile 0 of a ragged push)
-    bool out_hi;      // the slot holding the last sample of the tile's data is a hi slot
-    int r, sh, jl;    // samples in the injected slot, L - r, lane of the last slot
-    float m_lo, m_hi; // 1.0 in the lane/slot that receives the carried state
-};
-
 // One tile of one channel, samples already in lo/hi: S1..S7.  `buf` stages the outputs.
+// stab / buf / wst are float offsets into fk_smem.
 template <int L>
-__device__ __forceinline__ void process_tile(const PushParams& p, const float* __restrict__ stab, float* buf,
-                                             float* wst, float (&lo)[L], float (&hi)[L], int ch, int tile,
-                                             int lane, unsigned seen)
+__device__ __forceinline__ void process_tile(const PushParams& p, int stab, int buf, int wst, float (&lo)[L],
+                                             float (&hi)[L], int ch, int tile, int lane, unsigned seen)
 {
     using ST = SecTab<L>;
     const bool first = tile == 0, last = tile == p.n_tiles - 1;
-    const long long t0 = (long long)tile * Geo<L>::tile - p.pad0;
-    TileGeo g;
-    g.inj_hi = first && p.lead != 0;
-    g.r = first ? p.r : L;
-    g.sh = L - g.r;
-    g.jl = last ? p.last_lane : 31;
-    g.out_hi = last ? p.last_half != 0 : true;
-    g.m_lo = (lane == 0 && !g.inj_hi) ? 1.0f : 0.0f;
-    g.m_hi = (lane == 0 && g.inj_hi) ? 1.0f : 0.0f;
+    const int t0 = tile * Geo<L>::tile - p.pad0;
+    const bool inj_hi = first && p.lead != 0;   // carried state enters the hi slot of lane 0 (ragged tile 0)
+    const int r = first ? p.r : L;              // samples in the slot that receives the carried state
+    const int sh = L - r;
+    const int jl = last ? p.last_lane : 31;     // lane of the slot holding the tile's last sample
+    const bool out_hi = last ? p.last_half != 0 : true;
+    const float m_lo = (lane == 0 && !inj_hi) ? 1.0f : 0.0f;
+    const float m_hi = (lane == 0 && inj_hi) ? 1.0f : 0.0f;
     // per-lane fix-up table offset (floats) inside a section's table: lane 0's injected slot is
     // short by sh samples, so its rows are shifted down by sh
     int goff = ST::g0 + 2 * L;
-    if (lane == 0 && g.sh != 0) goff = (g.sh & 1) ? ST::g1 + 2 * (L - g.sh + 1) : ST::g0 + 2 * (L - g.sh);
+    if (lane == 0 && sh != 0) goff = (sh & 1) ? ST::g1 + 2 * (L - sh + 1) : ST::g0 + 2 * (L - sh);
 
     // ---- S1..S3 per section -------------------------------------------------------------------
     for (int k = 0; k < p.n_sec; ++k) {
-        const float* __restrict__ T = stab + k * ST::stride;
-        const int kind = __float_as_int(T[kOffKind]);
+        const int To = stab + k * ST::stride;
+        const int kind = __float_as_int(fk_smem[To + kOffKind]);
         float a1, a2, b1, b2;
         switch (kind) {
-            case kKindDF2: local_pass<L, kKindDF2>(lo, hi, T, a1, a2, b1, b2); break;
-            case kKindDelta: local_pass<L, kKindDelta>(lo, hi, T, a1, a2, b1, b2); break;
-            case kKindDeltaG: local_pass<L, kKindDeltaG>(lo, hi, T, a1, a2, b1, b2); break;
-            case kKindNormal: local_pass<L, kKindNormal>(lo, hi, T, a1, a2, b1, b2); break;
-            default: local_pass<L, kKindDF2G>(lo, hi, T, a1, a2, b1, b2); break;
+            case kKindDF2: local_pass<L, kKindDF2>(lo, hi, To, a1, a2, b1, b2); break;
+            case kKindDelta: local_pass<L, kKindDelta>(lo, hi, To, a1, a2, b1, b2); break;
+            case kKindDeltaG: local_pass<L, kKindDeltaG>(lo, hi, To, a1, a2, b1, b2); break;
+            case kKindNormal: local_pass<L, kKindNormal>(lo, hi, To, a1, a2, b1, b2); break;
+            default: local_pass<L, kKindDF2G>(lo, hi, To, a1, a2, b1, b2); break;
         }
         // S2: carried state S into its slot, then an inclusive scan of the lane totals
-        const float S1 = wst[2 * k], S2 = wst[2 * k + 1];
-        const float4 Pm = *reinterpret_cast<const float4*>(T + kOffP);               // A^L
+        const float2 S = *reinterpret_cast<const float2*>(&fk_smem[wst + 2 * k]);
+        const float4 Pm = *reinterpret_cast<const float4*>(&fk_smem[To + kOffP]);     // A^L
         const float4 Ar = *reinterpret_cast<const float4*>(&p.apow_r[k][0]);          // A^r (first slot)
         const float4 Au = first ? Ar : Pm;
-        const float i1 = fmaf(Au.x, S1, Au.y * S2), i2 = fmaf(Au.z, S1, Au.w * S2);
-        a1 = fmaf(g.m_lo, i1, a1); a2 = fmaf(g.m_lo, i2, a2);                        // state after the lo slot
-        b1 = fmaf(g.m_hi, i1, b1); b2 = fmaf(g.m_hi, i2, b2);
+        const float i1 = fmaf(Au.x, S.x, Au.y * S.y), i2 = fmaf(Au.z, S.x, Au.w * S.y);
+        a1 = fmaf(m_lo, i1, a1); a2 = fmaf(m_lo, i2, a2);                             // state after the lo slot
+        b1 = fmaf(m_hi, i1, b1); b2 = fmaf(m_hi, i2, b2);
         float W1 = fmaf(Pm.x, a1, fmaf(Pm.y, a2, b1)), W2 = fmaf(Pm.z, a1, fmaf(Pm.w, a2, b2));
-        const int nsteps = __float_as_int(T[kOffNSteps]);
+        const int nsteps = __float_as_int(fk_smem[To + kOffNSteps]);
 #pragma unroll
         for (int d = 0; d < kSteps; ++d) {
             if (d < nsteps) {
-                const float4 Q = *reinterpret_cast<const float4*>(T + kOffQ + 4 * d);
-                const float U1 = __shfl_up_sync(0xffffffffu, W1, 1 << d), U2 = __shfl_up_sync(0xffffffffu, W2, 1 << d);
-                if (lane >= (1 << d)) {
-                    W1 = fmaf(Q.x, U1, fmaf(Q.y, U2, W1));
-                    W2 = fmaf(Q.z, U1, fmaf(Q.w, U2, W2));
-                }
+                const float4 Q = *reinterpret_cast<const float4*>(&fk_smem[To + kOffQ + 4 * d]);
+                float U1 = __shfl_up_sync(0xffffffffu, W1, 1 << d), U2 = __shfl_up_sync(0xffffffffu, W2, 1 << d);
+                const bool act = lane >= (1 << d);
+                U1 = act ? U1 : 0.0f; U2 = act ? U2 : 0.0f;
+                W1 = fmaf(Q.x, U1, fmaf(Q.y, U2, W1));
+                W2 = fmaf(Q.z, U1, fmaf(Q.w, U2, W2));
             }
         }
         float E1 = __shfl_up_sync(0xffffffffu, W1, 1), E2 = __shfl_up_sync(0xffffffffu, W2, 1);
-        if (lane == 0) { E1 = 0.0f; E2 = 0.0f; }    // state entering the lane's lo slot
+        E1 = lane == 0 ? 0.0f : E1; E2 = lane == 0 ? 0.0f : E2;    // state entering the lane's lo slot
         // carry-in of the hi slot: P E + (state after lo from rest)
         float o1 = fmaf(Pm.x, E1, fmaf(Pm.y, E2, a1)), o2 = fmaf(Pm.z, E1, fmaf(Pm.w, E2, a2));
         // new carried state: state after the slot holding the last sample
-        const float n1 = __shfl_sync(0xffffffffu, g.out_hi ? W1 : o1, g.jl);
-        const float n2 = __shfl_sync(0xffffffffu, g.out_hi ? W2 : o2, g.jl);
+        const float n1 = __shfl_sync(0xffffffffu, out_hi ? W1 : o1, jl);
+        const float n2 = __shfl_sync(0xffffffffu, out_hi ? W2 : o2, jl);
         if (lane == 0) {
-            wst[2 * k] = n1; wst[2 * k + 1] = n2;
-            if (g.inj_hi) { o1 = S1; o2 = S2; } else { E1 = S1; E2 = S2; }
+            *reinterpret_cast<float2*>(&fk_smem[wst + 2 * k]) = make_float2(n1, n2);
+            if (inj_hi) { o1 = S.x; o2 = S.y; } else { E1 = S.x; E2 = S.y; }
         }
         // S3 fix-up: y[i] += g1[i] s1 + g2[i] s2
-        const float4* __restrict__ G = reinterpret_cast<const float4*>(T + goff);
+        const float4* G = reinterpret_cast<const float4*>(&fk_smem[To + goff]);
 #pragma unroll
         for (int i = 0; i < L; i += 2) {
             const float4 gg = G[i >> 1];
@@ -344,8 +343,8 @@ __device__ __forceinline__ void process_tile(const PushParams& p, const float* _
     }
 
     // ---- S4..S6: energy, the two averages, ratio --------------------------------------------
-    const float* __restrict__ AV = stab + p.n_sec * ST::stride;
-    const float as = AV[0], al = AV[1];
+    const int AV = stab + p.n_sec * ST::stride;
+    const float as = fk_smem[AV], al = fk_smem[AV + 1];
     float sa = 0.0f, la = 0.0f, sb = 0.0f, lb = 0.0f;       // (sta, lta) x (lo slot, hi slot) from rest
 #pragma unroll
     for (int i = 0; i < L; ++i) {
@@ -354,39 +353,42 @@ __device__ __forceinline__ void process_tile(const PushParams& p, const float* _
         sa = fmaf(as, sa, ea); la = fmaf(al, la, ea);
         sb = fmaf(as, sb, eb); lb = fmaf(al, lb, eb);
     }
-    const int ks = 2 * p.n_sec;
-    const float Ms = wst[ks], Ml = wst[ks + 1];
+    const int ks = wst + 2 * p.n_sec;
+    const float2 M = *reinterpret_cast<const float2*>(&fk_smem[ks]);           // carried (sta~, lta~)
     // carried averages into their slot: + alpha^len M = M - (1 - alpha^len) M
-    const float bLs = AV[kAvgBetaL], bLl = AV[kAvgBetaL + 1];
+    const float bLs = fk_smem[AV + kAvgBetaL], bLl = fk_smem[AV + kAvgBetaL + 1];
     const float brs = first ? p.beta_r[0] : bLs, brl = first ? p.beta_r[1] : bLl;
-    const float is = fmaf(-brs, Ms, Ms), il = fmaf(-brl, Ml, Ml);
-    sa = fmaf(g.m_lo, is, sa); la = fmaf(g.m_lo, il, la);
-    sb = fmaf(g.m_hi, is, sb); lb = fmaf(g.m_hi, il, lb);
+    const float is = fmaf(-brs, M.x, M.x), il = fmaf(-brl, M.y, M.y);
+    sa = fmaf(m_lo, is, sa); la = fmaf(m_lo, il, la);
+    sb = fmaf(m_hi, is, sb); lb = fmaf(m_hi, il, lb);
     float Ws = sb + fmaf(-bLs, sa, sa), Wl = lb + fmaf(-bLl, la, la);          // alpha^L lo + hi
 #pragma unroll
     for (int d = 0; d < kSteps; ++d) {
-        const float qs = AV[kAvgBetaQ + 2 * d], ql = AV[kAvgBetaQ + 2 * d + 1];
-        const float Us = __shfl_up_sync(0xffffffffu, Ws, 1 << d), Ul = __shfl_up_sync(0xffffffffu, Wl, 1 << d);
-        if (lane >= (1 << d)) { Ws += fmaf(-qs, Us, Us); Wl += fmaf(-ql, Ul, Ul); }
+        const float2 q = *reinterpret_cast<const float2*>(&fk_smem[AV + kAvgBetaQ + 2 * d]);
+        float Us = __shfl_up_sync(0xffffffffu, Ws, 1 << d), Ul = __shfl_up_sync(0xffffffffu, Wl, 1 << d);
+        const bool act = lane >= (1 << d);
+        Us = act ? Us : 0.0f; Ul = act ? Ul : 0.0f;
+        Ws += fmaf(-q.x, Us, Us); Wl += fmaf(-q.y, Ul, Ul);
     }
     float Es = __shfl_up_sync(0xffffffffu, Ws, 1), El = __shfl_up_sync(0xffffffffu, Wl, 1);
-    if (lane == 0) { Es = 0.0f; El = 0.0f; }
+    Es = lane == 0 ? 0.0f : Es; El = lane == 0 ? 0.0f : El;
     float Os = sa + fmaf(-bLs, Es, Es), Ol = la + fmaf(-bLl, El, El);          // carry-in of the hi slot
-    const float Ns = __shfl_sync(0xffffffffu, g.out_hi ? Ws : Os, g.jl);
-    const float Nl = __shfl_sync(0xffffffffu, g.out_hi ? Wl : Ol, g.jl);
+    const float Ns = __shfl_sync(0xffffffffu, out_hi ? Ws : Os, jl);
+    const float Nl = __shfl_sync(0xffffffffu, out_hi ? Wl : Ol, jl);
     if (lane == 0) {
-        wst[ks] = Ns; wst[ks + 1] = Nl;
+        *reinterpret_cast<float2*>(&fk_smem[ks]) = make_float2(Ns, Nl);
         // the short slot starts its second pass sh zeros early: M alpha^-sh decays to M on them
-        const float Mvs = first ? Ms * p.inv_sh[0] : Ms, Mvl = first ? Ml * p.inv_sh[1] : Ml;
-        if (g.inj_hi) { Os = Mvs; Ol = Mvl; } else { Es = Mvs; El = Mvl; }
+        const float Mvs = first ? M.x * p.inv_sh[0] : M.x, Mvl = first ? M.y * p.inv_sh[1] : M.y;
+        if (inj_hi) { Os = Mvs; Ol = Mvl; } else { Es = Mvs; El = Mvl; }
     }
 
     if (p.cf) {
         // warm-up (reading R10): samples whose index since create/reset is < lta_len give cf = 0
         const long long rem = (long long)p.lta_len - (long long)seen - t0;     // first tile position with cf != 0
         const float ratio = p.ratio, thr = p.lta_thr;
-        // l~ never drops below alpha^L times its carry-in inside a slot (e >= 0)
-        const bool live = fmaf(-bLl, El, El) > thr && fmaf(-bLl, Ol, Ol) > thr;
+        // l~ never drops below alpha^L times its carry-in inside a slot (e >= 0); the idle slot in
+        // front of a ragged push (lo slot of lane 0) holds no sample
+        const bool live = (fmaf(-bLl, El, El) > thr || (lane == 0 && inj_hi)) && fmaf(-bLl, Ol, Ol) > thr;
         if (rem <= 0 && __all_sync(0xffffffffu, live)) {
 #pragma unroll
             for (int i = 0; i < L; ++i) {
@@ -423,35 +425,31 @@ template <int L>
 __global__ void __launch_bounds__(cm_max_warps<L>() * 32, 1)
 filark_push_cm_kernel(const __grid_constant__ PushParams p)
 {
-    extern __shared__ __align__(16) float smem[];
     const int tab_floats = p.n_sec * SecTab<L>::stride + kAvgFloats;
-    float* stab = smem;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
-    float* wbase = smem + tab_floats + warp * warp_smem_floats<L>();
-    float* bufs[2] = { wbase, wbase + Geo<L>::buf_floats };
-    float* wsts[2] = { wbase + 2 * Geo<L>::buf_floats, wbase + 2 * Geo<L>::buf_floats + kStateSmem };
+    const int wbase = tab_floats + warp * warp_smem_floats<L>();      // two tile buffers, then two state copies
+    const int wst0 = wbase + 2 * Geo<L>::buf_floats;
 
     // warp (b, w) walks the channels b + grid (w + W i)
     const int stride = gridDim.x * W;
-    int ch = blockIdx.x + gridDim.x * warp, tile = 0, cur = 0;
-    if (ch < p.n_ch) issue_tile_load<L>(p, ch, 0, bufs[0], wsts[0], lane, true);
+    int ch = blockIdx.x + gridDim.x * warp, tile = 0, cur = 0, wcur = 0;
+    if (ch < p.n_ch) issue_tile_load<L>(p, ch, 0, wbase, wst0, lane, true);
     for (int i = threadIdx.x; i < tab_floats / 4; i += blockDim.x)
-        reinterpret_cast<float4*>(stab)[i] = __ldg(reinterpret_cast<const float4*>(p.tab) + i);
+        reinterpret_cast<float4*>(fk_smem)[i] = __ldg(reinterpret_cast<const float4*>(p.tab) + i);
     __syncthreads();
 
     const int ns = state_floats(p.n_sec);
-    int wcur = 0;                                    // which state copy belongs to the current channel
     unsigned seen = 0;
     while (ch < p.n_ch) {
         int nch = ch, ntile = tile + 1;
         if (ntile == p.n_tiles) { ntile = 0; nch = ch + stride; }
+        const int buf = wbase + cur * Geo<L>::buf_floats;
+        const int wst = wst0 + wcur * kStateSmem;
         cp_async_wait_all();
         __syncwarp();
-        float* buf = bufs[cur];
-        float* wst = wsts[wcur];
         float lo[L], hi[L];
         {
-            const float4* s = reinterpret_cast<const float4*>(buf + lane * Geo<L>::pitch);
+            const float4* s = reinterpret_cast<const float4*>(&fk_smem[buf + lane * Geo<L>::pitch]);
             const float gn = p.gain;
 #pragma unroll
             for (int q = 0; q < L / 4; ++q) {
@@ -460,20 +458,22 @@ filark_push_cm_kernel(const __grid_constant__ PushParams p)
                 hi[4 * q] = b.x * gn; hi[4 * q + 1] = b.y * gn; hi[4 * q + 2] = b.z * gn; hi[4 * q + 3] = b.w * gn;
             }
         }
-        if (tile == 0) seen = __float_as_uint(wst[ns - 2]);
+        if (tile == 0) seen = __float_as_uint(fk_smem[wst + ns - 2]);
         __syncwarp();
-        if (nch < p.n_ch) issue_tile_load<L>(p, nch, ntile, bufs[cur ^ 1], wsts[wcur ^ 1], lane, ntile == 0);
-        process_tile<L>(p, stab, buf, wst, lo, hi, ch, tile, lane, seen);
+        if (nch < p.n_ch)
+            issue_tile_load<L>(p, nch, ntile, wbase + (cur ^ 1) * Geo<L>::buf_floats,
+                               wst0 + (wcur ^ 1) * kStateSmem, lane, ntile == 0);
+        process_tile<L>(p, 0, buf, wst, lo, hi, ch, tile, lane, seen);
         if (ntile == 0) {
             // channel done: carried state and sample count back to global memory
             if (lane == 0) {
                 const unsigned long long s2 = (unsigned long long)seen + (unsigned long long)p.n_t;
-                wst[ns - 2] = __uint_as_float(s2 > kSeenMax ? kSeenMax : (unsigned)s2);
+                fk_smem[wst + ns - 2] = __uint_as_float(s2 > kSeenMax ? kSeenMax : (unsigned)s2);
             }
             __syncwarp();
             float* gst = p.state + (long long)ch * ns;
-            if (lane < ns) gst[lane] = wst[lane];
-            if (lane + 32 < ns) gst[lane + 32] = wst[lane + 32];
+            if (lane < ns) gst[lane] = fk_smem[wst + lane];
+            if (lane + 32 < ns) gst[lane + 32] = fk_smem[wst + lane + 32];
             wcur ^= 1;
         }
         ch = nch; tile = ntile; cur ^= 1;
