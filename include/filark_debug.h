@@ -24,14 +24,15 @@ extern "C" {
 int filark_debug_design(const double *sos, int n_sec, int *kinds, double *coefs, double *gain);
 
 /*
- * Slot geometry of one channel-major push of n_t >= 1 samples (csrc/filark_kernels.cuh): the time
- * axis is cut into slots of L samples aligned to the END of the push; a tile is 64 slots (lane l
- * owns slots 2l, 2l+1).  force_L = 0 lets the library choose L among its compiled variants
- * (8, 16, 24, 32, 48), otherwise L = force_L.  out7 = { L, n_tiles, lead (idle slots in front),
- * r (samples in the first, possibly short, slot), pad0 (zeros in front of sample 0),
- * last_lane, last_half (position in the last tile of the slot holding the last sample) }.
+ * Slot geometry of one channel-major push of n_t >= 1 samples that finds r0 raw samples of the
+ * previous push waiting in the handle (csrc/filark_kernels.cuh): the stream is cut into slots of
+ * L samples aligned to the stream (not to the push); a tile is 64 slots (lane l owns slots 2l,
+ * 2l+1); tile-space positions [0, r0) of the first tile are the waiting samples.  force_L = 0
+ * lets the library choose L among its compiled variants (8, 16, 24, 32, 48), otherwise
+ * L = force_L.  out5 = { L, n_tiles, q_last (full slots in the last tile, 0..64), r1 (samples
+ * of the trailing partial slot, kept for the next push), vec4 (16-byte accesses stay aligned) }.
  */
-int filark_debug_push_geometry(long long n_t, int force_L, int *out7);
+int filark_debug_push_geometry(long long n_t, int r0, int force_L, int *out5);
 
 /* out4 (row-major 2x2) = A^e for the state-space form chosen for one section (6 doubles). */
 int filark_debug_block_power(const double *sos6, long long e, double *out4);

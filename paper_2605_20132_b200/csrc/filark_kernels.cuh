@@ -6,29 +6,34 @@
 // each output is written once.
 //
 // Channel-major mapping (time contiguous): one warp owns one channel at a time.  The time axis
-// of a push is cut into sub-blocks of L samples ("slots"); a tile is 64 consecutive slots and
-// lane l owns slots 2l ("lo") and 2l+1 ("hi"), i.e. 2L contiguous samples, in registers through
-// every section and the STA/LTA.  The two slots of a lane are two independent recurrence chains
-// interleaved in program order (B200 issues FFMA2 at the cost of two FFMA, so plain scalar FFMA
-// on two chains is as fast and needs no register pairing -- DESIGN.md 6).  Tiles of a channel
-// are processed in time order by the same warp; the carried state sits in shared memory between
-// tiles and in global memory between pushes.
+// is cut into sub-blocks of L samples ("slots"); a tile is 64 consecutive slots and lane l owns
+// slots 2l ("lo") and 2l+1 ("hi"), i.e. 2L contiguous samples, as the two halves of L packed
+// f32x2 registers that stay in registers through every section and the STA/LTA.  Every
+// per-sample instruction is an FFMA2 whose third operand -- a section coefficient, a fix-up row
+// C A^i, an averaging constant -- is warp-uniform and comes from the kernel-parameter constant
+// bank through a uniform register: an FFMA2 with three register-file operands is limited to
+// about 2/3 of the FMA pipe by register-file bandwidth on B200, with a uniform operand it runs
+// at ~95 % (profiles/).
+//
+// Slots are aligned to the STREAM, not to the push: the carried state of a channel always
+// belongs to a slot boundary.  The samples of a push that do not fill a slot (r1 < L of them)
+// are filtered and written like all others (zero-padded slot, outputs of the padding dropped),
+// but the state is not advanced over them; their raw values are kept in the handle (`hist`)
+// and the next push starts with them (r0 = r1 positions of its first tile come from `hist`,
+// their outputs are recomputed and dropped).  Every slot that advances the state is therefore
+// full, every lane uses the same fix-up rows, and ragged pushes need no second code path.
+// r0 and the sample counter live in device memory (`Ctl`), so a push has no host-side mutable
+// argument and can be replayed from a CUDA graph.
 //
 // Persistent grid: one CTA per SM, W warps per CTA; warp (b, w) walks the channels
 // b + grid (w + W i), i = 0, 1, ...  While a tile is computed, the next tile (of the same or of
 // the warp's next channel) and that channel's carried state are already in flight into the
 // warp's second shared-memory buffer (cp.async, 16 B per lane, zero-filled outside the push).
 //
-// Ragged pushes need no second code path: slots are aligned to the END of the push, the first
-// slot is the short one (r <= L samples, zero-padded at its front -- a zero-state recurrence
-// stays at rest through leading zeros), and it always sits in the hi slot of lane 0 of tile 0
-// (one idle slot in front of it when r < L), so that its shifted fix-up table is a per-lane
-// table pointer.  Trailing idle slots hold zeros and are never stored.
-//
 // The recurrences are exact restatements of the oracle's definition:
 //   section:  s[n] = A s[n-1] + B x[n],  y[n] = C s[n-1] + D x[n]           (design.hpp)
 //   slot with carry-in s_in, local pass from zero state giving y_loc and end state v:
-//             y[i] = y_loc[i] + (C A^i) s_in,   s_out = A^len s_in + v
+//             y[i] = y_loc[i] + (C A^i) s_in,   s_out = A^L s_in + v
 //   averages: m~[n] = alpha m~[n-1] + e[n]  (m~ = m * N),  cf = (N_l/N_s) s~/l~
 #pragma once
 #include <cuda_runtime.h>
@@ -39,69 +44,91 @@ namespace filark {
 constexpr int kMaxSec = 16;
 constexpr int kMaxWarps = 16;          // warps per CTA (one CTA per SM)
 constexpr int kSteps = 5;              // log2(32) scan steps
+constexpr int kHist = 64;              // floats of raw history per channel (>= largest L)
 constexpr int kKindDF2 = 0, kKindDF2G = 1, kKindDelta = 2, kKindDeltaG = 3, kKindNormal = 4;
 
-// ---- device table of one sub-block length L (floats); see build_variant_table() ----------------
-// per section, stride SecTab<L>::stride:
-//   [0] kind (int bits)  [1..5] local-pass coefficients  [7] scan steps needed (int bits)
-//   [8..11]  P = A^L                       [12..31] Q[d] = A^(2L 2^d), d = 0..4 (row-major 2x2)
-//   G0: 2L rows (g1, g2): rows -L..-1 are zero, row i >= 0 is C A^i     (+ 4 floats pad)
-//   G1: the same shifted down by one row (row j holds G0 row j-1): 16-byte aligned odd shifts
-// after the sections, the averages block (kAvgFloats):
-//   [0] alpha_s [1] alpha_l  [2..3] 1 - alpha^L  [4..13] 1 - alpha^(2L 2^d) (s,l interleaved)
-//   [14] 1/N_s [15] 1/N_l
-// What depends on the push (the length r of its first slot) travels in PushParams.
-template <int L> struct SecTab {
-    static constexpr int g0 = 32;
-    static constexpr int gsz = 4 * L + 4;
-    static constexpr int g1 = g0 + gsz;
-    static constexpr int stride = g1 + gsz;
+// Device-resident control block of a handle (blocked channel-major kernels).
+struct Ctl {
+    unsigned long long seen;   // samples pushed since create/reset
+    unsigned int r0;           // samples waiting in `hist` (raw tail of the previous push)
+    unsigned int ticket;       // CTAs that have finished the running push
 };
-constexpr int kOffKind = 0, kOffCoef = 1, kOffNSteps = 7, kOffP = 8, kOffQ = 12;
-constexpr int kAvgBetaL = 2, kAvgBetaQ = 4, kAvgInvN = 14, kAvgFloats = 16;
+
+// One SOS section for sub-block length L; every member is warp-uniform and is read straight
+// from the constant bank.  Q[d] = A^(2L 2^d); g[i] = C A^i.
+template <int L> struct SecParams {
+    int kind, nsteps;
+    float c[5];
+    float pad;
+    float P[4];                // A^L, row-major 2x2
+    float Q[kSteps][4];
+    float g[L][2];
+};
+
+// The two exponential averages (index 0: STA, 1: LTA).  beta = 1 - alpha^n keeps full relative
+// precision for alpha next to 1; v alpha^n is evaluated as v - beta v.
+struct AvgParams {
+    float alpha[2];
+    float betaL[2];            // 1 - alpha^L
+    float betaQ[kSteps][2];    // 1 - alpha^(2L 2^d)
+    float invN[2];
+};
 
 // Carried state of one channel (floats): [0, 2 n_sec) section states, then sta~, lta~, the
-// number of samples seen since create/reset (uint32 bits, saturating), one pad word.
+// number of samples seen (serial kernel only; uint32 bits, saturating), one pad word.
 __host__ __device__ constexpr int state_floats(int n_sec) { return 2 * n_sec + 4; }
-constexpr unsigned kSeenMax = 0x7fffffffu;    // >= any lta_len; only ever moved as bits
+constexpr unsigned kSeenMax = 0x7fffffffu;
 
-struct PushParams {
+template <int L> struct PushParams {
     const float* in;
     float* filt;
     float* cf;
-    const float* tab;        // table of the chosen L (device)
-    float* state;            // channel-major: [n_ch][state_floats]; time-major kernels: [state_floats][n_ch]
-    long long n_t, in_pitch, out_pitch;
-    int n_ch, n_sec;
-    int n_tiles;             // tiles per channel
-    int lead;                // idle slots in front of the first one (0, or 1 when r < L)
-    int r;                   // samples in the first slot, 1..L
-    int pad0;                // zeros in front of sample 0: lead L + (L - r)
-    int last_lane, last_half;// lane / half of the slot holding the last sample (in the last tile)
-    int lta_len;
+    float* state;            // [n_ch][state_floats]
+    float* hist;             // [n_ch][kHist]
+    Ctl* ctl;
+    long long in_pitch, out_pitch;
+    int n_t, n_ch, n_sec, lta_len;
     int vec4;                // 16-byte global accesses are legal (alignment, pitch, n_t % 4 == 0)
     float gain, ratio, lta_thr;
-    float beta_r[2];         // 1 - alpha^r            (sta, lta): carry across the first slot
-    float inv_sh[2];         // alpha^-(L - r)         (sta, lta): second pass of the first slot
-    float apow_r[kMaxSec][4];// A^r per section, row-major 2x2
+    AvgParams avg;
+    SecParams<L> sec[kMaxSec];
 };
 
+// Per-push geometry, derived on the device from Ctl (host mirror: filark_debug_push_geometry).
+struct Geom {
+    int r0;                  // tile-space positions [0, r0) of tile 0 come from hist
+    int n_tiles;
+    int q_last;              // full slots in the last tile, 0..64
+    int r1;                  // samples of the trailing partial slot, 0..L-1
+    bool vec4;
+};
+template <int L>
+__host__ __device__ inline Geom make_geom(unsigned r0, int n_t, bool vec4)
+{
+    Geom g;
+    const long long total = (long long)r0 + n_t;
+    const long long n_full = total / L;
+    g.r0 = (int)r0;
+    g.r1 = (int)(total - n_full * L);
+    const long long slots = n_full + (g.r1 ? 1 : 0);
+    g.n_tiles = (int)((slots + 63) / 64);
+    g.q_last = (int)(n_full - 64LL * (g.n_tiles - 1));
+    g.vec4 = vec4 && (r0 & 3u) == 0;
+    return g;
+}
+
 // ---- small PTX wrappers ------------------------------------------------------------------------
-__device__ __forceinline__ void cp_async16(float* dst, const float* src, int src_bytes)
-{
-    const unsigned s = (unsigned)__cvta_generic_to_shared(dst);
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s), "l"(src), "r"(src_bytes) : "memory");
-}
-__device__ __forceinline__ void cp_async4(float* dst, const float* src, int src_bytes)
-{
-    const unsigned s = (unsigned)__cvta_generic_to_shared(dst);
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(s), "l"(src), "r"(src_bytes) : "memory");
-}
+__device__ __forceinline__ void cp_async16(int dst_off, const float* src, int src_bytes);
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void st_stream(float* p, float v) { __stcs(p, v); }
 __device__ __forceinline__ void st_stream4(float* p, float4 v) { __stcs(reinterpret_cast<float4*>(p), v); }
 __device__ __forceinline__ float rcp_fast(float a) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
+__device__ __forceinline__ float2 f2(float a) { return make_float2(a, a); }
+__device__ __forceinline__ float2 fma2(float a, float2 b, float2 c) { return __ffma2_rn(make_float2(a, a), b, c); }
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a, b); }
 
 template <int L> struct Geo {
     static constexpr int pitch = 2 * L + 4;        // floats per lane region: LDS.128 conflict-free
@@ -114,70 +141,98 @@ template <int L> struct Geo {
 // shared-memory access (32-bit addresses, LDS/STS instead of generic LD/ST).
 extern __shared__ __align__(16) float fk_smem[];
 
+__device__ __forceinline__ void cp_async16(int dst_off, const float* src, int src_bytes)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(&fk_smem[dst_off]);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(s), "l"(src), "r"(src_bytes) : "memory");
+}
+__device__ __forceinline__ void cp_async4(int dst_off, const float* src, int src_bytes)
+{
+    const unsigned s = (unsigned)__cvta_generic_to_shared(&fk_smem[dst_off]);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(s), "l"(src), "r"(src_bytes) : "memory");
+}
+
 // Shared memory of one warp: two tile buffers (input of tile k / staging of its outputs, and the
 // prefetched input of tile k+1) and two copies of the channel state.
 constexpr int kStateSmem = 40;                     // >= state_floats(kMaxSec), multiple of 4
 template <int L> __host__ __device__ constexpr int warp_smem_floats() { return 2 * Geo<L>::buf_floats + 2 * kStateSmem; }
 
 // S0: start the asynchronous copy of one tile of one channel into `buf` (padded lane regions:
-// tile-local sample e lives at buf[e + 4 (e / 2L)]) and of the channel's carried state into
-// `wst`.  t0 = time index (within the push) of the tile's position 0; samples outside [0, n_t)
-// are zero-filled.
+// tile-local sample e lives at buf[e + 4 (e / 2L)]) and, with the channel's first tile, of its
+// carried state into `wst`.  Tile-space position e of tile `tile` is input sample
+// t = tile 64L + e - r0; t < 0 reads hist[ch][r0 + t], t >= n_t is zero-filled.
 template <int L>
-__device__ __forceinline__ void issue_tile_load(const PushParams& p, int ch, int tile, int buf, int wst,
-                                                int lane, bool with_state)
+__device__ __forceinline__ void issue_tile_load(const PushParams<L>& p, const Geom& g, int ch, int tile, int buf,
+                                                int wst, int lane, bool with_state)
 {
-    const int t0 = tile * Geo<L>::tile - p.pad0;
-    const int n_t = (int)p.n_t;
+    const int t0 = tile * Geo<L>::tile - g.r0;
+    const int n_t = p.n_t;
     const float* __restrict__ src = p.in + (long long)ch * p.in_pitch;
-    if (p.vec4) {
-        // valid 16-byte chunks of this tile: [c_lo, c_hi)
-        const int c_lo = t0 < 0 ? (-t0 >> 2) : 0;
-        const int c_hi = min(Geo<L>::tile, n_t - t0) >> 2;
-        const unsigned span = (unsigned)(c_hi - c_lo);
-        const float* __restrict__ srct = src + t0;
+    const float* __restrict__ hsrc = p.hist + (long long)ch * kHist + g.r0;     // hsrc[t] for t in [-r0, 0)
+    if (g.vec4) {
+        if (t0 >= 0 && t0 + Geo<L>::tile <= n_t) {                   // interior tile: no bounds
+            const float* __restrict__ srct = src + t0 + 4 * lane;
 #pragma unroll
-        for (int m = 0; m < Geo<L>::chunks; ++m) {
-            const int c = 32 * m + lane;
-            const bool ok = (unsigned)(c - c_lo) < span;
-            cp_async16(&fk_smem[buf + 4 * c + 4 * (c / Geo<L>::chunks)], ok ? srct + 4 * c : src, ok ? 16 : 0);
+            for (int m = 0; m < Geo<L>::chunks; ++m) {
+                const int c = 32 * m + lane;
+                cp_async16(buf + 4 * c + 4 * (c / Geo<L>::chunks), srct + 128 * m, 16);
+            }
+        } else {
+#pragma unroll
+            for (int m = 0; m < Geo<L>::chunks; ++m) {
+                const int c = 32 * m + lane;
+                const int t = t0 + 4 * c;
+                const float* s = t < 0 ? hsrc + t : src + t;
+                const bool ok = t < n_t;
+                cp_async16(buf + 4 * c + 4 * (c / Geo<L>::chunks), ok ? s : src, ok ? 16 : 0);
+            }
         }
     } else {
-#pragma unroll 8
+#pragma unroll 1
         for (int m = 0; m < 2 * L; ++m) {
             const int e = 32 * m + lane;
             const int t = t0 + e;
-            const bool ok = (unsigned)t < (unsigned)n_t;
-            cp_async4(&fk_smem[buf + e + 4 * (e / (2 * L))], ok ? src + t : src, ok ? 4 : 0);
+            const float* s = t < 0 ? hsrc + t : src + t;
+            const bool ok = t < n_t;
+            cp_async4(buf + e + 4 * (e / (2 * L)), ok ? s : src, ok ? 4 : 0);
         }
     }
     if (with_state) {
         const int ns = state_floats(p.n_sec);
         const float* gst = p.state + (long long)ch * ns;
-        if (lane < ns) cp_async4(&fk_smem[wst + lane], gst + lane, 4);
-        if (lane + 32 < ns) cp_async4(&fk_smem[wst + lane + 32], gst + lane + 32, 4);
+        if (lane < ns) cp_async4(wst + lane, gst + lane, 4);
+        if (lane + 32 < ns) cp_async4(wst + lane + 32, gst + lane + 32, 4);
     }
     cp_async_commit();
 }
 
-// S7: the lane regions of `buf` -> one output array (coalesced 16-byte stores).
+// S7: the lane regions of `buf` -> one output array (coalesced 16-byte stores).  Positions that
+// map to t < 0 (recomputed history) or t >= n_t (padding) are dropped.
 template <int L>
-__device__ __forceinline__ void store_tile(const PushParams& p, float* __restrict__ dst, int buf, int lane, int t0)
+__device__ __forceinline__ void store_tile(const PushParams<L>& p, const Geom& g, float* __restrict__ dst, int buf,
+                                           int lane, int t0)
 {
-    const int n_t = (int)p.n_t;
-    if (p.vec4) {
-        const int c_lo = t0 < 0 ? (-t0 >> 2) : 0;
-        const int c_hi = min(Geo<L>::tile, n_t - t0) >> 2;
-        const unsigned span = (unsigned)(c_hi - c_lo);
-        float* __restrict__ dstt = dst + t0;
+    const int n_t = p.n_t;
+    if (g.vec4) {
+        if (t0 >= 0 && t0 + Geo<L>::tile <= n_t) {
+            float* __restrict__ dstt = dst + t0 + 4 * lane;
 #pragma unroll
-        for (int m = 0; m < Geo<L>::chunks; ++m) {
-            const int c = 32 * m + lane;
-            const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + 4 * c + 4 * (c / Geo<L>::chunks)]);
-            if ((unsigned)(c - c_lo) < span) st_stream4(dstt + 4 * c, v);
+            for (int m = 0; m < Geo<L>::chunks; ++m) {
+                const int c = 32 * m + lane;
+                const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + 4 * c + 4 * (c / Geo<L>::chunks)]);
+                st_stream4(dstt + 128 * m, v);
+            }
+        } else {
+            float* __restrict__ dstt = dst + t0;
+#pragma unroll
+            for (int m = 0; m < Geo<L>::chunks; ++m) {
+                const int c = 32 * m + lane;
+                const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + 4 * c + 4 * (c / Geo<L>::chunks)]);
+                if ((unsigned)(t0 + 4 * c) < (unsigned)n_t) st_stream4(dstt + 4 * c, v);
+            }
         }
     } else {
-#pragma unroll 8
+#pragma unroll 1
         for (int m = 0; m < 2 * L; ++m) {
             const int e = 32 * m + lane;
             const int t = t0 + e;
@@ -187,290 +242,259 @@ __device__ __forceinline__ void store_tile(const PushParams& p, float* __restric
     }
 }
 
+// Unpack the lane's pairs into its shared-memory region: lo samples then hi samples.
 template <int L>
-__device__ __forceinline__ void regs_to_buf(const float (&lo)[L], const float (&hi)[L], int buf, int lane)
+__device__ __forceinline__ void regs_to_buf(const float2 (&x)[L], int buf, int lane)
 {
     float4* d = reinterpret_cast<float4*>(&fk_smem[buf + lane * Geo<L>::pitch]);
 #pragma unroll
     for (int q = 0; q < L / 4; ++q) {
-        d[q] = make_float4(lo[4 * q], lo[4 * q + 1], lo[4 * q + 2], lo[4 * q + 3]);
-        d[L / 4 + q] = make_float4(hi[4 * q], hi[4 * q + 1], hi[4 * q + 2], hi[4 * q + 3]);
+        d[q] = make_float4(x[4 * q].x, x[4 * q + 1].x, x[4 * q + 2].x, x[4 * q + 3].x);
+        d[L / 4 + q] = make_float4(x[4 * q].y, x[4 * q + 1].y, x[4 * q + 2].y, x[4 * q + 3].y);
     }
 }
 
-// S1: zero-state response of one section on the lane's two slots; returns their end states.
+// S1: zero-state response of one section on the lane's two slots (the two halves of every
+// pair); returns the end states s1 = (lo state 1, hi state 1), s2 = (lo state 2, hi state 2).
 template <int L, int KIND>
-__device__ __forceinline__ void local_pass(float (&lo)[L], float (&hi)[L], int Toff,
-                                           float& a1, float& a2, float& b1, float& b2)
+__device__ __forceinline__ void local_pass(float2 (&x)[L], const SecParams<L>& T, float2& s1, float2& s2)
 {
-    const float* T = &fk_smem[Toff];
-    const float c0 = T[kOffCoef], c1 = T[kOffCoef + 1], c2 = T[kOffCoef + 2], c3 = T[kOffCoef + 3];
-    a1 = a2 = b1 = b2 = 0.0f;                       // (a1, a2): state of the lo slot, (b1, b2): hi slot
+    const float c0 = T.c[0], c1 = T.c[1], c2 = T.c[2], c3 = T.c[3];
+    s1 = s2 = make_float2(0.0f, 0.0f);
     if (KIND == kKindDF2) {
 #pragma unroll
         for (int i = 0; i < L; ++i) {
-            const float wa = fmaf(c0, a1, fmaf(c1, a2, lo[i]));
-            const float wb = fmaf(c0, b1, fmaf(c1, b2, hi[i]));
-            lo[i] = fmaf(c2, a1, fmaf(c3, a2, wa));
-            hi[i] = fmaf(c2, b1, fmaf(c3, b2, wb));
-            a2 = a1; a1 = wa; b2 = b1; b1 = wb;
+            const float2 w = fma2(c0, s1, fma2(c1, s2, x[i]));
+            x[i] = fma2(c2, s1, fma2(c3, s2, w));
+            s2 = s1; s1 = w;
         }
     } else if (KIND == kKindDelta) {
 #pragma unroll
         for (int i = 0; i < L; ++i) {
-            const float ua = fmaf(c0, a1, fmaf(c1, a2, lo[i]));
-            const float ub = fmaf(c0, b1, fmaf(c1, b2, hi[i]));
-            lo[i] = fmaf(c2, a1, ua);
-            hi[i] = fmaf(c2, b1, ub);
-            a2 += ua; a1 = ua; b2 += ub; b1 = ub;
+            const float2 u = fma2(c0, s1, fma2(c1, s2, x[i]));
+            x[i] = fma2(c2, s1, u);
+            s2 = add2(s2, u); s1 = u;
         }
     } else if (KIND == kKindDeltaG) {
 #pragma unroll
         for (int i = 0; i < L; ++i) {
-            const float ua = fmaf(c0, a1, fmaf(c1, a2, lo[i]));
-            const float ub = fmaf(c0, b1, fmaf(c1, b2, hi[i]));
-            lo[i] = fmaf(c3, a2, fmaf(c2, a1, ua));
-            hi[i] = fmaf(c3, b2, fmaf(c2, b1, ub));
-            a2 += ua; a1 = ua; b2 += ub; b1 = ub;
+            const float2 u = fma2(c0, s1, fma2(c1, s2, x[i]));
+            x[i] = fma2(c3, s2, fma2(c2, s1, u));
+            s2 = add2(s2, u); s1 = u;
         }
     } else if (KIND == kKindNormal) {
         const float nc1 = -c1;
 #pragma unroll
         for (int i = 0; i < L; ++i) {
-            const float xa = lo[i], xb = hi[i];
-            lo[i] = fmaf(c2, a1, fmaf(c3, a2, xa));
-            hi[i] = fmaf(c2, b1, fmaf(c3, b2, xb));
-            const float na = fmaf(c0, a1, fmaf(c1, a2, xa));
-            const float nb = fmaf(c0, b1, fmaf(c1, b2, xb));
-            a2 = fmaf(c0, a2, nc1 * a1); b2 = fmaf(c0, b2, nc1 * b1);
-            a1 = na; b1 = nb;
+            const float2 xi = x[i];
+            x[i] = fma2(c2, s1, fma2(c3, s2, xi));
+            const float2 n1 = fma2(c0, s1, fma2(c1, s2, xi));
+            s2 = fma2(c0, s2, mul2(f2(nc1), s1));
+            s1 = n1;
         }
     } else {                                        // kKindDF2G: explicit b0 = coefficient 4
-        const float c4 = T[kOffCoef + 4];
+        const float c4 = T.c[4];
 #pragma unroll
         for (int i = 0; i < L; ++i) {
-            const float wa = fmaf(c0, a1, fmaf(c1, a2, lo[i]));
-            const float wb = fmaf(c0, b1, fmaf(c1, b2, hi[i]));
-            lo[i] = fmaf(c2, a1, fmaf(c3, a2, c4 * wa));
-            hi[i] = fmaf(c2, b1, fmaf(c3, b2, c4 * wb));
-            a2 = a1; a1 = wa; b2 = b1; b1 = wb;
+            const float2 w = fma2(c0, s1, fma2(c1, s2, x[i]));
+            x[i] = fma2(c2, s1, fma2(c3, s2, mul2(f2(c4), w)));
+            s2 = s1; s1 = w;
         }
     }
 }
 
-// One tile of one channel, samples already in lo/hi: S1..S7.  `buf` stages the outputs.
-// stab / buf / wst are float offsets into fk_smem.
+// One tile of one channel, samples already in x (gain applied): S1..S7.  `buf` stages the
+// outputs.  buf / wst are float offsets into fk_smem.
 template <int L>
-__device__ __forceinline__ void process_tile(const PushParams& p, int stab, int buf, int wst, float (&lo)[L],
-                                             float (&hi)[L], int ch, int tile, int lane, unsigned seen)
+__device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom& g, int buf, int wst, float2 (&x)[L],
+                                             int ch, int tile, int lane, unsigned long long seen)
 {
-    using ST = SecTab<L>;
-    const bool first = tile == 0, last = tile == p.n_tiles - 1;
-    const int t0 = tile * Geo<L>::tile - p.pad0;
-    const bool inj_hi = first && p.lead != 0;   // carried state enters the hi slot of lane 0 (ragged tile 0)
-    const int r = first ? p.r : L;              // samples in the slot that receives the carried state
-    const int sh = L - r;
-    const int jl = last ? p.last_lane : 31;     // lane of the slot holding the tile's last sample
-    const bool out_hi = last ? p.last_half != 0 : true;
-    const float m_lo = (lane == 0 && !inj_hi) ? 1.0f : 0.0f;
-    const float m_hi = (lane == 0 && inj_hi) ? 1.0f : 0.0f;
-    // per-lane fix-up table offset (floats) inside a section's table: lane 0's injected slot is
-    // short by sh samples, so its rows are shifted down by sh
-    int goff = ST::g0 + 2 * L;
-    if (lane == 0 && sh != 0) goff = (sh & 1) ? ST::g1 + 2 * (L - sh + 1) : ST::g0 + 2 * (L - sh);
+    const bool last = tile == g.n_tiles - 1;
+    const int t0 = tile * Geo<L>::tile - g.r0;
+    // the carried state moves to the end of the tile's last FULL slot (slot q - 1)
+    const int q = last ? g.q_last : 64;
+    const bool keep = q == 0;
+    const int jl = keep ? 0 : (q - 1) >> 1;
+    const bool out_hi = ((q - 1) & 1) != 0;
 
     // ---- S1..S3 per section -------------------------------------------------------------------
     for (int k = 0; k < p.n_sec; ++k) {
-        const int To = stab + k * ST::stride;
-        const int kind = __float_as_int(fk_smem[To + kOffKind]);
-        float a1, a2, b1, b2;
-        switch (kind) {
-            case kKindDF2: local_pass<L, kKindDF2>(lo, hi, To, a1, a2, b1, b2); break;
-            case kKindDelta: local_pass<L, kKindDelta>(lo, hi, To, a1, a2, b1, b2); break;
-            case kKindDeltaG: local_pass<L, kKindDeltaG>(lo, hi, To, a1, a2, b1, b2); break;
-            case kKindNormal: local_pass<L, kKindNormal>(lo, hi, To, a1, a2, b1, b2); break;
-            default: local_pass<L, kKindDF2G>(lo, hi, To, a1, a2, b1, b2); break;
+        const SecParams<L>& T = p.sec[k];
+        float2 s1, s2;
+        switch (T.kind) {
+            case kKindDF2: local_pass<L, kKindDF2>(x, T, s1, s2); break;
+            case kKindDelta: local_pass<L, kKindDelta>(x, T, s1, s2); break;
+            case kKindDeltaG: local_pass<L, kKindDeltaG>(x, T, s1, s2); break;
+            case kKindNormal: local_pass<L, kKindNormal>(x, T, s1, s2); break;
+            default: local_pass<L, kKindDF2G>(x, T, s1, s2); break;
         }
-        // S2: carried state S into its slot, then an inclusive scan of the lane totals
+        // S2: lane total W = P a + b (a, b: end states of the lo / hi slot from rest); the carried
+        // state S enters lane 0's total through A^2L; inclusive scan over the lanes
         const float2 S = *reinterpret_cast<const float2*>(&fk_smem[wst + 2 * k]);
-        const float4 Pm = *reinterpret_cast<const float4*>(&fk_smem[To + kOffP]);     // A^L
-        const float4 Ar = *reinterpret_cast<const float4*>(&p.apow_r[k][0]);          // A^r (first slot)
-        const float4 Au = first ? Ar : Pm;
-        const float i1 = fmaf(Au.x, S.x, Au.y * S.y), i2 = fmaf(Au.z, S.x, Au.w * S.y);
-        a1 = fmaf(m_lo, i1, a1); a2 = fmaf(m_lo, i2, a2);                             // state after the lo slot
-        b1 = fmaf(m_hi, i1, b1); b2 = fmaf(m_hi, i2, b2);
-        float W1 = fmaf(Pm.x, a1, fmaf(Pm.y, a2, b1)), W2 = fmaf(Pm.z, a1, fmaf(Pm.w, a2, b2));
-        const int nsteps = __float_as_int(fk_smem[To + kOffNSteps]);
+        const float P0 = T.P[0], P1 = T.P[1], P2 = T.P[2], P3 = T.P[3];
+        float W1 = fmaf(P0, s1.x, fmaf(P1, s2.x, s1.y)), W2 = fmaf(P2, s1.x, fmaf(P3, s2.x, s2.y));
+        {
+            // (selects instead of branches: the table operands stay uniform-register reads)
+            const float S1 = lane == 0 ? S.x : 0.0f, S2 = lane == 0 ? S.y : 0.0f;
+            W1 = fmaf(T.Q[0][0], S1, fmaf(T.Q[0][1], S2, W1));
+            W2 = fmaf(T.Q[0][2], S1, fmaf(T.Q[0][3], S2, W2));
+        }
+        const int nsteps = T.nsteps;
 #pragma unroll
         for (int d = 0; d < kSteps; ++d) {
             if (d < nsteps) {
-                const float4 Q = *reinterpret_cast<const float4*>(&fk_smem[To + kOffQ + 4 * d]);
                 float U1 = __shfl_up_sync(0xffffffffu, W1, 1 << d), U2 = __shfl_up_sync(0xffffffffu, W2, 1 << d);
                 const bool act = lane >= (1 << d);
                 U1 = act ? U1 : 0.0f; U2 = act ? U2 : 0.0f;
-                W1 = fmaf(Q.x, U1, fmaf(Q.y, U2, W1));
-                W2 = fmaf(Q.z, U1, fmaf(Q.w, U2, W2));
+                W1 = fmaf(T.Q[d][0], U1, fmaf(T.Q[d][1], U2, W1));
+                W2 = fmaf(T.Q[d][2], U1, fmaf(T.Q[d][3], U2, W2));
             }
         }
         float E1 = __shfl_up_sync(0xffffffffu, W1, 1), E2 = __shfl_up_sync(0xffffffffu, W2, 1);
-        E1 = lane == 0 ? 0.0f : E1; E2 = lane == 0 ? 0.0f : E2;    // state entering the lane's lo slot
-        // carry-in of the hi slot: P E + (state after lo from rest)
-        float o1 = fmaf(Pm.x, E1, fmaf(Pm.y, E2, a1)), o2 = fmaf(Pm.z, E1, fmaf(Pm.w, E2, a2));
-        // new carried state: state after the slot holding the last sample
+        if (lane == 0) { E1 = S.x; E2 = S.y; }                      // state entering the lane's lo slot
+        const float o1 = fmaf(P0, E1, fmaf(P1, E2, s1.x)), o2 = fmaf(P2, E1, fmaf(P3, E2, s2.x));   // ... its hi slot
         const float n1 = __shfl_sync(0xffffffffu, out_hi ? W1 : o1, jl);
         const float n2 = __shfl_sync(0xffffffffu, out_hi ? W2 : o2, jl);
-        if (lane == 0) {
-            *reinterpret_cast<float2*>(&fk_smem[wst + 2 * k]) = make_float2(n1, n2);
-            if (inj_hi) { o1 = S.x; o2 = S.y; } else { E1 = S.x; E2 = S.y; }
-        }
+        if (lane == 0 && !keep) *reinterpret_cast<float2*>(&fk_smem[wst + 2 * k]) = make_float2(n1, n2);
         // S3 fix-up: y[i] += g1[i] s1 + g2[i] s2
-        const float4* G = reinterpret_cast<const float4*>(&fk_smem[To + goff]);
+        const float2 Ea = make_float2(E1, o1), Eb = make_float2(E2, o2);
 #pragma unroll
-        for (int i = 0; i < L; i += 2) {
-            const float4 gg = G[i >> 1];
-            lo[i] = fmaf(gg.x, E1, fmaf(gg.y, E2, lo[i]));
-            hi[i] = fmaf(gg.x, o1, fmaf(gg.y, o2, hi[i]));
-            lo[i + 1] = fmaf(gg.z, E1, fmaf(gg.w, E2, lo[i + 1]));
-            hi[i + 1] = fmaf(gg.z, o1, fmaf(gg.w, o2, hi[i + 1]));
-        }
+        for (int i = 0; i < L; ++i) x[i] = fma2(T.g[i][0], Ea, fma2(T.g[i][1], Eb, x[i]));
     }
 
     if (p.filt) {
-        regs_to_buf<L>(lo, hi, buf, lane);
+        regs_to_buf<L>(x, buf, lane);
         __syncwarp();
-        store_tile<L>(p, p.filt + (long long)ch * p.out_pitch, buf, lane, t0);
+        store_tile<L>(p, g, p.filt + (long long)ch * p.out_pitch, buf, lane, t0);
         __syncwarp();
     }
 
     // ---- S4..S6: energy, the two averages, ratio --------------------------------------------
-    const int AV = stab + p.n_sec * ST::stride;
-    const float as = fk_smem[AV], al = fk_smem[AV + 1];
-    float sa = 0.0f, la = 0.0f, sb = 0.0f, lb = 0.0f;       // (sta, lta) x (lo slot, hi slot) from rest
+    const float as = p.avg.alpha[0], al = p.avg.alpha[1];
+    float2 sp = make_float2(0.0f, 0.0f), lp = sp;                 // (lo slot, hi slot) from rest
 #pragma unroll
     for (int i = 0; i < L; ++i) {
-        const float ea = lo[i] * lo[i], eb = hi[i] * hi[i];
-        lo[i] = ea; hi[i] = eb;
-        sa = fmaf(as, sa, ea); la = fmaf(al, la, ea);
-        sb = fmaf(as, sb, eb); lb = fmaf(al, lb, eb);
+        const float2 e = mul2(x[i], x[i]);
+        x[i] = e;
+        sp = fma2(as, sp, e); lp = fma2(al, lp, e);
     }
     const int ks = wst + 2 * p.n_sec;
     const float2 M = *reinterpret_cast<const float2*>(&fk_smem[ks]);           // carried (sta~, lta~)
-    // carried averages into their slot: + alpha^len M = M - (1 - alpha^len) M
-    const float bLs = fk_smem[AV + kAvgBetaL], bLl = fk_smem[AV + kAvgBetaL + 1];
-    const float brs = first ? p.beta_r[0] : bLs, brl = first ? p.beta_r[1] : bLl;
-    const float is = fmaf(-brs, M.x, M.x), il = fmaf(-brl, M.y, M.y);
-    sa = fmaf(m_lo, is, sa); la = fmaf(m_lo, il, la);
-    sb = fmaf(m_hi, is, sb); lb = fmaf(m_hi, il, lb);
-    float Ws = sb + fmaf(-bLs, sa, sa), Wl = lb + fmaf(-bLl, la, la);          // alpha^L lo + hi
+    const float bLs = p.avg.betaL[0], bLl = p.avg.betaL[1];
+    float Ws = sp.y + fmaf(-bLs, sp.x, sp.x), Wl = lp.y + fmaf(-bLl, lp.x, lp.x);        // alpha^L lo + hi
+    {
+        const float Ms = lane == 0 ? M.x : 0.0f, Ml = lane == 0 ? M.y : 0.0f;
+        Ws += fmaf(-p.avg.betaQ[0][0], Ms, Ms); Wl += fmaf(-p.avg.betaQ[0][1], Ml, Ml);
+    }
 #pragma unroll
     for (int d = 0; d < kSteps; ++d) {
-        const float2 q = *reinterpret_cast<const float2*>(&fk_smem[AV + kAvgBetaQ + 2 * d]);
         float Us = __shfl_up_sync(0xffffffffu, Ws, 1 << d), Ul = __shfl_up_sync(0xffffffffu, Wl, 1 << d);
         const bool act = lane >= (1 << d);
         Us = act ? Us : 0.0f; Ul = act ? Ul : 0.0f;
-        Ws += fmaf(-q.x, Us, Us); Wl += fmaf(-q.y, Ul, Ul);
+        Ws += fmaf(-p.avg.betaQ[d][0], Us, Us); Wl += fmaf(-p.avg.betaQ[d][1], Ul, Ul);
     }
     float Es = __shfl_up_sync(0xffffffffu, Ws, 1), El = __shfl_up_sync(0xffffffffu, Wl, 1);
-    Es = lane == 0 ? 0.0f : Es; El = lane == 0 ? 0.0f : El;
-    float Os = sa + fmaf(-bLs, Es, Es), Ol = la + fmaf(-bLl, El, El);          // carry-in of the hi slot
+    if (lane == 0) { Es = M.x; El = M.y; }
+    const float Os = sp.x + fmaf(-bLs, Es, Es), Ol = lp.x + fmaf(-bLl, El, El);          // carry-in of the hi slot
     const float Ns = __shfl_sync(0xffffffffu, out_hi ? Ws : Os, jl);
     const float Nl = __shfl_sync(0xffffffffu, out_hi ? Wl : Ol, jl);
-    if (lane == 0) {
-        *reinterpret_cast<float2*>(&fk_smem[ks]) = make_float2(Ns, Nl);
-        // the short slot starts its second pass sh zeros early: M alpha^-sh decays to M on them
-        const float Mvs = first ? M.x * p.inv_sh[0] : M.x, Mvl = first ? M.y * p.inv_sh[1] : M.y;
-        if (inj_hi) { Os = Mvs; Ol = Mvl; } else { Es = Mvs; El = Mvl; }
-    }
+    if (lane == 0 && !keep) *reinterpret_cast<float2*>(&fk_smem[ks]) = make_float2(Ns, Nl);
 
     if (p.cf) {
         // warm-up (reading R10): samples whose index since create/reset is < lta_len give cf = 0
+        // (seen = samples pushed before this push; tile position e is sample seen + t0 + e of the stream)
         const long long rem = (long long)p.lta_len - (long long)seen - t0;     // first tile position with cf != 0
         const float ratio = p.ratio, thr = p.lta_thr;
-        // l~ never drops below alpha^L times its carry-in inside a slot (e >= 0); the idle slot in
-        // front of a ragged push (lo slot of lane 0) holds no sample
-        const bool live = (fmaf(-bLl, El, El) > thr || (lane == 0 && inj_hi)) && fmaf(-bLl, Ol, Ol) > thr;
+        float2 Ps = make_float2(Es, Os), Pl = make_float2(El, Ol);
+        // l~ never drops below alpha^L times its carry-in inside a slot (e >= 0)
+        const bool live = fmaf(-bLl, El, El) > thr && fmaf(-bLl, Ol, Ol) > thr;
         if (rem <= 0 && __all_sync(0xffffffffu, live)) {
 #pragma unroll
             for (int i = 0; i < L; ++i) {
-                Es = fmaf(as, Es, lo[i]); El = fmaf(al, El, lo[i]);
-                Os = fmaf(as, Os, hi[i]); Ol = fmaf(al, Ol, hi[i]);
-                lo[i] = (Es * ratio) * rcp_fast(El);
-                hi[i] = (Os * ratio) * rcp_fast(Ol);
+                Ps = fma2(as, Ps, x[i]); Pl = fma2(al, Pl, x[i]);
+                const float2 num = mul2(Ps, f2(ratio));
+                x[i].x = num.x * rcp_fast(Pl.x);
+                x[i].y = num.y * rcp_fast(Pl.y);
             }
         } else {
             const int wm = rem > (1 << 30) ? (1 << 30) : (rem < 0 ? 0 : (int)rem);
             const int base = 2 * lane * L;
 #pragma unroll
             for (int i = 0; i < L; ++i) {
-                Es = fmaf(as, Es, lo[i]); El = fmaf(al, El, lo[i]);
-                Os = fmaf(as, Os, hi[i]); Ol = fmaf(al, Ol, hi[i]);
-                const float qa = (Es * ratio) * rcp_fast(El), qb = (Os * ratio) * rcp_fast(Ol);
-                lo[i] = (El > thr && base + i >= wm) ? qa : 0.0f;
-                hi[i] = (Ol > thr && base + L + i >= wm) ? qb : 0.0f;
+                Ps = fma2(as, Ps, x[i]); Pl = fma2(al, Pl, x[i]);
+                const float qa = (Ps.x * ratio) * rcp_fast(Pl.x), qb = (Ps.y * ratio) * rcp_fast(Pl.y);
+                x[i].x = (Pl.x > thr && base + i >= wm) ? qa : 0.0f;
+                x[i].y = (Pl.y > thr && base + L + i >= wm) ? qb : 0.0f;
             }
         }
-        regs_to_buf<L>(lo, hi, buf, lane);
+        regs_to_buf<L>(x, buf, lane);
         __syncwarp();
-        store_tile<L>(p, p.cf + (long long)ch * p.out_pitch, buf, lane, t0);
+        store_tile<L>(p, g, p.cf + (long long)ch * p.out_pitch, buf, lane, t0);
     }
     __syncwarp();
 }
 
-// Warps per CTA the register file allows (one CTA per SM): 128 / 168 / 255 registers per thread.
+// Warps per CTA (one CTA per SM): bounded by shared memory (two tile buffers per warp).
 template <int L> __host__ __device__ constexpr int cm_max_warps() { return L <= 24 ? 16 : (L <= 32 ? 12 : 8); }
 
 // Channel-major push: grid <= SM count, block = W * 32 (W <= cm_max_warps<L>()); dynamic shared memory =
-// table + W * warp_smem_floats<L>() floats.
+// W * warp_smem_floats<L>() floats.
 template <int L>
 __global__ void __launch_bounds__(cm_max_warps<L>() * 32, 1)
-filark_push_cm_kernel(const __grid_constant__ PushParams p)
+filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
 {
-    const int tab_floats = p.n_sec * SecTab<L>::stride + kAvgFloats;
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, W = blockDim.x >> 5;
-    const int wbase = tab_floats + warp * warp_smem_floats<L>();      // two tile buffers, then two state copies
+    // the warp index through a shuffle: the compiler then knows that it -- and with it the channel
+    // walk, the section loop and every table index -- is warp-uniform, which is what lets the
+    // tables be read through uniform registers
+    const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
+    const int lane = threadIdx.x & 31, W = blockDim.x >> 5;
+    const int wbase = warp * warp_smem_floats<L>();                   // two tile buffers, then two state copies
     const int wst0 = wbase + 2 * Geo<L>::buf_floats;
+
+    const unsigned r0 = p.ctl->r0;
+    const unsigned long long seen = p.ctl->seen;
+    const Geom g = make_geom<L>(r0, p.n_t, p.vec4 != 0);
 
     // warp (b, w) walks the channels b + grid (w + W i)
     const int stride = gridDim.x * W;
     int ch = blockIdx.x + gridDim.x * warp, tile = 0, cur = 0, wcur = 0;
-    if (ch < p.n_ch) issue_tile_load<L>(p, ch, 0, wbase, wst0, lane, true);
-    for (int i = threadIdx.x; i < tab_floats / 4; i += blockDim.x)
-        reinterpret_cast<float4*>(fk_smem)[i] = __ldg(reinterpret_cast<const float4*>(p.tab) + i);
-    __syncthreads();
+    if (ch < p.n_ch) issue_tile_load<L>(p, g, ch, 0, wbase, wst0, lane, true);
 
     const int ns = state_floats(p.n_sec);
-    unsigned seen = 0;
     while (ch < p.n_ch) {
         int nch = ch, ntile = tile + 1;
-        if (ntile == p.n_tiles) { ntile = 0; nch = ch + stride; }
+        if (ntile == g.n_tiles) { ntile = 0; nch = ch + stride; }
         const int buf = wbase + cur * Geo<L>::buf_floats;
         const int wst = wst0 + wcur * kStateSmem;
         cp_async_wait_all();
         __syncwarp();
-        float lo[L], hi[L];
+        if (ntile == 0 && g.r1 != 0) {
+            // last tile of the channel: keep the raw samples of its trailing partial slot
+            const int e0 = g.q_last * L;                              // tile-space position of that slot
+            float* hd = p.hist + (long long)ch * kHist;
+            for (int j = lane; j < g.r1; j += 32) {
+                const int e = e0 + j;
+                hd[j] = fk_smem[buf + e + 4 * (e / (2 * L))];
+            }
+        }
+        float2 x[L];
         {
             const float4* s = reinterpret_cast<const float4*>(&fk_smem[buf + lane * Geo<L>::pitch]);
             const float gn = p.gain;
 #pragma unroll
             for (int q = 0; q < L / 4; ++q) {
                 const float4 a = s[q], b = s[L / 4 + q];
-                lo[4 * q] = a.x * gn; lo[4 * q + 1] = a.y * gn; lo[4 * q + 2] = a.z * gn; lo[4 * q + 3] = a.w * gn;
-                hi[4 * q] = b.x * gn; hi[4 * q + 1] = b.y * gn; hi[4 * q + 2] = b.z * gn; hi[4 * q + 3] = b.w * gn;
+                x[4 * q] = make_float2(a.x * gn, b.x * gn); x[4 * q + 1] = make_float2(a.y * gn, b.y * gn);
+                x[4 * q + 2] = make_float2(a.z * gn, b.z * gn); x[4 * q + 3] = make_float2(a.w * gn, b.w * gn);
             }
         }
-        if (tile == 0) seen = __float_as_uint(fk_smem[wst + ns - 2]);
         __syncwarp();
         if (nch < p.n_ch)
-            issue_tile_load<L>(p, nch, ntile, wbase + (cur ^ 1) * Geo<L>::buf_floats,
+            issue_tile_load<L>(p, g, nch, ntile, wbase + (cur ^ 1) * Geo<L>::buf_floats,
                                wst0 + (wcur ^ 1) * kStateSmem, lane, ntile == 0);
-        process_tile<L>(p, 0, buf, wst, lo, hi, ch, tile, lane, seen);
+        process_tile<L>(p, g, buf, wst, x, ch, tile, lane, seen);
         if (ntile == 0) {
-            // channel done: carried state and sample count back to global memory
-            if (lane == 0) {
-                const unsigned long long s2 = (unsigned long long)seen + (unsigned long long)p.n_t;
-                fk_smem[wst + ns - 2] = __uint_as_float(s2 > kSeenMax ? kSeenMax : (unsigned)s2);
-            }
-            __syncwarp();
+            // channel done: carried state back to global memory
             float* gst = p.state + (long long)ch * ns;
             if (lane < ns) gst[lane] = fk_smem[wst + lane];
             if (lane + 32 < ns) gst[lane + 32] = fk_smem[wst + lane + 32];
@@ -478,37 +502,53 @@ filark_push_cm_kernel(const __grid_constant__ PushParams p)
         }
         ch = nch; tile = ntile; cur ^= 1;
     }
+
+    // the last CTA to finish advances the control block (every CTA read it before it got here)
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        __threadfence();
+        const unsigned t = atomicAdd(&p.ctl->ticket, 1u);
+        if (t == gridDim.x - 1) {
+            p.ctl->r0 = (unsigned)g.r1;
+            p.ctl->seen = seen + (unsigned long long)p.n_t;
+            p.ctl->ticket = 0u;
+            __threadfence();
+        }
+    }
 }
 
 // Diagnostic kernel (FILARK_FLAG_SERIAL_SCAN; also the time-major path for now): one thread per
-// channel, serial in time, the same state-space sections and the same state contents, no blocked
-// scan.  Element (c, t) of a chunk is at c * sc + t * st; state word i of channel c is at
-// c * state_sc + i * state_sk.  tab = table of any L (only the coefficients and 1/N are read).
+// channel, serial in time, the same state-space sections, no blocked scan, no history: the
+// carried state is the state after the last sample of the push.  Element (c, t) of a chunk is
+// at c * sc + t * st; state word i of channel c is at c * state_sc + i * state_sk.
+struct SerialParams {
+    const float* in;
+    float* filt;
+    float* cf;
+    float* state;
+    long long n_t, sc_in, st_in, sc_out, st_out, state_sc, state_sk;
+    int n_ch, n_sec, lta_len;
+    float gain, ratio, lta_thr, inv_ns, inv_nl;
+    int kind[kMaxSec];
+    float c[kMaxSec][5];
+};
+
 __global__ void __launch_bounds__(128)
-filark_push_serial_kernel(const __grid_constant__ PushParams p, int sec_stride, long long sc_in,
-                          long long st_in, long long sc_out, long long st_out, long long state_sc,
-                          long long state_sk)
+filark_push_serial_kernel(const __grid_constant__ SerialParams p)
 {
-    __shared__ float coef[kMaxSec][8];
-    __shared__ float cinv[2];
-    for (int i = threadIdx.x; i < p.n_sec * 8; i += blockDim.x)
-        coef[i >> 3][i & 7] = p.tab[(i >> 3) * sec_stride + (i & 7)];
-    if (threadIdx.x < 2) cinv[threadIdx.x] = p.tab[p.n_sec * sec_stride + kAvgInvN + threadIdx.x];
-    __syncthreads();
     const int ch = blockIdx.x * blockDim.x + threadIdx.x;
     if (ch < p.n_ch) {
         float s[2 * kMaxSec + 2];
         const int nf = 2 * p.n_sec + 2;
-        for (int i = 0; i < nf; ++i) s[i] = p.state[ch * state_sc + i * state_sk];
-        const unsigned seen = __float_as_uint(p.state[ch * state_sc + nf * state_sk]);
-        const float cs = cinv[0], cl = cinv[1];
+        for (int i = 0; i < nf; ++i) s[i] = p.state[ch * p.state_sc + i * p.state_sk];
+        const unsigned seen = __float_as_uint(p.state[ch * p.state_sc + nf * p.state_sk]);
+        const float cs = p.inv_ns, cl = p.inv_nl;
         float ms = s[nf - 2], ml = s[nf - 1];
         for (long long t = 0; t < p.n_t; ++t) {
-            float v = p.in[ch * sc_in + t * st_in] * p.gain;
+            float v = p.in[ch * p.sc_in + t * p.st_in] * p.gain;
             for (int k = 0; k < p.n_sec; ++k) {
-                const float* T = coef[k];
-                const int kind = __float_as_int(T[kOffKind]);
-                const float c0 = T[1], c1 = T[2], c2 = T[3], c3 = T[4], c4 = T[5];
+                const int kind = p.kind[k];
+                const float c0 = p.c[k][0], c1 = p.c[k][1], c2 = p.c[k][2], c3 = p.c[k][3], c4 = p.c[k][4];
                 const float s1 = s[2 * k], s2 = s[2 * k + 1];
                 float y;
                 if (kind == kKindDF2 || kind == kKindDF2G) {
@@ -527,19 +567,19 @@ filark_push_serial_kernel(const __grid_constant__ PushParams p, int sec_stride, 
                 }
                 v = y;
             }
-            if (p.filt) p.filt[ch * sc_out + t * st_out] = v;
+            if (p.filt) p.filt[ch * p.sc_out + t * p.st_out] = v;
             const float e = v * v;
             ms = fmaf(-cs, ms, ms) + e;      // (1 - 1/N) m~ + e without rounding 1 - 1/N (reading R13)
             ml = fmaf(-cl, ml, ml) + e;
             if (p.cf)
-                p.cf[ch * sc_out + t * st_out] =
+                p.cf[ch * p.sc_out + t * p.st_out] =
                     (ml > p.lta_thr && (unsigned long long)seen + (unsigned long long)t >= (unsigned long long)p.lta_len)
                         ? p.ratio * __fdividef(ms, ml) : 0.0f;
         }
         s[nf - 2] = ms; s[nf - 1] = ml;
-        for (int i = 0; i < nf; ++i) p.state[ch * state_sc + i * state_sk] = s[i];
+        for (int i = 0; i < nf; ++i) p.state[ch * p.state_sc + i * p.state_sk] = s[i];
         const unsigned long long s2 = (unsigned long long)seen + (unsigned long long)p.n_t;
-        p.state[ch * state_sc + nf * state_sk] = __uint_as_float(s2 > kSeenMax ? kSeenMax : (unsigned)s2);
+        p.state[ch * p.state_sc + nf * p.state_sk] = __uint_as_float(s2 > kSeenMax ? kSeenMax : (unsigned)s2);
     }
 }
 

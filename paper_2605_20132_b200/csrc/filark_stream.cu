@@ -23,18 +23,18 @@ using namespace filark;
 static const int kVariantL[] = {8, 16, 24, 32, 48};
 constexpr int kNumVariants = 5;
 
-struct Geometry { int L, n_tiles, lead, r, pad0, last_lane, last_half; };
-
 struct filark_stream {
     int device;
     int n_ch, n_sec, sta_len, lta_len, layout;
     unsigned flags;
     Section sec[kMaxSec];
     double gain;
-    float* d_tab[kNumVariants];
-    size_t tab_floats[kNumVariants];
+    void* proto[kNumVariants];      // host PushParams<L> with every table filled; pointers patched per push
+    SerialParams serial;            // the same for the serial diagnostic kernel
     float* d_state;
     size_t state_floats;
+    float* d_hist;                  // [n_ch][kHist] raw tail of the previous push
+    Ctl* d_ctl;
     int n_sm;
     size_t smem_optin;
     int last_cuda_error;
@@ -55,136 +55,106 @@ static void put_mat(float* dst, const Mat2& m)
     dst[0] = (float)m.a; dst[1] = (float)m.b; dst[2] = (float)m.c; dst[3] = (float)m.d;
 }
 
-template <int L> static size_t variant_floats(int n_sec)
+// Everything of a push that does not depend on its buffers: tables in float64, rounded last.
+template <int L> static void build_proto(const filark_stream* h, PushParams<L>* p)
 {
-    return (size_t)n_sec * SecTab<L>::stride + kAvgFloats;
-}
-
-// Device table of sub-block length L (layout documented in filark_kernels.cuh).
-template <int L> static void build_variant_table(const filark_stream* h, float* tab)
-{
-    using ST = SecTab<L>;
-    std::memset(tab, 0, sizeof(float) * variant_floats<L>(h->n_sec));
+    std::memset(p, 0, sizeof(*p));
+    p->n_ch = h->n_ch; p->n_sec = h->n_sec; p->lta_len = h->lta_len;
+    p->gain = (float)h->gain;
+    p->ratio = (float)((double)h->lta_len / (double)h->sta_len);
+    p->lta_thr = (float)(1e-30 * (double)h->lta_len);      // lta <= 1e-30  <=>  lta~ <= 1e-30 N_l
     for (int k = 0; k < h->n_sec; ++k) {
         const Section& s = h->sec[k];
-        float* T = tab + (size_t)k * ST::stride;
-        std::memcpy(&T[kOffKind], &s.kind, sizeof(int));
-        for (int i = 0; i < 5; ++i) T[kOffCoef + i] = (float)s.coef[i];
-        put_mat(T + kOffP, mpow(s.A, L));
+        SecParams<L>& T = p->sec[k];
+        T.kind = s.kind;
+        for (int i = 0; i < 5; ++i) T.c[i] = (float)s.coef[i];
+        put_mat(T.P, mpow(s.A, L));
         Mat2 q = mpow(s.A, 2 * L);
         int nsteps = kSteps;
         for (int d = 0; d < kSteps; ++d) {
-            put_mat(T + kOffQ + 4 * d, q);
+            put_mat(T.Q[d], q);
             if (nsteps == kSteps && norm1(q) < 1e-10) nsteps = d;      // this and later steps add < 1e-10
             q = mul(q, q);
         }
-        std::memcpy(&T[kOffNSteps], &nsteps, sizeof(int));
+        T.nsteps = nsteps;
         double g[2 * L];
         fixup_rows(s, L, g);
-        for (int i = 0; i < L; ++i) {
-            T[ST::g0 + 2 * (L + i)] = (float)g[2 * i];         T[ST::g0 + 2 * (L + i) + 1] = (float)g[2 * i + 1];
-            T[ST::g1 + 2 * (L + i + 1)] = (float)g[2 * i];     T[ST::g1 + 2 * (L + i + 1) + 1] = (float)g[2 * i + 1];
-        }
-        // (row 2L of G1 would be g[L-1] shifted out of the table: it lands in the 4-float pad)
+        for (int i = 0; i < L; ++i) { T.g[i][0] = (float)g[2 * i]; T.g[i][1] = (float)g[2 * i + 1]; }
     }
-    float* AV = tab + (size_t)h->n_sec * ST::stride;
     const double cs = 1.0 / h->sta_len, cl = 1.0 / h->lta_len;
-    AV[0] = (float)(1.0 - cs); AV[1] = (float)(1.0 - cl);
-    AV[kAvgBetaL] = (float)one_minus_pow(cs, L); AV[kAvgBetaL + 1] = (float)one_minus_pow(cl, L);
+    AvgParams& a = p->avg;
+    a.alpha[0] = (float)(1.0 - cs); a.alpha[1] = (float)(1.0 - cl);
+    a.betaL[0] = (float)one_minus_pow(cs, L); a.betaL[1] = (float)one_minus_pow(cl, L);
     for (int d = 0; d < kSteps; ++d) {
         const double e = 2.0 * L * (double)(1 << d);
-        AV[kAvgBetaQ + 2 * d] = (float)one_minus_pow(cs, e);
-        AV[kAvgBetaQ + 2 * d + 1] = (float)one_minus_pow(cl, e);
+        a.betaQ[d][0] = (float)one_minus_pow(cs, e);
+        a.betaQ[d][1] = (float)one_minus_pow(cl, e);
     }
-    AV[kAvgInvN] = (float)cs; AV[kAvgInvN + 1] = (float)cl;
+    a.invN[0] = (float)cs; a.invN[1] = (float)cl;
 }
 
-// What a push needs beyond the table: powers for its first (possibly short) slot of r samples.
-static void fill_first_slot_params(const filark_stream* h, int L, int r, PushParams* p)
+static void build_serial(const filark_stream* h, SerialParams* p)
 {
-    const double cs = 1.0 / h->sta_len, cl = 1.0 / h->lta_len;
-    const int sh = L - r;
-    p->beta_r[0] = (float)one_minus_pow(cs, r); p->beta_r[1] = (float)one_minus_pow(cl, r);
-    // alpha^-sh; alpha = 0 (length-1 average) keeps no memory, any finite factor will do
-    p->inv_sh[0] = cs >= 1.0 ? (sh == 0 ? 1.0f : 0.0f) : (float)std::exp(-(double)sh * std::log1p(-cs));
-    p->inv_sh[1] = cl >= 1.0 ? (sh == 0 ? 1.0f : 0.0f) : (float)std::exp(-(double)sh * std::log1p(-cl));
-    for (int k = 0; k < h->n_sec; ++k) put_mat(&p->apow_r[k][0], mpow(h->sec[k].A, r));
+    std::memset(p, 0, sizeof(*p));
+    p->n_ch = h->n_ch; p->n_sec = h->n_sec; p->lta_len = h->lta_len;
+    p->gain = (float)h->gain;
+    p->ratio = (float)((double)h->lta_len / (double)h->sta_len);
+    p->lta_thr = (float)(1e-30 * (double)h->lta_len);
+    p->inv_ns = (float)(1.0 / h->sta_len); p->inv_nl = (float)(1.0 / h->lta_len);
+    for (int k = 0; k < h->n_sec; ++k) {
+        p->kind[k] = h->sec[k].kind;
+        for (int i = 0; i < 5; ++i) p->c[k][i] = (float)h->sec[k].coef[i];
+    }
 }
 
-static size_t variant_floats_rt(int v, int n_sec)
+static void* alloc_proto(int v, const filark_stream* h)
 {
     switch (kVariantL[v]) {
-        case 8: return variant_floats<8>(n_sec);
-        case 16: return variant_floats<16>(n_sec);
-        case 24: return variant_floats<24>(n_sec);
-        case 32: return variant_floats<32>(n_sec);
-        default: return variant_floats<48>(n_sec);
-    }
-}
-static void build_variant_rt(int v, const filark_stream* h, float* tab)
-{
-    switch (kVariantL[v]) {
-        case 8: build_variant_table<8>(h, tab); break;
-        case 16: build_variant_table<16>(h, tab); break;
-        case 24: build_variant_table<24>(h, tab); break;
-        case 32: build_variant_table<32>(h, tab); break;
-        default: build_variant_table<48>(h, tab); break;
-    }
-}
-static int sec_stride_rt(int v)
-{
-    switch (kVariantL[v]) {
-        case 8: return SecTab<8>::stride;
-        case 16: return SecTab<16>::stride;
-        case 24: return SecTab<24>::stride;
-        case 32: return SecTab<32>::stride;
-        default: return SecTab<48>::stride;
+#define FK_CASE(LL) case LL: { auto* p = (PushParams<LL>*)std::malloc(sizeof(PushParams<LL>)); if (p) build_proto<LL>(h, p); return p; }
+        FK_CASE(8) FK_CASE(16) FK_CASE(24) FK_CASE(32)
+        default: { auto* p = (PushParams<48>*)std::malloc(sizeof(PushParams<48>)); if (p) build_proto<48>(h, p); return p; }
+#undef FK_CASE
     }
 }
 
-// Slot geometry of a push of n_t >= 1 samples with sub-block length L: slots are aligned to the
-// end of the push; a short first slot (r < L) sits behind one idle slot (high half of lane 0).
-static Geometry geometry_for(long long n_t, int L)
-{
-    Geometry g{};
-    g.L = L;
-    const long long U = (n_t + L - 1) / L;                 // slots holding samples
-    g.r = (int)(n_t - (U - 1) * L);
-    g.lead = g.r < L ? 1 : 0;
-    g.pad0 = g.lead * L + (L - g.r);
-    const long long slots = U + g.lead;
-    g.n_tiles = (int)((slots + 63) / 64);
-    const int s_last = (int)((slots - 1) % 64);
-    g.last_lane = s_last >> 1; g.last_half = s_last & 1;
-    return g;
-}
-
-// Cheapest variant: a tile costs its L samples per lane-half plus a fixed part (scans, staging).
+// Cheapest variant for a push of n_t samples: a tile costs its L samples per lane-half plus a
+// fixed part (scans, staging); r0 is not known on the host, so it is taken as 0.
 static int choose_variant(long long n_t)
 {
     int best = 0; double best_cost = 1e300;
     for (int v = 0; v < kNumVariants; ++v) {
-        const Geometry g = geometry_for(n_t, kVariantL[v]);
-        const double cost = (double)g.n_tiles * (kVariantL[v] + 10.0);
+        const int L = kVariantL[v];
+        const long long slots = (n_t + L - 1) / L;
+        const double cost = (double)((slots + 63) / 64) * (L + 10.0);
         if (cost < best_cost) { best_cost = cost; best = v; }
     }
     return best;
 }
 
-// One CTA per SM; W warps per CTA as far as registers and shared memory allow; fewer, on more
-// SMs, when there are few channels.
-template <int L>
-static cudaError_t launch_cm(const filark_stream* h, const PushParams& p, cudaStream_t stream)
+static Geom geometry_rt(int L, unsigned r0, int n_t, bool vec4)
 {
-    const size_t tab_bytes = sizeof(float) * variant_floats<L>(p.n_sec);
+    switch (L) {
+        case 8: return make_geom<8>(r0, n_t, vec4);
+        case 16: return make_geom<16>(r0, n_t, vec4);
+        case 24: return make_geom<24>(r0, n_t, vec4);
+        case 32: return make_geom<32>(r0, n_t, vec4);
+        default: return make_geom<48>(r0, n_t, vec4);
+    }
+}
+
+// One CTA per SM; W warps per CTA as far as shared memory allows; fewer, on more SMs, when
+// there are few channels.
+template <int L>
+static cudaError_t launch_cm(const filark_stream* h, const PushParams<L>& p, cudaStream_t stream)
+{
     const size_t warp_bytes = sizeof(float) * (size_t)warp_smem_floats<L>();
     int W = cm_max_warps<L>();
-    const int fit = (int)((h->smem_optin - tab_bytes) / warp_bytes);
+    const int fit = (int)(h->smem_optin / warp_bytes);
     if (fit < W) W = fit;
     const int want = (p.n_ch + h->n_sm - 1) / h->n_sm;
     if (want < W) W = want;
     if (W < 1) return cudaErrorInvalidConfiguration;
-    const size_t smem = tab_bytes + (size_t)W * warp_bytes;
+    const size_t smem = (size_t)W * warp_bytes;
     static bool attr_done = false;           // per variant (template instance); idempotent
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(filark_push_cm_kernel<L>, cudaFuncAttributeMaxDynamicSharedMemorySize,
@@ -196,6 +166,17 @@ static cudaError_t launch_cm(const filark_stream* h, const PushParams& p, cudaSt
     if (grid > h->n_sm) grid = h->n_sm;
     filark_push_cm_kernel<L><<<grid, W * 32, smem, stream>>>(p);
     return cudaGetLastError();
+}
+
+template <int L>
+static cudaError_t push_variant(const filark_stream* h, int v, const float* d_in, int n_t, long long in_pitch,
+                                float* d_filt, float* d_cf, long long out_pitch, int vec4, cudaStream_t stream)
+{
+    PushParams<L> p = *(const PushParams<L>*)h->proto[v];
+    p.in = d_in; p.filt = d_filt; p.cf = d_cf;
+    p.state = h->d_state; p.hist = h->d_hist; p.ctl = h->d_ctl;
+    p.in_pitch = in_pitch; p.out_pitch = out_pitch; p.n_t = n_t; p.vec4 = vec4;
+    return launch_cm<L>(h, p, stream);
 }
 
 extern "C" {
@@ -267,21 +248,20 @@ filark_status_t filark_stream_create_ex(filark_stream_t** out, int n_ch, const d
     h->smem_optin = (size_t)optin;
     if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_state, sizeof(float) * h->state_floats);
     if (e == cudaSuccess) e = cudaMemset(h->d_state, 0, sizeof(float) * h->state_floats);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_hist, sizeof(float) * (size_t)n_ch * kHist);
+    if (e == cudaSuccess) e = cudaMemset(h->d_hist, 0, sizeof(float) * (size_t)n_ch * kHist);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_ctl, sizeof(Ctl));
+    if (e == cudaSuccess) e = cudaMemset(h->d_ctl, 0, sizeof(Ctl));
     bool host_oom = false;
+    build_serial(h, &h->serial);
     for (int v = 0; v < kNumVariants && e == cudaSuccess && !host_oom; ++v) {
-        h->tab_floats[v] = variant_floats_rt(v, n_sec);
-        float* tab = (float*)std::malloc(sizeof(float) * h->tab_floats[v]);
-        if (!tab) { host_oom = true; break; }
-        build_variant_rt(v, h, tab);
-        e = cudaMalloc((void**)&h->d_tab[v], sizeof(float) * h->tab_floats[v]);
-        if (e == cudaSuccess)
-            e = cudaMemcpy(h->d_tab[v], tab, sizeof(float) * h->tab_floats[v], cudaMemcpyHostToDevice);
-        std::free(tab);
+        h->proto[v] = alloc_proto(v, h);
+        if (!h->proto[v]) host_oom = true;
     }
     if (e != cudaSuccess || host_oom) {
         const bool oom = host_oom || e == cudaErrorMemoryAllocation;
-        for (int v = 0; v < kNumVariants; ++v) cudaFree(h->d_tab[v]);
-        cudaFree(h->d_state);
+        for (int v = 0; v < kNumVariants; ++v) std::free(h->proto[v]);
+        cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_ctl);
         delete h;
         cudaGetLastError();
         return oom ? FILARK_ERR_ALLOC : FILARK_ERR_CUDA;
@@ -301,8 +281,8 @@ filark_status_t filark_stream_destroy(filark_stream_t* h)
 {
     if (!h) return FILARK_OK;
     cudaDeviceSynchronize();
-    for (int v = 0; v < kNumVariants; ++v) cudaFree(h->d_tab[v]);
-    cudaFree(h->d_state);
+    for (int v = 0; v < kNumVariants; ++v) std::free(h->proto[v]);
+    cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_ctl);
     for (int i = 0; i < 3; ++i) cudaFree(h->d_stage[i]);
     delete h;
     return FILARK_OK;
@@ -316,6 +296,7 @@ filark_status_t filark_stream_reset(filark_stream_t* h, cudaStream_t stream)
     if (e != cudaSuccess) return cuda_fail(h, e);
     if (dev != h->device) return FILARK_ERR_DEVICE_MISMATCH;
     e = cudaMemsetAsync(h->d_state, 0, sizeof(float) * h->state_floats, stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->d_ctl, 0, sizeof(Ctl), stream);
     if (e != cudaSuccess) return cuda_fail(h, e);
     h->samples = 0;
     return FILARK_OK;
@@ -350,44 +331,31 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
     if (e != cudaSuccess) return cuda_fail(h, e);
     if (dev != h->device) return FILARK_ERR_DEVICE_MISMATCH;
 
-    PushParams p{};
-    p.in = d_in; p.filt = d_filt; p.cf = d_cf;
-    p.state = h->d_state;
-    p.n_t = n_t; p.in_pitch = in_pitch; p.out_pitch = out_pitch;
-    p.n_ch = h->n_ch; p.n_sec = h->n_sec;
-    p.lta_len = h->lta_len;
-    p.gain = (float)h->gain;
-    p.ratio = (float)((double)h->lta_len / (double)h->sta_len);
-    p.lta_thr = (float)(1e-30 * (double)h->lta_len);      // lta <= 1e-30  <=>  lta~ <= 1e-30 N_l
-    const int ns = state_floats(h->n_sec);
+    if (n_t > 0x7fff0000LL) return FILARK_ERR_INVALID_ARG;        // samples per channel of one push fit an int
 
     if ((h->flags & FILARK_FLAG_SERIAL_SCAN) || !cm) {
         // Serial diagnostic kernel; also the time-major path until the blocked time-major
         // kernel lands.
-        const long long sc_in = cm ? in_pitch : 1, st_in = cm ? 1 : in_pitch;
-        const long long sc_out = cm ? out_pitch : 1, st_out = cm ? 1 : out_pitch;
-        const long long state_sc = cm ? ns : 1, state_sk = cm ? 1 : h->n_ch;
+        const int ns = state_floats(h->n_sec);
+        SerialParams p = h->serial;
+        p.in = d_in; p.filt = d_filt; p.cf = d_cf; p.state = h->d_state; p.n_t = n_t;
+        p.sc_in = cm ? in_pitch : 1; p.st_in = cm ? 1 : in_pitch;
+        p.sc_out = cm ? out_pitch : 1; p.st_out = cm ? 1 : out_pitch;
+        p.state_sc = cm ? ns : 1; p.state_sk = cm ? 1 : h->n_ch;
         const int block = 128, grid = (h->n_ch + block - 1) / block;
-        p.tab = h->d_tab[0];
-        filark_push_serial_kernel<<<grid, block, 0, stream>>>(p, sec_stride_rt(0), sc_in, st_in, sc_out,
-                                                              st_out, state_sc, state_sk);
+        filark_push_serial_kernel<<<grid, block, 0, stream>>>(p);
         e = cudaGetLastError();
     } else {
         int v = choose_variant(n_t);
         for (int i = 0; i < kNumVariants; ++i) if (kVariantL[i] == (int)((h->flags >> 8) & 0xFF)) v = i;
-        const Geometry g = geometry_for(n_t, kVariantL[v]);
-        p.tab = h->d_tab[v];
-        p.n_tiles = g.n_tiles; p.lead = g.lead; p.r = g.r; p.pad0 = g.pad0;
-        p.last_lane = g.last_lane; p.last_half = g.last_half;
-        fill_first_slot_params(h, g.L, g.r, &p);
         const uintptr_t all = (uintptr_t)d_in | (uintptr_t)d_filt | (uintptr_t)d_cf;
-        p.vec4 = ((all & 15u) == 0 && (in_pitch & 3) == 0 && (out_pitch & 3) == 0 && (n_t & 3) == 0) ? 1 : 0;
-        switch (g.L) {
-            case 8: e = launch_cm<8>(h, p, stream); break;
-            case 16: e = launch_cm<16>(h, p, stream); break;
-            case 24: e = launch_cm<24>(h, p, stream); break;
-            case 32: e = launch_cm<32>(h, p, stream); break;
-            default: e = launch_cm<48>(h, p, stream); break;
+        const int vec4 = ((all & 15u) == 0 && (in_pitch & 3) == 0 && (out_pitch & 3) == 0 && (n_t & 3) == 0) ? 1 : 0;
+        switch (kVariantL[v]) {
+            case 8: e = push_variant<8>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, stream); break;
+            case 16: e = push_variant<16>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, stream); break;
+            case 24: e = push_variant<24>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, stream); break;
+            case 32: e = push_variant<32>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, stream); break;
+            default: e = push_variant<48>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, stream); break;
         }
     }
     if (e != cudaSuccess) return cuda_fail(h, e);
@@ -459,16 +427,15 @@ int filark_debug_design(const double* sos, int n_sec, int* kinds, double* coefs,
     return (int)FILARK_OK;
 }
 
-int filark_debug_push_geometry(long long n_t, int force_L, int* out7)
+int filark_debug_push_geometry(long long n_t, int r0, int force_L, int* out5)
 {
-    if (n_t < 1 || !out7) return (int)FILARK_ERR_INVALID_ARG;
+    if (n_t < 1 || n_t > 0x7fff0000LL || r0 < 0 || r0 >= kHist || !out5) return (int)FILARK_ERR_INVALID_ARG;
     int L = 0;
     if (force_L == 0) L = kVariantL[choose_variant(n_t)];
     else for (int v = 0; v < kNumVariants; ++v) if (kVariantL[v] == force_L) L = force_L;
     if (L == 0) return (int)FILARK_ERR_INVALID_ARG;
-    const Geometry g = geometry_for(n_t, L);
-    out7[0] = g.L; out7[1] = g.n_tiles; out7[2] = g.lead; out7[3] = g.r; out7[4] = g.pad0;
-    out7[5] = g.last_lane; out7[6] = g.last_half;
+    const Geom g = geometry_rt(L, (unsigned)r0, (int)n_t, true);
+    out5[0] = L; out5[1] = g.n_tiles; out5[2] = g.q_last; out5[3] = g.r1; out5[4] = g.vec4 ? 1 : 0;
     return (int)FILARK_OK;
 }
 

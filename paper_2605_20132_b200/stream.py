@@ -72,7 +72,7 @@ def load_library():
     lib.filark_debug_design.restype = ci
     lib.filark_debug_design.argtypes = [vp, ci, vp, vp, vp]
     lib.filark_debug_push_geometry.restype = ci
-    lib.filark_debug_push_geometry.argtypes = [ll, ci, vp]
+    lib.filark_debug_push_geometry.argtypes = [ll, ci, ci, vp]
     lib.filark_debug_block_power.restype = ci
     lib.filark_debug_block_power.argtypes = [vp, ll, vp]
     _lib = lib
@@ -199,14 +199,14 @@ def debug_design(sos):
     return kinds, coefs, float(gain.value)
 
 
-def debug_push_geometry(n_t: int, force_L: int = 0):
-    """dict(L, n_tiles, lead, r, pad0, last_lane, last_half) of a channel-major push of n_t samples."""
+def debug_push_geometry(n_t: int, r0: int = 0, force_L: int = 0):
+    """dict(L, n_tiles, q_last, r1, vec4) of a channel-major push of n_t samples behind r0 waiting ones."""
     lib = load_library()
-    out = np.zeros(7, dtype=np.int32)
-    st = lib.filark_debug_push_geometry(int(n_t), int(force_L), out.ctypes.data)
+    out = np.zeros(5, dtype=np.int32)
+    st = lib.filark_debug_push_geometry(int(n_t), int(r0), int(force_L), out.ctypes.data)
     if st != 0:
         raise FilarkError(st, "filark_debug_push_geometry")
-    return dict(zip(("L", "n_tiles", "lead", "r", "pad0", "last_lane", "last_half"), map(int, out)))
+    return dict(zip(("L", "n_tiles", "q_last", "r1", "vec4"), map(int, out)))
 
 
 def debug_block_power(sos6, e: int):
