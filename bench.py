@@ -49,6 +49,7 @@ def parse_args():
     ap.add_argument("--workload", default="cfg3")
     ap.add_argument("--mode", default="chunked", choices=["chunked", "whole"])
     ap.add_argument("--layout", default="cm", choices=["cm", "tm"])
+    ap.add_argument("--force-l", type=int, default=0, help="tuning: force the sub-block length variant")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-detail", action="store_true")
@@ -241,7 +242,7 @@ def main():
         del x
     filts = [torch.empty_like(t) for t in ins]
     cfs = [torch.empty_like(t) for t in ins]
-    stream = FilarkStream(w.n_ch, sos, w.sta_len, w.lta_len, layout)
+    stream = FilarkStream(w.n_ch, sos, w.sta_len, w.lta_len, layout, flags=args.force_l << 8)
     samples_per_step = w.n_ch * w.n_t
 
     def step():

@@ -98,7 +98,7 @@ inline DesignStatus design_section(const double* sos6, Section* out)
         s.A = { p, -q, p, 1.0 - q };
         s.B[0] = 1.0; s.B[1] = 1.0;
         s.C[0] = p - n2; s.C[1] = m - q;
-        s.coef[0] = p; s.coef[1] = -q; s.coef[2] = -n2; s.coef[3] = m;
+        s.coef[0] = p; s.coef[1] = -q; s.coef[2] = -n2; s.coef[3] = m; s.coef[4] = p - q;
     } else if (s.dist_m1 < kNearUnitCircle && disc < 0.0 && omega > 1e-7) {
         const double B1 = n1 - a1, B2 = n2 - a2;                 // DF2T input vector, D = 1
         const double sigma = -0.5 * a1;

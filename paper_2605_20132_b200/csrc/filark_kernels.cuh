@@ -52,6 +52,8 @@ struct Ctl {
     unsigned long long seen;   // samples pushed since create/reset
     unsigned int r0;           // samples waiting in `hist` (raw tail of the previous push)
     unsigned int ticket;       // CTAs that have finished the running push
+    unsigned int work;         // next unclaimed work item of the running push
+    unsigned int pad;
 };
 
 // One SOS section for sub-block length L; every member is warp-uniform and is read straight
@@ -86,6 +88,7 @@ template <int L> struct PushParams {
     float* state;            // [n_ch][state_floats]
     float* hist;             // [n_ch][kHist]
     Ctl* ctl;
+    unsigned* progress;      // [n_ch] segments of the running push completed per channel
     long long in_pitch, out_pitch;
     int n_t, n_ch, n_sec, lta_len;
     int vec4;                // 16-byte global accesses are legal (alignment, pitch, n_t % 4 == 0)
@@ -268,20 +271,23 @@ __device__ __forceinline__ void local_pass(float2 (&x)[L], const SecParams<L>& T
             x[i] = fma2(c2, s1, fma2(c3, s2, w));
             s2 = s1; s1 = w;
         }
-    } else if (KIND == kKindDelta) {
+    } else if (KIND == kKindDelta || KIND == kKindDeltaG) {
+        // u[n] = p u[n-1] - q w[n-1] + x[n] with w[n-1] = w[n-2] + u[n-1] substituted:
+        // u[n] = (p - q) u[n-1] + (x[n] - q w[n-2]), so that one FMA per sample sits on the
+        // critical path instead of three (c4 = p - q rounded from float64; 1 + a1 + a2 = q stays
+        // exact).  wl lags one sample behind the state w.
+        const float c4 = T.c[4];
+        float2 wl = s2;
 #pragma unroll
         for (int i = 0; i < L; ++i) {
-            const float2 u = fma2(c0, s1, fma2(c1, s2, x[i]));
+            const float2 t = fma2(c1, wl, x[i]);
+            wl = add2(wl, s1);
+            const float2 u = fma2(c4, s1, t);
             x[i] = fma2(c2, s1, u);
-            s2 = add2(s2, u); s1 = u;
+            if (KIND == kKindDeltaG) x[i] = fma2(c3, wl, x[i]);
+            s1 = u;
         }
-    } else if (KIND == kKindDeltaG) {
-#pragma unroll
-        for (int i = 0; i < L; ++i) {
-            const float2 u = fma2(c0, s1, fma2(c1, s2, x[i]));
-            x[i] = fma2(c3, s2, fma2(c2, s1, u));
-            s2 = add2(s2, u); s1 = u;
-        }
+        s2 = add2(wl, s1);
     } else if (KIND == kKindNormal) {
         const float nc1 = -c1;
 #pragma unroll
@@ -454,21 +460,60 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     const unsigned r0 = p.ctl->r0;
     const unsigned long long seen = p.ctl->seen;
     const Geom g = make_geom<L>(r0, p.n_t, p.vec4 != 0);
-
-    // warp (b, w) walks the channels b + grid (w + W i)
-    const int stride = gridDim.x * W;
-    int ch = blockIdx.x + gridDim.x * warp, tile = 0, cur = 0, wcur = 0;
-    if (ch < p.n_ch) issue_tile_load<L>(p, g, ch, 0, wbase, wst0, lane, true);
-
     const int ns = state_floats(p.n_sec);
-    while (ch < p.n_ch) {
-        int nch = ch, ntile = tile + 1;
-        if (ntile == g.n_tiles) { ntile = 0; nch = ch + stride; }
+
+    // Work items (segment, channel), segment-major; a segment is seg_tiles consecutive tiles of a
+    // channel, sized for about 8 items per warp; warp gw takes items gw, gw + n_warps, ...
+    // Segment s of a channel starts from the state its segment s - 1 left in global memory
+    // (`progress` says when).  That item has a lower index, every warp takes its items in
+    // rising order and all warps are resident (grid <= SM count, one CTA per SM), so the
+    // unfinished item with the lowest index can always run and the waits end.
+    const int n_warps = gridDim.x * W;
+    int seg_tiles = (int)(((long long)g.n_tiles * p.n_ch) / (8LL * n_warps));
+    seg_tiles = max(1, min(seg_tiles, g.n_tiles));
+    const int n_seg = (g.n_tiles + seg_tiles - 1) / seg_tiles;
+    const unsigned n_items = (unsigned)n_seg * (unsigned)p.n_ch;
+    unsigned item = blockIdx.x + gridDim.x * warp;
+    auto claim = [&](int& ch, int& tile, int& tend, int& seg) -> bool {
+        const unsigned it = item;
+        item += (unsigned)n_warps;
+        if (it >= n_items) return false;
+        seg = (int)(it / (unsigned)p.n_ch);
+        ch = (int)(it - (unsigned)seg * (unsigned)p.n_ch);
+        tile = seg * seg_tiles;
+        tend = min(g.n_tiles, tile + seg_tiles);
+        return true;
+    };
+
+    int ch = 0, tile = 0, tend = 0, seg = 0, cur = 0, wcur = 0;
+    bool have = claim(ch, tile, tend, seg);
+    if (have) issue_tile_load<L>(p, g, ch, tile, wbase, wst0, lane, seg == 0);
+
+    while (have) {
+        int nch = ch, ntile = tile + 1, ntend = tend, nseg = seg;
+        bool nhave = true;
+        const bool item_end = ntile == tend;
+        if (item_end) nhave = claim(nch, ntile, ntend, nseg);
         const int buf = wbase + cur * Geo<L>::buf_floats;
         const int wst = wst0 + wcur * kStateSmem;
         cp_async_wait_all();
         __syncwarp();
-        if (ntile == 0 && g.r1 != 0) {
+        if (seg > 0 && tile == seg * seg_tiles) {
+            // first tile of a later segment: wait for the segment before it, then fetch its state
+            // (every lane polls the same word and the value goes through a shuffle, so that the
+            // loop is warp-uniform for the compiler: a divergent wait loop makes it give up the
+            // uniform-register path for everything after it)
+            unsigned done;
+            do {
+                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(done) : "l"(p.progress + ch) : "memory");
+                done = __shfl_sync(0xffffffffu, done, 0);
+            } while (done < (unsigned)seg);
+            const float* gst = p.state + (long long)ch * ns;
+            if (lane < ns) fk_smem[wst + lane] = __ldcg(gst + lane);
+            if (lane + 32 < ns) fk_smem[wst + lane + 32] = __ldcg(gst + lane + 32);
+            __syncwarp();
+        }
+        if (tile == g.n_tiles - 1 && g.r1 != 0) {
             // last tile of the channel: keep the raw samples of its trailing partial slot
             const int e0 = g.q_last * L;                              // tile-space position of that slot
             float* hd = p.hist + (long long)ch * kHist;
@@ -489,18 +534,26 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
             }
         }
         __syncwarp();
-        if (nch < p.n_ch)
+        if (nhave)
             issue_tile_load<L>(p, g, nch, ntile, wbase + (cur ^ 1) * Geo<L>::buf_floats,
-                               wst0 + (wcur ^ 1) * kStateSmem, lane, ntile == 0);
+                               wst0 + (wcur ^ 1) * kStateSmem, lane, item_end && nseg == 0);
         process_tile<L>(p, g, buf, wst, x, ch, tile, lane, seen);
-        if (ntile == 0) {
-            // channel done: carried state back to global memory
+        if (item_end) {
+            // segment done: carried state back to global memory, then tell the next segment
             float* gst = p.state + (long long)ch * ns;
             if (lane < ns) gst[lane] = fk_smem[wst + lane];
             if (lane + 32 < ns) gst[lane + 32] = fk_smem[wst + lane + 32];
+            if (n_seg > 1) {
+                __syncwarp();
+                if (lane == 0) {
+                    const unsigned done = tend == g.n_tiles ? 0u : (unsigned)(seg + 1);
+                    __threadfence();
+                    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.progress + ch), "r"(done) : "memory");
+                }
+            }
             wcur ^= 1;
         }
-        ch = nch; tile = ntile; cur ^= 1;
+        ch = nch; tile = ntile; tend = ntend; seg = nseg; have = nhave; cur ^= 1;
     }
 
     // the last CTA to finish advances the control block (every CTA read it before it got here)

@@ -35,6 +35,7 @@ struct filark_stream {
     size_t state_floats;
     float* d_hist;                  // [n_ch][kHist] raw tail of the previous push
     Ctl* d_ctl;
+    unsigned* d_progress;           // [n_ch], self-resetting
     int n_sm;
     size_t smem_optin;
     int last_cuda_error;
@@ -117,16 +118,20 @@ static void* alloc_proto(int v, const filark_stream* h)
     }
 }
 
-// Cheapest variant for a push of n_t samples: a tile costs its L samples per lane-half plus a
-// fixed part (scans, staging); r0 is not known on the host, so it is taken as 0.
+// Variant for a push of n_t samples.  Measured on B200 (profiles/): L = 24 with 16 warps per SM
+// is the fastest per sample (larger L costs warps, smaller L more scans per sample), so it is
+// used unless a smaller L puts a short push into fewer lane-samples: the cost of a tile is its
+// L samples per lane-half plus a fixed part (scans, staging).  r0 is not known on the host
+// and is taken as 0.
 static int choose_variant(long long n_t)
 {
     int best = 0; double best_cost = 1e300;
     for (int v = 0; v < kNumVariants; ++v) {
         const int L = kVariantL[v];
+        if (L > 24) continue;
         const long long slots = (n_t + L - 1) / L;
         const double cost = (double)((slots + 63) / 64) * (L + 10.0);
-        if (cost < best_cost) { best_cost = cost; best = v; }
+        if (cost < best_cost * (1.0 - 1e-9) || (cost <= best_cost * (1.0 + 1e-9) && L == 24)) { best_cost = cost; best = v; }
     }
     return best;
 }
@@ -153,6 +158,10 @@ static cudaError_t launch_cm(const filark_stream* h, const PushParams<L>& p, cud
     if (fit < W) W = fit;
     const int want = (p.n_ch + h->n_sm - 1) / h->n_sm;
     if (want < W) W = want;
+    if (const char* t = std::getenv("FILARK_TUNE_WARPS")) {       // tuning experiments only
+        const int w = std::atoi(t);
+        if (w >= 1 && w <= W) W = w;
+    }
     if (W < 1) return cudaErrorInvalidConfiguration;
     const size_t smem = (size_t)W * warp_bytes;
     static bool attr_done = false;           // per variant (template instance); idempotent
@@ -174,7 +183,7 @@ static cudaError_t push_variant(const filark_stream* h, int v, const float* d_in
 {
     PushParams<L> p = *(const PushParams<L>*)h->proto[v];
     p.in = d_in; p.filt = d_filt; p.cf = d_cf;
-    p.state = h->d_state; p.hist = h->d_hist; p.ctl = h->d_ctl;
+    p.state = h->d_state; p.hist = h->d_hist; p.ctl = h->d_ctl; p.progress = h->d_progress;
     p.in_pitch = in_pitch; p.out_pitch = out_pitch; p.n_t = n_t; p.vec4 = vec4;
     return launch_cm<L>(h, p, stream);
 }
@@ -252,6 +261,8 @@ filark_status_t filark_stream_create_ex(filark_stream_t** out, int n_ch, const d
     if (e == cudaSuccess) e = cudaMemset(h->d_hist, 0, sizeof(float) * (size_t)n_ch * kHist);
     if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_ctl, sizeof(Ctl));
     if (e == cudaSuccess) e = cudaMemset(h->d_ctl, 0, sizeof(Ctl));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_progress, sizeof(unsigned) * (size_t)n_ch);
+    if (e == cudaSuccess) e = cudaMemset(h->d_progress, 0, sizeof(unsigned) * (size_t)n_ch);
     bool host_oom = false;
     build_serial(h, &h->serial);
     for (int v = 0; v < kNumVariants && e == cudaSuccess && !host_oom; ++v) {
@@ -261,7 +272,7 @@ filark_status_t filark_stream_create_ex(filark_stream_t** out, int n_ch, const d
     if (e != cudaSuccess || host_oom) {
         const bool oom = host_oom || e == cudaErrorMemoryAllocation;
         for (int v = 0; v < kNumVariants; ++v) std::free(h->proto[v]);
-        cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_ctl);
+        cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_ctl); cudaFree(h->d_progress);
         delete h;
         cudaGetLastError();
         return oom ? FILARK_ERR_ALLOC : FILARK_ERR_CUDA;
@@ -282,7 +293,7 @@ filark_status_t filark_stream_destroy(filark_stream_t* h)
     if (!h) return FILARK_OK;
     cudaDeviceSynchronize();
     for (int v = 0; v < kNumVariants; ++v) std::free(h->proto[v]);
-    cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_ctl);
+    cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_ctl); cudaFree(h->d_progress);
     for (int i = 0; i < 3; ++i) cudaFree(h->d_stage[i]);
     delete h;
     return FILARK_OK;
@@ -297,6 +308,7 @@ filark_status_t filark_stream_reset(filark_stream_t* h, cudaStream_t stream)
     if (dev != h->device) return FILARK_ERR_DEVICE_MISMATCH;
     e = cudaMemsetAsync(h->d_state, 0, sizeof(float) * h->state_floats, stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(h->d_ctl, 0, sizeof(Ctl), stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->d_progress, 0, sizeof(unsigned) * (size_t)h->n_ch, stream);
     if (e != cudaSuccess) return cuda_fail(h, e);
     h->samples = 0;
     return FILARK_OK;
