@@ -457,6 +457,21 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     const int wbase = warp * warp_smem_floats<L>();                   // two tile buffers, then two state copies
     const int wst0 = wbase + 2 * Geo<L>::buf_floats;
 
+    // Programmatic dependent launch: let the next push of the stream be scheduled as soon as SMs
+    // free up, and, before waiting for the previous push to complete, pull this warp's first rows
+    // into L2 (the input does not depend on the previous push; Ctl, state and hist do).
+    asm volatile("griddepcontrol.launch_dependents;");
+    {
+        const int ch0 = blockIdx.x + gridDim.x * warp;
+        if (ch0 < p.n_ch) {
+            const char* row = reinterpret_cast<const char*>(p.in + (long long)ch0 * p.in_pitch);
+            const int bytes = 4 * min(p.n_t, Geo<L>::tile);
+            for (int o = 128 * lane; o < bytes; o += 128 * 32)
+                asm volatile("prefetch.global.L2 [%0];" ::"l"(row + o));
+        }
+    }
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+
     const unsigned r0 = p.ctl->r0;
     const unsigned long long seen = p.ctl->seen;
     const Geom g = make_geom<L>(r0, p.n_t, p.vec4 != 0);

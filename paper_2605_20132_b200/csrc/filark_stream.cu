@@ -16,6 +16,7 @@
 #include "../../include/filark_debug.h"
 #include "design.hpp"
 #include "filark_kernels.cuh"
+#include "filark_kernels_tm.cuh"
 
 using namespace filark;
 
@@ -33,7 +34,9 @@ struct filark_stream {
     SerialParams serial;            // the same for the serial diagnostic kernel
     float* d_state;
     size_t state_floats;
-    float* d_hist;                  // [n_ch][kHist] raw tail of the previous push
+    float* d_hist;                  // raw tail of the previous push: [n_ch][kHist] (channel-major) or
+                                    // [2][kHist][n_ch] (time-major, double-buffered by push parity)
+    int tm_grid;                    // resident CTAs of the time-major kernel
     Ctl* d_ctl;
     unsigned* d_progress;           // [n_ch], self-resetting
     int n_sm;
@@ -77,7 +80,7 @@ template <int L> static void build_proto(const filark_stream* h, PushParams<L>* 
             if (nsteps == kSteps && norm1(q) < 1e-10) nsteps = d;      // this and later steps add < 1e-10
             q = mul(q, q);
         }
-        T.nsteps = nsteps;
+        T.nsteps = std::getenv("FILARK_TUNE_NOSCAN") ? 0 : nsteps;   // timing experiments only (wrong results)
         double g[2 * L];
         fixup_rows(s, L, g);
         for (int i = 0; i < L; ++i) { T.g[i][0] = (float)g[2 * i]; T.g[i][1] = (float)g[2 * i + 1]; }
@@ -173,8 +176,16 @@ static cudaError_t launch_cm(const filark_stream* h, const PushParams<L>& p, cud
     }
     int grid = (p.n_ch + W - 1) / W;
     if (grid > h->n_sm) grid = h->n_sm;
-    filark_push_cm_kernel<L><<<grid, W * 32, smem, stream>>>(p);
-    return cudaGetLastError();
+    // programmatic stream serialization: a push may be scheduled while the push before it drains
+    // (the kernel waits with griddepcontrol.wait before it touches anything that push writes)
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)(W * 32));
+    cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = std::getenv("FILARK_TUNE_PDL") ? 1 : 0;   // off: measured slower
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L>, p);
 }
 
 template <int L>
@@ -257,8 +268,8 @@ filark_status_t filark_stream_create_ex(filark_stream_t** out, int n_ch, const d
     h->smem_optin = (size_t)optin;
     if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_state, sizeof(float) * h->state_floats);
     if (e == cudaSuccess) e = cudaMemset(h->d_state, 0, sizeof(float) * h->state_floats);
-    if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_hist, sizeof(float) * (size_t)n_ch * kHist);
-    if (e == cudaSuccess) e = cudaMemset(h->d_hist, 0, sizeof(float) * (size_t)n_ch * kHist);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_hist, sizeof(float) * 2 * (size_t)n_ch * kHist);
+    if (e == cudaSuccess) e = cudaMemset(h->d_hist, 0, sizeof(float) * 2 * (size_t)n_ch * kHist);
     if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_ctl, sizeof(Ctl));
     if (e == cudaSuccess) e = cudaMemset(h->d_ctl, 0, sizeof(Ctl));
     if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_progress, sizeof(unsigned) * (size_t)n_ch);
@@ -345,9 +356,8 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
 
     if (n_t > 0x7fff0000LL) return FILARK_ERR_INVALID_ARG;        // samples per channel of one push fit an int
 
-    if ((h->flags & FILARK_FLAG_SERIAL_SCAN) || !cm) {
-        // Serial diagnostic kernel; also the time-major path until the blocked time-major
-        // kernel lands.
+    if (h->flags & FILARK_FLAG_SERIAL_SCAN) {
+        // Serial diagnostic kernel (either layout).
         const int ns = state_floats(h->n_sec);
         SerialParams p = h->serial;
         p.in = d_in; p.filt = d_filt; p.cf = d_cf; p.state = h->d_state; p.n_t = n_t;
@@ -356,6 +366,31 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
         p.state_sc = cm ? ns : 1; p.state_sk = cm ? 1 : h->n_ch;
         const int block = 128, grid = (h->n_ch + block - 1) / block;
         filark_push_serial_kernel<<<grid, block, 0, stream>>>(p);
+        e = cudaGetLastError();
+    } else if (!cm) {
+        // Time-major blocked kernel: tables of the L = kTmL variant.
+        int v = 0;
+        for (int i = 0; i < kNumVariants; ++i) if (kVariantL[i] == kTmL) v = i;
+        PushParams<kTmL> p = *(const PushParams<kTmL>*)h->proto[v];
+        p.in = d_in; p.filt = d_filt; p.cf = d_cf;
+        p.state = h->d_state; p.hist = nullptr; p.ctl = h->d_ctl; p.progress = nullptr;
+        p.in_pitch = in_pitch; p.out_pitch = out_pitch; p.n_t = (int)n_t; p.vec4 = 0;
+        TmArgs a{};
+        a.hist2 = h->d_hist; a.progress = h->d_progress;
+        const uintptr_t all = (uintptr_t)d_in | (uintptr_t)d_filt | (uintptr_t)d_cf;
+        a.vec2 = ((all & 7u) == 0 && (in_pitch & 1) == 0 && (out_pitch & 1) == 0) ? 1 : 0;
+        if (h->tm_grid == 0) {
+            int per_sm = 0;
+            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, filark_push_tm_kernel<kTmL, kTmWarps>,
+                                                              kTmWarps * 32, 0);
+            if (e != cudaSuccess) return cuda_fail(h, e);
+            if (per_sm < 1) return cuda_fail(h, cudaErrorInvalidConfiguration);
+            h->tm_grid = per_sm * h->n_sm;               // every CTA resident: the progress waits rely on it
+        }
+        const long long slots = (n_t + kHist + kTmL - 1) / kTmL;             // upper bound (r0 < kHist)
+        const long long items = ((slots + kTmWarps - 1) / kTmWarps) * ((h->n_ch + 63) / 64);
+        const int grid = (int)(items < h->tm_grid ? items : h->tm_grid);
+        filark_push_tm_kernel<kTmL, kTmWarps><<<grid, kTmWarps * 32, 0, stream>>>(p, a);
         e = cudaGetLastError();
     } else {
         int v = choose_variant(n_t);
