@@ -129,12 +129,15 @@ filark_status_t filark_stream_push_pitched(filark_stream_t *h, const float *d_in
 /*
  * filark_stream_push_host -- end-to-end variant for callers whose chunk lives in HOST memory
  * (the paper's pipeline executor hands the operator host arrays): copies the
- * dense chunk host->device into staging buffers owned by the handle, runs push, and copies
- * the requested outputs device->host, all asynchronously on `stream`.  h_in / h_filt / h_cf
- * are HOST pointers (pinned memory for true asynchrony), n_ch*n_t floats each in the handle's
- * layout; h_filt or h_cf may be NULL.  The staging buffers grow on demand: a push larger than
- * any before it synchronises `stream` and allocates (the only allocation in the push family).
- * The caller synchronises `stream` before reading the outputs.
+ * dense chunk host->device into staging buffers owned by the handle, runs push on `stream`, and
+ * copies the requested outputs device->host.  h_in / h_filt / h_cf are HOST pointers (pinned
+ * memory for true asynchrony), n_ch*n_t floats each in the handle's layout; h_filt or h_cf may
+ * be NULL.  The copies run on two streams owned by the handle (two alternating sets of staging
+ * buffers), so that the upload of a chunk overlaps the download of the one before it; `stream`
+ * is made to wait for the download, so the caller synchronises `stream` -- and nothing else --
+ * before reading the outputs or changing h_in.  The staging buffers grow on demand: a push
+ * larger than any before it synchronises and allocates (the only allocation in the push
+ * family; not capturable in a CUDA graph).
  * Errors: as push, plus ALLOC.
  */
 filark_status_t filark_stream_push_host(filark_stream_t *h, const float *h_in, long long n_t,

@@ -43,9 +43,14 @@ struct filark_stream {
     size_t smem_optin;
     int last_cuda_error;
     long long launches, samples;
-    // staging for push_host
-    float* d_stage[3];
+    // staging for push_host: two sets of (in, filt, cf) used alternately, an upload and a download
+    // stream of the handle's own, and the events that order them against the caller's stream
+    float* d_stage[2][3];
     size_t stage_elems;
+    cudaStream_t s_h2d, s_d2h;
+    cudaEvent_t ev_h2d[2], ev_kernel[2], ev_d2h[2];
+    bool host_ready, ev_pending[2];
+    unsigned host_pushes;
 };
 
 static filark_status_t cuda_fail(filark_stream* h, cudaError_t e)
@@ -305,7 +310,11 @@ filark_status_t filark_stream_destroy(filark_stream_t* h)
     cudaDeviceSynchronize();
     for (int v = 0; v < kNumVariants; ++v) std::free(h->proto[v]);
     cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_ctl); cudaFree(h->d_progress);
-    for (int i = 0; i < 3; ++i) cudaFree(h->d_stage[i]);
+    for (int j = 0; j < 2; ++j) for (int i = 0; i < 3; ++i) cudaFree(h->d_stage[j][i]);
+    if (h->host_ready) {
+        cudaStreamDestroy(h->s_h2d); cudaStreamDestroy(h->s_d2h);
+        for (int j = 0; j < 2; ++j) { cudaEventDestroy(h->ev_h2d[j]); cudaEventDestroy(h->ev_kernel[j]); cudaEventDestroy(h->ev_d2h[j]); }
+    }
     delete h;
     return FILARK_OK;
 }
@@ -427,29 +436,63 @@ filark_status_t filark_stream_push_host(filark_stream_t* h, const float* h_in, l
     if (!h_in || (!h_filt && !h_cf)) return FILARK_ERR_INVALID_ARG;
     const size_t elems = (size_t)h->n_ch * (size_t)n_t;
     cudaError_t e = cudaSuccess;
+    if (!h->host_ready) {
+        e = cudaStreamCreateWithFlags(&h->s_h2d, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&h->s_d2h, cudaStreamNonBlocking);
+        for (int j = 0; j < 2 && e == cudaSuccess; ++j) {
+            e = cudaEventCreateWithFlags(&h->ev_h2d[j], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_kernel[j], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&h->ev_d2h[j], cudaEventDisableTiming);
+        }
+        if (e != cudaSuccess) return cuda_fail(h, e);
+        h->host_ready = true;
+    }
     if (elems > h->stage_elems) {
-        cudaStreamSynchronize(stream);
-        for (int i = 0; i < 3; ++i) { cudaFree(h->d_stage[i]); h->d_stage[i] = nullptr; }
+        cudaStreamSynchronize(stream); cudaStreamSynchronize(h->s_h2d); cudaStreamSynchronize(h->s_d2h);
+        for (int j = 0; j < 2; ++j) for (int i = 0; i < 3; ++i) { cudaFree(h->d_stage[j][i]); h->d_stage[j][i] = nullptr; }
         h->stage_elems = 0;
-        for (int i = 0; i < 3 && e == cudaSuccess; ++i)
-            e = cudaMalloc((void**)&h->d_stage[i], sizeof(float) * elems);
+        for (int j = 0; j < 2; ++j)
+            for (int i = 0; i < 3 && e == cudaSuccess; ++i)
+                e = cudaMalloc((void**)&h->d_stage[j][i], sizeof(float) * elems);
         if (e != cudaSuccess) {
-            for (int i = 0; i < 3; ++i) { cudaFree(h->d_stage[i]); h->d_stage[i] = nullptr; }
+            for (int j = 0; j < 2; ++j) for (int i = 0; i < 3; ++i) { cudaFree(h->d_stage[j][i]); h->d_stage[j][i] = nullptr; }
             cudaGetLastError();
             h->last_cuda_error = (int)e;
             return e == cudaErrorMemoryAllocation ? FILARK_ERR_ALLOC : FILARK_ERR_CUDA;
         }
         h->stage_elems = elems;
+        h->ev_pending[0] = h->ev_pending[1] = false;
     }
-    e = cudaMemcpyAsync(h->d_stage[0], h_in, sizeof(float) * elems, cudaMemcpyHostToDevice, stream);
+    // Upload on the handle's upload stream, kernel on the caller's stream, download on the handle's
+    // download stream: the upload of this chunk overlaps the download of the one before it (PCIe is
+    // full duplex).  The caller's stream waits for the download at the end, so that synchronising
+    // it still means "outputs are in host memory".
+    const int j = (int)(h->host_pushes & 1u);
+    float* const* st = h->d_stage[j];
+    if (h->ev_pending[j]) {
+        // set j was last used two pushes ago: its kernel must have read the input buffer, its
+        // download must have read the output buffers
+        e = cudaStreamWaitEvent(h->s_h2d, h->ev_kernel[j], 0);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(stream, h->ev_d2h[j], 0);
+        if (e != cudaSuccess) return cuda_fail(h, e);
+    }
+    e = cudaMemcpyAsync(st[0], h_in, sizeof(float) * elems, cudaMemcpyHostToDevice, h->s_h2d);
+    if (e == cudaSuccess) e = cudaEventRecord(h->ev_h2d[j], h->s_h2d);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(stream, h->ev_h2d[j], 0);
     if (e != cudaSuccess) return cuda_fail(h, e);
-    const filark_status_t st = filark_stream_push(h, h->d_stage[0], n_t, h_filt ? h->d_stage[1] : nullptr,
-                                                  h_cf ? h->d_stage[2] : nullptr, stream);
-    if (st != FILARK_OK) return st;
-    if (h_filt) e = cudaMemcpyAsync(h_filt, h->d_stage[1], sizeof(float) * elems, cudaMemcpyDeviceToHost, stream);
+    const filark_status_t stt = filark_stream_push(h, st[0], n_t, h_filt ? st[1] : nullptr, h_cf ? st[2] : nullptr, stream);
+    if (stt != FILARK_OK) return stt;
+    e = cudaEventRecord(h->ev_kernel[j], stream);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(h->s_d2h, h->ev_kernel[j], 0);
+    if (e == cudaSuccess && h_filt)
+        e = cudaMemcpyAsync(h_filt, st[1], sizeof(float) * elems, cudaMemcpyDeviceToHost, h->s_d2h);
     if (e == cudaSuccess && h_cf)
-        e = cudaMemcpyAsync(h_cf, h->d_stage[2], sizeof(float) * elems, cudaMemcpyDeviceToHost, stream);
+        e = cudaMemcpyAsync(h_cf, st[2], sizeof(float) * elems, cudaMemcpyDeviceToHost, h->s_d2h);
+    if (e == cudaSuccess) e = cudaEventRecord(h->ev_d2h[j], h->s_d2h);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(stream, h->ev_d2h[j], 0);
     if (e != cudaSuccess) return cuda_fail(h, e);
+    h->ev_pending[j] = true;
+    h->host_pushes += 1;
     return FILARK_OK;
 }
 

@@ -199,3 +199,11 @@ def _add_moving(x, w, t0, c0, v, f, amp, sigma):
 def checksum(x: torch.Tensor) -> float:
     """Cheap content fingerprint recorded beside measurements."""
     return float(x.double().abs().sum().item())
+
+
+def channel_shard(n_ch: int, rank: int, world: int):
+    """[lo, hi) channel range of `rank` when one record is sharded over `world` GPUs: channels are
+    independent (no halo, no exchange step), so contiguous, balanced row ranges are all there is."""
+    base, extra = divmod(int(n_ch), int(world))
+    lo = rank * base + min(rank, extra)
+    return lo, lo + base + (1 if rank < extra else 0)

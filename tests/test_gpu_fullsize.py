@@ -1,0 +1,107 @@
+"""Full-size parity in the launch configuration bench.py times (BASELINE.json configs[2], cfg3:
+6,000 ch x 90,000 samples, 60 pushes of 1,500 samples, channel-major): the record is generated on
+the device, streamed through the C ABI exactly as the bench does, and SAMPLED channels are checked
+element by element against the float64 oracle, which computes those channels one by one from the
+same input rows.  Also: chunked vs whole GPU output at full size, and cfg4's shape (10,000
+channels, 1,000-sample pushes) on a shorter record."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2605_20132_b200.workloads import CHANNEL_MAJOR, TIME_MAJOR, CONFIGS, design_sos, generate, push_schedule
+from tests._util import assert_parity, run_oracle
+
+pytestmark = pytest.mark.gpu
+
+
+def _stream_record(w, x, layout=CHANNEL_MAJOR):
+    from paper_2605_20132_b200.stream import FilarkStream
+    s = FilarkStream(w.n_ch, design_sos(w), w.sta_len, w.lta_len, layout)
+    filt = torch.empty_like(x); cf = torch.empty_like(x)
+    p = 0
+    for c in push_schedule(w):
+        xin = x[:, p:p + c].contiguous()
+        f = torch.empty_like(xin); q = torch.empty_like(xin)
+        s.push(xin, f, q)
+        filt[:, p:p + c] = f; cf[:, p:p + c] = q
+        p += c
+    torch.cuda.synchronize()
+    n_launch = s.launch_count
+    return s, filt, cf, n_launch
+
+
+def test_cfg3_full_size_as_benched(cuda_device):
+    w = CONFIGS["cfg3"]
+    x = generate(w, device=cuda_device)
+    s, filt, cf, n_launch = _stream_record(w, x)
+    assert n_launch == 60
+    # sampled channels: first, last, around the persistent grid's strides, and random ones
+    rng = np.random.default_rng(11)
+    chans = sorted(set([0, 1, 147, 148, 2367, 2368, 4735, 4736, w.n_ch - 1] + rng.integers(0, w.n_ch, 23).tolist()))
+    xs = x[chans].cpu().numpy()
+    ref_f, ref_c = run_oracle(xs, design_sos(w), w.sta_len, w.lta_len)
+    r_f = assert_parity(filt[chans].cpu().numpy(), ref_f, "cfg3 full-size filt")
+    r_c = assert_parity(cf[chans].cpu().numpy(), ref_c, "cfg3 full-size cf")
+    print("cfg3 full size: filt rel-L2 %.2e max %.2e; cf rel-L2 %.2e max %.2e" % (r_f + r_c))
+    # properties that hold at any size, on every channel
+    assert torch.isfinite(filt).all() and torch.isfinite(cf).all()
+    assert (cf >= 0).all() and float(cf.max()) <= w.lta_len / w.sta_len * (1 + 1e-5)
+    assert (cf[:, :w.lta_len] == 0).all()
+    # whole-record push of the same record on the same handle after reset: same tolerance
+    s.reset()
+    f2 = torch.empty_like(x); c2 = torch.empty_like(x)
+    s.push(x, f2, c2)
+    torch.cuda.synchronize()
+    sel = chans[::3]
+    assert_parity(f2[sel].cpu().numpy(), filt[sel].cpu().numpy(), "whole vs chunked filt")
+    assert_parity(c2[sel].cpu().numpy(), cf[sel].cpu().numpy(), "whole vs chunked cf")
+    assert_parity(f2[chans].cpu().numpy(), ref_f, "cfg3 whole filt")
+    assert_parity(c2[chans].cpu().numpy(), ref_c, "cfg3 whole cf")
+    s.destroy()
+
+
+def test_cfg4_shape_small_chunks(cuda_device):
+    """10,000 channels, 1,000-sample pushes (small-chunk state carry), 20,000 samples."""
+    w = CONFIGS["cfg4"].scaled(n_ch=10_000, n_t=20_000)
+    x = generate(w, device=cuda_device)
+    s, filt, cf, n_launch = _stream_record(w, x)
+    assert n_launch == 20
+    chans = [0, 3, 4999, 9998, 9999]
+    ref_f, ref_c = run_oracle(x[chans].cpu().numpy(), design_sos(w), w.sta_len, w.lta_len)
+    assert_parity(filt[chans].cpu().numpy(), ref_f, "cfg4 filt")
+    assert_parity(cf[chans].cpu().numpy(), ref_c, "cfg4 cf")
+    s.destroy()
+
+
+def test_cfg5_random_chunks_against_whole_record_oracle(cuda_device):
+    """cfg5's filter (0.5-100 Hz, the worst-conditioned one) and its random push lengths 64..6000 on
+    a 600-channel x 300,000-sample slice; compared with the whole-record oracle."""
+    w = CONFIGS["cfg5"].scaled(n_ch=600, n_t=300_000)
+    x = generate(w, device=cuda_device)
+    s, filt, cf, _ = _stream_record(w, x)
+    chans = [0, 1, 299, 598, 599]
+    ref_f, ref_c = run_oracle(x[chans].cpu().numpy(), design_sos(w), w.sta_len, w.lta_len)
+    r_f = assert_parity(filt[chans].cpu().numpy(), ref_f, "cfg5 filt")
+    r_c = assert_parity(cf[chans].cpu().numpy(), ref_c, "cfg5 cf")
+    print("cfg5 slice: filt rel-L2 %.2e; cf rel-L2 %.2e" % (r_f[0], r_c[0]))
+    s.destroy()
+
+
+def test_time_major_full_width(cuda_device):
+    """Time-major kernel over the full 6,000-channel width (94 column blocks, odd tail block)."""
+    w = CONFIGS["cfg3"].scaled(n_ch=6000, n_t=6000)
+    x = generate(w, device=cuda_device)                      # [n_ch][n_t]
+    xt = x.t().contiguous()
+    from paper_2605_20132_b200.stream import FilarkStream
+    s = FilarkStream(w.n_ch, design_sos(w), w.sta_len, w.lta_len, TIME_MAJOR)
+    filt = torch.empty_like(xt); cf = torch.empty_like(xt)
+    p = 0
+    for c in [1500, 1499, 1, 3000]:
+        xin = xt[p:p + c].contiguous(); f = torch.empty_like(xin); q = torch.empty_like(xin)
+        s.push(xin, f, q); filt[p:p + c] = f; cf[p:p + c] = q; p += c
+    torch.cuda.synchronize()
+    chans = [0, 1, 63, 64, 65, 3001, 5998, 5999]
+    ref_f, ref_c = run_oracle(x[chans].cpu().numpy(), design_sos(w), w.sta_len, w.lta_len)
+    assert_parity(filt[:, chans].t().cpu().numpy(), ref_f, "tm filt")
+    assert_parity(cf[:, chans].t().cpu().numpy(), ref_c, "tm cf")
+    s.destroy()
