@@ -292,15 +292,18 @@ def main():
     bytes_per_launch = ALG_BYTES_PER_SAMPLE * samples_per_step / len(sched)
     ach = ALG_BYTES_PER_SAMPLE * samples_per_step / (ms_per_step * 1e-3) / 1e9 / 1.0
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")       # written from an ncu --set full capture
+    tpath = os.path.join(ROOT, "profiles", "r01_traffic.csv")    # from the ncu --set full captures (profiles/r01_traffic.md)
     try:
         with open(tpath) as f:
-            traffic = json.load(f).get(f"{w.name}_{args.mode}_{args.layout}")
+            for line in f.read().splitlines()[1:]:
+                k, v = line.split(",")
+                if k == f"{w.name}_{args.mode}_{args.layout}":
+                    traffic = float(v)
     except Exception:
         pass
     out["roofline"] = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s",
                        "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
-                       "kernel": "filark_push_cm_kernel" if layout == CHANNEL_MAJOR else "filark_push_tm_kernel",
+                       "kernel": "filark_push_cm_kernel<24>" if layout == CHANNEL_MAJOR else "filark_push_tm_kernel<16,8>",
                        "algorithmic_bytes_per_launch": bytes_per_launch,
                        "mean_launch_ms": per_launch_ms, "frac_of_nominal_8TBs": ach / HBM_NOMINAL_GBS,
                        "note": "achieved = 12 B/sample x samples per step / CUDA-event time of the step "
