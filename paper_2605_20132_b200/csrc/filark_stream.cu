@@ -39,6 +39,8 @@ struct filark_stream {
     int tm_grid;                    // resident CTAs of the time-major kernel
     Ctl* d_ctl;
     unsigned* d_progress;           // [n_ch], self-resetting
+    float4* d_tm_carry;             // time-major look-back ring [n_cb][2][kTmStages][32]
+    unsigned* d_tm_pub;             // [n_cb][32] published-tile counts, self-resetting
     int n_sm;
     size_t smem_optin;
     int last_cuda_error;
@@ -279,6 +281,13 @@ filark_status_t filark_stream_create_ex(filark_stream_t** out, int n_ch, const d
     if (e == cudaSuccess) e = cudaMemset(h->d_ctl, 0, sizeof(Ctl));
     if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_progress, sizeof(unsigned) * (size_t)n_ch);
     if (e == cudaSuccess) e = cudaMemset(h->d_progress, 0, sizeof(unsigned) * (size_t)n_ch);
+    if (layout == FILARK_LAYOUT_TIME_MAJOR) {
+        const size_t n_cb = ((size_t)n_ch + 63) / 64;
+        if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_tm_carry, sizeof(float4) * n_cb * 2 * kTmStages * 32);
+        if (e == cudaSuccess) e = cudaMemset(h->d_tm_carry, 0, sizeof(float4) * n_cb * 2 * kTmStages * 32);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_tm_pub, sizeof(unsigned) * n_cb * 32);
+        if (e == cudaSuccess) e = cudaMemset(h->d_tm_pub, 0, sizeof(unsigned) * n_cb * 32);
+    }
     bool host_oom = false;
     build_serial(h, &h->serial);
     for (int v = 0; v < kNumVariants && e == cudaSuccess && !host_oom; ++v) {
@@ -289,6 +298,7 @@ filark_status_t filark_stream_create_ex(filark_stream_t** out, int n_ch, const d
         const bool oom = host_oom || e == cudaErrorMemoryAllocation;
         for (int v = 0; v < kNumVariants; ++v) std::free(h->proto[v]);
         cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_ctl); cudaFree(h->d_progress);
+        cudaFree(h->d_tm_carry); cudaFree(h->d_tm_pub);
         delete h;
         cudaGetLastError();
         return oom ? FILARK_ERR_ALLOC : FILARK_ERR_CUDA;
@@ -310,6 +320,7 @@ filark_status_t filark_stream_destroy(filark_stream_t* h)
     cudaDeviceSynchronize();
     for (int v = 0; v < kNumVariants; ++v) std::free(h->proto[v]);
     cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_ctl); cudaFree(h->d_progress);
+    cudaFree(h->d_tm_carry); cudaFree(h->d_tm_pub);
     for (int j = 0; j < 2; ++j) for (int i = 0; i < 3; ++i) cudaFree(h->d_stage[j][i]);
     if (h->host_ready) {
         cudaStreamDestroy(h->s_h2d); cudaStreamDestroy(h->s_d2h);
@@ -329,6 +340,8 @@ filark_status_t filark_stream_reset(filark_stream_t* h, cudaStream_t stream)
     e = cudaMemsetAsync(h->d_state, 0, sizeof(float) * h->state_floats, stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(h->d_ctl, 0, sizeof(Ctl), stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(h->d_progress, 0, sizeof(unsigned) * (size_t)h->n_ch, stream);
+    if (e == cudaSuccess && h->d_tm_pub)
+        e = cudaMemsetAsync(h->d_tm_pub, 0, sizeof(unsigned) * (((size_t)h->n_ch + 63) / 64) * 32, stream);
     if (e != cudaSuccess) return cuda_fail(h, e);
     h->samples = 0;
     return FILARK_OK;
@@ -385,7 +398,7 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
         p.state = h->d_state; p.hist = nullptr; p.ctl = h->d_ctl; p.progress = nullptr;
         p.in_pitch = in_pitch; p.out_pitch = out_pitch; p.n_t = (int)n_t; p.vec4 = 0;
         TmArgs a{};
-        a.hist2 = h->d_hist; a.progress = h->d_progress;
+        a.hist2 = h->d_hist; a.carry = h->d_tm_carry; a.published = h->d_tm_pub;
         const uintptr_t all = (uintptr_t)d_in | (uintptr_t)d_filt | (uintptr_t)d_cf;
         a.vec2 = ((all & 7u) == 0 && (in_pitch & 1) == 0 && (out_pitch & 1) == 0) ? 1 : 0;
         if (h->tm_grid == 0) {
