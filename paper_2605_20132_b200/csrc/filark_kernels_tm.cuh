@@ -60,7 +60,7 @@ __device__ __forceinline__ void tm_step(const float (&P)[4], float2& e1, float2&
 }
 
 template <int L, int W>
-__global__ void __launch_bounds__(W * 32, 2)
+__global__ void __launch_bounds__(W * 32, 3)
 filark_push_tm_kernel(const __grid_constant__ PushParams<L> p, const __grid_constant__ TmArgs a)
 {
     // end states of the W slots: [0], [1] by section parity, [2] the averages (own copy: no barrier
@@ -136,13 +136,20 @@ filark_push_tm_kernel(const __grid_constant__ PushParams<L> p, const __grid_cons
 
         // ---- S0: load (history for t < 0, zeros for t >= n_t) ----------------------------------
         float2 x[L];
+        const bool inside = t0 >= 0 && t0 + L <= n_t;                // the slot lies inside the push (uniform)
+        if (inside) {
+            const float* row = p.in + (size_t)t0 * p.in_pitch;
 #pragma unroll
-        for (int i = 0; i < L; ++i) {
-            const int t = t0 + i;
-            float2 v = make_float2(0.0f, 0.0f);
-            if (t < 0) v = tm_load(hrd + (size_t)((int)r0 + t) * n_ch, c, v0, v1, hvec2);
-            else if (t < n_t) v = tm_load(p.in + (size_t)t * p.in_pitch, c, v0, v1, vec2);
-            x[i] = v;
+            for (int i = 0; i < L; ++i) x[i] = tm_load(row + (size_t)i * p.in_pitch, c, v0, v1, vec2);
+        } else {
+#pragma unroll
+            for (int i = 0; i < L; ++i) {
+                const int t = t0 + i;
+                float2 v = make_float2(0.0f, 0.0f);
+                if (t < 0) v = tm_load(hrd + (size_t)((int)r0 + t) * n_ch, c, v0, v1, hvec2);
+                else if (t < n_t) v = tm_load(p.in + (size_t)t * p.in_pitch, c, v0, v1, vec2);
+                x[i] = v;
+            }
         }
         if (slot == n_full && r1 != 0) {
             // the trailing partial slot: its raw samples wait for the next push
@@ -185,10 +192,16 @@ filark_push_tm_kernel(const __grid_constant__ PushParams<L> p, const __grid_cons
             for (int i = 0; i < L; ++i) x[i] = fma2(T.g[i][0], e1, fma2(T.g[i][1], e2, x[i]));
         }
         if (p.filt) {
+            if (inside) {
+                float* row = p.filt + (size_t)t0 * p.out_pitch;
 #pragma unroll
-            for (int i = 0; i < L; ++i) {
-                const int t = t0 + i;
-                if (t >= 0 && t < n_t) tm_store(p.filt + (size_t)t * p.out_pitch, c, v0, v1, vec2, x[i]);
+                for (int i = 0; i < L; ++i) tm_store(row + (size_t)i * p.out_pitch, c, v0, v1, vec2, x[i]);
+            } else {
+#pragma unroll
+                for (int i = 0; i < L; ++i) {
+                    const int t = t0 + i;
+                    if (t >= 0 && t < n_t) tm_store(p.filt + (size_t)t * p.out_pitch, c, v0, v1, vec2, x[i]);
+                }
             }
         }
         // ---- S4..S6: energy, the two averages, ratio --------------------------------------------
@@ -227,7 +240,7 @@ filark_push_tm_kernel(const __grid_constant__ PushParams<L> p, const __grid_cons
                 o.x = (el.x > thr && i >= wm) ? qa : 0.0f;
                 o.y = (el.y > thr && i >= wm) ? qb : 0.0f;
                 const int t = t0 + i;
-                if (t >= 0 && t < n_t) tm_store(p.cf + (size_t)t * p.out_pitch, c, v0, v1, vec2, o);
+                if (inside || (t >= 0 && t < n_t)) tm_store(p.cf + (size_t)t * p.out_pitch, c, v0, v1, vec2, o);
             }
         }
     }
