@@ -460,7 +460,6 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     // Programmatic dependent launch: let the next push of the stream be scheduled as soon as SMs
     // free up, and, before waiting for the previous push to complete, pull this warp's first rows
     // into L2 (the input does not depend on the previous push; Ctl, state and hist do).
-    asm volatile("griddepcontrol.launch_dependents;");
     {
         const int ch0 = blockIdx.x + gridDim.x * warp;
         if (ch0 < p.n_ch) {
@@ -571,6 +570,9 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         ch = nch; tile = ntile; tend = ntend; seg = nseg; have = nhave; cur ^= 1;
     }
 
+    // let the next push of the stream start launching while this one drains (it waits for our
+    // completion before it reads anything we write)
+    asm volatile("griddepcontrol.launch_dependents;");
     // the last CTA to finish advances the control block (every CTA read it before it got here)
     __syncthreads();
     if (threadIdx.x == 0) {
