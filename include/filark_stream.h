@@ -67,6 +67,9 @@ typedef enum filark_status {
 #define FILARK_FLAG_SERIAL_SCAN 1u  /* diagnostic kernel: one thread per channel, serial in time,
                                        same state-space arithmetic, no blocked scan             */
 
+#define FILARK_FLAG_STRICT_ORDER 2u /* every push waits for ALL work before it in the stream before it
+                                       touches memory (see "Ordering" at filark_stream_push)     */
+
 #define FILARK_FLAG_FORCE_L(L) ((unsigned)(L) << 8)  /* tuning/testing: use the kernel variant with
                                        sub-block length L (8, 16, 24, 32 or 48) for every push
                                        instead of the one chosen from n_t                        */
@@ -111,6 +114,16 @@ filark_status_t filark_stream_create_ex(filark_stream_t **out, int n_ch, const d
  * no allocation, and may be captured into a CUDA graph.  The caller owns all three buffers and
  * keeps them alive until the stream reaches the push.  Outputs must not alias the input or
  * each other (in-place is rejected).
+ * Ordering (channel-major layout): a push is a dependent launch of whatever precedes it in
+ * `stream` and sees all of that work completed -- with one exception that the library arranges
+ * itself: when the operation directly before it in the stream is the previous push of the SAME
+ * handle and the two pushes share no buffer (other than both reading the same input), the new
+ * push starts on the device while the previous one drains and orders itself against it channel by
+ * channel through the carried state (at most two pushes of a handle are in flight; outputs are
+ * identical either way).  Work after a push in the stream sees that push and all earlier ones
+ * completed.  A caller-written kernel between two pushes that signals programmatic launch
+ * completion early (cudaTriggerProgrammaticLaunchCompletion) must not produce the next push's
+ * input or read its output buffers; FILARK_FLAG_STRICT_ORDER removes the exception altogether.
  * Errors: INVALID_ARG (null handle/d_in, n_t < 0, both outputs NULL, aliasing), ALIGNMENT,
  * DEVICE_MISMATCH, CUDA (launch failure).
  */

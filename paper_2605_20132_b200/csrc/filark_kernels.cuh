@@ -56,6 +56,26 @@ struct Ctl {
     unsigned int pad;
 };
 
+// Control block of the channel-major kernel.  Consecutive pushes of a handle overlap on the device
+// (programmatic dependent launch, see filark_push_cm_kernel), so what a push needs to know about
+// its predecessors is double-buffered by push parity: push number e (since create/reset) reads
+// slot[e & 1]; the last of its CTAs to have read it writes slot[(e + 1) & 1] and publishes
+// epoch = e + 1 before the grid lets its dependents launch.
+struct CmSlot {
+    unsigned long long seen;   // samples pushed before this push
+    unsigned int r0;           // samples waiting in `hist`
+    unsigned int seq0;         // segments completed per channel before this push (cumulative, wraps)
+    unsigned int cum[2];       // CTAs launched by the earlier pushes of each parity (cumulative, wraps)
+};
+struct CmCtl {
+    CmSlot slot[2];
+    unsigned int epoch;        // pushes started since create/reset
+    unsigned int ticket;       // CTAs of the starting push that have read their slot
+    unsigned int exited[2];    // CTAs finished, by push parity (cumulative): push e - 2 is complete when
+                               // exited[e & 1] has reached slot[e & 1].cum[e & 1]
+};
+static_assert(sizeof(CmCtl) == 64, "the control block is read by one warp in one access");
+
 // One SOS section for sub-block length L; every member is warp-uniform and is read straight
 // from the constant bank.  Q[d] = A^(2L 2^d); g[i] = C A^i.
 template <int L> struct SecParams {
@@ -78,7 +98,8 @@ struct AvgParams {
 
 // Carried state of one channel (floats): [0, 2 n_sec) section states, then sta~, lta~, the
 // number of samples seen (serial kernel only; uint32 bits, saturating), one pad word.
-__host__ __device__ constexpr int state_floats(int n_sec) { return 2 * n_sec + 4; }
+// (padded to a multiple of four words: the state moves in 16-byte pieces)
+__host__ __device__ constexpr int state_floats(int n_sec) { return (2 * n_sec + 4 + 3) & ~3; }
 constexpr unsigned kSeenMax = 0x7fffffffu;
 
 template <int L> struct PushParams {
@@ -87,11 +108,13 @@ template <int L> struct PushParams {
     float* cf;
     float* state;            // [n_ch][state_floats]
     float* hist;             // [n_ch][kHist]
-    Ctl* ctl;
-    unsigned* progress;      // [n_ch] segments of the running push completed per channel
+    Ctl* ctl;                // time-major kernel
+    CmCtl* cctl;             // channel-major kernel
+    unsigned* progress;      // [n_ch] segments completed per channel since create/reset (cumulative, wraps)
     long long in_pitch, out_pitch;
     int n_t, n_ch, n_sec, lta_len;
     int vec4;                // 16-byte global accesses are legal (alignment, pitch, n_t % 4 == 0)
+    int wait_prior;          // wait for everything before this launch in the stream before touching memory
     float gain, ratio, lta_thr;
     AvgParams avg;
     SecParams<L> sec[kMaxSec];
@@ -127,6 +150,26 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 __device__ __forceinline__ void st_stream(float* p, float v) { __stcs(p, v); }
 __device__ __forceinline__ void st_stream4(float* p, float4 v) { __stcs(reinterpret_cast<float4*>(p), v); }
 __device__ __forceinline__ float rcp_fast(float a) { float r; asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(a)); return r; }
+__device__ __forceinline__ unsigned ld_acquire(const unsigned* p)
+{
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+// Polls of `progress` and of the control block are relaxed loads at gpu scope (served by L2, no
+// fence behind them, so that they can be issued early and consumed late).  Everything they guard
+// (state, hist, control slots) was written before a release at gpu scope and is only ever read
+// with loads that bypass L1 (cp.async.cg, ld.global.cg) issued after the poll has returned.
+__device__ __forceinline__ unsigned ld_relaxed(const unsigned* p)
+{
+    unsigned v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_release(unsigned* p, unsigned v)
+{
+    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
 __device__ __forceinline__ float2 f2(float a) { return make_float2(a, a); }
 __device__ __forceinline__ float2 fma2(float a, float2 b, float2 c) { return __ffma2_rn(make_float2(a, a), b, c); }
 __device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) { return __ffma2_rn(a, b, c); }
@@ -165,13 +208,11 @@ template <int L> __host__ __device__ constexpr int warp_smem_floats() { return 2
 // carried state into `wst`.  Tile-space position e of tile `tile` is input sample
 // t = tile 64L + e - r0; t < 0 reads hist[ch][r0 + t], t >= n_t is zero-filled.
 template <int L>
-__device__ __forceinline__ void issue_tile_load(const PushParams<L>& p, const Geom& g, int ch, int tile, int buf,
-                                                int wst, int lane, bool with_state)
+__device__ __forceinline__ void issue_tile_input(const PushParams<L>& p, const Geom& g, int ch, int tile, int buf, int lane)
 {
     const int t0 = tile * Geo<L>::tile - g.r0;
     const int n_t = p.n_t;
     const float* __restrict__ src = p.in + (long long)ch * p.in_pitch;
-    const float* __restrict__ hsrc = p.hist + (long long)ch * kHist + g.r0;     // hsrc[t] for t in [-r0, 0)
     if (g.vec4) {
         if (t0 >= 0 && t0 + Geo<L>::tile <= n_t) {                   // interior tile: no bounds
             const float* __restrict__ srct = src + t0 + 4 * lane;
@@ -185,9 +226,8 @@ __device__ __forceinline__ void issue_tile_load(const PushParams<L>& p, const Ge
             for (int m = 0; m < Geo<L>::chunks; ++m) {
                 const int c = 32 * m + lane;
                 const int t = t0 + 4 * c;
-                const float* s = t < 0 ? hsrc + t : src + t;
                 const bool ok = t < n_t;
-                cp_async16(buf + 4 * c + 4 * (c / Geo<L>::chunks), ok ? s : src, ok ? 16 : 0);
+                if (t >= 0) cp_async16(buf + 4 * c + 4 * (c / Geo<L>::chunks), ok ? src + t : src, ok ? 16 : 0);
             }
         }
     } else {
@@ -195,17 +235,29 @@ __device__ __forceinline__ void issue_tile_load(const PushParams<L>& p, const Ge
         for (int m = 0; m < 2 * L; ++m) {
             const int e = 32 * m + lane;
             const int t = t0 + e;
-            const float* s = t < 0 ? hsrc + t : src + t;
             const bool ok = t < n_t;
-            cp_async4(buf + e + 4 * (e / (2 * L)), ok ? s : src, ok ? 4 : 0);
+            if (t >= 0) cp_async4(buf + e + 4 * (e / (2 * L)), src + (ok ? t : 0), ok ? 4 : 0);
         }
     }
-    if (with_state) {
-        const int ns = state_floats(p.n_sec);
-        const float* gst = p.state + (long long)ch * ns;
-        if (lane < ns) cp_async4(wst + lane, gst + lane, 4);
-        if (lane + 32 < ns) cp_async4(wst + lane + 32, gst + lane + 32, 4);
+    cp_async_commit();
+}
+
+// S0, what the channel carries into its tile 0: the r0 raw samples waiting in `hist` (tile-space
+// positions [0, r0)) and the carried state into `wst`.  Both are rewritten by pushes that overlap
+// this one on the device: never read through L1, and only after `progress` says they are there.
+template <int L>
+__device__ __forceinline__ void issue_tile_carry(const PushParams<L>& p, const Geom& g, int ch, int buf, int wst, int lane)
+{
+    const float* __restrict__ hist = p.hist + (long long)ch * kHist;
+    if (g.vec4) {
+        const int c = lane;                                           // r0 < L: at most L / 4 <= 12 chunks
+        if (4 * c < g.r0) cp_async16(buf + 4 * c + 4 * (c / Geo<L>::chunks), hist + 4 * c, 16);
+    } else {
+        for (int e = lane; e < g.r0; e += 32) fk_smem[buf + e + 4 * (e / (2 * L))] = __ldcg(hist + e);
     }
+    const int ns = state_floats(p.n_sec);
+    const float* gst = p.state + (long long)ch * ns;
+    if (4 * lane < ns) cp_async16(wst + 4 * lane, gst + 4 * lane, 16);
     cp_async_commit();
 }
 
@@ -440,13 +492,64 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
     __syncwarp();
 }
 
-// Warps per CTA (one CTA per SM): bounded by shared memory (two tile buffers per warp).
-template <int L> __host__ __device__ constexpr int cm_max_warps() { return L <= 24 ? 16 : (L <= 32 ? 12 : 8); }
+#ifdef FK_TRACE
+// timeline instrumentation for tuning builds only (never in the product library):
+// fk_trace_buf[epoch % 16][warp of the grid < 4096][event slot < 16] = (time, tag)
+__device__ unsigned long long fk_trace_buf[16 * 4096 * 16 * 2];
+__device__ unsigned fk_trace_pos;
+__device__ __forceinline__ unsigned long long fk_now()
+{
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
+__device__ __forceinline__ void fk_trace(unsigned epoch, int gw, int lane, unsigned ev, unsigned& k, unsigned long long t)
+{
+    if (lane == 0 && k < 16 && gw < 4096) {
+        unsigned smid;
+        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
+        const size_t i = (((size_t)(epoch & 15u) * 4096 + gw) * 16 + k) * 2;
+        fk_trace_buf[i] = t;
+        fk_trace_buf[i + 1] = ((unsigned long long)epoch << 48) | ((unsigned long long)gw << 32) |
+                              ((unsigned long long)smid << 20) | ev | 0x800ull;
+    }
+    k += 1;
+}
+#define FK_TR(ev) fk_trace(tr_epoch, tr_gw, lane, ev, tr_k, fk_now())
+#else
+#define FK_TR(ev)
+#endif
 
-// Channel-major push: grid <= SM count, block = W * 32 (W <= cm_max_warps<L>()); dynamic shared memory =
+// Warps per SM (bounded by shared memory: two tile buffers per warp) and per CTA.  kCmCtasPerSm
+// CTAs share an SM so that the CTAs of the next push can move in as soon as some of this push's
+// CTAs have left, not only when the last warp of the SM is done.
+#ifndef FK_CTAS
+#define FK_CTAS 4
+#endif
+constexpr int kCmCtasPerSm = FK_CTAS;
+template <int L> __host__ __device__ constexpr int cm_max_warps() { return L <= 24 ? 16 : (L <= 32 ? 12 : 8); }
+template <int L> __host__ __device__ constexpr int cm_cta_warps() { return cm_max_warps<L>() / kCmCtasPerSm; }
+
+// Channel-major push: grid <= kCmCtasPerSm * SM count (every CTA of a push is resident once the
+// pushes before it have drained), block = W * 32 (W <= cm_cta_warps<L>()); dynamic shared memory =
 // W * warp_smem_floats<L>() floats.
+//
+// Overlap of consecutive pushes.  A push of 6,000 channels x 1,500 samples is 2.5 tiles per
+// resident warp and ~8 us of launch / first-load / drain latency that nothing inside one launch can
+// hide.  The kernel is therefore launched with programmatic stream serialization and signals
+// `launch_dependents` as soon as it has read its control slot: the CTAs of push e + 1 start on the
+// SMs as the CTAs of push e leave, and the only ordering between the two is the real one -- channel
+// c of push e + 1 starts from the state (and raw history) that push e left for channel c.
+// `progress[c]` counts the segments completed on channel c since create/reset; item (seg, c) of a
+// push whose slot says seq0 runs when progress[c] == seq0 + seg and then publishes seq0 + seg + 1
+// (release/acquire at gpu scope).  At most two pushes are in flight: push e starts only when push
+// e - 2 has completed (done[e & 1]), so the host only has to compare a push's buffers with those of
+// the push before it (p.wait_prior = 1 on a conflict, on another stream, after foreign work, or
+// with FILARK_FLAG_STRICT_ORDER: then the kernel begins with griddepcontrol.wait like any
+// dependent launch).  Every CTA ends with griddepcontrol.wait, so a push never completes before the
+// push in front of it.
 template <int L>
-__global__ void __launch_bounds__(cm_max_warps<L>() * 32, 1)
+__global__ void __launch_bounds__(cm_cta_warps<L>() * 32, kCmCtasPerSm)
 filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
 {
     // the warp index through a shuffle: the compiler then knows that it -- and with it the channel
@@ -456,38 +559,67 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     const int lane = threadIdx.x & 31, W = blockDim.x >> 5;
     const int wbase = warp * warp_smem_floats<L>();                   // two tile buffers, then two state copies
     const int wst0 = wbase + 2 * Geo<L>::buf_floats;
+    const int gw = (p.wait_prior & 2) ? (int)(blockIdx.x + gridDim.x * warp) : (int)(blockIdx.x * W + warp);   // warp index in the grid
+    __shared__ unsigned sh_ctl[16];
+    __shared__ unsigned sh_flag;
+    if (threadIdx.x == 0) sh_flag = 0u;
+#ifdef FK_TRACE
+    unsigned tr_epoch = 0, tr_k = 0;
+    const int tr_gw = blockIdx.x * (blockDim.x >> 5) + warp;
+    const unsigned long long tr_t0 = fk_now();
+#endif
 
-    // Programmatic dependent launch: let the next push of the stream be scheduled as soon as SMs
-    // free up, and, before waiting for the previous push to complete, pull this warp's first rows
-    // into L2 (the input does not depend on the previous push; Ctl, state and hist do).
-    {
-        const int ch0 = blockIdx.x + gridDim.x * warp;
-        if (ch0 < p.n_ch) {
-            const char* row = reinterpret_cast<const char*>(p.in + (long long)ch0 * p.in_pitch);
-            const int bytes = 4 * min(p.n_t, Geo<L>::tile);
-            for (int o = 128 * lane; o < bytes; o += 128 * 32)
-                asm volatile("prefetch.global.L2 [%0];" ::"l"(row + o));
-        }
+    // pull this warp's first rows into L2 while the control block is read (the input never
+    // depends on the previous push; the control block, state and hist do)
+    if (gw < p.n_ch) {
+        const char* row = reinterpret_cast<const char*>(p.in + (long long)gw * p.in_pitch);
+        const int bytes = 4 * min(p.n_t, Geo<L>::tile);
+        for (int o = 128 * lane; o < bytes; o += 128 * 32)
+            asm volatile("prefetch.global.L2 [%0];" ::"l"(row + o));
     }
-    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (p.wait_prior & 1) asm volatile("griddepcontrol.wait;" ::: "memory");
 
-    const unsigned r0 = p.ctl->r0;
-    const unsigned long long seen = p.ctl->seen;
+    // ---- control slot of this push.  Nothing changes epoch or slot[epoch & 1] between the launch of
+    // this grid (after every CTA of the previous push had taken its ticket and the last of them
+    // had published both) and the last ticket of this grid: one 64-byte read by warp 0 suffices.
+    CmCtl* const cc = p.cctl;
+    if (warp == 0) {
+        const unsigned* cw = reinterpret_cast<const unsigned*>(cc);
+        unsigned v = ld_relaxed(cw + (lane & 15));
+        const unsigned e = __shfl_sync(0xffffffffu, v, 12);
+        const unsigned par = e & 1u;
+        const unsigned need = __shfl_sync(0xffffffffu, v, 6 * par + 4 + par);     // slot[par].cum[par]
+        unsigned ex = __shfl_sync(0xffffffffu, v, 14 + par);
+        while ((int)(ex - need) < 0)                                   // push e - 2 must have completed
+            ex = __shfl_sync(0xffffffffu, ld_relaxed(&cc->exited[par]), 0);
+        if (lane < 16) sh_ctl[lane] = v;
+    }
+    __syncthreads();
+    const unsigned epoch = sh_ctl[12];
+#ifdef FK_TRACE
+    tr_epoch = epoch;
+    fk_trace(tr_epoch, tr_gw, lane, 0, tr_k, tr_t0);
+    FK_TR(1);
+#endif
+    const unsigned* sl = &sh_ctl[6 * (epoch & 1u)];
+    const unsigned long long seen = (unsigned long long)sl[0] | ((unsigned long long)sl[1] << 32);
+    const unsigned r0 = sl[2], seq0 = sl[3];
     const Geom g = make_geom<L>(r0, p.n_t, p.vec4 != 0);
     const int ns = state_floats(p.n_sec);
 
     // Work items (segment, channel), segment-major; a segment is seg_tiles consecutive tiles of a
     // channel, sized for about 8 items per warp; warp gw takes items gw, gw + n_warps, ...
     // Segment s of a channel starts from the state its segment s - 1 left in global memory
-    // (`progress` says when).  That item has a lower index, every warp takes its items in
-    // rising order and all warps are resident (grid <= SM count, one CTA per SM), so the
-    // unfinished item with the lowest index can always run and the waits end.
+    // (`progress` says when).  Within a push that item has a lower index, every warp takes its
+    // items in rising order and all warps of the push become resident (nothing an earlier push
+    // needs depends on a later one), so the unfinished item with the lowest index can always run.
     const int n_warps = gridDim.x * W;
     int seg_tiles = (int)(((long long)g.n_tiles * p.n_ch) / (8LL * n_warps));
     seg_tiles = max(1, min(seg_tiles, g.n_tiles));
     const int n_seg = (g.n_tiles + seg_tiles - 1) / seg_tiles;
     const unsigned n_items = (unsigned)n_seg * (unsigned)p.n_ch;
-    unsigned item = blockIdx.x + gridDim.x * warp;
+
+    unsigned item = (unsigned)gw;
     auto claim = [&](int& ch, int& tile, int& tend, int& seg) -> bool {
         const unsigned it = item;
         item += (unsigned)n_warps;
@@ -498,30 +630,79 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         tend = min(g.n_tiles, tile + seg_tiles);
         return true;
     };
+    // (every lane polls the same word and the value goes through a shuffle, so that the loop is
+    // warp-uniform for the compiler: a divergent wait loop makes it give up the uniform-register
+    // path for everything after it)
+    auto wait_progress = [&](int ch, unsigned need, unsigned have_val) {
+        unsigned done = __shfl_sync(0xffffffffu, have_val, 0);
+        while ((int)(done - need) < 0) done = __shfl_sync(0xffffffffu, ld_relaxed(p.progress + ch), 0);
+    };
 
     int ch = 0, tile = 0, tend = 0, seg = 0, cur = 0, wcur = 0;
+    // ---- hand the control block to the next push, then let it launch.  The ticket's round trip
+    // runs while the first rows are requested; only warp 0 waits for it, the other warps look at
+    // the flag when their first tile has arrived.
+    unsigned tk = 0;
+    if (warp == 0 && lane == 0) tk = atomicAdd(&cc->ticket, 1u);
+
     bool have = claim(ch, tile, tend, seg);
-    if (have) issue_tile_load<L>(p, g, ch, tile, wbase, wst0, lane, seg == 0);
+    unsigned pr0 = 0;
+    if (have) {
+        issue_tile_input<L>(p, g, ch, tile, wbase, lane);
+        if (seg == 0) pr0 = ld_relaxed(p.progress + ch);
+    }
+    if (warp == 0) {
+        tk = __shfl_sync(0xffffffffu, tk, 0);
+        if (lane == 0) {
+            if (tk == gridDim.x - 1) {                                // every CTA has read slot[e & 1]
+                CmSlot* nx = &cc->slot[(epoch + 1u) & 1u];
+                __stcg(&nx->seen, seen + (unsigned long long)p.n_t);
+                __stcg(&nx->r0, (unsigned)g.r1);
+                __stcg(&nx->seq0, seq0 + (unsigned)n_seg);
+                __stcg(&nx->cum[epoch & 1u], sl[4 + (epoch & 1u)] + gridDim.x);
+                __stcg(&nx->cum[(epoch & 1u) ^ 1u], sl[4 + ((epoch & 1u) ^ 1u)]);
+                __stcg(&cc->ticket, 0u);
+                st_release(&cc->epoch, epoch + 1u);
+                __threadfence();
+            }
+            *reinterpret_cast<volatile unsigned*>(&sh_flag) = 1u;
+        }
+    }
+    // the first segment of a channel needs what the previous push left (state, hist): wait before
+    // those loads are issued (a wait on an EARLIER push cannot be part of a cycle)
+    if (have && seg == 0) {
+        wait_progress(ch, seq0, pr0);
+        issue_tile_carry<L>(p, g, ch, wbase, wst0, lane);
+    }
+    if (have) cp_async_wait_all();
+    {
+        unsigned f;
+        do f = __shfl_sync(0xffffffffu, *reinterpret_cast<volatile unsigned*>(&sh_flag), 0); while (f == 0u);
+    }
+    asm volatile("griddepcontrol.launch_dependents;");
+    FK_TR(2);
 
     while (have) {
         int nch = ch, ntile = tile + 1, ntend = tend, nseg = seg;
         bool nhave = true;
         const bool item_end = ntile == tend;
-        if (item_end) nhave = claim(nch, ntile, ntend, nseg);
+        unsigned npr = 0;
+        if (item_end) {
+            nhave = claim(nch, ntile, ntend, nseg);
+#ifndef FK_NO_EARLY_POLL
+            if (nhave && nseg == 0) npr = ld_relaxed(p.progress + nch);      // used after the tile is in registers
+#else
+            npr = seq0 - 1u;
+#endif
+        }
         const int buf = wbase + cur * Geo<L>::buf_floats;
         const int wst = wst0 + wcur * kStateSmem;
         cp_async_wait_all();
         __syncwarp();
+        FK_TR(3);
         if (seg > 0 && tile == seg * seg_tiles) {
             // first tile of a later segment: wait for the segment before it, then fetch its state
-            // (every lane polls the same word and the value goes through a shuffle, so that the
-            // loop is warp-uniform for the compiler: a divergent wait loop makes it give up the
-            // uniform-register path for everything after it)
-            unsigned done;
-            do {
-                asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(done) : "l"(p.progress + ch) : "memory");
-                done = __shfl_sync(0xffffffffu, done, 0);
-            } while (done < (unsigned)seg);
+            wait_progress(ch, seq0 + (unsigned)seg, ld_relaxed(p.progress + ch));
             const float* gst = p.state + (long long)ch * ns;
             if (lane < ns) fk_smem[wst + lane] = __ldcg(gst + lane);
             if (lane + 32 < ns) fk_smem[wst + lane + 32] = __ldcg(gst + lane + 32);
@@ -548,43 +729,37 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
             }
         }
         __syncwarp();
-        if (nhave)
-            issue_tile_load<L>(p, g, nch, ntile, wbase + (cur ^ 1) * Geo<L>::buf_floats,
-                               wst0 + (wcur ^ 1) * kStateSmem, lane, item_end && nseg == 0);
-        process_tile<L>(p, g, buf, wst, x, ch, tile, lane, seen);
-        if (item_end) {
-            // segment done: carried state back to global memory, then tell the next segment
-            float* gst = p.state + (long long)ch * ns;
-            if (lane < ns) gst[lane] = fk_smem[wst + lane];
-            if (lane + 32 < ns) gst[lane + 32] = fk_smem[wst + lane + 32];
-            if (n_seg > 1) {
-                __syncwarp();
-                if (lane == 0) {
-                    const unsigned done = tend == g.n_tiles ? 0u : (unsigned)(seg + 1);
-                    __threadfence();
-                    asm volatile("st.release.gpu.global.u32 [%0], %1;" ::"l"(p.progress + ch), "r"(done) : "memory");
-                }
+        if (nhave) {
+            const int nbuf = wbase + (cur ^ 1) * Geo<L>::buf_floats;
+            issue_tile_input<L>(p, g, nch, ntile, nbuf, lane);
+            if (item_end && nseg == 0) {
+                wait_progress(nch, seq0, npr);
+                issue_tile_carry<L>(p, g, nch, nbuf, wst0 + (wcur ^ 1) * kStateSmem, lane);
             }
+        }
+        process_tile<L>(p, g, buf, wst, x, ch, tile, lane, seen);
+        FK_TR(4);
+        if (item_end) {
+            // segment done: carried state back to global memory, then tell whoever continues the channel
+            // (the next segment of this push or the first segment of the next push)
+            float* gst = p.state + (long long)ch * ns;
+            if (lane < ns) __stcg(gst + lane, fk_smem[wst + lane]);
+            if (lane + 32 < ns) __stcg(gst + lane + 32, fk_smem[wst + lane + 32]);
+            __syncwarp();
+            if (lane == 0) st_release(p.progress + ch, seq0 + (unsigned)seg + 1u);
             wcur ^= 1;
         }
         ch = nch; tile = ntile; tend = ntend; seg = nseg; have = nhave; cur ^= 1;
     }
 
-    // let the next push of the stream start launching while this one drains (it waits for our
-    // completion before it reads anything we write)
-    asm volatile("griddepcontrol.launch_dependents;");
-    // the last CTA to finish advances the control block (every CTA read it before it got here)
+    FK_TR(5);
+    // completion: count this CTA out (push e + 2 waits until all of them are)
     __syncthreads();
-    if (threadIdx.x == 0) {
-        __threadfence();
-        const unsigned t = atomicAdd(&p.ctl->ticket, 1u);
-        if (t == gridDim.x - 1) {
-            p.ctl->r0 = (unsigned)g.r1;
-            p.ctl->seen = seen + (unsigned long long)p.n_t;
-            p.ctl->ticket = 0u;
-            __threadfence();
-        }
-    }
+    if (threadIdx.x == 0)
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(&cc->exited[epoch & 1u]) : "memory");
+    // a push never completes before the push in front of it
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    FK_TR(6);
 }
 
 // Diagnostic kernel (FILARK_FLAG_SERIAL_SCAN; also the time-major path for now): one thread per

@@ -10,7 +10,9 @@
 #include <cstdint>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
+#include <unordered_map>
 
 #include "../../include/filark_stream.h"
 #include "../../include/filark_debug.h"
@@ -38,7 +40,13 @@ struct filark_stream {
                                     // [2][kHist][n_ch] (time-major, double-buffered by push parity)
     int tm_grid;                    // resident CTAs of the time-major kernel
     Ctl* d_ctl;
-    unsigned* d_progress;           // [n_ch], self-resetting
+    CmCtl* d_cctl;                  // channel-major kernel: double-buffered control slots (filark_kernels.cuh)
+    unsigned* d_progress;           // [n_ch] segments completed per channel (cumulative)
+    // what the previous channel-major push touched: a push may overlap the one before it on the
+    // device only if it follows it directly in the same stream and their buffers are disjoint
+    bool prev_valid;
+    cudaStream_t prev_stream;
+    uintptr_t prev_lo[3], prev_hi[3];
     float4* d_tm_carry;             // time-major look-back ring [n_cb][2][kTmStages][32]
     unsigned* d_tm_pub;             // [n_cb][32] published-tile counts, self-resetting
     int n_sm;
@@ -54,6 +62,29 @@ struct filark_stream {
     bool host_ready, ev_pending[2];
     unsigned host_pushes;
 };
+
+// Last handle that launched on a stream (process-wide): a push that follows ANOTHER handle's push
+// in the same stream must not start early either (its input may be that push's output).
+static std::mutex g_reg_mutex;
+static std::unordered_map<cudaStream_t, const filark_stream*> g_last_on_stream;
+
+static bool registry_is_last(cudaStream_t s, const filark_stream* h)
+{
+    std::lock_guard<std::mutex> lock(g_reg_mutex);
+    auto it = g_last_on_stream.find(s);
+    return it != g_last_on_stream.end() && it->second == h;
+}
+static void registry_set(cudaStream_t s, const filark_stream* h)
+{
+    std::lock_guard<std::mutex> lock(g_reg_mutex);
+    g_last_on_stream[s] = h;
+}
+static void registry_forget(const filark_stream* h)
+{
+    std::lock_guard<std::mutex> lock(g_reg_mutex);
+    for (auto it = g_last_on_stream.begin(); it != g_last_on_stream.end();)
+        it = it->second == h ? g_last_on_stream.erase(it) : ++it;
+}
 
 static filark_status_t cuda_fail(filark_stream* h, cudaError_t e)
 {
@@ -157,15 +188,17 @@ static Geom geometry_rt(int L, unsigned r0, int n_t, bool vec4)
     }
 }
 
-// One CTA per SM; W warps per CTA as far as shared memory allows; fewer, on more SMs, when
-// there are few channels.
+// kCmCtasPerSm CTAs per SM, W warps per CTA; fewer warps per CTA, on more SMs, when there are few
+// channels.  Every CTA of a push fits on the device at once (the segment waits rely on it).
 template <int L>
 static cudaError_t launch_cm(const filark_stream* h, const PushParams<L>& p, cudaStream_t stream)
 {
     const size_t warp_bytes = sizeof(float) * (size_t)warp_smem_floats<L>();
-    int W = cm_max_warps<L>();
-    const int fit = (int)(h->smem_optin / warp_bytes);
-    if (fit < W) W = fit;
+    int per_sm = cm_max_warps<L>();                      // warps per SM
+    const int fit = (int)((h->smem_optin - 64) / warp_bytes);
+    if (fit < per_sm) per_sm = fit;
+    int W = cm_cta_warps<L>();
+    if (W > per_sm) W = per_sm;
     const int want = (p.n_ch + h->n_sm - 1) / h->n_sm;
     if (want < W) W = want;
     if (const char* t = std::getenv("FILARK_TUNE_WARPS")) {       // tuning experiments only
@@ -177,15 +210,16 @@ static cudaError_t launch_cm(const filark_stream* h, const PushParams<L>& p, cud
     static bool attr_done = false;           // per variant (template instance); idempotent
     if (!attr_done) {
         cudaError_t e = cudaFuncSetAttribute(filark_push_cm_kernel<L>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)h->smem_optin);
+                                             (int)((size_t)cm_cta_warps<L>() * warp_bytes));
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
     int grid = (p.n_ch + W - 1) / W;
-    if (grid > h->n_sm) grid = h->n_sm;
-    // programmatic stream serialization: the kernel triggers its dependents when its work loop is
-    // done, so the next push of the stream is launched while this one drains (+4.5 % on 1,500-sample
-    // pushes); the next kernel waits with griddepcontrol.wait before it touches anything we write
+    const int resident = h->n_sm * (per_sm / W < 16 ? per_sm / W : 16);
+    if (grid > resident) grid = resident;
+    // programmatic stream serialization: the kernel lets its dependents launch as soon as it has read
+    // its control slot, and orders itself against the previous push channel by channel
+    // (filark_kernels.cuh); p.wait_prior = 1 makes it an ordinary dependent launch
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)(W * 32));
     cfg.dynamicSmemBytes = smem; cfg.stream = stream;
@@ -193,17 +227,20 @@ static cudaError_t launch_cm(const filark_stream* h, const PushParams<L>& p, cud
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = std::getenv("FILARK_TUNE_NOPDL") ? 0 : 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
+    if (std::getenv("FILARK_TUNE_CARVE")) cudaFuncSetAttribute(filark_push_cm_kernel<L>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
     return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L>, p);
 }
 
 template <int L>
 static cudaError_t push_variant(const filark_stream* h, int v, const float* d_in, int n_t, long long in_pitch,
-                                float* d_filt, float* d_cf, long long out_pitch, int vec4, cudaStream_t stream)
+                                float* d_filt, float* d_cf, long long out_pitch, int vec4, int wait_prior,
+                                cudaStream_t stream)
 {
     PushParams<L> p = *(const PushParams<L>*)h->proto[v];
     p.in = d_in; p.filt = d_filt; p.cf = d_cf;
-    p.state = h->d_state; p.hist = h->d_hist; p.ctl = h->d_ctl; p.progress = h->d_progress;
+    p.state = h->d_state; p.hist = h->d_hist; p.ctl = h->d_ctl; p.cctl = h->d_cctl; p.progress = h->d_progress;
     p.in_pitch = in_pitch; p.out_pitch = out_pitch; p.n_t = n_t; p.vec4 = vec4;
+    p.wait_prior = wait_prior | (std::getenv("FILARK_TUNE_MAP") ? 2 : 0);
     return launch_cm<L>(h, p, stream);
 }
 
@@ -247,7 +284,7 @@ static filark_status_t check_create_args(const void* out, int n_ch, const double
     if (!out || !sos || n_ch <= 0 || n_sec <= 0 || n_sec > FILARK_MAX_SECTIONS) return FILARK_ERR_INVALID_ARG;
     if (sta_len < 1 || lta_len < sta_len) return FILARK_ERR_INVALID_ARG;
     if (layout != FILARK_LAYOUT_CHANNEL_MAJOR && layout != FILARK_LAYOUT_TIME_MAJOR) return FILARK_ERR_INVALID_ARG;
-    if (flags & ~(FILARK_FLAG_SERIAL_SCAN | 0xFF00u)) return FILARK_ERR_INVALID_ARG;
+    if (flags & ~(FILARK_FLAG_SERIAL_SCAN | FILARK_FLAG_STRICT_ORDER | 0xFF00u)) return FILARK_ERR_INVALID_ARG;
     if (flags & 0xFF00u) {
         bool ok = false;
         for (int v = 0; v < kNumVariants; ++v) ok = ok || kVariantL[v] == (int)((flags >> 8) & 0xFF);
@@ -280,6 +317,8 @@ filark_status_t filark_stream_create_ex(filark_stream_t** out, int n_ch, const d
     if (e == cudaSuccess) e = cudaMemset(h->d_hist, 0, sizeof(float) * 2 * (size_t)n_ch * kHist);
     if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_ctl, sizeof(Ctl));
     if (e == cudaSuccess) e = cudaMemset(h->d_ctl, 0, sizeof(Ctl));
+    if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_cctl, sizeof(CmCtl));
+    if (e == cudaSuccess) e = cudaMemset(h->d_cctl, 0, sizeof(CmCtl));
     if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_progress, sizeof(unsigned) * (size_t)n_ch);
     if (e == cudaSuccess) e = cudaMemset(h->d_progress, 0, sizeof(unsigned) * (size_t)n_ch);
     if (layout == FILARK_LAYOUT_TIME_MAJOR) {
@@ -298,7 +337,7 @@ filark_status_t filark_stream_create_ex(filark_stream_t** out, int n_ch, const d
     if (e != cudaSuccess || host_oom) {
         const bool oom = host_oom || e == cudaErrorMemoryAllocation;
         for (int v = 0; v < kNumVariants; ++v) std::free(h->proto[v]);
-        cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_ctl); cudaFree(h->d_progress);
+        cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_ctl); cudaFree(h->d_cctl); cudaFree(h->d_progress);
         cudaFree(h->d_tm_carry); cudaFree(h->d_tm_pub);
         delete h;
         cudaGetLastError();
@@ -318,9 +357,10 @@ filark_status_t filark_stream_create(filark_stream_t** out, int n_ch, const doub
 filark_status_t filark_stream_destroy(filark_stream_t* h)
 {
     if (!h) return FILARK_OK;
+    registry_forget(h);
     cudaDeviceSynchronize();
     for (int v = 0; v < kNumVariants; ++v) std::free(h->proto[v]);
-    cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_ctl); cudaFree(h->d_progress);
+    cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_ctl); cudaFree(h->d_cctl); cudaFree(h->d_progress);
     cudaFree(h->d_tm_carry); cudaFree(h->d_tm_pub);
     for (int j = 0; j < 2; ++j) for (int i = 0; i < 3; ++i) cudaFree(h->d_stage[j][i]);
     if (h->host_ready) {
@@ -340,6 +380,8 @@ filark_status_t filark_stream_reset(filark_stream_t* h, cudaStream_t stream)
     if (dev != h->device) return FILARK_ERR_DEVICE_MISMATCH;
     e = cudaMemsetAsync(h->d_state, 0, sizeof(float) * h->state_floats, stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(h->d_ctl, 0, sizeof(Ctl), stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(h->d_cctl, 0, sizeof(CmCtl), stream);
+    h->prev_valid = false;
     if (e == cudaSuccess) e = cudaMemsetAsync(h->d_progress, 0, sizeof(unsigned) * (size_t)h->n_ch, stream);
     if (e == cudaSuccess && h->d_tm_pub)
         e = cudaMemsetAsync(h->d_tm_pub, 0, sizeof(unsigned) * (((size_t)h->n_ch + 63) / 64) * 32, stream);
@@ -420,14 +462,35 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
         for (int i = 0; i < kNumVariants; ++i) if (kVariantL[i] == (int)((h->flags >> 8) & 0xFF)) v = i;
         const uintptr_t all = (uintptr_t)d_in | (uintptr_t)d_filt | (uintptr_t)d_cf;
         const int vec4 = ((all & 15u) == 0 && (in_pitch & 3) == 0 && (out_pitch & 3) == 0 && (n_t & 3) == 0) ? 1 : 0;
+        // May this push overlap the one before it?  Only if that was this handle's own push, directly
+        // before it in the same stream as far as this library launched anything, and the two share no
+        // buffer (filark_stream.h, "Ordering").
+        const uintptr_t lo[3] = {(uintptr_t)d_in, (uintptr_t)d_filt, (uintptr_t)d_cf};
+        const uintptr_t hi[3] = {lo[0] + in_bytes, d_filt ? lo[1] + out_bytes : 0, d_cf ? lo[2] + out_bytes : 0};
+        int wait_prior = 1;
+        if (!(h->flags & FILARK_FLAG_STRICT_ORDER) && h->prev_valid && h->prev_stream == stream &&
+            registry_is_last(stream, h)) {
+            bool clash = false;
+            for (int i = 0; i < 3; ++i)
+                for (int j = 0; j < 3; ++j)
+                    if ((i > 0 || j > 0) && hi[i] && h->prev_hi[j] && lo[i] < h->prev_hi[j] && h->prev_lo[j] < hi[i])
+                        clash = true;
+            wait_prior = clash ? 1 : 0;
+        }
+        h->prev_valid = false;
         switch (kVariantL[v]) {
-            case 8: e = push_variant<8>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, stream); break;
-            case 16: e = push_variant<16>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, stream); break;
-            case 24: e = push_variant<24>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, stream); break;
-            case 32: e = push_variant<32>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, stream); break;
-            default: e = push_variant<48>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, stream); break;
+            case 8: e = push_variant<8>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, wait_prior, stream); break;
+            case 16: e = push_variant<16>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, wait_prior, stream); break;
+            case 24: e = push_variant<24>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, wait_prior, stream); break;
+            case 32: e = push_variant<32>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, wait_prior, stream); break;
+            default: e = push_variant<48>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, wait_prior, stream); break;
+        }
+        if (e == cudaSuccess) {
+            h->prev_valid = true; h->prev_stream = stream;
+            for (int i = 0; i < 3; ++i) { h->prev_lo[i] = lo[i]; h->prev_hi[i] = hi[i]; }
         }
     }
+    registry_set(stream, h);
     if (e != cudaSuccess) return cuda_fail(h, e);
     h->launches += 1;
     h->samples += n_t;
@@ -509,6 +572,17 @@ filark_status_t filark_stream_push_host(filark_stream_t* h, const float* h_in, l
     h->host_pushes += 1;
     return FILARK_OK;
 }
+
+#ifdef FK_TRACE
+int filark_trace_read(unsigned long long* out, unsigned max_words, int reset)
+{
+    const unsigned n = 16u * 4096u * 16u * 2u;
+    cudaDeviceSynchronize();
+    if (out && max_words >= n) cudaMemcpyFromSymbol(out, fk_trace_buf, sizeof(unsigned long long) * n);
+    if (reset) { void* d = nullptr; cudaGetSymbolAddress(&d, fk_trace_buf); cudaMemset(d, 0, sizeof(unsigned long long) * n); }
+    return (int)n;
+}
+#endif
 
 // ---- debug / introspection (include/filark_debug.h): host only, no CUDA calls -----------------
 int filark_debug_design(const double* sos, int n_sec, int* kinds, double* coefs, double* gain)
