@@ -61,20 +61,24 @@ struct Ctl {
 // its predecessors is double-buffered by push parity: push number e (since create/reset) reads
 // slot[e & 1]; the last of its CTAs to have read it writes slot[(e + 1) & 1] and publishes
 // epoch = e + 1 before the grid lets its dependents launch.
+constexpr int kCmDepth = 3;        // pushes of a handle in flight at most
 struct CmSlot {
     unsigned long long seen;   // samples pushed before this push
     unsigned int r0;           // samples waiting in `hist`
     unsigned int seq0;         // segments completed per channel before this push (cumulative, wraps)
-    unsigned int cum[2];       // CTAs launched by the earlier pushes of each parity (cumulative, wraps)
+    unsigned int cum[kCmDepth];    // CTAs launched by the earlier pushes e' with e' % kCmDepth == j (cumulative, wraps)
+    unsigned int pad;
 };
 struct CmCtl {
-    CmSlot slot[2];
-    unsigned int epoch;        // pushes started since create/reset
-    unsigned int ticket;       // CTAs of the starting push that have read their slot
-    unsigned int exited[2];    // CTAs finished, by push parity (cumulative): push e - 2 is complete when
-                               // exited[e & 1] has reached slot[e & 1].cum[e & 1]
+    CmSlot slot[2];            // words 0..7, 8..15
+    unsigned int epoch;        // word 16: pushes started since create/reset
+    unsigned int ticket;       // word 17: CTAs of the starting push that have read their slot
+    unsigned int exited[kCmDepth];   // words 18..20: CTAs finished, by push number % kCmDepth (cumulative): push
+                               // e - kCmDepth and all before it are complete when exited[e % kCmDepth] has
+                               // reached slot[e & 1].cum[e % kCmDepth]
+    unsigned int pad[11];
 };
-static_assert(sizeof(CmCtl) == 64, "the control block is read by one warp in one access");
+static_assert(sizeof(CmSlot) == 32 && sizeof(CmCtl) == 128, "the control block is read by one warp in one access");
 
 // One SOS section for sub-block length L; every member is warp-uniform and is read straight
 // from the constant bank.  Q[d] = A^(2L 2^d); g[i] = C A^i.
@@ -505,7 +509,8 @@ __device__ __forceinline__ unsigned long long fk_now()
 }
 __device__ __forceinline__ void fk_trace(unsigned epoch, int gw, int lane, unsigned ev, unsigned& k, unsigned long long t)
 {
-    if (lane == 0 && k < 16 && gw < 4096) {
+    if (ev >= 5) k = 9 + ev;
+    if (lane == 0 && k < 16 && (ev >= 5 || k < 14) && gw < 4096) {
         unsigned smid;
         asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
         const size_t i = (((size_t)(epoch & 15u) * 4096 + gw) * 16 + k) * 2;
@@ -520,18 +525,20 @@ __device__ __forceinline__ void fk_trace(unsigned epoch, int gw, int lane, unsig
 #define FK_TR(ev)
 #endif
 
-// Warps per SM (bounded by shared memory: two tile buffers per warp) and per CTA.  kCmCtasPerSm
-// CTAs share an SM so that the CTAs of the next push can move in as soon as some of this push's
-// CTAs have left, not only when the last warp of the SM is done.
-#ifndef FK_CTAS
-#define FK_CTAS 4
-#endif
-constexpr int kCmCtasPerSm = FK_CTAS;
+// Warps per SM (bounded by shared memory: two tile buffers per warp) and per CTA.  The kernel is
+// built for two launch shapes: CTAS = kCmCtasPerSm small CTAs per SM for ordinary pushes, so that
+// the CTAs of the next push can move in as soon as some of this push's CTAs have left, not only
+// when the last warp of an SM is done; and CTAS = 1 (one CTA of all the SM's warps, warps of a CTA
+// interleaved over the channels) for pushes long enough that the hand-over between pushes does
+// not matter: with several CTAs per SM the hardware favours the older CTAs, the younger ones fall
+// behind by 20 % and a long push ends with a tail (measured: 342 vs 377 Gsample/s on a 90,000-
+// sample push).
+constexpr int kCmCtasPerSm = 4;
 template <int L> __host__ __device__ constexpr int cm_max_warps() { return L <= 24 ? 16 : (L <= 32 ? 12 : 8); }
-template <int L> __host__ __device__ constexpr int cm_cta_warps() { return cm_max_warps<L>() / kCmCtasPerSm; }
+template <int L, int CTAS> __host__ __device__ constexpr int cm_cta_warps() { return cm_max_warps<L>() / CTAS; }
 
-// Channel-major push: grid <= kCmCtasPerSm * SM count (every CTA of a push is resident once the
-// pushes before it have drained), block = W * 32 (W <= cm_cta_warps<L>()); dynamic shared memory =
+// Channel-major push: grid <= CTAS * SM count (every CTA of a push is resident once the
+// pushes before it have drained), block = W * 32 (W <= cm_cta_warps<L, CTAS>()); dynamic shared memory =
 // W * warp_smem_floats<L>() floats.
 //
 // Overlap of consecutive pushes.  A push of 6,000 channels x 1,500 samples is 2.5 tiles per
@@ -542,14 +549,14 @@ template <int L> __host__ __device__ constexpr int cm_cta_warps() { return cm_ma
 // c of push e + 1 starts from the state (and raw history) that push e left for channel c.
 // `progress[c]` counts the segments completed on channel c since create/reset; item (seg, c) of a
 // push whose slot says seq0 runs when progress[c] == seq0 + seg and then publishes seq0 + seg + 1
-// (release/acquire at gpu scope).  At most two pushes are in flight: push e starts only when push
-// e - 2 has completed (done[e & 1]), so the host only has to compare a push's buffers with those of
-// the push before it (p.wait_prior = 1 on a conflict, on another stream, after foreign work, or
+// (release at gpu scope, L2-scope polls).  At most kCmDepth pushes are in flight: push e starts only
+// when push e - kCmDepth has completed (`exited`), so the host only has to compare a push's buffers
+// with those of the kCmDepth - 1 pushes before it (p.wait_prior = 1 on a conflict, on another stream, after foreign work, or
 // with FILARK_FLAG_STRICT_ORDER: then the kernel begins with griddepcontrol.wait like any
 // dependent launch).  Every CTA ends with griddepcontrol.wait, so a push never completes before the
 // push in front of it.
-template <int L>
-__global__ void __launch_bounds__(cm_cta_warps<L>() * 32, kCmCtasPerSm)
+template <int L, int CTAS>
+__global__ void __launch_bounds__(cm_cta_warps<L, CTAS>() * 32, CTAS)
 filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
 {
     // the warp index through a shuffle: the compiler then knows that it -- and with it the channel
@@ -559,8 +566,8 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     const int lane = threadIdx.x & 31, W = blockDim.x >> 5;
     const int wbase = warp * warp_smem_floats<L>();                   // two tile buffers, then two state copies
     const int wst0 = wbase + 2 * Geo<L>::buf_floats;
-    const int gw = (p.wait_prior & 2) ? (int)(blockIdx.x + gridDim.x * warp) : (int)(blockIdx.x * W + warp);   // warp index in the grid
-    __shared__ unsigned sh_ctl[16];
+    const int gw = CTAS == 1 ? (int)(blockIdx.x + gridDim.x * warp) : (int)(blockIdx.x * W + warp);   // warp index in the grid
+    __shared__ unsigned sh_ctl[32];
     __shared__ unsigned sh_flag;
     if (threadIdx.x == 0) sh_flag = 0u;
 #ifdef FK_TRACE
@@ -577,7 +584,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         for (int o = 128 * lane; o < bytes; o += 128 * 32)
             asm volatile("prefetch.global.L2 [%0];" ::"l"(row + o));
     }
-    if (p.wait_prior & 1) asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (p.wait_prior) asm volatile("griddepcontrol.wait;" ::: "memory");
 
     // ---- control slot of this push.  Nothing changes epoch or slot[epoch & 1] between the launch of
     // this grid (after every CTA of the previous push had taken its ticket and the last of them
@@ -585,23 +592,24 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     CmCtl* const cc = p.cctl;
     if (warp == 0) {
         const unsigned* cw = reinterpret_cast<const unsigned*>(cc);
-        unsigned v = ld_relaxed(cw + (lane & 15));
-        const unsigned e = __shfl_sync(0xffffffffu, v, 12);
-        const unsigned par = e & 1u;
-        const unsigned need = __shfl_sync(0xffffffffu, v, 6 * par + 4 + par);     // slot[par].cum[par]
-        unsigned ex = __shfl_sync(0xffffffffu, v, 14 + par);
-        while ((int)(ex - need) < 0)                                   // push e - 2 must have completed
-            ex = __shfl_sync(0xffffffffu, ld_relaxed(&cc->exited[par]), 0);
-        if (lane < 16) sh_ctl[lane] = v;
+        unsigned v = ld_relaxed(cw + lane);
+        const unsigned e = __shfl_sync(0xffffffffu, v, 16);
+        const unsigned ring = e % (unsigned)kCmDepth;
+        const unsigned need = __shfl_sync(0xffffffffu, v, 8 * (e & 1u) + 4 + ring);   // slot[e & 1].cum[ring]
+        unsigned ex = __shfl_sync(0xffffffffu, v, 18 + ring);
+        while ((int)(ex - need) < 0)                                   // push e - kCmDepth must have completed
+            ex = __shfl_sync(0xffffffffu, ld_relaxed(&cc->exited[ring]), 0);
+        sh_ctl[lane] = v;
     }
     __syncthreads();
-    const unsigned epoch = sh_ctl[12];
+    const unsigned epoch = sh_ctl[16];
+    const unsigned ring = epoch % (unsigned)kCmDepth;
 #ifdef FK_TRACE
     tr_epoch = epoch;
     fk_trace(tr_epoch, tr_gw, lane, 0, tr_k, tr_t0);
     FK_TR(1);
 #endif
-    const unsigned* sl = &sh_ctl[6 * (epoch & 1u)];
+    const unsigned* sl = &sh_ctl[8 * (epoch & 1u)];
     const unsigned long long seen = (unsigned long long)sl[0] | ((unsigned long long)sl[1] << 32);
     const unsigned r0 = sl[2], seq0 = sl[3];
     const Geom g = make_geom<L>(r0, p.n_t, p.vec4 != 0);
@@ -659,8 +667,8 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
                 __stcg(&nx->seen, seen + (unsigned long long)p.n_t);
                 __stcg(&nx->r0, (unsigned)g.r1);
                 __stcg(&nx->seq0, seq0 + (unsigned)n_seg);
-                __stcg(&nx->cum[epoch & 1u], sl[4 + (epoch & 1u)] + gridDim.x);
-                __stcg(&nx->cum[(epoch & 1u) ^ 1u], sl[4 + ((epoch & 1u) ^ 1u)]);
+                for (unsigned j = 0; j < (unsigned)kCmDepth; ++j)
+                    __stcg(&nx->cum[j], sl[4 + j] + (j == ring ? gridDim.x : 0u));
                 __stcg(&cc->ticket, 0u);
                 st_release(&cc->epoch, epoch + 1u);
                 __threadfence();
@@ -756,7 +764,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     // completion: count this CTA out (push e + 2 waits until all of them are)
     __syncthreads();
     if (threadIdx.x == 0)
-        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(&cc->exited[epoch & 1u]) : "memory");
+        asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(&cc->exited[ring]) : "memory");
     // a push never completes before the push in front of it
     asm volatile("griddepcontrol.wait;" ::: "memory");
     FK_TR(6);

@@ -44,9 +44,9 @@ struct filark_stream {
     unsigned* d_progress;           // [n_ch] segments completed per channel (cumulative)
     // what the previous channel-major push touched: a push may overlap the one before it on the
     // device only if it follows it directly in the same stream and their buffers are disjoint
-    bool prev_valid;
+    int prev_valid;                 // how many of the entries below describe pushes that may still run
     cudaStream_t prev_stream;
-    uintptr_t prev_lo[3], prev_hi[3];
+    uintptr_t prev_lo[kCmDepth - 1][3], prev_hi[kCmDepth - 1][3];     // [0] = the push before, [1] = the one before that
     float4* d_tm_carry;             // time-major look-back ring [n_cb][2][kTmStages][32]
     unsigned* d_tm_pub;             // [n_cb][32] published-tile counts, self-resetting
     int n_sm;
@@ -188,16 +188,16 @@ static Geom geometry_rt(int L, unsigned r0, int n_t, bool vec4)
     }
 }
 
-// kCmCtasPerSm CTAs per SM, W warps per CTA; fewer warps per CTA, on more SMs, when there are few
+// CTAS CTAs per SM, W warps per CTA; fewer warps per CTA, on more SMs, when there are few
 // channels.  Every CTA of a push fits on the device at once (the segment waits rely on it).
-template <int L>
-static cudaError_t launch_cm(const filark_stream* h, const PushParams<L>& p, cudaStream_t stream)
+template <int L, int CTAS>
+static cudaError_t launch_cm_shape(const filark_stream* h, const PushParams<L>& p, cudaStream_t stream)
 {
     const size_t warp_bytes = sizeof(float) * (size_t)warp_smem_floats<L>();
     int per_sm = cm_max_warps<L>();                      // warps per SM
-    const int fit = (int)((h->smem_optin - 64) / warp_bytes);
+    const int fit = (int)((h->smem_optin - 256) / warp_bytes);
     if (fit < per_sm) per_sm = fit;
-    int W = cm_cta_warps<L>();
+    int W = cm_cta_warps<L, CTAS>();
     if (W > per_sm) W = per_sm;
     const int want = (p.n_ch + h->n_sm - 1) / h->n_sm;
     if (want < W) W = want;
@@ -207,10 +207,10 @@ static cudaError_t launch_cm(const filark_stream* h, const PushParams<L>& p, cud
     }
     if (W < 1) return cudaErrorInvalidConfiguration;
     const size_t smem = (size_t)W * warp_bytes;
-    static bool attr_done = false;           // per variant (template instance); idempotent
+    static bool attr_done = false;           // per template instance; idempotent
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(filark_push_cm_kernel<L>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)((size_t)cm_cta_warps<L>() * warp_bytes));
+        cudaError_t e = cudaFuncSetAttribute(filark_push_cm_kernel<L, CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                             (int)((size_t)cm_cta_warps<L, CTAS>() * warp_bytes));
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
@@ -227,8 +227,20 @@ static cudaError_t launch_cm(const filark_stream* h, const PushParams<L>& p, cud
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = std::getenv("FILARK_TUNE_NOPDL") ? 0 : 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    if (std::getenv("FILARK_TUNE_CARVE")) cudaFuncSetAttribute(filark_push_cm_kernel<L>, cudaFuncAttributePreferredSharedMemoryCarveout, 100);
-    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L>, p);
+    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, CTAS>, p);
+}
+
+// Launch shape (filark_kernels.cuh): one CTA per SM when every resident warp gets a long run of tiles
+// anyway, small CTAs otherwise.  (L = 24 is the only variant long pushes ever use.)
+template <int L>
+static cudaError_t launch_cm(const filark_stream* h, const PushParams<L>& p, cudaStream_t stream)
+{
+    if constexpr (L == 24) {
+        const long long tiles = ((long long)p.n_t + kHist + Geo<L>::tile - 1) / Geo<L>::tile * p.n_ch;
+        const bool long_push = tiles >= 12LL * h->n_sm * cm_max_warps<L>();
+        if (long_push && !std::getenv("FILARK_TUNE_SMALL_CTAS")) return launch_cm_shape<24, 1>(h, p, stream);
+    }
+    return launch_cm_shape<L, kCmCtasPerSm>(h, p, stream);
 }
 
 template <int L>
@@ -240,7 +252,7 @@ static cudaError_t push_variant(const filark_stream* h, int v, const float* d_in
     p.in = d_in; p.filt = d_filt; p.cf = d_cf;
     p.state = h->d_state; p.hist = h->d_hist; p.ctl = h->d_ctl; p.cctl = h->d_cctl; p.progress = h->d_progress;
     p.in_pitch = in_pitch; p.out_pitch = out_pitch; p.n_t = n_t; p.vec4 = vec4;
-    p.wait_prior = wait_prior | (std::getenv("FILARK_TUNE_MAP") ? 2 : 0);
+    p.wait_prior = wait_prior;
     return launch_cm<L>(h, p, stream);
 }
 
@@ -381,7 +393,7 @@ filark_status_t filark_stream_reset(filark_stream_t* h, cudaStream_t stream)
     e = cudaMemsetAsync(h->d_state, 0, sizeof(float) * h->state_floats, stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(h->d_ctl, 0, sizeof(Ctl), stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(h->d_cctl, 0, sizeof(CmCtl), stream);
-    h->prev_valid = false;
+    h->prev_valid = 0;
     if (e == cudaSuccess) e = cudaMemsetAsync(h->d_progress, 0, sizeof(unsigned) * (size_t)h->n_ch, stream);
     if (e == cudaSuccess && h->d_tm_pub)
         e = cudaMemsetAsync(h->d_tm_pub, 0, sizeof(unsigned) * (((size_t)h->n_ch + 63) / 64) * 32, stream);
@@ -468,16 +480,19 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
         const uintptr_t lo[3] = {(uintptr_t)d_in, (uintptr_t)d_filt, (uintptr_t)d_cf};
         const uintptr_t hi[3] = {lo[0] + in_bytes, d_filt ? lo[1] + out_bytes : 0, d_cf ? lo[2] + out_bytes : 0};
         int wait_prior = 1;
-        if (!(h->flags & FILARK_FLAG_STRICT_ORDER) && h->prev_valid && h->prev_stream == stream &&
+        if (!(h->flags & FILARK_FLAG_STRICT_ORDER) && h->prev_valid > 0 && h->prev_stream == stream &&
             registry_is_last(stream, h)) {
             bool clash = false;
-            for (int i = 0; i < 3; ++i)
-                for (int j = 0; j < 3; ++j)
-                    if ((i > 0 || j > 0) && hi[i] && h->prev_hi[j] && lo[i] < h->prev_hi[j] && h->prev_lo[j] < hi[i])
-                        clash = true;
+            for (int q = 0; q < h->prev_valid; ++q)
+                for (int i = 0; i < 3; ++i)
+                    for (int j = 0; j < 3; ++j)
+                        if ((i > 0 || j > 0) && hi[i] && h->prev_hi[q][j] && lo[i] < h->prev_hi[q][j] &&
+                            h->prev_lo[q][j] < hi[i])
+                            clash = true;
             wait_prior = clash ? 1 : 0;
         }
-        h->prev_valid = false;
+        const int n_prev = wait_prior ? 0 : h->prev_valid;       // a waiting push leaves nothing in flight behind it
+        h->prev_valid = 0;
         switch (kVariantL[v]) {
             case 8: e = push_variant<8>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, wait_prior, stream); break;
             case 16: e = push_variant<16>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, wait_prior, stream); break;
@@ -486,8 +501,11 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
             default: e = push_variant<48>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, wait_prior, stream); break;
         }
         if (e == cudaSuccess) {
-            h->prev_valid = true; h->prev_stream = stream;
-            for (int i = 0; i < 3; ++i) { h->prev_lo[i] = lo[i]; h->prev_hi[i] = hi[i]; }
+            const int keep = n_prev < kCmDepth - 2 ? n_prev : kCmDepth - 2;
+            for (int q = keep; q > 0; --q)
+                for (int i = 0; i < 3; ++i) { h->prev_lo[q][i] = h->prev_lo[q - 1][i]; h->prev_hi[q][i] = h->prev_hi[q - 1][i]; }
+            for (int i = 0; i < 3; ++i) { h->prev_lo[0][i] = lo[i]; h->prev_hi[0][i] = hi[i]; }
+            h->prev_valid = keep + 1; h->prev_stream = stream;
         }
     }
     registry_set(stream, h);
