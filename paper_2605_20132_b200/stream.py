@@ -17,6 +17,7 @@ from .workloads import CHANNEL_MAJOR, TIME_MAJOR
 
 FLAG_NONE = 0
 FLAG_SERIAL_SCAN = 1
+FLAG_STRICT_ORDER = 2       # every push waits for all earlier work in its stream (filark_stream.h, "Ordering")
 MAX_SECTIONS = 16
 
 STATUS_NAMES = {0: "FILARK_OK", 1: "FILARK_ERR_INVALID_ARG", 2: "FILARK_ERR_UNSTABLE",

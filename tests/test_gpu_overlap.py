@@ -1,0 +1,170 @@
+"""GPU: consecutive pushes of a handle overlap on the device (include/filark_stream.h, "Ordering";
+csrc/filark_kernels.cuh).  Back-to-back pushes with nothing between them in the stream must give
+bit-identical outputs to the same pushes under FILARK_FLAG_STRICT_ORDER (every push an ordinary
+dependent launch) and match the float64 oracle; pushes whose buffers clash with the ones before
+them, and pushes of another handle in the same stream, must be ordered like any stream work."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2605_20132_b200.stream import FLAG_STRICT_ORDER, FilarkStream
+from paper_2605_20132_b200.workloads import CHANNEL_MAJOR, CONFIGS, design_sos, generate
+from tests._util import assert_parity, run_oracle, split
+
+pytestmark = pytest.mark.gpu
+
+
+def _back_to_back(s, chunks, outs_f, outs_c):
+    """Nothing but pushes goes into the stream: this is the case in which they overlap."""
+    for x, f, c in zip(chunks, outs_f, outs_c):
+        s.push(x, f, c)
+
+
+def _alloc(chunks):
+    return [torch.empty_like(x) for x in chunks], [torch.empty_like(x) for x in chunks]
+
+
+@pytest.mark.parametrize("n_ch,n_t,sizes", [
+    (3000, 12_000, [1500]),                 # the bench's push shape: 16-byte path, r0 alternates 0 / 12
+    (2500, 9_000, [700, 333, 1501, 64]),    # ragged: 4-byte path, hist crosses pushes
+    (6000, 6_000, [1000]),                  # more channels than resident warps
+    (700, 40_000, [16_000, 8_000]),         # several segments per channel and push
+])
+def test_overlapped_equals_strict_order_and_oracle(cuda_device, n_ch, n_t, sizes):
+    w = CONFIGS["cfg3"].scaled(n_ch=n_ch, n_t=n_t)
+    sos = design_sos(w)
+    x = generate(w, device="cpu")
+    xd = x.to(cuda_device)
+    chunks = [xd[:, a:b].contiguous() for a, b in split(n_t, sizes)]
+    res = {}
+    for flags in (0, FLAG_STRICT_ORDER):
+        s = FilarkStream(n_ch, sos, w.sta_len, w.lta_len, CHANNEL_MAJOR, flags)
+        of, oc = _alloc(chunks)
+        for rep in range(3):                               # reset + replay: counters start over
+            torch.cuda.synchronize()
+            _back_to_back(s, chunks, of, oc)
+            torch.cuda.synchronize()
+            if rep < 2:
+                s.reset()
+        res[flags] = (torch.cat(of, 1).cpu().numpy(), torch.cat(oc, 1).cpu().numpy())
+        s.destroy()
+    assert np.array_equal(res[0][0], res[FLAG_STRICT_ORDER][0]), "filt differs from strict order"
+    assert np.array_equal(res[0][1], res[FLAG_STRICT_ORDER][1]), "cf differs from strict order"
+    pick = np.unique(np.r_[0, 1, n_ch // 3, n_ch // 2, n_ch - 2, n_ch - 1,
+                           np.random.default_rng(5).integers(0, n_ch, 26)])
+    ref_f, ref_c = run_oracle(x.numpy()[pick], sos, w.sta_len, w.lta_len)
+    assert_parity(res[0][0][pick], ref_f, "overlapped filt")
+    assert_parity(res[0][1][pick], ref_c, "overlapped cf")
+
+
+def test_long_run_of_overlapped_pushes(cuda_device):
+    """200 pushes in flight behind each other: counters, slot parity and the in-flight bound."""
+    n_ch, chunk, n_push = 1200, 252, 200
+    w = CONFIGS["cfg4"].scaled(n_ch=n_ch, n_t=chunk * n_push)
+    sos = design_sos(w)
+    x = generate(w, device="cpu")
+    xd = x.to(cuda_device)
+    chunks = [xd[:, a:b].contiguous() for a, b in split(w.n_t, [chunk])]
+    s = FilarkStream(n_ch, sos, w.sta_len, w.lta_len)
+    of, oc = _alloc(chunks)
+    _back_to_back(s, chunks, of, oc)
+    torch.cuda.synchronize()
+    assert s.launch_count == n_push
+    pick = np.arange(0, n_ch, 97)
+    ref_f, ref_c = run_oracle(x.numpy()[pick], sos, w.sta_len, w.lta_len)
+    assert_parity(torch.cat(of, 1).cpu().numpy()[pick], ref_f, "200 pushes filt")
+    assert_parity(torch.cat(oc, 1).cpu().numpy()[pick], ref_c, "200 pushes cf")
+    s.destroy()
+
+
+def test_clashing_buffers_are_ordered(cuda_device):
+    """(a) every push writes the SAME output buffers; (b) a push reads what the push before it
+    wrote.  Both must behave as plain stream order says."""
+    n_ch, chunk, n_push = 2400, 1500, 6
+    w = CONFIGS["cfg3"].scaled(n_ch=n_ch, n_t=chunk * n_push)
+    sos = design_sos(w)
+    xd = generate(w, device="cpu").to(cuda_device)
+    chunks = [xd[:, a:b].contiguous() for a, b in split(w.n_t, [chunk])]
+    # reference: strict order, separate buffers
+    s = FilarkStream(n_ch, sos, w.sta_len, w.lta_len, CHANNEL_MAJOR, FLAG_STRICT_ORDER)
+    of, oc = _alloc(chunks)
+    _back_to_back(s, chunks, of, oc)
+    torch.cuda.synchronize()
+    s.destroy()
+    # (a) one pair of output buffers for all pushes: the last push must win everywhere
+    s = FilarkStream(n_ch, sos, w.sta_len, w.lta_len)
+    f1 = torch.empty_like(chunks[0]); c1 = torch.empty_like(chunks[0])
+    for xk in chunks:
+        s.push(xk, f1, c1)
+    torch.cuda.synchronize()
+    assert torch.equal(f1, of[-1]) and torch.equal(c1, oc[-1])
+    s.destroy()
+    # (b) second handle-free chain: push k + 1 filters the filt output of push k again
+    for flags in (0, FLAG_STRICT_ORDER):
+        s = FilarkStream(n_ch, sos, w.sta_len, w.lta_len, CHANNEL_MAJOR, flags)
+        bufs = [chunks[0]] + [torch.empty_like(chunks[0]) for _ in range(n_push)]
+        for k in range(n_push):
+            s.push(bufs[k], bufs[k + 1], None)
+        torch.cuda.synchronize()
+        if flags == 0:
+            got = [b.clone() for b in bufs[1:]]
+        else:
+            for a, b in zip(got, bufs[1:]):
+                assert torch.equal(a, b), "a push read its input before the push before it had written it"
+        s.destroy()
+
+
+def test_two_handles_chained_in_one_stream(cuda_device):
+    """Handle B filters what handle A wrote, push by push, in one stream: B's pushes follow A's
+    pushes directly and must still see A's output complete."""
+    n_ch, chunk, n_push = 2400, 1500, 5
+    w = CONFIGS["cfg3"].scaled(n_ch=n_ch, n_t=chunk * n_push)
+    sos = design_sos(w)
+    xd = generate(w, device="cpu").to(cuda_device)
+    chunks = [xd[:, a:b].contiguous() for a, b in split(w.n_t, [chunk])]
+    out = {}
+    for flags in (0, FLAG_STRICT_ORDER):
+        a = FilarkStream(n_ch, sos, w.sta_len, w.lta_len, CHANNEL_MAJOR, flags)
+        b = FilarkStream(n_ch, sos[:2], w.sta_len, w.lta_len, CHANNEL_MAJOR, flags)
+        fa, _ = _alloc(chunks); fb, cb = _alloc(chunks)
+        for k in range(n_push):
+            a.push(chunks[k], fa[k], None)
+            b.push(fa[k], fb[k], cb[k])
+        torch.cuda.synchronize()
+        out[flags] = (torch.cat(fb, 1), torch.cat(cb, 1))
+        a.destroy(); b.destroy()
+    assert torch.equal(out[0][0], out[FLAG_STRICT_ORDER][0])
+    assert torch.equal(out[0][1], out[FLAG_STRICT_ORDER][1])
+
+
+def test_graph_of_back_to_back_pushes(cuda_device):
+    """Several pushes captured into ONE graph (programmatic edges between them), replayed."""
+    n_ch, chunk, per_graph, n_rep = 2000, 1500, 4, 3
+    w = CONFIGS["cfg3"].scaled(n_ch=n_ch, n_t=chunk * per_graph * n_rep)
+    sos = design_sos(w)
+    x = generate(w, device="cpu")
+    xd = x.to(cuda_device)
+    s = FilarkStream(n_ch, sos, w.sta_len, w.lta_len)
+    xin = [torch.empty((n_ch, chunk), device=cuda_device) for _ in range(per_graph)]
+    of, oc = _alloc(xin)
+    side = torch.cuda.Stream()
+    g = torch.cuda.CUDAGraph()
+    with torch.cuda.stream(side):
+        s.push(xin[0], of[0], oc[0]); s.reset()             # warm-up outside capture
+        torch.cuda.synchronize()
+        with torch.cuda.graph(g, stream=side):
+            for k in range(per_graph):
+                s.push(xin[k], of[k], oc[k])
+    got_f, got_c = [], []
+    for r in range(n_rep):
+        for k in range(per_graph):
+            a = (r * per_graph + k) * chunk
+            xin[k].copy_(xd[:, a:a + chunk])
+        g.replay()
+        torch.cuda.synchronize()
+        got_f += [t.clone() for t in of]; got_c += [t.clone() for t in oc]
+    pick = np.arange(0, n_ch, 131)
+    ref_f, ref_c = run_oracle(x.numpy()[pick], sos, w.sta_len, w.lta_len)
+    assert_parity(torch.cat(got_f, 1).cpu().numpy()[pick], ref_f, "graph of pushes filt")
+    assert_parity(torch.cat(got_c, 1).cpu().numpy()[pick], ref_c, "graph of pushes cf")
+    s.destroy()
