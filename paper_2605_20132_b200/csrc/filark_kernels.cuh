@@ -117,6 +117,8 @@ template <int L> struct PushParams {
     unsigned* progress;      // [n_ch] segments completed per channel since create/reset (cumulative, wraps)
     long long in_pitch, out_pitch;
     int n_t, n_ch, n_sec, lta_len;
+    int n_base, n_rem;       // n_t = n_base L + n_rem
+    int seg_tiles;           // tiles per work item (host heuristic: about 8 items per resident warp)
     int vec4;                // 16-byte global accesses are legal (alignment, pitch, n_t % 4 == 0)
     int wait_prior;          // wait for everything before this launch in the stream before touching memory
     float gain, ratio, lta_thr;
@@ -132,20 +134,25 @@ struct Geom {
     int r1;                  // samples of the trailing partial slot, 0..L-1
     bool vec4;
 };
+// n_t = n_base L + n_rem is split on the host, so that the device needs no division (every CTA
+// of every push derives the geometry in its prologue, a serial chain of scalar instructions).
 template <int L>
-__host__ __device__ inline Geom make_geom(unsigned r0, int n_t, bool vec4)
+__host__ __device__ inline Geom make_geom(unsigned r0, int n_base, int n_rem, bool vec4)
 {
     Geom g;
-    const long long total = (long long)r0 + n_t;
-    const long long n_full = total / L;
+    // (r0 < kHist is the tail of the previous push, which may have used a longer L; n_rem < L)
+    const int carry = ((int)r0 + n_rem) / L;               // small numerator, compile-time divisor
+    const int n_full = n_base + carry;                     // full slots of r0 + n_t samples
     g.r0 = (int)r0;
-    g.r1 = (int)(total - n_full * L);
-    const long long slots = n_full + (g.r1 ? 1 : 0);
-    g.n_tiles = (int)((slots + 63) / 64);
-    g.q_last = (int)(n_full - 64LL * (g.n_tiles - 1));
+    g.r1 = (int)r0 + n_rem - carry * L;
+    const int slots = n_full + (g.r1 ? 1 : 0);
+    g.n_tiles = (slots + 63) >> 6;
+    g.q_last = n_full - 64 * (g.n_tiles - 1);
     g.vec4 = vec4 && (r0 & 3u) == 0;
     return g;
 }
+template <int L>
+__host__ __device__ inline Geom make_geom(unsigned r0, int n_t, bool vec4) { return make_geom<L>(r0, n_t / L, n_t % L, vec4); }
 
 // ---- small PTX wrappers ------------------------------------------------------------------------
 __device__ __forceinline__ void cp_async16(int dst_off, const float* src, int src_bytes);
@@ -369,7 +376,8 @@ __device__ __forceinline__ void local_pass(float2 (&x)[L], const SecParams<L>& T
 // outputs.  buf / wst are float offsets into fk_smem.
 template <int L>
 __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom& g, int buf, int wst, float2 (&x)[L],
-                                             int ch, int tile, int lane, unsigned long long seen)
+                                             int ch, int tile, int lane, unsigned long long seen,
+                                             bool item_end, unsigned rel_val)
 {
     const bool last = tile == g.n_tiles - 1;
     const int t0 = tile * Geo<L>::tile - g.r0;
@@ -462,6 +470,20 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
     const float Nl = __shfl_sync(0xffffffffu, out_hi ? Wl : Ol, jl);
     if (lane == 0 && !keep) *reinterpret_cast<float2*>(&fk_smem[ks]) = make_float2(Ns, Nl);
 
+    // Last tile of a work item: the carried state is final here.  It goes back to global memory
+    // now, and `progress` is released after the ratio loop below: the fence of the release waits for
+    // the stores the warp has in flight, and by then these are a loop old (at the very end of the
+    // tile, behind the cf stores, it cost about a microsecond per item).  What is stored after the
+    // release are outputs only; nobody who waits on `progress` reads them (the host orders pushes
+    // that share a buffer), the end of the grid publishes them.
+    if (item_end) {
+        __syncwarp();
+        const int ns = state_floats(p.n_sec);
+        float* gst = p.state + (long long)ch * ns;
+        if (lane < ns) __stcg(gst + lane, fk_smem[wst + lane]);
+        if (lane + 32 < ns) __stcg(gst + lane + 32, fk_smem[wst + lane + 32]);
+    }
+
     if (p.cf) {
         // warm-up (reading R10): samples whose index since create/reset is < lta_len give cf = 0
         // (seen = samples pushed before this push; tile position e is sample seen + t0 + e of the stream)
@@ -491,7 +513,11 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
         }
         regs_to_buf<L>(x, buf, lane);
         __syncwarp();
+        if (item_end && lane == 0) st_release(p.progress + ch, rel_val);
         store_tile<L>(p, g, p.cf + (long long)ch * p.out_pitch, buf, lane, t0);
+    } else if (item_end) {
+        __syncwarp();
+        if (lane == 0) st_release(p.progress + ch, rel_val);
     }
     __syncwarp();
 }
@@ -509,7 +535,7 @@ __device__ __forceinline__ unsigned long long fk_now()
 }
 __device__ __forceinline__ void fk_trace(unsigned epoch, int gw, int lane, unsigned ev, unsigned& k, unsigned long long t)
 {
-    if (ev >= 5) k = 9 + ev;
+    if (ev >= 5 && ev <= 6) k = 9 + ev;
     if (lane == 0 && k < 16 && (ev >= 5 || k < 14) && gw < 4096) {
         unsigned smid;
         asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
@@ -576,15 +602,11 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     const unsigned long long tr_t0 = fk_now();
 #endif
 
-    // pull this warp's first rows into L2 while the control block is read (the input never
-    // depends on the previous push; the control block, state and hist do)
-    if (gw < p.n_ch) {
-        const char* row = reinterpret_cast<const char*>(p.in + (long long)gw * p.in_pitch);
-        const int bytes = 4 * min(p.n_t, Geo<L>::tile);
-        for (int o = 128 * lane; o < bytes; o += 128 * 32)
-            asm volatile("prefetch.global.L2 [%0];" ::"l"(row + o));
-    }
     if (p.wait_prior) asm volatile("griddepcontrol.wait;" ::: "memory");
+    // the warp's first item is always (segment 0, channel gw): ask for its progress word now, so that
+    // the answer is there when the control slot says what to compare it with
+    unsigned pr0 = 0;
+    if (gw < p.n_ch) pr0 = ld_relaxed(p.progress + gw);
 
     // ---- control slot of this push.  Nothing changes epoch or slot[epoch & 1] between the launch of
     // this grid (after every CTA of the previous push had taken its ticket and the last of them
@@ -612,7 +634,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     const unsigned* sl = &sh_ctl[8 * (epoch & 1u)];
     const unsigned long long seen = (unsigned long long)sl[0] | ((unsigned long long)sl[1] << 32);
     const unsigned r0 = sl[2], seq0 = sl[3];
-    const Geom g = make_geom<L>(r0, p.n_t, p.vec4 != 0);
+    const Geom g = make_geom<L>(r0, p.n_base, p.n_rem, p.vec4 != 0);
     const int ns = state_floats(p.n_sec);
 
     // Work items (segment, channel), segment-major; a segment is seg_tiles consecutive tiles of a
@@ -622,9 +644,8 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     // items in rising order and all warps of the push become resident (nothing an earlier push
     // needs depends on a later one), so the unfinished item with the lowest index can always run.
     const int n_warps = gridDim.x * W;
-    int seg_tiles = (int)(((long long)g.n_tiles * p.n_ch) / (8LL * n_warps));
-    seg_tiles = max(1, min(seg_tiles, g.n_tiles));
-    const int n_seg = (g.n_tiles + seg_tiles - 1) / seg_tiles;
+    const int seg_tiles = min(p.seg_tiles, g.n_tiles);
+    const int n_seg = seg_tiles == g.n_tiles ? 1 : (g.n_tiles + seg_tiles - 1) / seg_tiles;
     const unsigned n_items = (unsigned)n_seg * (unsigned)p.n_ch;
 
     unsigned item = (unsigned)gw;
@@ -632,7 +653,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         const unsigned it = item;
         item += (unsigned)n_warps;
         if (it >= n_items) return false;
-        seg = (int)(it / (unsigned)p.n_ch);
+        seg = n_seg == 1 ? 0 : (int)(it / (unsigned)p.n_ch);
         ch = (int)(it - (unsigned)seg * (unsigned)p.n_ch);
         tile = seg * seg_tiles;
         tend = min(g.n_tiles, tile + seg_tiles);
@@ -654,11 +675,14 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     if (warp == 0 && lane == 0) tk = atomicAdd(&cc->ticket, 1u);
 
     bool have = claim(ch, tile, tend, seg);
-    unsigned pr0 = 0;
-    if (have) {
-        issue_tile_input<L>(p, g, ch, tile, wbase, lane);
-        if (seg == 0) pr0 = ld_relaxed(p.progress + ch);
+    if (have) issue_tile_input<L>(p, g, ch, tile, wbase, lane);
+    // the first segment of a channel needs what the previous push left (state, hist): wait before
+    // those loads are issued (a wait on an EARLIER push cannot be part of a cycle)
+    if (have && seg == 0) {
+        wait_progress(ch, seq0, pr0);
+        issue_tile_carry<L>(p, g, ch, wbase, wst0, lane);
     }
+    FK_TR(7);
     if (warp == 0) {
         tk = __shfl_sync(0xffffffffu, tk, 0);
         if (lane == 0) {
@@ -676,13 +700,8 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
             *reinterpret_cast<volatile unsigned*>(&sh_flag) = 1u;
         }
     }
-    // the first segment of a channel needs what the previous push left (state, hist): wait before
-    // those loads are issued (a wait on an EARLIER push cannot be part of a cycle)
-    if (have && seg == 0) {
-        wait_progress(ch, seq0, pr0);
-        issue_tile_carry<L>(p, g, ch, wbase, wst0, lane);
-    }
     if (have) cp_async_wait_all();
+    FK_TR(8);
     {
         unsigned f;
         do f = __shfl_sync(0xffffffffu, *reinterpret_cast<volatile unsigned*>(&sh_flag), 0); while (f == 0u);
@@ -697,11 +716,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         unsigned npr = 0;
         if (item_end) {
             nhave = claim(nch, ntile, ntend, nseg);
-#ifndef FK_NO_EARLY_POLL
             if (nhave && nseg == 0) npr = ld_relaxed(p.progress + nch);      // used after the tile is in registers
-#else
-            npr = seq0 - 1u;
-#endif
         }
         const int buf = wbase + cur * Geo<L>::buf_floats;
         const int wst = wst0 + wcur * kStateSmem;
@@ -745,18 +760,11 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
                 issue_tile_carry<L>(p, g, nch, nbuf, wst0 + (wcur ^ 1) * kStateSmem, lane);
             }
         }
-        process_tile<L>(p, g, buf, wst, x, ch, tile, lane, seen);
+        // (a segment's end writes the carried state back and tells whoever continues the channel:
+        // the next segment of this push or the first segment of the next push)
+        process_tile<L>(p, g, buf, wst, x, ch, tile, lane, seen, item_end, seq0 + (unsigned)seg + 1u);
         FK_TR(4);
-        if (item_end) {
-            // segment done: carried state back to global memory, then tell whoever continues the channel
-            // (the next segment of this push or the first segment of the next push)
-            float* gst = p.state + (long long)ch * ns;
-            if (lane < ns) __stcg(gst + lane, fk_smem[wst + lane]);
-            if (lane + 32 < ns) __stcg(gst + lane + 32, fk_smem[wst + lane + 32]);
-            __syncwarp();
-            if (lane == 0) st_release(p.progress + ch, seq0 + (unsigned)seg + 1u);
-            wcur ^= 1;
-        }
+        if (item_end) wcur ^= 1;
         ch = nch; tile = ntile; tend = ntend; seg = nseg; have = nhave; cur ^= 1;
     }
 

@@ -217,6 +217,13 @@ static cudaError_t launch_cm_shape(const filark_stream* h, const PushParams<L>& 
     int grid = (p.n_ch + W - 1) / W;
     const int resident = h->n_sm * (per_sm / W < 16 ? per_sm / W : 16);
     if (grid > resident) grid = resident;
+    // work items: runs of seg_tiles tiles of a channel, about 8 items per warp of the grid
+    PushParams<L> q = p;
+    {
+        const long long n_tiles = ((long long)p.n_t + L - 1) / L / 64 + 1;          // r0 = 0 estimate, >= 1
+        long long st = n_tiles * p.n_ch / (8LL * grid * W);
+        q.seg_tiles = (int)(st < 1 ? 1 : (st > 0x3fffffff ? 0x3fffffff : st));
+    }
     // programmatic stream serialization: the kernel lets its dependents launch as soon as it has read
     // its control slot, and orders itself against the previous push channel by channel
     // (filark_kernels.cuh); p.wait_prior = 1 makes it an ordinary dependent launch
@@ -227,7 +234,7 @@ static cudaError_t launch_cm_shape(const filark_stream* h, const PushParams<L>& 
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = std::getenv("FILARK_TUNE_NOPDL") ? 0 : 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, CTAS>, p);
+    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, CTAS>, q);
 }
 
 // Launch shape (filark_kernels.cuh): one CTA per SM when every resident warp gets a long run of tiles
@@ -252,6 +259,7 @@ static cudaError_t push_variant(const filark_stream* h, int v, const float* d_in
     p.in = d_in; p.filt = d_filt; p.cf = d_cf;
     p.state = h->d_state; p.hist = h->d_hist; p.ctl = h->d_ctl; p.cctl = h->d_cctl; p.progress = h->d_progress;
     p.in_pitch = in_pitch; p.out_pitch = out_pitch; p.n_t = n_t; p.vec4 = vec4;
+    p.n_base = n_t / L; p.n_rem = n_t % L;
     p.wait_prior = wait_prior;
     return launch_cm<L>(h, p, stream);
 }

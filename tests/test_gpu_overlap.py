@@ -27,6 +27,7 @@ def _alloc(chunks):
 @pytest.mark.parametrize("n_ch,n_t,sizes", [
     (3000, 12_000, [1500]),                 # the bench's push shape: 16-byte path, r0 alternates 0 / 12
     (2500, 9_000, [700, 333, 1501, 64]),    # ragged: 4-byte path, hist crosses pushes
+    (2000, 9_000, [1500, 100, 1000, 7]),    # the variant changes from push to push: r0 >= L of the next one
     (6000, 6_000, [1000]),                  # more channels than resident warps
     (700, 40_000, [16_000, 8_000]),         # several segments per channel and push
 ])
