@@ -117,10 +117,10 @@ filark_status_t filark_stream_create_ex(filark_stream_t **out, int n_ch, const d
  * Ordering (channel-major layout): a push is a dependent launch of whatever precedes it in
  * `stream` and sees all of that work completed -- with one exception that the library arranges
  * itself: when the operation directly before it in the stream is the previous push of the SAME
- * handle and the two pushes share no buffer (other than both reading the same input), the new
- * push starts on the device while the previous one drains and orders itself against it channel by
- * channel through the carried state (at most two pushes of a handle are in flight; outputs are
- * identical either way).  Work after a push in the stream sees that push and all earlier ones
+ * handle and the new push shares no buffer with the two pushes before it (other than reading the
+ * same input), the new push starts on the device while they drain and orders itself against them
+ * channel by channel through the carried state (at most three pushes of a handle are in flight;
+ * outputs are identical either way).  Work after a push in the stream sees that push and all earlier ones
  * completed.  A caller-written kernel between two pushes that signals programmatic launch
  * completion early (cudaTriggerProgrammaticLaunchCompletion) must not produce the next push's
  * input or read its output buffers; FILARK_FLAG_STRICT_ORDER removes the exception altogether.
