@@ -119,7 +119,8 @@ template <int L> struct PushParams {
     int n_t, n_ch, n_sec, lta_len;
     int n_base, n_rem;       // n_t = n_base L + n_rem
     int seg_tiles;           // tiles per work item (host heuristic: about 8 items per resident warp)
-    int vec4;                // 16-byte global accesses are legal (alignment, pitch, n_t % 4 == 0)
+    int vec4;                // host's view of the alignment (introspection only: the kernel derives the
+                             // shift of every row itself, see "Alignment")
     int wait_prior;          // wait for everything before this launch in the stream before touching memory
     float gain, ratio, lta_thr;
     AvgParams avg;
@@ -190,7 +191,7 @@ __device__ __forceinline__ float2 add2(float2 a, float2 b) { return __fadd2_rn(a
 template <int L> struct Geo {
     static constexpr int pitch = 2 * L + 4;        // floats per lane region: LDS.128 conflict-free
     static constexpr int tile = 64 * L;            // samples per tile
-    static constexpr int buf_floats = 32 * pitch;
+    static constexpr int buf_floats = 32 * pitch + 4;  // + one chunk: a shifted tile (below) ends in "region 32"
     static constexpr int chunks = L / 2;           // 16-byte chunks per lane region
 };
 
@@ -212,7 +213,23 @@ __device__ __forceinline__ void cp_async4(int dst_off, const float* src, int src
 // Shared memory of one warp: two tile buffers (input of tile k / staging of its outputs, and the
 // prefetched input of tile k+1) and two copies of the channel state.
 constexpr int kStateSmem = 40;                     // >= state_floats(kMaxSec), multiple of 4
-template <int L> __host__ __device__ constexpr int warp_smem_floats() { return 2 * Geo<L>::buf_floats + 2 * kStateSmem; }
+constexpr int kHistSmem = 48;                      // raw history of the next item's channel (r0 < 48)
+template <int L> __host__ __device__ constexpr int warp_smem_floats() { return 2 * Geo<L>::buf_floats + 2 * kStateSmem + kHistSmem; }
+
+// Alignment.  Global rows start anywhere (4-byte aligned pointers, any pitch, any n_t) and tile
+// position e of a push is input sample t = e - r0 (+ tile offset), so in general neither the row
+// nor the tile is 16-byte aligned.  The tile is therefore held in shared memory SHIFTED by
+// s = (row address / 4 - r0) mod 4 floats: "raw" position p = e + s has the same alignment as the
+// global element it holds, 16-byte chunks of the row are copied to 16-byte chunks of the buffer
+// (cp.async 16 B in, STG.128 out; only the at most three elements at either end of a row move one
+// by one), and the shift is undone where the lane regions meet the registers (scalar LDS/STS
+// instead of 128-bit ones when s != 0).  Input, filt and cf rows each have their own shift.
+__device__ __forceinline__ int row_shift(const float* row, int r0)
+{
+    return (int)(((unsigned)((uintptr_t)row >> 2) - (unsigned)r0) & 3u);
+}
+// index in a tile buffer of raw position p (padded lane regions)
+template <int L> __device__ __forceinline__ int raw_index(int p) { return p + 4 * (p / (2 * L)); }
 
 // S0: start the asynchronous copy of one tile of one channel into `buf` (padded lane regions:
 // tile-local sample e lives at buf[e + 4 (e / 2L)]) and, with the channel's first tile, of its
@@ -224,30 +241,40 @@ __device__ __forceinline__ void issue_tile_input(const PushParams<L>& p, const G
     const int t0 = tile * Geo<L>::tile - g.r0;
     const int n_t = p.n_t;
     const float* __restrict__ src = p.in + (long long)ch * p.in_pitch;
-    if (g.vec4) {
-        if (t0 >= 0 && t0 + Geo<L>::tile <= n_t) {                   // interior tile: no bounds
-            const float* __restrict__ srct = src + t0 + 4 * lane;
+    const int s = row_shift(src, g.r0);
+    if (s == 0 && t0 >= 0 && t0 + Geo<L>::tile <= n_t) {             // aligned interior tile: no bounds
+        const float* __restrict__ srct = src + t0 + 4 * lane;
 #pragma unroll
-            for (int m = 0; m < Geo<L>::chunks; ++m) {
-                const int c = 32 * m + lane;
-                cp_async16(buf + 4 * c + 4 * (c / Geo<L>::chunks), srct + 128 * m, 16);
-            }
-        } else {
+        for (int m = 0; m < Geo<L>::chunks; ++m) {
+            const int c = 32 * m + lane;
+            cp_async16(buf + 4 * c + 4 * (c / Geo<L>::chunks), srct + 128 * m, 16);
+        }
+    } else if (s == 0 && ((g.r0 | n_t) & 3) == 0) {                 // aligned edge tile, whole chunks only
 #pragma unroll
-            for (int m = 0; m < Geo<L>::chunks; ++m) {
-                const int c = 32 * m + lane;
-                const int t = t0 + 4 * c;
-                const bool ok = t < n_t;
-                if (t >= 0) cp_async16(buf + 4 * c + 4 * (c / Geo<L>::chunks), ok ? src + t : src, ok ? 16 : 0);
-            }
+        for (int m = 0; m < Geo<L>::chunks; ++m) {
+            const int c = 32 * m + lane;
+            const int t = t0 + 4 * c;
+            const bool ok = t < n_t;
+            if (t >= 0) cp_async16(buf + 4 * c + 4 * (c / Geo<L>::chunks), ok ? src + t : src, ok ? 16 : 0);
         }
     } else {
+        // raw chunk c holds input samples tf .. tf + 3; samples before the row (t < 0) are history
+        // (issue_tile_carry), samples behind it (t >= n_t) are zero-filled; one chunk more than a
+        // tile has, because of the shift (what it loads beyond the tile is not used)
 #pragma unroll 1
-        for (int m = 0; m < 2 * L; ++m) {
-            const int e = 32 * m + lane;
-            const int t = t0 + e;
-            const bool ok = t < n_t;
-            if (t >= 0) cp_async4(buf + e + 4 * (e / (2 * L)), src + (ok ? t : 0), ok ? 4 : 0);
+        for (int c = lane; c <= 32 * Geo<L>::chunks; c += 32) {
+            const int tf = t0 + 4 * c - s;
+            const int d = buf + 4 * c + 4 * (c / Geo<L>::chunks);
+            if (tf >= 0) {
+                const int rem = n_t - tf;
+                const int bytes = rem >= 4 ? 16 : (rem > 0 ? 4 * rem : 0);
+                cp_async16(d, bytes ? src + tf : p.hist, bytes);
+            } else if (tf > -4) {
+                for (int j = 1; j < 4; ++j) {
+                    const int t = tf + j;
+                    if (t >= 0) cp_async4(d + j, src + (t < n_t ? t : 0), t < n_t ? 4 : 0);
+                }
+            }
         }
     }
     cp_async_commit();
@@ -257,15 +284,12 @@ __device__ __forceinline__ void issue_tile_input(const PushParams<L>& p, const G
 // positions [0, r0)) and the carried state into `wst`.  Both are rewritten by pushes that overlap
 // this one on the device: never read through L1, and only after `progress` says they are there.
 template <int L>
-__device__ __forceinline__ void issue_tile_carry(const PushParams<L>& p, const Geom& g, int ch, int buf, int wst, int lane)
+__device__ __forceinline__ void issue_tile_carry(const PushParams<L>& p, const Geom& g, int ch, int whs, int wst, int lane)
 {
+    // (history goes to the warp's scratch first: where it belongs in the tile buffer depends on the
+    // row's shift, and it is moved there when the tile is taken up)
     const float* __restrict__ hist = p.hist + (long long)ch * kHist;
-    if (g.vec4) {
-        const int c = lane;                                           // r0 < L: at most L / 4 <= 12 chunks
-        if (4 * c < g.r0) cp_async16(buf + 4 * c + 4 * (c / Geo<L>::chunks), hist + 4 * c, 16);
-    } else {
-        for (int e = lane; e < g.r0; e += 32) fk_smem[buf + e + 4 * (e / (2 * L))] = __ldcg(hist + e);
-    }
+    if (4 * lane < g.r0) cp_async16(whs + 4 * lane, hist + 4 * lane, 16);
     const int ns = state_floats(p.n_sec);
     const float* gst = p.state + (long long)ch * ns;
     if (4 * lane < ns) cp_async16(wst + 4 * lane, gst + 4 * lane, 16);
@@ -276,47 +300,90 @@ __device__ __forceinline__ void issue_tile_carry(const PushParams<L>& p, const G
 // map to t < 0 (recomputed history) or t >= n_t (padding) are dropped.
 template <int L>
 __device__ __forceinline__ void store_tile(const PushParams<L>& p, const Geom& g, float* __restrict__ dst, int buf,
-                                           int lane, int t0)
+                                           int lane, int t0, int s)
 {
     const int n_t = p.n_t;
-    if (g.vec4) {
-        if (t0 >= 0 && t0 + Geo<L>::tile <= n_t) {
-            float* __restrict__ dstt = dst + t0 + 4 * lane;
+    if (s == 0 && t0 >= 0 && t0 + Geo<L>::tile <= n_t) {
+        float* __restrict__ dstt = dst + t0 + 4 * lane;
 #pragma unroll
-            for (int m = 0; m < Geo<L>::chunks; ++m) {
-                const int c = 32 * m + lane;
-                const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + 4 * c + 4 * (c / Geo<L>::chunks)]);
-                st_stream4(dstt + 128 * m, v);
-            }
-        } else {
-            float* __restrict__ dstt = dst + t0;
+        for (int m = 0; m < Geo<L>::chunks; ++m) {
+            const int c = 32 * m + lane;
+            const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + 4 * c + 4 * (c / Geo<L>::chunks)]);
+            st_stream4(dstt + 128 * m, v);
+        }
+    } else if (s == 0 && ((g.r0 | n_t) & 3) == 0) {                 // aligned edge tile, whole chunks only
+        float* __restrict__ dstt = dst + t0;
 #pragma unroll
-            for (int m = 0; m < Geo<L>::chunks; ++m) {
-                const int c = 32 * m + lane;
-                const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + 4 * c + 4 * (c / Geo<L>::chunks)]);
-                if ((unsigned)(t0 + 4 * c) < (unsigned)n_t) st_stream4(dstt + 4 * c, v);
-            }
+        for (int m = 0; m < Geo<L>::chunks; ++m) {
+            const int c = 32 * m + lane;
+            const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + 4 * c + 4 * (c / Geo<L>::chunks)]);
+            if ((unsigned)(t0 + 4 * c) < (unsigned)n_t) st_stream4(dstt + 4 * c, v);
         }
     } else {
+        // element j of raw chunk c is tile position e = 4 c + j - s: only 0 <= e < tile belongs to
+        // this tile (the first chunk starts with the previous tile's last samples, the extra chunk
+        // ends with the next tile's first ones), and only 0 <= t < n_t exists
 #pragma unroll 1
-        for (int m = 0; m < 2 * L; ++m) {
-            const int e = 32 * m + lane;
-            const int t = t0 + e;
-            const float v = fk_smem[buf + e + 4 * (e / (2 * L))];
-            if ((unsigned)t < (unsigned)n_t) st_stream(dst + t, v);
+        for (int c = lane; c <= 32 * Geo<L>::chunks; c += 32) {
+            const int e = 4 * c - s;
+            const int tf = t0 + e;
+            const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + 4 * c + 4 * (c / Geo<L>::chunks)]);
+            if (e >= 0 && e + 4 <= Geo<L>::tile && tf >= 0 && tf + 4 <= n_t) {
+                st_stream4(dst + tf, v);
+            } else {
+                const float vv[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    if ((unsigned)(e + j) < (unsigned)Geo<L>::tile && (unsigned)(tf + j) < (unsigned)n_t)
+                        st_stream(dst + tf + j, vv[j]);
+            }
         }
     }
 }
 
-// Unpack the lane's pairs into its shared-memory region: lo samples then hi samples.
+// Unpack the lane's pairs into its shared-memory region: lo samples then hi samples (raw positions
+// 2L lane + s ...: the last few hi samples of a shifted tile fall into the next region).
 template <int L>
-__device__ __forceinline__ void regs_to_buf(const float2 (&x)[L], int buf, int lane)
+__device__ __forceinline__ void regs_to_buf(const float2 (&x)[L], int buf, int lane, int s)
 {
-    float4* d = reinterpret_cast<float4*>(&fk_smem[buf + lane * Geo<L>::pitch]);
+    if (s == 0) {
+        float4* d = reinterpret_cast<float4*>(&fk_smem[buf + lane * Geo<L>::pitch]);
 #pragma unroll
-    for (int q = 0; q < L / 4; ++q) {
-        d[q] = make_float4(x[4 * q].x, x[4 * q + 1].x, x[4 * q + 2].x, x[4 * q + 3].x);
-        d[L / 4 + q] = make_float4(x[4 * q].y, x[4 * q + 1].y, x[4 * q + 2].y, x[4 * q + 3].y);
+        for (int q = 0; q < L / 4; ++q) {
+            d[q] = make_float4(x[4 * q].x, x[4 * q + 1].x, x[4 * q + 2].x, x[4 * q + 3].x);
+            d[L / 4 + q] = make_float4(x[4 * q].y, x[4 * q + 1].y, x[4 * q + 2].y, x[4 * q + 3].y);
+        }
+    } else {
+        const int base = buf + lane * Geo<L>::pitch + s;
+#pragma unroll
+        for (int i = 0; i < L; ++i) {
+            fk_smem[base + i] = x[i].x;
+            const int o = L + i;
+            fk_smem[base + o + ((i >= L - 3 && s + o >= 2 * L) ? 4 : 0)] = x[i].y;
+        }
+    }
+}
+
+// The reverse: the lane's region -> packed pairs, times the cascade's gain.
+template <int L>
+__device__ __forceinline__ void buf_to_regs(float2 (&x)[L], int buf, int lane, int s, float gn)
+{
+    if (s == 0) {
+        const float4* r = reinterpret_cast<const float4*>(&fk_smem[buf + lane * Geo<L>::pitch]);
+#pragma unroll
+        for (int q = 0; q < L / 4; ++q) {
+            const float4 a = r[q], b = r[L / 4 + q];
+            x[4 * q] = make_float2(a.x * gn, b.x * gn); x[4 * q + 1] = make_float2(a.y * gn, b.y * gn);
+            x[4 * q + 2] = make_float2(a.z * gn, b.z * gn); x[4 * q + 3] = make_float2(a.w * gn, b.w * gn);
+        }
+    } else {
+        const int base = buf + lane * Geo<L>::pitch + s;
+#pragma unroll
+        for (int i = 0; i < L; ++i) {
+            const int o = L + i;
+            x[i] = make_float2(fk_smem[base + i] * gn,
+                               fk_smem[base + o + ((i >= L - 3 && s + o >= 2 * L) ? 4 : 0)] * gn);
+        }
     }
 }
 
@@ -433,9 +500,11 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
     }
 
     if (p.filt) {
-        regs_to_buf<L>(x, buf, lane);
+        float* row = p.filt + (long long)ch * p.out_pitch;
+        const int sf = row_shift(row, g.r0);
+        regs_to_buf<L>(x, buf, lane, sf);
         __syncwarp();
-        store_tile<L>(p, g, p.filt + (long long)ch * p.out_pitch, buf, lane, t0);
+        store_tile<L>(p, g, row, buf, lane, t0, sf);
         __syncwarp();
     }
 
@@ -511,10 +580,12 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
                 x[i].y = (Pl.y > thr && base + L + i >= wm) ? qb : 0.0f;
             }
         }
-        regs_to_buf<L>(x, buf, lane);
+        float* row = p.cf + (long long)ch * p.out_pitch;
+        const int sc = row_shift(row, g.r0);
+        regs_to_buf<L>(x, buf, lane, sc);
         __syncwarp();
         if (item_end && lane == 0) st_release(p.progress + ch, rel_val);
-        store_tile<L>(p, g, p.cf + (long long)ch * p.out_pitch, buf, lane, t0);
+        store_tile<L>(p, g, row, buf, lane, t0, sc);
     } else if (item_end) {
         __syncwarp();
         if (lane == 0) st_release(p.progress + ch, rel_val);
@@ -592,6 +663,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     const int lane = threadIdx.x & 31, W = blockDim.x >> 5;
     const int wbase = warp * warp_smem_floats<L>();                   // two tile buffers, then two state copies
     const int wst0 = wbase + 2 * Geo<L>::buf_floats;
+    const int whs = wst0 + 2 * kStateSmem;                            // history scratch
     const int gw = CTAS == 1 ? (int)(blockIdx.x + gridDim.x * warp) : (int)(blockIdx.x * W + warp);   // warp index in the grid
     __shared__ unsigned sh_ctl[32];
     __shared__ unsigned sh_flag;
@@ -680,7 +752,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     // those loads are issued (a wait on an EARLIER push cannot be part of a cycle)
     if (have && seg == 0) {
         wait_progress(ch, seq0, pr0);
-        issue_tile_carry<L>(p, g, ch, wbase, wst0, lane);
+        issue_tile_carry<L>(p, g, ch, whs, wst0, lane);
     }
     FK_TR(7);
     if (warp == 0) {
@@ -731,33 +803,27 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
             if (lane + 32 < ns) fk_smem[wst + lane + 32] = __ldcg(gst + lane + 32);
             __syncwarp();
         }
+        const int sin = row_shift(p.in + (long long)ch * p.in_pitch, g.r0);
+        if (tile == 0 && g.r0 != 0) {
+            // first tile of the channel: the waiting raw samples from the scratch to the head of the tile
+            for (int e = lane; e < g.r0; e += 32) fk_smem[buf + raw_index<L>(e + sin)] = fk_smem[whs + e];
+            __syncwarp();
+        }
         if (tile == g.n_tiles - 1 && g.r1 != 0) {
             // last tile of the channel: keep the raw samples of its trailing partial slot
             const int e0 = g.q_last * L;                              // tile-space position of that slot
             float* hd = p.hist + (long long)ch * kHist;
-            for (int j = lane; j < g.r1; j += 32) {
-                const int e = e0 + j;
-                hd[j] = fk_smem[buf + e + 4 * (e / (2 * L))];
-            }
+            for (int j = lane; j < g.r1; j += 32) hd[j] = fk_smem[buf + raw_index<L>(e0 + j + sin)];
         }
         float2 x[L];
-        {
-            const float4* s = reinterpret_cast<const float4*>(&fk_smem[buf + lane * Geo<L>::pitch]);
-            const float gn = p.gain;
-#pragma unroll
-            for (int q = 0; q < L / 4; ++q) {
-                const float4 a = s[q], b = s[L / 4 + q];
-                x[4 * q] = make_float2(a.x * gn, b.x * gn); x[4 * q + 1] = make_float2(a.y * gn, b.y * gn);
-                x[4 * q + 2] = make_float2(a.z * gn, b.z * gn); x[4 * q + 3] = make_float2(a.w * gn, b.w * gn);
-            }
-        }
+        buf_to_regs<L>(x, buf, lane, sin, p.gain);
         __syncwarp();
         if (nhave) {
             const int nbuf = wbase + (cur ^ 1) * Geo<L>::buf_floats;
             issue_tile_input<L>(p, g, nch, ntile, nbuf, lane);
             if (item_end && nseg == 0) {
                 wait_progress(nch, seq0, npr);
-                issue_tile_carry<L>(p, g, nch, nbuf, wst0 + (wcur ^ 1) * kStateSmem, lane);
+                issue_tile_carry<L>(p, g, nch, whs, wst0 + (wcur ^ 1) * kStateSmem, lane);
             }
         }
         // (a segment's end writes the carried state back and tells whoever continues the channel:

@@ -600,6 +600,14 @@ filark_status_t filark_stream_push_host(filark_stream_t* h, const float* h_in, l
 }
 
 #ifdef FK_TRACE
+int filark_trace_occupancy(int warps)
+{
+    int n = -1;
+    const size_t smem = (size_t)warps * sizeof(float) * warp_smem_floats<24>();
+    cudaFuncSetAttribute(filark_push_cm_kernel<24, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, filark_push_cm_kernel<24, 4>, warps * 32, smem);
+    return n;
+}
 int filark_trace_read(unsigned long long* out, unsigned max_words, int reset)
 {
     const unsigned n = 16u * 4096u * 16u * 2u;
