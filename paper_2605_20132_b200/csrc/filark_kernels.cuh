@@ -235,21 +235,23 @@ template <int L> __device__ __forceinline__ int raw_index(int p) { return p + 4 
 // tile-local sample e lives at buf[e + 4 (e / 2L)]) and, with the channel's first tile, of its
 // carried state into `wst`.  Tile-space position e of tile `tile` is input sample
 // t = tile 64L + e - r0; t < 0 reads hist[ch][r0 + t], t >= n_t is zero-filled.
-template <int L>
+template <int L, bool kInterior>
 __device__ __forceinline__ void issue_tile_input(const PushParams<L>& p, const Geom& g, int ch, int tile, int buf, int lane)
 {
     const int t0 = tile * Geo<L>::tile - g.r0;
     const int n_t = p.n_t;
     const float* __restrict__ src = p.in + (long long)ch * p.in_pitch;
     const int s = row_shift(src, g.r0);
-    if (s == 0 && t0 >= 0 && t0 + Geo<L>::tile <= n_t) {             // aligned interior tile: no bounds
+    if (kInterior && s == 0 && t0 >= 0 && t0 + Geo<L>::tile <= n_t) {   // aligned interior tile: no bounds
+        // (only in the kernel built for long pushes: elsewhere the instruction cache is the scarcer
+        // resource and one path serves interior and edge tiles)
         const float* __restrict__ srct = src + t0 + 4 * lane;
 #pragma unroll
         for (int m = 0; m < Geo<L>::chunks; ++m) {
             const int c = 32 * m + lane;
             cp_async16(buf + 4 * c + 4 * (c / Geo<L>::chunks), srct + 128 * m, 16);
         }
-    } else if (s == 0 && ((g.r0 | n_t) & 3) == 0) {                 // aligned edge tile, whole chunks only
+    } else if (s == 0 && ((g.r0 | n_t) & 3) == 0) {                  // aligned rows, whole chunks only
 #pragma unroll
         for (int m = 0; m < Geo<L>::chunks; ++m) {
             const int c = 32 * m + lane;
@@ -298,12 +300,12 @@ __device__ __forceinline__ void issue_tile_carry(const PushParams<L>& p, const G
 
 // S7: the lane regions of `buf` -> one output array (coalesced 16-byte stores).  Positions that
 // map to t < 0 (recomputed history) or t >= n_t (padding) are dropped.
-template <int L>
+template <int L, bool kInterior>
 __device__ __forceinline__ void store_tile(const PushParams<L>& p, const Geom& g, float* __restrict__ dst, int buf,
                                            int lane, int t0, int s)
 {
     const int n_t = p.n_t;
-    if (s == 0 && t0 >= 0 && t0 + Geo<L>::tile <= n_t) {
+    if (kInterior && s == 0 && t0 >= 0 && t0 + Geo<L>::tile <= n_t) {
         float* __restrict__ dstt = dst + t0 + 4 * lane;
 #pragma unroll
         for (int m = 0; m < Geo<L>::chunks; ++m) {
@@ -311,7 +313,7 @@ __device__ __forceinline__ void store_tile(const PushParams<L>& p, const Geom& g
             const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + 4 * c + 4 * (c / Geo<L>::chunks)]);
             st_stream4(dstt + 128 * m, v);
         }
-    } else if (s == 0 && ((g.r0 | n_t) & 3) == 0) {                 // aligned edge tile, whole chunks only
+    } else if (s == 0 && ((g.r0 | n_t) & 3) == 0) {                  // aligned rows, whole chunks only
         float* __restrict__ dstt = dst + t0;
 #pragma unroll
         for (int m = 0; m < Geo<L>::chunks; ++m) {
@@ -441,7 +443,7 @@ __device__ __forceinline__ void local_pass(float2 (&x)[L], const SecParams<L>& T
 
 // One tile of one channel, samples already in x (gain applied): S1..S7.  `buf` stages the
 // outputs.  buf / wst are float offsets into fk_smem.
-template <int L>
+template <int L, bool kInterior, bool kAllKinds>
 __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom& g, int buf, int wst, float2 (&x)[L],
                                              int ch, int tile, int lane, unsigned long long seen,
                                              bool item_end, unsigned rel_val)
@@ -458,12 +460,19 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
     for (int k = 0; k < p.n_sec; ++k) {
         const SecParams<L>& T = p.sec[k];
         float2 s1, s2;
-        switch (T.kind) {
-            case kKindDF2: local_pass<L, kKindDF2>(x, T, s1, s2); break;
-            case kKindDelta: local_pass<L, kKindDelta>(x, T, s1, s2); break;
-            case kKindDeltaG: local_pass<L, kKindDeltaG>(x, T, s1, s2); break;
-            case kKindNormal: local_pass<L, kKindNormal>(x, T, s1, s2); break;
-            default: local_pass<L, kKindDF2G>(x, T, s1, s2); break;
+        // (kAllKinds = false: the kernel for cascades made of the two common section forms only --
+        // what a Butterworth bandpass gives -- without the code of the other three)
+        if (kAllKinds) {
+            switch (T.kind) {
+                case kKindDF2: local_pass<L, kKindDF2>(x, T, s1, s2); break;
+                case kKindDelta: local_pass<L, kKindDelta>(x, T, s1, s2); break;
+                case kKindDeltaG: local_pass<L, kKindDeltaG>(x, T, s1, s2); break;
+                case kKindNormal: local_pass<L, kKindNormal>(x, T, s1, s2); break;
+                default: local_pass<L, kKindDF2G>(x, T, s1, s2); break;
+            }
+        } else {
+            if (T.kind == kKindDF2) local_pass<L, kKindDF2>(x, T, s1, s2);
+            else local_pass<L, kKindDelta>(x, T, s1, s2);
         }
         // S2: lane total W = P a + b (a, b: end states of the lo / hi slot from rest); the carried
         // state S enters lane 0's total through A^2L; inclusive scan over the lanes
@@ -504,7 +513,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
         const int sf = row_shift(row, g.r0);
         regs_to_buf<L>(x, buf, lane, sf);
         __syncwarp();
-        store_tile<L>(p, g, row, buf, lane, t0, sf);
+        store_tile<L, kInterior>(p, g, row, buf, lane, t0, sf);
         __syncwarp();
     }
 
@@ -585,7 +594,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
         regs_to_buf<L>(x, buf, lane, sc);
         __syncwarp();
         if (item_end && lane == 0) st_release(p.progress + ch, rel_val);
-        store_tile<L>(p, g, row, buf, lane, t0, sc);
+        store_tile<L, kInterior>(p, g, row, buf, lane, t0, sc);
     } else if (item_end) {
         __syncwarp();
         if (lane == 0) st_release(p.progress + ch, rel_val);
@@ -652,7 +661,7 @@ template <int L, int CTAS> __host__ __device__ constexpr int cm_cta_warps() { re
 // with FILARK_FLAG_STRICT_ORDER: then the kernel begins with griddepcontrol.wait like any
 // dependent launch).  Every CTA ends with griddepcontrol.wait, so a push never completes before the
 // push in front of it.
-template <int L, int CTAS>
+template <int L, int CTAS, bool kAllKinds>
 __global__ void __launch_bounds__(cm_cta_warps<L, CTAS>() * 32, CTAS)
 filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
 {
@@ -747,7 +756,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     if (warp == 0 && lane == 0) tk = atomicAdd(&cc->ticket, 1u);
 
     bool have = claim(ch, tile, tend, seg);
-    if (have) issue_tile_input<L>(p, g, ch, tile, wbase, lane);
+    if (have) issue_tile_input<L, CTAS == 1>(p, g, ch, tile, wbase, lane);
     // the first segment of a channel needs what the previous push left (state, hist): wait before
     // those loads are issued (a wait on an EARLIER push cannot be part of a cycle)
     if (have && seg == 0) {
@@ -820,7 +829,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         __syncwarp();
         if (nhave) {
             const int nbuf = wbase + (cur ^ 1) * Geo<L>::buf_floats;
-            issue_tile_input<L>(p, g, nch, ntile, nbuf, lane);
+            issue_tile_input<L, CTAS == 1>(p, g, nch, ntile, nbuf, lane);
             if (item_end && nseg == 0) {
                 wait_progress(nch, seq0, npr);
                 issue_tile_carry<L>(p, g, nch, whs, wst0 + (wcur ^ 1) * kStateSmem, lane);
@@ -828,7 +837,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         }
         // (a segment's end writes the carried state back and tells whoever continues the channel:
         // the next segment of this push or the first segment of the next push)
-        process_tile<L>(p, g, buf, wst, x, ch, tile, lane, seen, item_end, seq0 + (unsigned)seg + 1u);
+        process_tile<L, CTAS == 1, kAllKinds>(p, g, buf, wst, x, ch, tile, lane, seen, item_end, seq0 + (unsigned)seg + 1u);
         FK_TR(4);
         if (item_end) wcur ^= 1;
         ch = nch; tile = ntile; tend = ntend; seg = nseg; have = nhave; cur ^= 1;

@@ -31,6 +31,7 @@ struct filark_stream {
     int n_ch, n_sec, sta_len, lta_len, layout;
     unsigned flags;
     Section sec[kMaxSec];
+    bool lean_kinds;                // every section is kKindDF2 or kKindDelta: the smaller kernel serves
     double gain;
     void* proto[kNumVariants];      // host PushParams<L> with every table filled; pointers patched per push
     SerialParams serial;            // the same for the serial diagnostic kernel
@@ -190,7 +191,7 @@ static Geom geometry_rt(int L, unsigned r0, int n_t, bool vec4)
 
 // CTAS CTAs per SM, W warps per CTA; fewer warps per CTA, on more SMs, when there are few
 // channels.  Every CTA of a push fits on the device at once (the segment waits rely on it).
-template <int L, int CTAS>
+template <int L, int CTAS, bool kAllKinds>
 static cudaError_t launch_cm_shape(const filark_stream* h, const PushParams<L>& p, cudaStream_t stream)
 {
     const size_t warp_bytes = sizeof(float) * (size_t)warp_smem_floats<L>();
@@ -209,7 +210,7 @@ static cudaError_t launch_cm_shape(const filark_stream* h, const PushParams<L>& 
     const size_t smem = (size_t)W * warp_bytes;
     static bool attr_done = false;           // per template instance; idempotent
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(filark_push_cm_kernel<L, CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+        cudaError_t e = cudaFuncSetAttribute(filark_push_cm_kernel<L, CTAS, kAllKinds>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                              (int)((size_t)cm_cta_warps<L, CTAS>() * warp_bytes));
         if (e != cudaSuccess) return e;
         attr_done = true;
@@ -234,7 +235,7 @@ static cudaError_t launch_cm_shape(const filark_stream* h, const PushParams<L>& 
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = std::getenv("FILARK_TUNE_NOPDL") ? 0 : 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, CTAS>, q);
+    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, CTAS, kAllKinds>, q);
 }
 
 // Launch shape (filark_kernels.cuh): one CTA per SM when every resident warp gets a long run of tiles
@@ -245,9 +246,11 @@ static cudaError_t launch_cm(const filark_stream* h, const PushParams<L>& p, cud
     if constexpr (L == 24) {
         const long long tiles = ((long long)p.n_t + kHist + Geo<L>::tile - 1) / Geo<L>::tile * p.n_ch;
         const bool long_push = tiles >= 12LL * h->n_sm * cm_max_warps<L>();
-        if (long_push && !std::getenv("FILARK_TUNE_SMALL_CTAS")) return launch_cm_shape<24, 1>(h, p, stream);
+        if (long_push && !std::getenv("FILARK_TUNE_SMALL_CTAS"))
+            return h->lean_kinds ? launch_cm_shape<24, 1, false>(h, p, stream) : launch_cm_shape<24, 1, true>(h, p, stream);
     }
-    return launch_cm_shape<L, kCmCtasPerSm>(h, p, stream);
+    return h->lean_kinds ? launch_cm_shape<L, kCmCtasPerSm, false>(h, p, stream)
+                         : launch_cm_shape<L, kCmCtasPerSm, true>(h, p, stream);
 }
 
 template <int L>
@@ -323,6 +326,8 @@ filark_status_t filark_stream_create_ex(filark_stream_t** out, int n_ch, const d
     std::memset(h, 0, sizeof(*h));
     st = design_all(sos, n_sec, h->sec, &h->gain);
     if (st != FILARK_OK) { delete h; return st; }
+    h->lean_kinds = !std::getenv("FILARK_TUNE_ALL_KINDS");
+    for (int k = 0; k < n_sec; ++k) h->lean_kinds = h->lean_kinds && (h->sec[k].kind == kKindDF2 || h->sec[k].kind == kKindDelta);
     h->n_ch = n_ch; h->n_sec = n_sec; h->sta_len = sta_len; h->lta_len = lta_len;
     h->layout = layout; h->flags = flags;
     h->state_floats = (size_t)n_ch * (size_t)state_floats(n_sec);
@@ -604,8 +609,8 @@ int filark_trace_occupancy(int warps)
 {
     int n = -1;
     const size_t smem = (size_t)warps * sizeof(float) * warp_smem_floats<24>();
-    cudaFuncSetAttribute(filark_push_cm_kernel<24, 4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, filark_push_cm_kernel<24, 4>, warps * 32, smem);
+    cudaFuncSetAttribute(filark_push_cm_kernel<24, 4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, filark_push_cm_kernel<24, 4, false>, warps * 32, smem);
     return n;
 }
 int filark_trace_read(unsigned long long* out, unsigned max_words, int reset)

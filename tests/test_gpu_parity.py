@@ -244,3 +244,26 @@ def test_push_host_end_to_end(cuda_device):
     assert_parity(torch.cat(fs, 1).numpy(), ref_f, "push_host filt")
     assert_parity(torch.cat(cs, 1).numpy(), ref_c, "push_host cf")
     s.destroy()
+
+
+@pytest.mark.parametrize("sizes", [[0], [1500], [700, 333, 1501, 64]])
+def test_all_section_forms(cuda_device, sizes):
+    """A cascade that needs every section form of csrc/design.hpp (b0 = 0, first order, identity,
+    double real pole, poles near z = 1 with and without zeros there, poles near z = -1): the
+    general kernel, not the one built for Butterworth-type cascades only."""
+    from paper_2605_20132_b200.stream import FilarkStream, debug_design
+    sos = np.array([[0.0, 1.0, 0.0, 1.0, -1.9, 0.9025 + 1e-4],
+                    [2.0, 0.5, 0.0, 2.0, -1.0, 0.0],
+                    [1.0, 0.0, 0.0, 1.0, 0.0, 0.0],
+                    [0.3, 0.1, 0.2, 1.0, -1.6, 0.64],
+                    [1.0, 2.0, 1.0, 1.0, -1.95, 0.9512],
+                    [1.0, -1.0, 0.0, 1.0, -0.999, 0.0],
+                    [0.5, 0.3, 0.5, 1.0, 1.9, 0.9125]])
+    assert set(debug_design(sos)[0]) == {0, 1, 2, 3, 4}
+    n_ch, n_t = 37, 20_000
+    x = torch.from_numpy(np.random.default_rng(11).standard_normal((n_ch, n_t)).astype(np.float32))
+    ref_f, ref_c = run_oracle(x.numpy(), sos, 40, 900)
+    s = FilarkStream(n_ch, sos, 40, 900)
+    f, c = run_gpu(s, x.to(cuda_device), CHANNEL_MAJOR, [(0, n_t)] if sizes == [0] else split(n_t, sizes))
+    _check(f, c, ref_f, ref_c, CHANNEL_MAJOR, f"all section forms {sizes}")
+    s.destroy()
