@@ -389,6 +389,104 @@ __device__ __forceinline__ void buf_to_regs(float2 (&x)[L], int buf, int lane, i
     }
 }
 
+// ---- time-major chunks ([n_t][n_ch], PAPER.md:160 dims='nt_nc') --------------------------------
+// The same kernel serves them through a transpose in shared memory: a CTA of kTmChannels warps
+// owns kTmChannels ADJACENT channels (one per warp, exactly as in the channel-major mapping), and
+// its threads move a tile together: thread (c, j) = (tid mod kTmChannels, tid / kTmChannels)
+// copies element (time j + 32 k, channel c) for k = 0, 1, ... -- 64 contiguous bytes of a time row
+// per 16 threads -- into / out of warp c's tile buffer.  No shift (nothing is wider than 4 bytes).
+constexpr int kTmChannels = 16;
+// distance between the shared-memory areas of two warps: = 4 (mod 32) floats in the time-major
+// mapping, so that the 16 channels of one time sample fall into 8 different banks
+template <int L, bool kTM> __host__ __device__ constexpr int warp_stride()
+{
+    return kTM ? warp_smem_floats<L>() + ((36 - warp_smem_floats<L>() % 32) % 32) : warp_smem_floats<L>();
+}
+
+// (addresses advance incrementally -- 32 time samples per step, a hop over the 16-byte pad whenever
+// a lane region of 2L floats ends: these loops run once per element and must stay a few
+// instructions long)
+template <int L> struct TmWalk {
+    static constexpr int R = 2 * L;                 // floats per lane region
+    unsigned sa;                                    // shared-space byte address of the element
+    int r;                                          // its position inside the lane region
+    __device__ __forceinline__ TmWalk(int float_off, int e0)
+    {
+        sa = (unsigned)__cvta_generic_to_shared(&fk_smem[float_off + raw_index<L>(e0)]);
+        r = e0 % R;
+    }
+    __device__ __forceinline__ void step()
+    {
+        sa += 128u + 16u * (32 / R);
+        r += 32 % R;
+        if (32 % R != 0 && r >= R) { r -= R; sa += 16u; }
+    }
+};
+
+template <int L>
+__device__ __forceinline__ void issue_tile_input_tm(const PushParams<L>& p, const Geom& g, int cg, int tile, int bufoff)
+{
+    constexpr int S = warp_stride<L, true>();
+    const int c = threadIdx.x & (kTmChannels - 1), j = threadIdx.x / kTmChannels;
+    const int ch = cg * kTmChannels + c;
+    const int t0 = tile * Geo<L>::tile - g.r0;
+    const bool chok = ch < p.n_ch;
+    TmWalk<L> w(c * S + bufoff, j);
+    const float* gp = p.in + ch + (long long)(t0 + j) * p.in_pitch;
+    const long long gstep = 32LL * p.in_pitch;
+    if (chok && t0 >= 0 && t0 + Geo<L>::tile <= p.n_t) {
+#pragma unroll 4
+        for (int k = 0; k < Geo<L>::tile / 32; ++k) {
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(w.sa), "l"(gp) : "memory");
+            gp += gstep; w.step();
+        }
+    } else {
+        int t = t0 + j;
+#pragma unroll 2
+        for (int k = 0; k < Geo<L>::tile / 32; ++k) {
+            const bool ok = chok && t < p.n_t;
+            if (t >= 0)
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(w.sa), "l"(ok ? gp : p.in), "r"(ok ? 4 : 0) : "memory");
+            gp += gstep; t += 32; w.step();
+        }
+    }
+    cp_async_commit();
+}
+
+template <int L>
+__device__ __forceinline__ void store_tile_tm(const PushParams<L>& p, const Geom& g, float* __restrict__ out, int cg,
+                                              int bufoff, int t0)
+{
+    constexpr int S = warp_stride<L, true>();
+    const int c = threadIdx.x & (kTmChannels - 1), j = threadIdx.x / kTmChannels;
+    const int ch = cg * kTmChannels + c;
+    if (ch < p.n_ch) {
+        TmWalk<L> w(c * S + bufoff, j);
+        float* gp = out + ch + (long long)(t0 + j) * p.out_pitch;
+        const long long gstep = 32LL * p.out_pitch;
+        if (t0 >= 0 && t0 + Geo<L>::tile <= p.n_t) {
+#pragma unroll 4
+            for (int k = 0; k < Geo<L>::tile / 32; ++k) {
+                float v;
+                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(w.sa));
+                st_stream(gp, v);
+                gp += gstep; w.step();
+            }
+        } else {
+            int t = t0 + j;
+#pragma unroll 2
+            for (int k = 0; k < Geo<L>::tile / 32; ++k) {
+                if ((unsigned)t < (unsigned)p.n_t) {
+                    float v;
+                    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(w.sa));
+                    st_stream(gp, v);
+                }
+                gp += gstep; t += 32; w.step();
+            }
+        }
+    }
+}
+
 // S1: zero-state response of one section on the lane's two slots (the two halves of every
 // pair); returns the end states s1 = (lo state 1, hi state 1), s2 = (lo state 2, hi state 2).
 template <int L, int KIND>
@@ -443,10 +541,13 @@ __device__ __forceinline__ void local_pass(float2 (&x)[L], const SecParams<L>& T
 
 // One tile of one channel, samples already in x (gain applied): S1..S7.  `buf` stages the
 // outputs.  buf / wst are float offsets into fk_smem.
-template <int L, bool kInterior, bool kAllKinds>
+// (kTM: time-major chunk; the CTA's warps hold the channels cg kTmChannels + warp and store together;
+// `bufoff` = buf relative to the warp's shared-memory area; `item_end` is false for a warp whose
+// channel does not exist)
+template <int L, bool kInterior, bool kAllKinds, bool kTM>
 __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom& g, int buf, int wst, float2 (&x)[L],
                                              int ch, int tile, int lane, unsigned long long seen,
-                                             bool item_end, unsigned rel_val)
+                                             bool item_end, unsigned rel_val, int cg, int bufoff)
 {
     const bool last = tile == g.n_tiles - 1;
     const int t0 = tile * Geo<L>::tile - g.r0;
@@ -509,12 +610,19 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
     }
 
     if (p.filt) {
-        float* row = p.filt + (long long)ch * p.out_pitch;
-        const int sf = row_shift(row, g.r0);
-        regs_to_buf<L>(x, buf, lane, sf);
-        __syncwarp();
-        store_tile<L, kInterior>(p, g, row, buf, lane, t0, sf);
-        __syncwarp();
+        if (kTM) {
+            regs_to_buf<L>(x, buf, lane, 0);
+            __syncthreads();
+            store_tile_tm<L>(p, g, p.filt, cg, bufoff, t0);
+            __syncthreads();
+        } else {
+            float* row = p.filt + (long long)ch * p.out_pitch;
+            const int sf = row_shift(row, g.r0);
+            regs_to_buf<L>(x, buf, lane, sf);
+            __syncwarp();
+            store_tile<L, kInterior>(p, g, row, buf, lane, t0, sf);
+            __syncwarp();
+        }
     }
 
     // ---- S4..S6: energy, the two averages, ratio --------------------------------------------
@@ -589,12 +697,19 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
                 x[i].y = (Pl.y > thr && base + L + i >= wm) ? qb : 0.0f;
             }
         }
-        float* row = p.cf + (long long)ch * p.out_pitch;
-        const int sc = row_shift(row, g.r0);
-        regs_to_buf<L>(x, buf, lane, sc);
-        __syncwarp();
-        if (item_end && lane == 0) st_release(p.progress + ch, rel_val);
-        store_tile<L, kInterior>(p, g, row, buf, lane, t0, sc);
+        if (kTM) {
+            regs_to_buf<L>(x, buf, lane, 0);
+            __syncthreads();
+            if (item_end && lane == 0) st_release(p.progress + ch, rel_val);
+            store_tile_tm<L>(p, g, p.cf, cg, bufoff, t0);
+        } else {
+            float* row = p.cf + (long long)ch * p.out_pitch;
+            const int sc = row_shift(row, g.r0);
+            regs_to_buf<L>(x, buf, lane, sc);
+            __syncwarp();
+            if (item_end && lane == 0) st_release(p.progress + ch, rel_val);
+            store_tile<L, kInterior>(p, g, row, buf, lane, t0, sc);
+        }
     } else if (item_end) {
         __syncwarp();
         if (lane == 0) st_release(p.progress + ch, rel_val);
@@ -661,7 +776,9 @@ template <int L, int CTAS> __host__ __device__ constexpr int cm_cta_warps() { re
 // with FILARK_FLAG_STRICT_ORDER: then the kernel begins with griddepcontrol.wait like any
 // dependent launch).  Every CTA ends with griddepcontrol.wait, so a push never completes before the
 // push in front of it.
-template <int L, int CTAS, bool kAllKinds>
+// kTM: time-major chunks through the transpose in shared memory (above): CTAS = 1, kTmChannels warps;
+// the work items are (segment, group of kTmChannels channels) and belong to the CTA as a whole.
+template <int L, int CTAS, bool kAllKinds, bool kTM = false>
 __global__ void __launch_bounds__(cm_cta_warps<L, CTAS>() * 32, CTAS)
 filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
 {
@@ -670,10 +787,11 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     // tables be read through uniform registers
     const int warp = __shfl_sync(0xffffffffu, (int)(threadIdx.x >> 5), 0);
     const int lane = threadIdx.x & 31, W = blockDim.x >> 5;
-    const int wbase = warp * warp_smem_floats<L>();                   // two tile buffers, then two state copies
+    const int wbase = warp * warp_stride<L, kTM>();                   // two tile buffers, two state copies, history scratch
     const int wst0 = wbase + 2 * Geo<L>::buf_floats;
     const int whs = wst0 + 2 * kStateSmem;                            // history scratch
-    const int gw = CTAS == 1 ? (int)(blockIdx.x + gridDim.x * warp) : (int)(blockIdx.x * W + warp);   // warp index in the grid
+    const int gw = kTM ? (int)(blockIdx.x * kTmChannels + warp)       // (time-major: the channel of the first item)
+                       : CTAS == 1 ? (int)(blockIdx.x + gridDim.x * warp) : (int)(blockIdx.x * W + warp);   // warp index in the grid
     __shared__ unsigned sh_ctl[32];
     __shared__ unsigned sh_flag;
     if (threadIdx.x == 0) sh_flag = 0u;
@@ -727,15 +845,18 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     const int n_warps = gridDim.x * W;
     const int seg_tiles = min(p.seg_tiles, g.n_tiles);
     const int n_seg = seg_tiles == g.n_tiles ? 1 : (g.n_tiles + seg_tiles - 1) / seg_tiles;
-    const unsigned n_items = (unsigned)n_seg * (unsigned)p.n_ch;
+    const unsigned n_units = kTM ? (unsigned)((p.n_ch + kTmChannels - 1) / kTmChannels) : (unsigned)p.n_ch;
+    const unsigned n_items = (unsigned)n_seg * n_units;
 
-    unsigned item = (unsigned)gw;
-    auto claim = [&](int& ch, int& tile, int& tend, int& seg) -> bool {
+    unsigned item = kTM ? blockIdx.x : (unsigned)gw;
+    auto claim = [&](int& ch, int& tile, int& tend, int& seg, int& cg) -> bool {
         const unsigned it = item;
-        item += (unsigned)n_warps;
+        item += kTM ? gridDim.x : (unsigned)n_warps;
         if (it >= n_items) return false;
-        seg = n_seg == 1 ? 0 : (int)(it / (unsigned)p.n_ch);
-        ch = (int)(it - (unsigned)seg * (unsigned)p.n_ch);
+        seg = n_seg == 1 ? 0 : (int)(it / n_units);
+        const int u = (int)(it - (unsigned)seg * n_units);
+        cg = kTM ? u : 0;
+        ch = kTM ? u * kTmChannels + warp : u;
         tile = seg * seg_tiles;
         tend = min(g.n_tiles, tile + seg_tiles);
         return true;
@@ -748,18 +869,21 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         while ((int)(done - need) < 0) done = __shfl_sync(0xffffffffu, ld_relaxed(p.progress + ch), 0);
     };
 
-    int ch = 0, tile = 0, tend = 0, seg = 0, cur = 0, wcur = 0;
+    int ch = 0, tile = 0, tend = 0, seg = 0, cg = 0, cur = 0, wcur = 0;
     // ---- hand the control block to the next push, then let it launch.  The ticket's round trip
     // runs while the first rows are requested; only warp 0 waits for it, the other warps look at
     // the flag when their first tile has arrived.
     unsigned tk = 0;
     if (warp == 0 && lane == 0) tk = atomicAdd(&cc->ticket, 1u);
 
-    bool have = claim(ch, tile, tend, seg);
-    if (have) issue_tile_input<L, CTAS == 1>(p, g, ch, tile, wbase, lane);
+    bool have = claim(ch, tile, tend, seg, cg);
+    if (have) {
+        if (kTM) issue_tile_input_tm<L>(p, g, cg, tile, 0);
+        else issue_tile_input<L, CTAS == 1>(p, g, ch, tile, wbase, lane);
+    }
     // the first segment of a channel needs what the previous push left (state, hist): wait before
     // those loads are issued (a wait on an EARLIER push cannot be part of a cycle)
-    if (have && seg == 0) {
+    if (have && seg == 0 && ch < p.n_ch) {
         wait_progress(ch, seq0, pr0);
         issue_tile_carry<L>(p, g, ch, whs, wst0, lane);
     }
@@ -791,20 +915,21 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     FK_TR(2);
 
     while (have) {
-        int nch = ch, ntile = tile + 1, ntend = tend, nseg = seg;
+        int nch = ch, ntile = tile + 1, ntend = tend, nseg = seg, ncg = cg;
         bool nhave = true;
         const bool item_end = ntile == tend;
+        const bool valid = !kTM || ch < p.n_ch;        // (time-major: the last group may have idle warps)
         unsigned npr = 0;
         if (item_end) {
-            nhave = claim(nch, ntile, ntend, nseg);
-            if (nhave && nseg == 0) npr = ld_relaxed(p.progress + nch);      // used after the tile is in registers
+            nhave = claim(nch, ntile, ntend, nseg, ncg);
+            if (nhave && nseg == 0 && nch < p.n_ch) npr = ld_relaxed(p.progress + nch);      // used after the tile is in registers
         }
         const int buf = wbase + cur * Geo<L>::buf_floats;
         const int wst = wst0 + wcur * kStateSmem;
         cp_async_wait_all();
-        __syncwarp();
+        if (kTM) __syncthreads(); else __syncwarp();   // (time-major: every thread's part of the tile has landed)
         FK_TR(3);
-        if (seg > 0 && tile == seg * seg_tiles) {
+        if (valid && seg > 0 && tile == seg * seg_tiles) {
             // first tile of a later segment: wait for the segment before it, then fetch its state
             wait_progress(ch, seq0 + (unsigned)seg, ld_relaxed(p.progress + ch));
             const float* gst = p.state + (long long)ch * ns;
@@ -812,13 +937,13 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
             if (lane + 32 < ns) fk_smem[wst + lane + 32] = __ldcg(gst + lane + 32);
             __syncwarp();
         }
-        const int sin = row_shift(p.in + (long long)ch * p.in_pitch, g.r0);
-        if (tile == 0 && g.r0 != 0) {
+        const int sin = kTM ? 0 : row_shift(p.in + (long long)ch * p.in_pitch, g.r0);
+        if (valid && tile == 0 && g.r0 != 0) {
             // first tile of the channel: the waiting raw samples from the scratch to the head of the tile
             for (int e = lane; e < g.r0; e += 32) fk_smem[buf + raw_index<L>(e + sin)] = fk_smem[whs + e];
             __syncwarp();
         }
-        if (tile == g.n_tiles - 1 && g.r1 != 0) {
+        if (valid && tile == g.n_tiles - 1 && g.r1 != 0) {
             // last tile of the channel: keep the raw samples of its trailing partial slot
             const int e0 = g.q_last * L;                              // tile-space position of that slot
             float* hd = p.hist + (long long)ch * kHist;
@@ -829,18 +954,20 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         __syncwarp();
         if (nhave) {
             const int nbuf = wbase + (cur ^ 1) * Geo<L>::buf_floats;
-            issue_tile_input<L, CTAS == 1>(p, g, nch, ntile, nbuf, lane);
-            if (item_end && nseg == 0) {
+            if (kTM) issue_tile_input_tm<L>(p, g, ncg, ntile, (cur ^ 1) * Geo<L>::buf_floats);
+            else issue_tile_input<L, CTAS == 1>(p, g, nch, ntile, nbuf, lane);
+            if (item_end && nseg == 0 && nch < p.n_ch) {
                 wait_progress(nch, seq0, npr);
                 issue_tile_carry<L>(p, g, nch, whs, wst0 + (wcur ^ 1) * kStateSmem, lane);
             }
         }
         // (a segment's end writes the carried state back and tells whoever continues the channel:
         // the next segment of this push or the first segment of the next push)
-        process_tile<L, CTAS == 1, kAllKinds>(p, g, buf, wst, x, ch, tile, lane, seen, item_end, seq0 + (unsigned)seg + 1u);
+        process_tile<L, CTAS == 1, kAllKinds, kTM>(p, g, buf, wst, x, ch, tile, lane, seen, item_end && valid,
+                                                    seq0 + (unsigned)seg + 1u, cg, cur * Geo<L>::buf_floats);
         FK_TR(4);
         if (item_end) wcur ^= 1;
-        ch = nch; tile = ntile; tend = ntend; seg = nseg; have = nhave; cur ^= 1;
+        ch = nch; tile = ntile; tend = ntend; seg = nseg; cg = ncg; have = nhave; cur ^= 1;
     }
 
     FK_TR(5);

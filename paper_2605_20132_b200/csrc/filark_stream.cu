@@ -253,6 +253,46 @@ static cudaError_t launch_cm(const filark_stream* h, const PushParams<L>& p, cud
                          : launch_cm_shape<L, kCmCtasPerSm, true>(h, p, stream);
 }
 
+// Time-major chunks: the same kernel with the transpose in shared memory (filark_kernels.cuh): one CTA
+// of kTmChannels warps per SM, work items = (segment, group of kTmChannels adjacent channels).
+template <int L, bool kAllKinds>
+static cudaError_t launch_tm_kinds(const filark_stream* h, const PushParams<L>& p, cudaStream_t stream)
+{
+    const size_t smem = sizeof(float) * (size_t)kTmChannels * (size_t)warp_stride<L, true>();
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(filark_push_cm_kernel<L, 1, kAllKinds, true>,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    const int n_cg = (p.n_ch + kTmChannels - 1) / kTmChannels;
+    const int grid = n_cg < h->n_sm ? n_cg : h->n_sm;
+    PushParams<L> q = p;
+    {
+        const long long n_tiles = ((long long)p.n_t + L - 1) / L / 64 + 1;
+        long long st = n_tiles * n_cg / (8LL * grid);
+        q.seg_tiles = (int)(st < 1 ? 1 : (st > 0x3fffffff ? 0x3fffffff : st));
+    }
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)(kTmChannels * 32));
+    cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = std::getenv("FILARK_TUNE_NOPDL") ? 0 : 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, 1, kAllKinds, true>, q);
+}
+template <int L>
+static cudaError_t launch_tm(const filark_stream* h, const PushParams<L>& p, cudaStream_t stream)
+{
+    if constexpr (L <= 24) {
+        return h->lean_kinds ? launch_tm_kinds<L, false>(h, p, stream) : launch_tm_kinds<L, true>(h, p, stream);
+    } else {
+        return cudaErrorInvalidConfiguration;            // (the caller maps longer variants to L = 24)
+    }
+}
+
 template <int L>
 static cudaError_t push_variant(const filark_stream* h, int v, const float* d_in, int n_t, long long in_pitch,
                                 float* d_filt, float* d_cf, long long out_pitch, int vec4, int wait_prior,
@@ -264,6 +304,7 @@ static cudaError_t push_variant(const filark_stream* h, int v, const float* d_in
     p.in_pitch = in_pitch; p.out_pitch = out_pitch; p.n_t = n_t; p.vec4 = vec4;
     p.n_base = n_t / L; p.n_rem = n_t % L;
     p.wait_prior = wait_prior;
+    if (h->layout == FILARK_LAYOUT_TIME_MAJOR) return launch_tm<L>(h, p, stream);
     return launch_cm<L>(h, p, stream);
 }
 
@@ -457,8 +498,8 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
         const int block = 128, grid = (h->n_ch + block - 1) / block;
         filark_push_serial_kernel<<<grid, block, 0, stream>>>(p);
         e = cudaGetLastError();
-    } else if (!cm) {
-        // Time-major blocked kernel: tables of the L = kTmL variant.
+    } else if (!cm && std::getenv("FILARK_TUNE_OLD_TM")) {
+        // The first time-major kernel (scan across warps, per-section look-back), kept for comparison.
         int v = 0;
         for (int i = 0; i < kNumVariants; ++i) if (kVariantL[i] == kTmL) v = i;
         PushParams<kTmL> p = *(const PushParams<kTmL>*)h->proto[v];
@@ -485,6 +526,7 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
     } else {
         int v = choose_variant(n_t);
         for (int i = 0; i < kNumVariants; ++i) if (kVariantL[i] == (int)((h->flags >> 8) & 0xFF)) v = i;
+        if (!cm && kVariantL[v] > 24) v = 2;             // time-major: 16 warps per CTA, L <= 24
         const uintptr_t all = (uintptr_t)d_in | (uintptr_t)d_filt | (uintptr_t)d_cf;
         const int vec4 = ((all & 15u) == 0 && (in_pitch & 3) == 0 && (out_pitch & 3) == 0 && (n_t & 3) == 0) ? 1 : 0;
         // May this push overlap the one before it?  Only if that was this handle's own push, directly
