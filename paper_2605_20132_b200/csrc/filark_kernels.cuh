@@ -423,66 +423,102 @@ template <int L> struct TmWalk {
     }
 };
 
+// The load of a tile is issued in portions (between the sections of the tile before it): 48
+// four-byte copies per thread in one go fill the load/store queue and hold the warp up.
+template <int L> struct TmPrefetch {
+    TmWalk<L> w;
+    const float* gp;
+    const float* dummy;
+    long long gstep;
+    int t, n_t, left;
+    bool chok, interior;
+    __device__ __forceinline__ TmPrefetch(const PushParams<L>& p, const Geom& g, int cg, int tile, int bufoff)
+        : w((int)(threadIdx.x & (kTmChannels - 1)) * warp_stride<L, true>() + bufoff, (int)(threadIdx.x / kTmChannels))
+    {
+        const int c = threadIdx.x & (kTmChannels - 1), j = threadIdx.x / kTmChannels;
+        const int ch = cg * kTmChannels + c;
+        const int t0 = tile * Geo<L>::tile - g.r0;
+        chok = ch < p.n_ch;
+        gp = p.in + ch + (long long)(t0 + j) * p.in_pitch;
+        dummy = p.in;
+        gstep = 32LL * p.in_pitch;
+        t = t0 + j; n_t = p.n_t; left = Geo<L>::tile / 32;
+        interior = chok && t0 >= 0 && t0 + Geo<L>::tile <= p.n_t;
+    }
+    __device__ __forceinline__ void issue(int n)
+    {
+        n = min(n, left);
+        left -= n;
+        if (interior) {
+#pragma unroll 2
+            for (int k = 0; k < n; ++k) {
+                asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(w.sa), "l"(gp) : "memory");
+                gp += gstep; w.step();
+            }
+        } else {
+#pragma unroll 2
+            for (int k = 0; k < n; ++k) {
+                const bool ok = chok && t < n_t;
+                if (t >= 0)
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(w.sa), "l"(ok ? gp : dummy), "r"(ok ? 4 : 0) : "memory");
+                gp += gstep; t += 32; w.step();
+            }
+        }
+    }
+    __device__ __forceinline__ void finish() { issue(left); cp_async_commit(); }
+};
+
 template <int L>
 __device__ __forceinline__ void issue_tile_input_tm(const PushParams<L>& p, const Geom& g, int cg, int tile, int bufoff)
 {
-    constexpr int S = warp_stride<L, true>();
-    const int c = threadIdx.x & (kTmChannels - 1), j = threadIdx.x / kTmChannels;
-    const int ch = cg * kTmChannels + c;
-    const int t0 = tile * Geo<L>::tile - g.r0;
-    const bool chok = ch < p.n_ch;
-    TmWalk<L> w(c * S + bufoff, j);
-    const float* gp = p.in + ch + (long long)(t0 + j) * p.in_pitch;
-    const long long gstep = 32LL * p.in_pitch;
-    if (chok && t0 >= 0 && t0 + Geo<L>::tile <= p.n_t) {
-#pragma unroll 4
-        for (int k = 0; k < Geo<L>::tile / 32; ++k) {
-            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(w.sa), "l"(gp) : "memory");
-            gp += gstep; w.step();
-        }
-    } else {
-        int t = t0 + j;
-#pragma unroll 2
-        for (int k = 0; k < Geo<L>::tile / 32; ++k) {
-            const bool ok = chok && t < p.n_t;
-            if (t >= 0)
-                asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(w.sa), "l"(ok ? gp : p.in), "r"(ok ? 4 : 0) : "memory");
-            gp += gstep; t += 32; w.step();
-        }
-    }
-    cp_async_commit();
+    TmPrefetch<L> pf(p, g, cg, tile, bufoff);
+    pf.finish();
 }
 
+// Stores: thread (q, j) = (tid mod 4, tid / 4) gathers the samples of channels 4q .. 4q + 3 at time
+// j + 128 k from four warps' buffers and writes them with one 16-byte store (8 time rows of 64 bytes
+// per warp instruction) when the rows are 16-byte aligned (p.vec4), one by one otherwise.
 template <int L>
 __device__ __forceinline__ void store_tile_tm(const PushParams<L>& p, const Geom& g, float* __restrict__ out, int cg,
                                               int bufoff, int t0)
 {
     constexpr int S = warp_stride<L, true>();
+    if (p.vec4 && (cg + 1) * kTmChannels <= p.n_ch) {
+        const int q = threadIdx.x & 3, j = threadIdx.x >> 2;           // j = 0 .. 127
+        const int t1 = min(p.n_t - t0, Geo<L>::tile);                  // tile positions [max(0, -t0), t1) exist
+        float* gp = out + (long long)cg * kTmChannels + 4 * q + (long long)(t0 + j) * p.out_pitch;
+        const long long gstep = 128LL * p.out_pitch;
+        const unsigned sa0 = (unsigned)__cvta_generic_to_shared(&fk_smem[4 * q * S + bufoff]);
+#pragma unroll 2
+        for (int e = j; e < Geo<L>::tile; e += 128) {
+            if (e + t0 >= 0 && e < t1) {
+                const unsigned sa = sa0 + 4u * (unsigned)raw_index<L>(e);
+                float4 v;
+                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v.x) : "r"(sa));
+                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v.y) : "r"(sa + 4u * S));
+                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v.z) : "r"(sa + 8u * S));
+                asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v.w) : "r"(sa + 12u * S));
+                st_stream4(gp, v);
+            }
+            gp += gstep;
+        }
+        return;
+    }
     const int c = threadIdx.x & (kTmChannels - 1), j = threadIdx.x / kTmChannels;
     const int ch = cg * kTmChannels + c;
     if (ch < p.n_ch) {
         TmWalk<L> w(c * S + bufoff, j);
         float* gp = out + ch + (long long)(t0 + j) * p.out_pitch;
         const long long gstep = 32LL * p.out_pitch;
-        if (t0 >= 0 && t0 + Geo<L>::tile <= p.n_t) {
-#pragma unroll 4
-            for (int k = 0; k < Geo<L>::tile / 32; ++k) {
+        int t = t0 + j;
+#pragma unroll 2
+        for (int k = 0; k < Geo<L>::tile / 32; ++k) {
+            if ((unsigned)t < (unsigned)p.n_t) {
                 float v;
                 asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(w.sa));
                 st_stream(gp, v);
-                gp += gstep; w.step();
             }
-        } else {
-            int t = t0 + j;
-#pragma unroll 2
-            for (int k = 0; k < Geo<L>::tile / 32; ++k) {
-                if ((unsigned)t < (unsigned)p.n_t) {
-                    float v;
-                    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(w.sa));
-                    st_stream(gp, v);
-                }
-                gp += gstep; t += 32; w.step();
-            }
+            gp += gstep; t += 32; w.step();
         }
     }
 }
@@ -547,7 +583,8 @@ __device__ __forceinline__ void local_pass(float2 (&x)[L], const SecParams<L>& T
 template <int L, bool kInterior, bool kAllKinds, bool kTM>
 __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom& g, int buf, int wst, float2 (&x)[L],
                                              int ch, int tile, int lane, unsigned long long seen,
-                                             bool item_end, unsigned rel_val, int cg, int bufoff)
+                                             bool item_end, unsigned rel_val, int cg, int bufoff,
+                                             TmPrefetch<L>* pf = nullptr)
 {
     const bool last = tile == g.n_tiles - 1;
     const int t0 = tile * Geo<L>::tile - g.r0;
@@ -558,9 +595,11 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
     const bool out_hi = ((q - 1) & 1) != 0;
 
     // ---- S1..S3 per section -------------------------------------------------------------------
+    const int pf_part = kTM ? (Geo<L>::tile / 32 + p.n_sec - 1) / p.n_sec : 0;
     for (int k = 0; k < p.n_sec; ++k) {
         const SecParams<L>& T = p.sec[k];
         float2 s1, s2;
+        if (kTM && pf != nullptr) pf->issue(pf_part);
         // (kAllKinds = false: the kernel for cascades made of the two common section forms only --
         // what a Butterworth bandpass gives -- without the code of the other three)
         if (kAllKinds) {
@@ -609,6 +648,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
         for (int i = 0; i < L; ++i) x[i] = fma2(T.g[i][0], Ea, fma2(T.g[i][1], Eb, x[i]));
     }
 
+    if (kTM && pf != nullptr) pf->finish();
     if (p.filt) {
         if (kTM) {
             regs_to_buf<L>(x, buf, lane, 0);
@@ -954,8 +994,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         __syncwarp();
         if (nhave) {
             const int nbuf = wbase + (cur ^ 1) * Geo<L>::buf_floats;
-            if (kTM) issue_tile_input_tm<L>(p, g, ncg, ntile, (cur ^ 1) * Geo<L>::buf_floats);
-            else issue_tile_input<L, CTAS == 1>(p, g, nch, ntile, nbuf, lane);
+            if (!kTM) issue_tile_input<L, CTAS == 1>(p, g, nch, ntile, nbuf, lane);
             if (item_end && nseg == 0 && nch < p.n_ch) {
                 wait_progress(nch, seq0, npr);
                 issue_tile_carry<L>(p, g, nch, whs, wst0 + (wcur ^ 1) * kStateSmem, lane);
@@ -963,8 +1002,16 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         }
         // (a segment's end writes the carried state back and tells whoever continues the channel:
         // the next segment of this push or the first segment of the next push)
-        process_tile<L, CTAS == 1, kAllKinds, kTM>(p, g, buf, wst, x, ch, tile, lane, seen, item_end && valid,
-                                                    seq0 + (unsigned)seg + 1u, cg, cur * Geo<L>::buf_floats);
+        if (kTM) {
+            // (time-major: the next tile is requested in portions while this one is computed)
+            TmPrefetch<L> pf(p, g, ncg, ntile, (cur ^ 1) * Geo<L>::buf_floats);
+            process_tile<L, true, kAllKinds, true>(p, g, buf, wst, x, ch, tile, lane, seen, item_end && valid,
+                                                   seq0 + (unsigned)seg + 1u, cg, cur * Geo<L>::buf_floats,
+                                                   nhave ? &pf : nullptr);
+        } else {
+            process_tile<L, CTAS == 1, kAllKinds, false>(p, g, buf, wst, x, ch, tile, lane, seen, item_end && valid,
+                                                         seq0 + (unsigned)seg + 1u, cg, cur * Geo<L>::buf_floats);
+        }
         FK_TR(4);
         if (item_end) wcur ^= 1;
         ch = nch; tile = ntile; tend = ntend; seg = nseg; cg = ncg; have = nhave; cur ^= 1;

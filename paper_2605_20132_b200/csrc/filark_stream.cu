@@ -528,7 +528,9 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
         for (int i = 0; i < kNumVariants; ++i) if (kVariantL[i] == (int)((h->flags >> 8) & 0xFF)) v = i;
         if (!cm && kVariantL[v] > 24) v = 2;             // time-major: 16 warps per CTA, L <= 24
         const uintptr_t all = (uintptr_t)d_in | (uintptr_t)d_filt | (uintptr_t)d_cf;
-        const int vec4 = ((all & 15u) == 0 && (in_pitch & 3) == 0 && (out_pitch & 3) == 0 && (n_t & 3) == 0) ? 1 : 0;
+        // (channel-major: introspection only; time-major: output rows allow 16-byte stores)
+        const int vec4 = cm ? (((all & 15u) == 0 && (in_pitch & 3) == 0 && (out_pitch & 3) == 0 && (n_t & 3) == 0) ? 1 : 0)
+                            : (((((uintptr_t)d_filt | (uintptr_t)d_cf) & 15u) == 0 && (out_pitch & 3) == 0) ? 1 : 0);
         // May this push overlap the one before it?  Only if that was this handle's own push, directly
         // before it in the same stream as far as this library launched anything, and the two share no
         // buffer (filark_stream.h, "Ordering").
