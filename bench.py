@@ -303,7 +303,7 @@ def main():
         pass
     out["roofline"] = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s",
                        "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
-                       "kernel": "filark_push_cm_kernel<24,4>" if layout == CHANNEL_MAJOR else "filark_push_tm_kernel<16,8>",
+                       "kernel": "filark_push_cm_kernel<24,4,lean>" if layout == CHANNEL_MAJOR else "filark_push_cm_kernel<24,1,lean,time-major>",
                        "algorithmic_bytes_per_launch": bytes_per_launch,
                        "mean_launch_ms": per_launch_ms, "frac_of_nominal_8TBs": ach / HBM_NOMINAL_GBS,
                        "note": "achieved = 12 B/sample x samples per step / CUDA-event time of the step "

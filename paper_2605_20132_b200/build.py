@@ -12,7 +12,7 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_PKG, "csrc")
 LIB_PATH = os.path.join(_PKG, "libfilark_stream.so")
 SOURCES = [os.path.join(_CSRC, "filark_stream.cu")]
-DEPENDS = SOURCES + [os.path.join(_CSRC, "filark_kernels.cuh"), os.path.join(_CSRC, "filark_kernels_tm.cuh"), os.path.join(_CSRC, "design.hpp"),
+DEPENDS = SOURCES + [os.path.join(_CSRC, "filark_kernels.cuh"), os.path.join(_CSRC, "design.hpp"),
                      os.path.join(os.path.dirname(_PKG), "include", "filark_stream.h"),
                      os.path.join(os.path.dirname(_PKG), "include", "filark_debug.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",

@@ -22,13 +22,15 @@
 // and the next push starts with them (r0 = r1 positions of its first tile come from `hist`,
 // their outputs are recomputed and dropped).  Every slot that advances the state is therefore
 // full, every lane uses the same fix-up rows, and ragged pushes need no second code path.
-// r0 and the sample counter live in device memory (`Ctl`), so a push has no host-side mutable
+// r0 and the sample counter live in device memory (`CmCtl`), so a push has no host-side mutable
 // argument and can be replayed from a CUDA graph.
 //
-// Persistent grid: one CTA per SM, W warps per CTA; warp (b, w) walks the channels
-// b + grid (w + W i), i = 0, 1, ...  While a tile is computed, the next tile (of the same or of
+// Persistent grid, 16 warps per SM (four small CTAs, or one for long pushes): a warp walks work
+// items (segment of tiles, channel).  While a tile is computed, the next tile (of the same or of
 // the warp's next channel) and that channel's carried state are already in flight into the
 // warp's second shared-memory buffer (cp.async, 16 B per lane, zero-filled outside the push).
+// Consecutive pushes of a handle overlap on the device (see filark_push_cm_kernel).  Time-major
+// chunks ([n_t][n_ch]) go through the same kernel with a transpose in shared memory (kTM).
 //
 // The recurrences are exact restatements of the oracle's definition:
 //   section:  s[n] = A s[n-1] + B x[n],  y[n] = C s[n-1] + D x[n]           (design.hpp)
@@ -47,16 +49,7 @@ constexpr int kSteps = 5;              // log2(32) scan steps
 constexpr int kHist = 64;              // floats of raw history per channel (>= largest L)
 constexpr int kKindDF2 = 0, kKindDF2G = 1, kKindDelta = 2, kKindDeltaG = 3, kKindNormal = 4;
 
-// Device-resident control block of a handle (blocked channel-major kernels).
-struct Ctl {
-    unsigned long long seen;   // samples pushed since create/reset
-    unsigned int r0;           // samples waiting in `hist` (raw tail of the previous push)
-    unsigned int ticket;       // CTAs that have finished the running push
-    unsigned int work;         // next unclaimed work item of the running push
-    unsigned int pad;
-};
-
-// Control block of the channel-major kernel.  Consecutive pushes of a handle overlap on the device
+// Device-resident control block of a handle.  Consecutive pushes of a handle overlap on the device
 // (programmatic dependent launch, see filark_push_cm_kernel), so what a push needs to know about
 // its predecessors is double-buffered by push parity: push number e (since create/reset) reads
 // slot[e & 1]; the last of its CTAs to have read it writes slot[(e + 1) & 1] and publishes
@@ -66,16 +59,17 @@ struct CmSlot {
     unsigned long long seen;   // samples pushed before this push
     unsigned int r0;           // samples waiting in `hist`
     unsigned int seq0;         // segments completed per channel before this push (cumulative, wraps)
-    unsigned int cum[kCmDepth];    // CTAs launched by the earlier pushes e' with e' % kCmDepth == j (cumulative, wraps)
-    unsigned int pad;
+    unsigned int cum[kCmDepth];    // CTAs launched by the earlier pushes of ring position j (cumulative, wraps)
+    unsigned int ring;         // this push's position in the ring of kCmDepth pushes in flight (kept here, not
+                               // taken as epoch % kCmDepth: 2^32 is not a multiple of 3)
 };
 struct CmCtl {
     CmSlot slot[2];            // words 0..7, 8..15
     unsigned int epoch;        // word 16: pushes started since create/reset
     unsigned int ticket;       // word 17: CTAs of the starting push that have read their slot
-    unsigned int exited[kCmDepth];   // words 18..20: CTAs finished, by push number % kCmDepth (cumulative): push
-                               // e - kCmDepth and all before it are complete when exited[e % kCmDepth] has
-                               // reached slot[e & 1].cum[e % kCmDepth]
+    unsigned int exited[kCmDepth];   // words 18..20: CTAs finished, by ring position (cumulative): push
+                               // e - kCmDepth and all before it are complete when exited[ring] has
+                               // reached slot[e & 1].cum[ring]
     unsigned int pad[11];
 };
 static_assert(sizeof(CmSlot) == 32 && sizeof(CmCtl) == 128, "the control block is read by one warp in one access");
@@ -112,8 +106,7 @@ template <int L> struct PushParams {
     float* cf;
     float* state;            // [n_ch][state_floats]
     float* hist;             // [n_ch][kHist]
-    Ctl* ctl;                // time-major kernel
-    CmCtl* cctl;             // channel-major kernel
+    CmCtl* cctl;
     unsigned* progress;      // [n_ch] segments completed per channel since create/reset (cumulative, wraps)
     long long in_pitch, out_pitch;
     int n_t, n_ch, n_sec, lta_len;
@@ -127,7 +120,7 @@ template <int L> struct PushParams {
     SecParams<L> sec[kMaxSec];
 };
 
-// Per-push geometry, derived on the device from Ctl (host mirror: filark_debug_push_geometry).
+// Per-push geometry, derived on the device from the control block (host mirror: filark_debug_push_geometry).
 struct Geom {
     int r0;                  // tile-space positions [0, r0) of tile 0 come from hist
     int n_tiles;
@@ -855,7 +848,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         const unsigned* cw = reinterpret_cast<const unsigned*>(cc);
         unsigned v = ld_relaxed(cw + lane);
         const unsigned e = __shfl_sync(0xffffffffu, v, 16);
-        const unsigned ring = e % (unsigned)kCmDepth;
+        const unsigned ring = __shfl_sync(0xffffffffu, v, 8 * (e & 1u) + 7);
         const unsigned need = __shfl_sync(0xffffffffu, v, 8 * (e & 1u) + 4 + ring);   // slot[e & 1].cum[ring]
         unsigned ex = __shfl_sync(0xffffffffu, v, 18 + ring);
         while ((int)(ex - need) < 0)                                   // push e - kCmDepth must have completed
@@ -864,7 +857,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     }
     __syncthreads();
     const unsigned epoch = sh_ctl[16];
-    const unsigned ring = epoch % (unsigned)kCmDepth;
+    const unsigned ring = sh_ctl[8 * (epoch & 1u) + 7];
 #ifdef FK_TRACE
     tr_epoch = epoch;
     fk_trace(tr_epoch, tr_gw, lane, 0, tr_k, tr_t0);
@@ -938,6 +931,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
                 __stcg(&nx->seq0, seq0 + (unsigned)n_seg);
                 for (unsigned j = 0; j < (unsigned)kCmDepth; ++j)
                     __stcg(&nx->cum[j], sl[4 + j] + (j == ring ? gridDim.x : 0u));
+                __stcg(&nx->ring, ring + 1u == (unsigned)kCmDepth ? 0u : ring + 1u);
                 __stcg(&cc->ticket, 0u);
                 st_release(&cc->epoch, epoch + 1u);
                 __threadfence();
@@ -1027,7 +1021,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     FK_TR(6);
 }
 
-// Diagnostic kernel (FILARK_FLAG_SERIAL_SCAN; also the time-major path for now): one thread per
+// Diagnostic kernel (FILARK_FLAG_SERIAL_SCAN, either layout): one thread per
 // channel, serial in time, the same state-space sections, no blocked scan, no history: the
 // carried state is the state after the last sample of the push.  Element (c, t) of a chunk is
 // at c * sc + t * st; state word i of channel c is at c * state_sc + i * state_sk.

@@ -18,7 +18,6 @@
 #include "../../include/filark_debug.h"
 #include "design.hpp"
 #include "filark_kernels.cuh"
-#include "filark_kernels_tm.cuh"
 
 using namespace filark;
 
@@ -39,8 +38,6 @@ struct filark_stream {
     size_t state_floats;
     float* d_hist;                  // raw tail of the previous push: [n_ch][kHist] (channel-major) or
                                     // [2][kHist][n_ch] (time-major, double-buffered by push parity)
-    int tm_grid;                    // resident CTAs of the time-major kernel
-    Ctl* d_ctl;
     CmCtl* d_cctl;                  // channel-major kernel: double-buffered control slots (filark_kernels.cuh)
     unsigned* d_progress;           // [n_ch] segments completed per channel (cumulative)
     // what the previous channel-major push touched: a push may overlap the one before it on the
@@ -48,8 +45,6 @@ struct filark_stream {
     int prev_valid;                 // how many of the entries below describe pushes that may still run
     cudaStream_t prev_stream;
     uintptr_t prev_lo[kCmDepth - 1][3], prev_hi[kCmDepth - 1][3];     // [0] = the push before, [1] = the one before that
-    float4* d_tm_carry;             // time-major look-back ring [n_cb][2][kTmStages][32]
-    unsigned* d_tm_pub;             // [n_cb][32] published-tile counts, self-resetting
     int n_sm;
     size_t smem_optin;
     int last_cuda_error;
@@ -300,7 +295,7 @@ static cudaError_t push_variant(const filark_stream* h, int v, const float* d_in
 {
     PushParams<L> p = *(const PushParams<L>*)h->proto[v];
     p.in = d_in; p.filt = d_filt; p.cf = d_cf;
-    p.state = h->d_state; p.hist = h->d_hist; p.ctl = h->d_ctl; p.cctl = h->d_cctl; p.progress = h->d_progress;
+    p.state = h->d_state; p.hist = h->d_hist; p.cctl = h->d_cctl; p.progress = h->d_progress;
     p.in_pitch = in_pitch; p.out_pitch = out_pitch; p.n_t = n_t; p.vec4 = vec4;
     p.n_base = n_t / L; p.n_rem = n_t % L;
     p.wait_prior = wait_prior;
@@ -381,19 +376,10 @@ filark_status_t filark_stream_create_ex(filark_stream_t** out, int n_ch, const d
     if (e == cudaSuccess) e = cudaMemset(h->d_state, 0, sizeof(float) * h->state_floats);
     if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_hist, sizeof(float) * 2 * (size_t)n_ch * kHist);
     if (e == cudaSuccess) e = cudaMemset(h->d_hist, 0, sizeof(float) * 2 * (size_t)n_ch * kHist);
-    if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_ctl, sizeof(Ctl));
-    if (e == cudaSuccess) e = cudaMemset(h->d_ctl, 0, sizeof(Ctl));
     if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_cctl, sizeof(CmCtl));
     if (e == cudaSuccess) e = cudaMemset(h->d_cctl, 0, sizeof(CmCtl));
     if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_progress, sizeof(unsigned) * (size_t)n_ch);
     if (e == cudaSuccess) e = cudaMemset(h->d_progress, 0, sizeof(unsigned) * (size_t)n_ch);
-    if (layout == FILARK_LAYOUT_TIME_MAJOR) {
-        const size_t n_cb = ((size_t)n_ch + 63) / 64;
-        if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_tm_carry, sizeof(float4) * n_cb * 2 * kTmStages * 32);
-        if (e == cudaSuccess) e = cudaMemset(h->d_tm_carry, 0, sizeof(float4) * n_cb * 2 * kTmStages * 32);
-        if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_tm_pub, sizeof(unsigned) * n_cb * 32);
-        if (e == cudaSuccess) e = cudaMemset(h->d_tm_pub, 0, sizeof(unsigned) * n_cb * 32);
-    }
     bool host_oom = false;
     build_serial(h, &h->serial);
     for (int v = 0; v < kNumVariants && e == cudaSuccess && !host_oom; ++v) {
@@ -403,8 +389,7 @@ filark_status_t filark_stream_create_ex(filark_stream_t** out, int n_ch, const d
     if (e != cudaSuccess || host_oom) {
         const bool oom = host_oom || e == cudaErrorMemoryAllocation;
         for (int v = 0; v < kNumVariants; ++v) std::free(h->proto[v]);
-        cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_ctl); cudaFree(h->d_cctl); cudaFree(h->d_progress);
-        cudaFree(h->d_tm_carry); cudaFree(h->d_tm_pub);
+        cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_cctl); cudaFree(h->d_progress);
         delete h;
         cudaGetLastError();
         return oom ? FILARK_ERR_ALLOC : FILARK_ERR_CUDA;
@@ -426,8 +411,7 @@ filark_status_t filark_stream_destroy(filark_stream_t* h)
     registry_forget(h);
     cudaDeviceSynchronize();
     for (int v = 0; v < kNumVariants; ++v) std::free(h->proto[v]);
-    cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_ctl); cudaFree(h->d_cctl); cudaFree(h->d_progress);
-    cudaFree(h->d_tm_carry); cudaFree(h->d_tm_pub);
+    cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_cctl); cudaFree(h->d_progress);
     for (int j = 0; j < 2; ++j) for (int i = 0; i < 3; ++i) cudaFree(h->d_stage[j][i]);
     if (h->host_ready) {
         cudaStreamDestroy(h->s_h2d); cudaStreamDestroy(h->s_d2h);
@@ -445,12 +429,9 @@ filark_status_t filark_stream_reset(filark_stream_t* h, cudaStream_t stream)
     if (e != cudaSuccess) return cuda_fail(h, e);
     if (dev != h->device) return FILARK_ERR_DEVICE_MISMATCH;
     e = cudaMemsetAsync(h->d_state, 0, sizeof(float) * h->state_floats, stream);
-    if (e == cudaSuccess) e = cudaMemsetAsync(h->d_ctl, 0, sizeof(Ctl), stream);
     if (e == cudaSuccess) e = cudaMemsetAsync(h->d_cctl, 0, sizeof(CmCtl), stream);
     h->prev_valid = 0;
     if (e == cudaSuccess) e = cudaMemsetAsync(h->d_progress, 0, sizeof(unsigned) * (size_t)h->n_ch, stream);
-    if (e == cudaSuccess && h->d_tm_pub)
-        e = cudaMemsetAsync(h->d_tm_pub, 0, sizeof(unsigned) * (((size_t)h->n_ch + 63) / 64) * 32, stream);
     if (e != cudaSuccess) return cuda_fail(h, e);
     h->samples = 0;
     return FILARK_OK;
@@ -497,31 +478,6 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
         p.state_sc = cm ? ns : 1; p.state_sk = cm ? 1 : h->n_ch;
         const int block = 128, grid = (h->n_ch + block - 1) / block;
         filark_push_serial_kernel<<<grid, block, 0, stream>>>(p);
-        e = cudaGetLastError();
-    } else if (!cm && std::getenv("FILARK_TUNE_OLD_TM")) {
-        // The first time-major kernel (scan across warps, per-section look-back), kept for comparison.
-        int v = 0;
-        for (int i = 0; i < kNumVariants; ++i) if (kVariantL[i] == kTmL) v = i;
-        PushParams<kTmL> p = *(const PushParams<kTmL>*)h->proto[v];
-        p.in = d_in; p.filt = d_filt; p.cf = d_cf;
-        p.state = h->d_state; p.hist = nullptr; p.ctl = h->d_ctl; p.progress = nullptr;
-        p.in_pitch = in_pitch; p.out_pitch = out_pitch; p.n_t = (int)n_t; p.vec4 = 0;
-        TmArgs a{};
-        a.hist2 = h->d_hist; a.carry = h->d_tm_carry; a.published = h->d_tm_pub;
-        const uintptr_t all = (uintptr_t)d_in | (uintptr_t)d_filt | (uintptr_t)d_cf;
-        a.vec2 = ((all & 7u) == 0 && (in_pitch & 1) == 0 && (out_pitch & 1) == 0) ? 1 : 0;
-        if (h->tm_grid == 0) {
-            int per_sm = 0;
-            e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, filark_push_tm_kernel<kTmL, kTmWarps>,
-                                                              kTmWarps * 32, 0);
-            if (e != cudaSuccess) return cuda_fail(h, e);
-            if (per_sm < 1) return cuda_fail(h, cudaErrorInvalidConfiguration);
-            h->tm_grid = per_sm * h->n_sm;               // every CTA resident: the progress waits rely on it
-        }
-        const long long slots = (n_t + kHist + kTmL - 1) / kTmL;             // upper bound (r0 < kHist)
-        const long long items = ((slots + kTmWarps - 1) / kTmWarps) * ((h->n_ch + 63) / 64);
-        const int grid = (int)(items < h->tm_grid ? items : h->tm_grid);
-        filark_push_tm_kernel<kTmL, kTmWarps><<<grid, kTmWarps * 32, 0, stream>>>(p, a);
         e = cudaGetLastError();
     } else {
         int v = choose_variant(n_t);
