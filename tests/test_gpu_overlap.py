@@ -58,6 +58,35 @@ def test_overlapped_equals_strict_order_and_oracle(cuda_device, n_ch, n_t, sizes
     assert_parity(res[0][1][pick], ref_c, "overlapped cf")
 
 
+@pytest.mark.parametrize("n_ch,n_t,sizes", [(3001, 9_000, [1500]), (1000, 7_000, [700, 333, 1501, 64])])
+def test_time_major_overlapped_equals_strict_order_and_oracle(cuda_device, n_ch, n_t, sizes):
+    """The same for time-major chunks ([n_t][n_ch]; the last group of 16 channels is partial)."""
+    from paper_2605_20132_b200.workloads import TIME_MAJOR
+    w = CONFIGS["cfg3"].scaled(n_ch=n_ch, n_t=n_t)
+    sos = design_sos(w)
+    x = generate(w, device="cpu")
+    xd = x.t().contiguous().to(cuda_device)
+    chunks = [xd[a:b, :].contiguous() for a, b in split(n_t, sizes)]
+    res = {}
+    for flags in (0, FLAG_STRICT_ORDER):
+        s = FilarkStream(n_ch, sos, w.sta_len, w.lta_len, TIME_MAJOR, flags)
+        of, oc = _alloc(chunks)
+        for rep in range(2):
+            torch.cuda.synchronize()
+            _back_to_back(s, chunks, of, oc)
+            torch.cuda.synchronize()
+            if rep < 1:
+                s.reset()
+        res[flags] = (torch.cat(of, 0).t().contiguous().cpu().numpy(), torch.cat(oc, 0).t().contiguous().cpu().numpy())
+        s.destroy()
+    assert np.array_equal(res[0][0], res[FLAG_STRICT_ORDER][0]), "filt differs from strict order"
+    assert np.array_equal(res[0][1], res[FLAG_STRICT_ORDER][1]), "cf differs from strict order"
+    pick = np.unique(np.r_[0, 15, 16, n_ch - 17, n_ch - 1, np.random.default_rng(6).integers(0, n_ch, 20)])
+    ref_f, ref_c = run_oracle(x.numpy()[pick], sos, w.sta_len, w.lta_len)
+    assert_parity(res[0][0][pick], ref_f, "time-major overlapped filt")
+    assert_parity(res[0][1][pick], ref_c, "time-major overlapped cf")
+
+
 def test_long_run_of_overlapped_pushes(cuda_device):
     """200 pushes in flight behind each other: counters, slot parity and the in-flight bound."""
     n_ch, chunk, n_push = 1200, 252, 200
