@@ -44,7 +44,7 @@
 namespace filark {
 
 constexpr int kMaxSec = 16;
-constexpr int kMaxWarps = 16;          // warps per CTA (one CTA per SM)
+constexpr int kMaxWarps = 16;          // warps per SM
 constexpr int kSteps = 5;              // log2(32) scan steps
 constexpr int kHist = 64;              // floats of raw history per channel (>= largest L)
 constexpr int kKindDF2 = 0, kKindDF2G = 1, kKindDelta = 2, kKindDeltaG = 3, kKindNormal = 4;
@@ -1012,7 +1012,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     }
 
     FK_TR(5);
-    // completion: count this CTA out (push e + 2 waits until all of them are)
+    // completion: count this CTA out (push e + kCmDepth waits until all of them are)
     __syncthreads();
     if (threadIdx.x == 0)
         asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(&cc->exited[ring]) : "memory");
