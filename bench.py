@@ -193,6 +193,8 @@ def workload_config(w, args, sched):
             "layout": "channel-major [n_ch][n_t]" if args.layout == "cm" else "time-major [n_t][n_ch]",
             "pushes_per_step": len(sched), "chunk_samples": sched[0] if len(set(sched)) == 1 else "mixed",
             "l2": "inputs larger than L2: each push reads a distinct chunk; 6.5 GB traffic per step",
+            "push_overlap": "consecutive pushes of the stream overlap on the device (programmatic dependent "
+                            "launch, ordered per channel through the carried state; include/filark_stream.h)",
             "parallelism": "independent channel shards, one stream handle per GPU, no collective"}
 
 
