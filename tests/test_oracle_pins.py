@@ -356,3 +356,38 @@ def test_golden_fixture_regression():
     f, c = o.push(x)
     got = np.stack([x.ravel(), f.ravel(), c.ravel()], axis=1)
     assert np.array_equal(got.astype(np.float32), tab.astype(np.float32))
+
+
+# --------------------------------------------------------------------------- the fused path as a whole
+@pytest.mark.parametrize("name", ["cfg1", "cfg3", "cfg5"])
+def test_fused_path_matches_the_scipy_composition(name):
+    """The whole path (cascade -> energy of the UNROUNDED output -> two averages -> ratio with the
+    warm-up and the guard, state carried over ragged pushes) against the same chain built from
+    library routines: scipy.signal.sosfilt, then lfilter for each average.  Pins the composition,
+    not only its parts: order of the steps, which signal is squared, which average divides which,
+    where the warm-up counter starts, what a chunk boundary does."""
+    w = CONFIGS[name]
+    sos = design_sos(w)
+    sta, lta = 40, 700                      # short enough for the warm-up to end inside the record
+    rng = np.random.default_rng(2024)
+    n_ch, n_t = 3, 6000
+    x = rng.standard_normal((n_ch, n_t)).astype(np.float32)
+    x[1] *= 1e-3
+    x[2, 2500:] = 0.0                       # a channel that dies: the averages decay, the guard never trips
+    o = Oracle(n_ch, sos, sta, lta)
+    fs, cs, p = [], [], 0
+    for c in [1, 999, 1500, 7, 2048, 1445]:
+        f, cf = o.push(np.ascontiguousarray(x[:, p:p + c]))
+        fs.append(f); cs.append(cf); p += c
+    o.close()
+    assert p == n_t
+    filt, cf = np.concatenate(fs, 1), np.concatenate(cs, 1)
+    for ch in range(n_ch):
+        y = signal.sosfilt(sos, x[ch].astype(np.float64))
+        e = y * y
+        s = signal.lfilter([1.0 / sta], [1.0, -(1.0 - 1.0 / sta)], e)
+        l = signal.lfilter([1.0 / lta], [1.0, -(1.0 - 1.0 / lta)], e)
+        ref_cf = np.where((np.arange(n_t) >= lta) & (l > 1e-30), s / np.where(l > 1e-30, l, 1.0), 0.0)
+        assert np.max(np.abs(filt[ch] - y)) <= 1e-6 * np.max(np.abs(y))            # float32 rounding of y
+        assert np.all(cf[ch, :lta] == 0.0) and cf[ch, lta] != 0.0                  # warm-up: exactly lta_len zeros
+        assert np.max(np.abs(cf[ch] - ref_cf)) <= 2e-6 * np.max(np.abs(ref_cf))
