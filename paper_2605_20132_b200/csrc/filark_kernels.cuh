@@ -622,11 +622,11 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
 #pragma unroll
         for (int d = 0; d < kSteps; ++d) {
             if (d < nsteps) {
-                float U1 = __shfl_up_sync(0xffffffffu, W1, 1 << d), U2 = __shfl_up_sync(0xffffffffu, W2, 1 << d);
-                const bool act = lane >= (1 << d);
-                U1 = act ? U1 : 0.0f; U2 = act ? U2 : 0.0f;
-                W1 = fmaf(T.Q[d][0], U1, fmaf(T.Q[d][1], U2, W1));
-                W2 = fmaf(T.Q[d][2], U1, fmaf(T.Q[d][3], U2, W2));
+                const float U1 = __shfl_up_sync(0xffffffffu, W1, 1 << d), U2 = __shfl_up_sync(0xffffffffu, W2, 1 << d);
+                // (predicated updates instead of zeroed operands: two selects fewer per step)
+                const float N1 = fmaf(T.Q[d][0], U1, fmaf(T.Q[d][1], U2, W1));
+                const float N2 = fmaf(T.Q[d][2], U1, fmaf(T.Q[d][3], U2, W2));
+                if (lane >= (1 << d)) { W1 = N1; W2 = N2; }
             }
         }
         float E1 = __shfl_up_sync(0xffffffffu, W1, 1), E2 = __shfl_up_sync(0xffffffffu, W2, 1);
@@ -677,10 +677,9 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
     }
 #pragma unroll
     for (int d = 0; d < kSteps; ++d) {
-        float Us = __shfl_up_sync(0xffffffffu, Ws, 1 << d), Ul = __shfl_up_sync(0xffffffffu, Wl, 1 << d);
-        const bool act = lane >= (1 << d);
-        Us = act ? Us : 0.0f; Ul = act ? Ul : 0.0f;
-        Ws += fmaf(-p.avg.betaQ[d][0], Us, Us); Wl += fmaf(-p.avg.betaQ[d][1], Ul, Ul);
+        const float Us = __shfl_up_sync(0xffffffffu, Ws, 1 << d), Ul = __shfl_up_sync(0xffffffffu, Wl, 1 << d);
+        const float Ns_ = Ws + fmaf(-p.avg.betaQ[d][0], Us, Us), Nl_ = Wl + fmaf(-p.avg.betaQ[d][1], Ul, Ul);
+        if (lane >= (1 << d)) { Ws = Ns_; Wl = Nl_; }
     }
     float Es = __shfl_up_sync(0xffffffffu, Ws, 1), El = __shfl_up_sync(0xffffffffu, Wl, 1);
     if (lane == 0) { Es = M.x; El = M.y; }
