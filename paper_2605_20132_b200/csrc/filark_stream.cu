@@ -82,6 +82,22 @@ static void registry_forget(const filark_stream* h)
         it = it->second == h ? g_last_on_stream.erase(it) : ++it;
 }
 
+// Tuning switches, read once: a push is a few microseconds of host work and short
+// pushes are bound by it.
+struct Tune { int warps; bool nopdl, small_ctas; };
+static const Tune& tune()
+{
+    static const Tune t = [] {
+        Tune v{};
+        const char* w = std::getenv("FILARK_TUNE_WARPS");
+        v.warps = w ? std::atoi(w) : 0;
+        v.nopdl = std::getenv("FILARK_TUNE_NOPDL") != nullptr;
+        v.small_ctas = std::getenv("FILARK_TUNE_SMALL_CTAS") != nullptr;
+        return v;
+    }();
+    return t;
+}
+
 static filark_status_t cuda_fail(filark_stream* h, cudaError_t e)
 {
     if (h) h->last_cuda_error = (int)e;
@@ -187,7 +203,7 @@ static Geom geometry_rt(int L, unsigned r0, int n_t, bool vec4)
 // CTAS CTAs per SM, W warps per CTA; fewer warps per CTA, on more SMs, when there are few
 // channels.  Every CTA of a push fits on the device at once (the segment waits rely on it).
 template <int L, int CTAS, bool kAllKinds>
-static cudaError_t launch_cm_shape(const filark_stream* h, const PushParams<L>& p, cudaStream_t stream)
+static cudaError_t launch_cm_shape(const filark_stream* h, PushParams<L>& p, cudaStream_t stream)
 {
     const size_t warp_bytes = sizeof(float) * (size_t)warp_smem_floats<L>();
     int per_sm = cm_max_warps<L>();                      // warps per SM
@@ -197,10 +213,7 @@ static cudaError_t launch_cm_shape(const filark_stream* h, const PushParams<L>& 
     if (W > per_sm) W = per_sm;
     const int want = (p.n_ch + h->n_sm - 1) / h->n_sm;
     if (want < W) W = want;
-    if (const char* t = std::getenv("FILARK_TUNE_WARPS")) {       // tuning experiments only
-        const int w = std::atoi(t);
-        if (w >= 1 && w <= W) W = w;
-    }
+    if (tune().warps >= 1 && tune().warps <= W) W = tune().warps;       // tuning experiments only
     if (W < 1) return cudaErrorInvalidConfiguration;
     const size_t smem = (size_t)W * warp_bytes;
     static bool attr_done = false;           // per template instance; idempotent
@@ -214,11 +227,10 @@ static cudaError_t launch_cm_shape(const filark_stream* h, const PushParams<L>& 
     const int resident = h->n_sm * (per_sm / W < 16 ? per_sm / W : 16);
     if (grid > resident) grid = resident;
     // work items: runs of seg_tiles tiles of a channel, about 8 items per warp of the grid
-    PushParams<L> q = p;
     {
         const long long n_tiles = ((long long)p.n_t + L - 1) / L / 64 + 1;          // r0 = 0 estimate, >= 1
         long long st = n_tiles * p.n_ch / (8LL * grid * W);
-        q.seg_tiles = (int)(st < 1 ? 1 : (st > 0x3fffffff ? 0x3fffffff : st));
+        p.seg_tiles = (int)(st < 1 ? 1 : (st > 0x3fffffff ? 0x3fffffff : st));
     }
     // programmatic stream serialization: the kernel lets its dependents launch as soon as it has read
     // its control slot, and orders itself against the previous push channel by channel
@@ -228,20 +240,20 @@ static cudaError_t launch_cm_shape(const filark_stream* h, const PushParams<L>& 
     cfg.dynamicSmemBytes = smem; cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = std::getenv("FILARK_TUNE_NOPDL") ? 0 : 1;
+    attr[0].val.programmaticStreamSerializationAllowed = tune().nopdl ? 0 : 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, CTAS, kAllKinds>, q);
+    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, CTAS, kAllKinds>, p);
 }
 
 // Launch shape (filark_kernels.cuh): one CTA per SM when every resident warp gets a long run of tiles
 // anyway, small CTAs otherwise.  (L = 24 is the only variant long pushes ever use.)
 template <int L>
-static cudaError_t launch_cm(const filark_stream* h, const PushParams<L>& p, cudaStream_t stream)
+static cudaError_t launch_cm(const filark_stream* h, PushParams<L>& p, cudaStream_t stream)
 {
     if constexpr (L == 24) {
         const long long tiles = ((long long)p.n_t + kHist + Geo<L>::tile - 1) / Geo<L>::tile * p.n_ch;
         const bool long_push = tiles >= 12LL * h->n_sm * cm_max_warps<L>();
-        if (long_push && !std::getenv("FILARK_TUNE_SMALL_CTAS"))
+        if (long_push && !tune().small_ctas)
             return h->lean_kinds ? launch_cm_shape<24, 1, false>(h, p, stream) : launch_cm_shape<24, 1, true>(h, p, stream);
     }
     return h->lean_kinds ? launch_cm_shape<L, kCmCtasPerSm, false>(h, p, stream)
@@ -251,7 +263,7 @@ static cudaError_t launch_cm(const filark_stream* h, const PushParams<L>& p, cud
 // Time-major chunks: the same kernel with the transpose in shared memory (filark_kernels.cuh): one CTA
 // of kTmChannels warps per SM, work items = (segment, group of kTmChannels adjacent channels).
 template <int L, bool kAllKinds>
-static cudaError_t launch_tm_kinds(const filark_stream* h, const PushParams<L>& p, cudaStream_t stream)
+static cudaError_t launch_tm_kinds(const filark_stream* h, PushParams<L>& p, cudaStream_t stream)
 {
     const size_t smem = sizeof(float) * (size_t)kTmChannels * (size_t)warp_stride<L, true>();
     static bool attr_done = false;
@@ -263,23 +275,22 @@ static cudaError_t launch_tm_kinds(const filark_stream* h, const PushParams<L>& 
     }
     const int n_cg = (p.n_ch + kTmChannels - 1) / kTmChannels;
     const int grid = n_cg < h->n_sm ? n_cg : h->n_sm;
-    PushParams<L> q = p;
     {
         const long long n_tiles = ((long long)p.n_t + L - 1) / L / 64 + 1;
         long long st = n_tiles * n_cg / (8LL * grid);
-        q.seg_tiles = (int)(st < 1 ? 1 : (st > 0x3fffffff ? 0x3fffffff : st));
+        p.seg_tiles = (int)(st < 1 ? 1 : (st > 0x3fffffff ? 0x3fffffff : st));
     }
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)(kTmChannels * 32));
     cfg.dynamicSmemBytes = smem; cfg.stream = stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = std::getenv("FILARK_TUNE_NOPDL") ? 0 : 1;
+    attr[0].val.programmaticStreamSerializationAllowed = tune().nopdl ? 0 : 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, 1, kAllKinds, true>, q);
+    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, 1, kAllKinds, true>, p);
 }
 template <int L>
-static cudaError_t launch_tm(const filark_stream* h, const PushParams<L>& p, cudaStream_t stream)
+static cudaError_t launch_tm(const filark_stream* h, PushParams<L>& p, cudaStream_t stream)
 {
     if constexpr (L <= 24) {
         return h->lean_kinds ? launch_tm_kinds<L, false>(h, p, stream) : launch_tm_kinds<L, true>(h, p, stream);
