@@ -267,3 +267,42 @@ def test_all_section_forms(cuda_device, sizes):
     f, c = run_gpu(s, x.to(cuda_device), CHANNEL_MAJOR, [(0, n_t)] if sizes == [0] else split(n_t, sizes))
     _check(f, c, ref_f, ref_c, CHANNEL_MAJOR, f"all section forms {sizes}")
     s.destroy()
+
+
+@pytest.mark.parametrize("layout", [CHANNEL_MAJOR, TIME_MAJOR])
+def test_no_write_outside_the_chunk(cuda_device, layout):
+    """Outputs are windows of canary-filled buffers at odd offsets and pitches (rows start at every
+    alignment, chunks of odd lengths): everything outside the windows must still hold the canary
+    afterwards (compute-sanitizer is not available on the GPU pool), everything inside must match
+    the oracle."""
+    w = CONFIGS["cfg4"].scaled(n_ch=19, n_t=4321)
+    x_cm = generate(w, device="cpu", layout=CHANNEL_MAJOR)
+    ref_f, ref_c = run_oracle(x_cm.numpy(), design_sos(w), w.sta_len, w.lta_len)
+    s = _stream(w, layout)
+    canary = 12345.0
+    got_f = np.zeros((w.n_ch, w.n_t), np.float32); got_c = np.zeros_like(got_f)
+    p = 0
+    for k, c in enumerate([1501, 7, 1024, 333, 1, 1455]):
+        blk = x_cm[:, p:p + c]
+        rows, cols = (w.n_ch, c) if layout == CHANNEL_MAJOR else (c, w.n_ch)
+        pitch_in, pitch_out = cols + 3 + (k % 3), cols + 5 + (k % 2)
+        off_in, off_out = 1 + k % 4, 2 + (k * 3) % 5
+        xin = torch.full((off_in + rows * pitch_in + 9,), 777.0, device=cuda_device)
+        src = (blk if layout == CHANNEL_MAJOR else blk.t()).contiguous().to(cuda_device)
+        xin[off_in:off_in + rows * pitch_in].view(rows, pitch_in)[:, :cols] = src
+        bf = torch.full((off_out + rows * pitch_out + 9,), canary, device=cuda_device)
+        bc = torch.full_like(bf, canary)
+        s.push_pitched(xin, c, pitch_in, bf, bc, pitch_out, in_offset=off_in, out_offset=off_out)
+        torch.cuda.synchronize()
+        for buf, got in ((bf, got_f), (bc, got_c)):
+            h = buf.cpu().numpy()
+            body = h[off_out:off_out + rows * pitch_out].reshape(rows, pitch_out)
+            assert np.all(h[:off_out] == canary) and np.all(h[off_out + rows * pitch_out:] == canary), "wrote outside the buffer window"
+            assert np.all(body[:, cols:] == canary), "wrote into the gap between rows"
+            win = body[:, :cols]
+            got[:, p:p + c] = win if layout == CHANNEL_MAJOR else win.T
+        p += c
+    assert p == w.n_t
+    assert_parity(got_f, ref_f, "canary windows filt")
+    assert_parity(got_c, ref_c, "canary windows cf")
+    s.destroy()
