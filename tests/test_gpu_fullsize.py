@@ -105,3 +105,40 @@ def test_time_major_full_width(cuda_device):
     assert_parity(filt[:, chans].t().cpu().numpy(), ref_f, "tm filt")
     assert_parity(cf[:, chans].t().cpu().numpy(), ref_c, "tm cf")
     s.destroy()
+
+
+def test_cfg3_full_size_back_to_back_pushes(cuda_device):
+    """Exactly the bench's loop: one dense tensor per push, separate outputs, nothing between the
+    pushes in the stream, so that consecutive pushes overlap on the device.  Sampled channels
+    against the oracle, and every bit of both outputs against the same pushes under
+    FILARK_FLAG_STRICT_ORDER, several times over (2,400 overlapped pushes of 6,000 channels were run
+    this way without a difference while the overlap was developed)."""
+    from paper_2605_20132_b200.stream import FLAG_STRICT_ORDER, FilarkStream
+    w = CONFIGS["cfg3"]
+    sos = design_sos(w)
+    x = generate(w, device=cuda_device)
+    rng = np.random.default_rng(12)
+    chans = sorted(set([0, 3, 4, 2367, 2368, w.n_ch - 1] + rng.integers(0, w.n_ch, 18).tolist()))
+    ref_f, ref_c = run_oracle(x[chans].cpu().numpy(), sos, w.sta_len, w.lta_len)
+    ins, p = [], 0
+    for c in push_schedule(w):
+        ins.append(x[:, p:p + c].contiguous()); p += c
+    del x
+    fs = [torch.empty_like(t) for t in ins]; cs = [torch.empty_like(t) for t in ins]
+
+    def checksum(ts):
+        return int(torch.stack([t.view(torch.int32).sum(dtype=torch.int64) for t in ts]).sum().item())
+
+    sums = {}
+    for flags, reps in ((FLAG_STRICT_ORDER, 1), (0, 5)):
+        s = FilarkStream(w.n_ch, sos, w.sta_len, w.lta_len, CHANNEL_MAJOR, flags)
+        for _ in range(reps):
+            s.reset()
+            for a, f, c in zip(ins, fs, cs):
+                s.push(a, f, c)
+            torch.cuda.synchronize()
+            sums.setdefault(flags, []).append((checksum(fs), checksum(cs)))
+        s.destroy()
+    assert all(v == sums[FLAG_STRICT_ORDER][0] for v in sums[0]), sums
+    assert_parity(torch.cat([f[chans] for f in fs], 1).cpu().numpy(), ref_f, "back-to-back filt")
+    assert_parity(torch.cat([c[chans] for c in cs], 1).cpu().numpy(), ref_c, "back-to-back cf")
