@@ -830,9 +830,9 @@ template <int L, int CTAS> __host__ __device__ constexpr int cm_cta_warps() { re
 // push whose slot says seq0 runs when progress[c] == seq0 + seg and then publishes seq0 + seg + 1
 // (release at gpu scope, L2-scope polls).  At most kCmDepth pushes are in flight: push e starts only
 // when push e - kCmDepth has completed (`exited`), so the host only has to compare a push's buffers
-// with those of the kCmDepth - 1 pushes before it (p.wait_prior = 1 on a conflict, on another stream, after foreign work, or
-// with FILARK_FLAG_STRICT_ORDER: then the kernel begins with griddepcontrol.wait like any
-// dependent launch).  Every CTA ends with griddepcontrol.wait, so a push never completes before the
+// with those of the kCmDepth - 1 pushes before it (p.wait_prior = 1 on a conflict, on another
+// stream, after foreign work, or with FILARK_FLAG_STRICT_ORDER: then the kernel begins with
+// griddepcontrol.wait like any dependent launch).  Every CTA ends with griddepcontrol.wait, so a push never completes before the
 // push in front of it.
 // kTM: time-major chunks through the transpose in shared memory (above): CTAS = 1, kTmChannels warps;
 // the work items are (segment, group of kTmChannels channels) and belong to the CTA as a whole.
