@@ -193,7 +193,8 @@ def workload_config(w, args, sched):
             "layout": "channel-major [n_ch][n_t]" if args.layout == "cm" else "time-major [n_t][n_ch]",
             "pushes_per_step": len(sched), "chunk_samples": sched[0] if len(set(sched)) == 1 else "mixed",
             "l2": "inputs larger than L2: each push reads a distinct chunk; 6.5 GB traffic per step",
-            "push_overlap": "consecutive pushes of the stream overlap on the device (programmatic dependent "
+            "api": "filark_stream_reset + ONE filark_stream_push_many call per step (one kernel per push)",
+            "push_overlap": "the pushes of a push_many call overlap on the device (programmatic dependent "
                             "launch, ordered per channel through the carried state; include/filark_stream.h)",
             "parallelism": "independent channel shards, one stream handle per GPU, no collective"}
 
@@ -211,7 +212,7 @@ def main():
     import numpy as np
     import torch
     import torch.distributed as dist
-    from paper_2605_20132_b200.stream import FilarkStream, load_library
+    from paper_2605_20132_b200.stream import FilarkStream, PushBatch, load_library
     from paper_2605_20132_b200.workloads import (CHANNEL_MAJOR, TIME_MAJOR, CONFIGS, design_sos,
                                                   generate, push_schedule)
     if not torch.cuda.is_available():
@@ -246,11 +247,11 @@ def main():
     cfs = [torch.empty_like(t) for t in ins]
     stream = FilarkStream(w.n_ch, sos, w.sta_len, w.lta_len, layout, flags=args.force_l << 8)
     samples_per_step = w.n_ch * w.n_t
+    batch = PushBatch(stream, ins, filts, cfs)       # the step's schedule, marshalled once
 
     def step():
         stream.reset()
-        for xi, fi, ci in zip(ins, filts, cfs):
-            stream.push(xi, fi, ci)
+        stream.push_many(batch)                      # one host call enqueues every push of the record
 
     def barrier():
         if world > 1:

@@ -28,7 +28,7 @@ int filark_debug_design(const double *sos, int n_sec, int *kinds, double *coefs,
  * previous push waiting in the handle (csrc/filark_kernels.cuh): the stream is cut into slots of
  * L samples aligned to the stream (not to the push); a tile is 64 slots (lane l owns slots 2l,
  * 2l+1); tile-space positions [0, r0) of the first tile are the waiting samples.  force_L = 0
- * lets the library choose L among its compiled variants (8, 16, 24, 32, 48), otherwise
+ * lets the library choose L among its compiled variants (8, 16, 24), otherwise
  * L = force_L.  out5 = { L, n_tiles, q_last (full slots in the last tile, 0..64), r1 (samples
  * of the trailing partial slot, kept for the next push), vec4 (16-byte accesses stay aligned) }.
  */

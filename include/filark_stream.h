@@ -67,12 +67,18 @@ typedef enum filark_status {
 #define FILARK_FLAG_SERIAL_SCAN 1u  /* diagnostic kernel: one thread per channel, serial in time,
                                        same state-space arithmetic, no blocked scan             */
 
-#define FILARK_FLAG_STRICT_ORDER 2u /* every push waits for ALL work before it in the stream before it
-                                       touches memory (see "Ordering" at filark_stream_push)     */
+#define FILARK_FLAG_STRICT_ORDER 2u /* never overlap pushes, not even inside filark_stream_push_many
+                                       (wins over FILARK_FLAG_OVERLAP_PUSHES)                     */
+
+#define FILARK_FLAG_OVERLAP_PUSHES 4u /* the caller promises that, in the stream, NOTHING but this
+                                       library's calls on this handle lies between one push and
+                                       the next that writes the next push's input or touches its
+                                       output buffers: consecutive push calls may then overlap on
+                                       the device (see "Ordering" at filark_stream_push)         */
 
 #define FILARK_FLAG_FORCE_L(L) ((unsigned)(L) << 8)  /* tuning/testing: use the kernel variant with
-                                       sub-block length L (8, 16, 24, 32 or 48) for every push
-                                       instead of the one chosen from n_t                        */
+                                       sub-block length L (8, 16 or 24) for every push instead of
+                                       the one chosen from n_t                                   */
 
 #define FILARK_MAX_SECTIONS 16
 
@@ -114,21 +120,42 @@ filark_status_t filark_stream_create_ex(filark_stream_t **out, int n_ch, const d
  * no allocation, and may be captured into a CUDA graph.  The caller owns all three buffers and
  * keeps them alive until the stream reaches the push.  Outputs must not alias the input or
  * each other (in-place is rejected).
- * Ordering (channel-major layout): a push is a dependent launch of whatever precedes it in
- * `stream` and sees all of that work completed -- with one exception that the library arranges
- * itself: when the operation directly before it in the stream is the previous push of the SAME
- * handle and the new push shares no buffer with the two pushes before it (other than reading the
- * same input), the new push starts on the device while they drain and orders itself against them
- * channel by channel through the carried state (at most three pushes of a handle are in flight;
- * outputs are identical either way).  Work after a push in the stream sees that push and all earlier ones
- * completed.  A caller-written kernel between two pushes that signals programmatic launch
- * completion early (cudaTriggerProgrammaticLaunchCompletion) must not produce the next push's
- * input or read its output buffers; FILARK_FLAG_STRICT_ORDER removes the exception altogether.
+ * Ordering.  By default a push behaves like any kernel in `stream`: it sees all work enqueued
+ * before it completed, and work enqueued after it sees the push (and all earlier pushes)
+ * completed.  Consecutive pushes of one handle CAN overlap on the device -- the next push starts
+ * while the previous one drains and orders itself against it channel by channel through the
+ * carried state; at most three pushes of a handle are in flight and the outputs are bit-identical
+ * either way -- but only where the library knows what lies between them in the stream:
+ *   - between the pushes of one filark_stream_push_many call (nothing does), and
+ *   - between separate push calls of a handle created with FILARK_FLAG_OVERLAP_PUSHES, by which
+ *     the caller promises that no other work enqueued between two pushes produces the later
+ *     push's input or touches its output buffers (the host cannot see foreign kernels, and a
+ *     dependent launch that does not wait is not guaranteed to see their writes).
+ * Even then a push waits like an ordinary kernel when the call before it in the stream (as far as
+ * this library launched it) was not the same handle's push, or when it shares a buffer with the
+ * two pushes before it (other than reading the same input).  Every push completes after all
+ * earlier pushes of the handle.
  * Errors: INVALID_ARG (null handle/d_in, n_t < 0, both outputs NULL, aliasing), ALIGNMENT,
  * DEVICE_MISMATCH, CUDA (launch failure).
  */
 filark_status_t filark_stream_push(filark_stream_t *h, const float *d_in, long long n_t,
                                    float *d_filt, float *d_cf, cudaStream_t stream);
+
+/*
+ * filark_stream_push_many -- enqueue a schedule of n_push consecutive dense pushes with one host
+ * call (the pipeline executor's chunk loop; a folder of files is one
+ * stream of chunks).  Exactly the same result as calling filark_stream_push n_push times in order;
+ * the pushes of one call overlap on the device where their buffers allow (see "Ordering").
+ *   d_in    [host, in]  n_push DEVICE pointers, chunk i holding n_ch*n_t[i] floats.
+ *   n_t     [host, in]  n_push chunk lengths (>= 0; a zero-length chunk is skipped).
+ *   d_filt, d_cf  [host, in]  n_push DEVICE pointers each; either array may be NULL (that output is
+ *           not wanted for any chunk) and single entries may be NULL, but every chunk needs at
+ *           least one output.
+ * Stops at the first failing push and returns its status (earlier pushes stay enqueued).
+ */
+filark_status_t filark_stream_push_many(filark_stream_t *h, int n_push, const float *const *d_in,
+                                        const long long *n_t, float *const *d_filt,
+                                        float *const *d_cf, cudaStream_t stream);
 
 /*
  * filark_stream_push_pitched -- as push, for a sub-view of a larger record: consecutive
@@ -163,7 +190,8 @@ filark_status_t filark_stream_push_host(filark_stream_t *h, const float *h_in, l
  */
 filark_status_t filark_stream_reset(filark_stream_t *h, cudaStream_t stream);
 
-/* Free the handle and its device memory.  NULL is accepted.  Synchronises the device. */
+/* Free the handle and its device memory (on the handle's device, whichever device is current).
+ * NULL is accepted.  Synchronises the handle's device. */
 filark_status_t filark_stream_destroy(filark_stream_t *h);
 
 /* Static description of a status code; never NULL. */

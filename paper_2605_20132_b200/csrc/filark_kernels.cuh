@@ -55,24 +55,28 @@ constexpr int kKindDF2 = 0, kKindDF2G = 1, kKindDelta = 2, kKindDeltaG = 3, kKin
 // slot[e & 1]; the last of its CTAs to have read it writes slot[(e + 1) & 1] and publishes
 // epoch = e + 1 before the grid lets its dependents launch.
 constexpr int kCmDepth = 3;        // pushes of a handle in flight at most
-struct CmSlot {
+struct CmSlot {                // 12 words
     unsigned long long seen;   // samples pushed before this push
     unsigned int r0;           // samples waiting in `hist`
     unsigned int seq0;         // segments completed per channel before this push (cumulative, wraps)
     unsigned int cum[kCmDepth];    // CTAs launched by the earlier pushes of ring position j (cumulative, wraps)
     unsigned int ring;         // this push's position in the ring of kCmDepth pushes in flight (kept here, not
                                // taken as epoch % kCmDepth: 2^32 is not a multiple of 3)
+    unsigned int wbase[kCmDepth];  // value of work[j] at which the next push of ring position j starts claiming
+    unsigned int pad;
 };
 struct CmCtl {
-    CmSlot slot[2];            // words 0..7, 8..15
-    unsigned int epoch;        // word 16: pushes started since create/reset
-    unsigned int ticket;       // word 17: CTAs of the starting push that have read their slot
-    unsigned int exited[kCmDepth];   // words 18..20: CTAs finished, by ring position (cumulative): push
+    CmSlot slot[2];            // words 0..11, 12..23
+    unsigned int epoch;        // word 24: pushes started since create/reset
+    unsigned int ticket;       // word 25: CTAs of the starting push that have read their slot
+    unsigned int exited[kCmDepth];   // words 26..28: CTAs finished, by ring position (cumulative): push
                                // e - kCmDepth and all before it are complete when exited[ring] has
                                // reached slot[e & 1].cum[ring]
-    unsigned int pad[11];
+    unsigned int work[kCmDepth];     // words 29..31: work items claimed, by ring position (cumulative, never
+                               // reset: push e claims work[ring] - slot[e & 1].wbase[ring]), see "Work items"
 };
-static_assert(sizeof(CmSlot) == 32 && sizeof(CmCtl) == 128, "the control block is read by one warp in one access");
+constexpr int kCtlSlotWords = 12, kCtlEpoch = 24, kCtlExited = 26;
+static_assert(sizeof(CmSlot) == 4 * kCtlSlotWords && sizeof(CmCtl) == 128, "the control block is read by one warp in one access");
 
 // One SOS section for sub-block length L; every member is warp-uniform and is read straight
 // from the constant bank.  Q[d] = A^(2L 2^d); g[i] = C A^i.
@@ -169,6 +173,14 @@ __device__ __forceinline__ unsigned ld_relaxed(const unsigned* p)
 {
     unsigned v;
     asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+// (guarded data read with plain instructions: volatile + memory clobber, so that the compiler cannot
+// move the load above the poll that guards it -- the __ldcg intrinsic is a pure asm and may be)
+__device__ __forceinline__ float ld_relaxed_f32(const float* p)
+{
+    float v;
+    asm volatile("ld.relaxed.gpu.global.f32 %0, [%1];" : "=f"(v) : "l"(p) : "memory");
     return v;
 }
 __device__ __forceinline__ void st_release(unsigned* p, unsigned v)
@@ -775,34 +787,6 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
     __syncwarp();
 }
 
-#ifdef FK_TRACE
-// timeline instrumentation for tuning builds only (never in the product library):
-// fk_trace_buf[epoch % 16][warp of the grid < 4096][event slot < 16] = (time, tag)
-__device__ unsigned long long fk_trace_buf[16 * 4096 * 16 * 2];
-__device__ unsigned fk_trace_pos;
-__device__ __forceinline__ unsigned long long fk_now()
-{
-    unsigned long long t;
-    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-    return t;
-}
-__device__ __forceinline__ void fk_trace(unsigned epoch, int gw, int lane, unsigned ev, unsigned& k, unsigned long long t)
-{
-    if (ev >= 5 && ev <= 6) k = 9 + ev;
-    if (lane == 0 && k < 16 && (ev >= 5 || k < 14) && gw < 4096) {
-        unsigned smid;
-        asm volatile("mov.u32 %0, %%smid;" : "=r"(smid));
-        const size_t i = (((size_t)(epoch & 15u) * 4096 + gw) * 16 + k) * 2;
-        fk_trace_buf[i] = t;
-        fk_trace_buf[i + 1] = ((unsigned long long)epoch << 48) | ((unsigned long long)gw << 32) |
-                              ((unsigned long long)smid << 20) | ev | 0x800ull;
-    }
-    k += 1;
-}
-#define FK_TR(ev) fk_trace(tr_epoch, tr_gw, lane, ev, tr_k, fk_now())
-#else
-#define FK_TR(ev)
-#endif
 
 // Warps per SM (bounded by shared memory: two tile buffers per warp) and per CTA.  The kernel is
 // built for two launch shapes: CTAS = kCmCtasPerSm small CTAs per SM for ordinary pushes, so that
@@ -836,7 +820,7 @@ template <int L, int CTAS> __host__ __device__ constexpr int cm_cta_warps() { re
 // push in front of it.
 // kTM: time-major chunks through the transpose in shared memory (above): CTAS = 1, kTmChannels warps;
 // the work items are (segment, group of kTmChannels channels) and belong to the CTA as a whole.
-template <int L, int CTAS, bool kAllKinds, bool kTM = false>
+template <int L, int CTAS, bool kAllKinds, bool kTM, bool kDyn>
 __global__ void __launch_bounds__(cm_cta_warps<L, CTAS>() * 32, CTAS)
 filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
 {
@@ -852,64 +836,80 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
                        : CTAS == 1 ? (int)(blockIdx.x + gridDim.x * warp) : (int)(blockIdx.x * W + warp);   // warp index in the grid
     __shared__ unsigned sh_ctl[32];
     __shared__ unsigned sh_flag;
+    __shared__ unsigned sh_item;
     if (threadIdx.x == 0) sh_flag = 0u;
-#ifdef FK_TRACE
-    unsigned tr_epoch = 0, tr_k = 0;
-    const int tr_gw = blockIdx.x * (blockDim.x >> 5) + warp;
-    const unsigned long long tr_t0 = fk_now();
-#endif
 
     if (p.wait_prior) asm volatile("griddepcontrol.wait;" ::: "memory");
     // the warp's first item is always (segment 0, channel gw): ask for its progress word now, so that
     // the answer is there when the control slot says what to compare it with
+    // (static work distribution only: a claimed first item can be any channel)
     unsigned pr0 = 0;
-    if (gw < p.n_ch) pr0 = ld_relaxed(p.progress + gw);
+    if (!kDyn && gw < p.n_ch) pr0 = ld_relaxed(p.progress + gw);
 
     // ---- control slot of this push.  Nothing changes epoch or slot[epoch & 1] between the launch of
     // this grid (after every CTA of the previous push had taken its ticket and the last of them
-    // had published both) and the last ticket of this grid: one 64-byte read by warp 0 suffices.
+    // had published both) and the last ticket of this grid: one 128-byte read by warp 0 suffices.
     CmCtl* const cc = p.cctl;
     if (warp == 0) {
         const unsigned* cw = reinterpret_cast<const unsigned*>(cc);
         unsigned v = ld_relaxed(cw + lane);
-        const unsigned e = __shfl_sync(0xffffffffu, v, 16);
-        const unsigned ring = __shfl_sync(0xffffffffu, v, 8 * (e & 1u) + 7);
-        const unsigned need = __shfl_sync(0xffffffffu, v, 8 * (e & 1u) + 4 + ring);   // slot[e & 1].cum[ring]
-        unsigned ex = __shfl_sync(0xffffffffu, v, 18 + ring);
+        const unsigned e = __shfl_sync(0xffffffffu, v, kCtlEpoch);
+        const unsigned ring = __shfl_sync(0xffffffffu, v, kCtlSlotWords * (e & 1u) + 7);
+        const unsigned need = __shfl_sync(0xffffffffu, v, kCtlSlotWords * (e & 1u) + 4 + ring);   // slot[e & 1].cum[ring]
+        unsigned ex = __shfl_sync(0xffffffffu, v, kCtlExited + ring);
         while ((int)(ex - need) < 0)                                   // push e - kCmDepth must have completed
             ex = __shfl_sync(0xffffffffu, ld_relaxed(&cc->exited[ring]), 0);
         sh_ctl[lane] = v;
     }
     __syncthreads();
-    const unsigned epoch = sh_ctl[16];
-    const unsigned ring = sh_ctl[8 * (epoch & 1u) + 7];
-#ifdef FK_TRACE
-    tr_epoch = epoch;
-    fk_trace(tr_epoch, tr_gw, lane, 0, tr_k, tr_t0);
-    FK_TR(1);
-#endif
-    const unsigned* sl = &sh_ctl[8 * (epoch & 1u)];
+    const unsigned epoch = sh_ctl[kCtlEpoch];
+    const unsigned ring = sh_ctl[kCtlSlotWords * (epoch & 1u) + 7];
+    const unsigned* sl = &sh_ctl[kCtlSlotWords * (epoch & 1u)];
     const unsigned long long seen = (unsigned long long)sl[0] | ((unsigned long long)sl[1] << 32);
     const unsigned r0 = sl[2], seq0 = sl[3];
     const Geom g = make_geom<L>(r0, p.n_base, p.n_rem, p.vec4 != 0);
     const int ns = state_floats(p.n_sec);
 
     // Work items (segment, channel), segment-major; a segment is seg_tiles consecutive tiles of a
-    // channel, sized for about 8 items per warp; warp gw takes items gw, gw + n_warps, ...
-    // Segment s of a channel starts from the state its segment s - 1 left in global memory
-    // (`progress` says when).  Within a push that item has a lower index, every warp takes its
-    // items in rising order and all warps of the push become resident (nothing an earlier push
-    // needs depends on a later one), so the unfinished item with the lowest index can always run.
+    // channel, sized for about 8 items per warp.  Segment s of a channel starts from the state its
+    // segment s - 1 left in global memory (`progress` says when), i.e. item (s, c) waits for an item
+    // of LOWER index of the same push (or, for s = 0, for the push before).
+    //  - One segment per channel (ordinary pushes, kDyn = false): no waits inside the push; warp gw takes
+    //    items gw, gw + n_warps, ... statically.  What such a warp waits for belongs to an EARLIER push,
+    //    every CTA of which had started before this grid could launch.
+    //  - Several segments per channel (long pushes, kDyn = true): items are CLAIMED from work[ring], a counter
+    //    in the control block, in rising order.  The holder of a claimed item is therefore a
+    //    resident warp, and so is the holder of every item it waits for (lower index = claimed
+    //    earlier): the unfinished item of lowest index can always run, whether or not the other
+    //    CTAs of the grid have been scheduled yet (two handles pushing on two streams share the SMs
+    //    in any proportion).  The counter is never reset: push e claims work[ring] - wbase[ring],
+    //    and every warp (time-major: CTA) makes exactly two claims beyond the last item, so the
+    //    next push of this ring position starts at wbase + n_items + 2 claimers.
     const int n_warps = gridDim.x * W;
     const int seg_tiles = min(p.seg_tiles, g.n_tiles);
     const int n_seg = seg_tiles == g.n_tiles ? 1 : (g.n_tiles + seg_tiles - 1) / seg_tiles;
     const unsigned n_units = kTM ? (unsigned)((p.n_ch + kTmChannels - 1) / kTmChannels) : (unsigned)p.n_ch;
     const unsigned n_items = (unsigned)n_seg * n_units;
+    constexpr bool dyn = kDyn;          // (chosen on the host: kDyn = false only if n_seg = 1 whatever r0 is)
 
     unsigned item = kTM ? blockIdx.x : (unsigned)gw;
-    auto claim = [&](int& ch, int& tile, int& tend, int& seg, int& cg) -> bool {
-        const unsigned it = item;
-        item += kTM ? gridDim.x : (unsigned)n_warps;
+    // Claimed items: the claim for the item AFTER the next one is always in flight (`pend`, raw counter
+    // value, lane 0 of the warp / thread 0 of a time-major CTA), so that the round trip of the atomic
+    // is never waited for except at the very start; every claimer ends with two claims beyond the
+    // last item.  Holding an item while working on a lower one does not change the argument above.
+    unsigned pend = 0;
+    auto claim_issue = [&]() {
+        if (kTM ? threadIdx.x == 0 : lane == 0) pend = atomicAdd(&cc->work[ring], 1u);
+    };
+    // (time-major: thread 0 publishes `pend` in sh_item before a CTA barrier, claim_take runs after it)
+    auto claim_take = [&](int& ch, int& tile, int& tend, int& seg, int& cg) -> bool {
+        unsigned it;
+        if (dyn) {
+            it = (kTM ? sh_item : __shfl_sync(0xffffffffu, pend, 0)) - sl[8 + ring];
+        } else {
+            it = item;
+            item += kTM ? gridDim.x : (unsigned)n_warps;
+        }
         if (it >= n_items) return false;
         seg = n_seg == 1 ? 0 : (int)(it / n_units);
         const int u = (int)(it - (unsigned)seg * n_units);
@@ -934,7 +934,15 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     unsigned tk = 0;
     if (warp == 0 && lane == 0) tk = atomicAdd(&cc->ticket, 1u);
 
-    bool have = claim(ch, tile, tend, seg, cg);
+    if (dyn) {
+        claim_issue();
+        if (kTM) { if (threadIdx.x == 0) sh_item = pend; __syncthreads(); }
+    }
+    bool have = claim_take(ch, tile, tend, seg, cg);
+    if (dyn) {
+        if (kTM) __syncthreads();                    // (sh_item is rewritten at the next item's end)
+        claim_issue();
+    }
     if (have) {
         if (kTM) issue_tile_input_tm<L>(p, g, cg, tile, 0);
         else issue_tile_input<L, CTAS == 1>(p, g, ch, tile, wbase, lane);
@@ -942,10 +950,9 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     // the first segment of a channel needs what the previous push left (state, hist): wait before
     // those loads are issued (a wait on an EARLIER push cannot be part of a cycle)
     if (have && seg == 0 && ch < p.n_ch) {
-        wait_progress(ch, seq0, pr0);
+        wait_progress(ch, seq0, kDyn ? ld_relaxed(p.progress + ch) : pr0);
         issue_tile_carry<L>(p, g, ch, whs, wst0, lane);
     }
-    FK_TR(7);
     if (warp == 0) {
         tk = __shfl_sync(0xffffffffu, tk, 0);
         if (lane == 0) {
@@ -954,8 +961,10 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
                 __stcg(&nx->seen, seen + (unsigned long long)p.n_t);
                 __stcg(&nx->r0, (unsigned)g.r1);
                 __stcg(&nx->seq0, seq0 + (unsigned)n_seg);
-                for (unsigned j = 0; j < (unsigned)kCmDepth; ++j)
+                for (unsigned j = 0; j < (unsigned)kCmDepth; ++j) {
                     __stcg(&nx->cum[j], sl[4 + j] + (j == ring ? gridDim.x : 0u));
+                    __stcg(&nx->wbase[j], sl[8 + j] + (j == ring && dyn ? n_items + 2u * (kTM ? gridDim.x : (unsigned)n_warps) : 0u));
+                }
                 __stcg(&nx->ring, ring + 1u == (unsigned)kCmDepth ? 0u : ring + 1u);
                 __stcg(&cc->ticket, 0u);
                 st_release(&cc->epoch, epoch + 1u);
@@ -965,13 +974,11 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         }
     }
     if (have) cp_async_wait_all();
-    FK_TR(8);
     {
         unsigned f;
         do f = __shfl_sync(0xffffffffu, *reinterpret_cast<volatile unsigned*>(&sh_flag), 0); while (f == 0u);
     }
     asm volatile("griddepcontrol.launch_dependents;");
-    FK_TR(2);
 
     while (have) {
         int nch = ch, ntile = tile + 1, ntend = tend, nseg = seg, ncg = cg;
@@ -980,20 +987,29 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         const bool valid = !kTM || ch < p.n_ch;        // (time-major: the last group may have idle warps)
         unsigned npr = 0;
         if (item_end) {
-            nhave = claim(nch, ntile, ntend, nseg, ncg);
-            if (nhave && nseg == 0 && nch < p.n_ch) npr = ld_relaxed(p.progress + nch);      // used after the tile is in registers
+            if (!dyn || !kTM) {
+                nhave = claim_take(nch, ntile, ntend, nseg, ncg);
+                if (dyn) claim_issue();
+                if (nhave && nseg == 0 && nch < p.n_ch) npr = ld_relaxed(p.progress + nch);      // used after the tile is in registers
+            } else if (threadIdx.x == 0) {
+                sh_item = pend;
+            }
         }
         const int buf = wbase + cur * Geo<L>::buf_floats;
         const int wst = wst0 + wcur * kStateSmem;
         cp_async_wait_all();
         if (kTM) __syncthreads(); else __syncwarp();   // (time-major: every thread's part of the tile has landed)
-        FK_TR(3);
+        if (kTM && dyn && item_end) {
+            nhave = claim_take(nch, ntile, ntend, nseg, ncg);
+            claim_issue();
+            if (nhave && nseg == 0 && nch < p.n_ch) npr = ld_relaxed(p.progress + nch);
+        }
         if (valid && seg > 0 && tile == seg * seg_tiles) {
             // first tile of a later segment: wait for the segment before it, then fetch its state
             wait_progress(ch, seq0 + (unsigned)seg, ld_relaxed(p.progress + ch));
             const float* gst = p.state + (long long)ch * ns;
-            if (lane < ns) fk_smem[wst + lane] = __ldcg(gst + lane);
-            if (lane + 32 < ns) fk_smem[wst + lane + 32] = __ldcg(gst + lane + 32);
+            if (lane < ns) fk_smem[wst + lane] = ld_relaxed_f32(gst + lane);
+            if (lane + 32 < ns) fk_smem[wst + lane + 32] = ld_relaxed_f32(gst + lane + 32);
             __syncwarp();
         }
         const int sin = kTM ? 0 : row_shift(p.in + (long long)ch * p.in_pitch, g.r0);
@@ -1031,19 +1047,15 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
             process_tile<L, CTAS == 1, kAllKinds, false>(p, g, buf, wst, x, ch, tile, lane, seen, item_end && valid,
                                                          seq0 + (unsigned)seg + 1u, cg, cur * Geo<L>::buf_floats);
         }
-        FK_TR(4);
         if (item_end) wcur ^= 1;
         ch = nch; tile = ntile; tend = ntend; seg = nseg; cg = ncg; have = nhave; cur ^= 1;
     }
-
-    FK_TR(5);
     // completion: count this CTA out (push e + kCmDepth waits until all of them are)
     __syncthreads();
     if (threadIdx.x == 0)
         asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(&cc->exited[ring]) : "memory");
     // a push never completes before the push in front of it
     asm volatile("griddepcontrol.wait;" ::: "memory");
-    FK_TR(6);
 }
 
 // Diagnostic kernel (FILARK_FLAG_SERIAL_SCAN, either layout): one thread per

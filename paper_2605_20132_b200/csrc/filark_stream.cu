@@ -6,6 +6,7 @@
 // (cached), ONE kernel launch on the caller's stream.  No synchronisation, no allocation.
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cmath>
 #include <cstdint>
 #include <cstdlib>
@@ -22,8 +23,10 @@
 using namespace filark;
 
 // Sub-block lengths compiled as kernel variants; a push picks the cheapest for its n_t.
-static const int kVariantL[] = {8, 16, 24, 32, 48};
-constexpr int kNumVariants = 5;
+static const int kVariantL[] = {8, 16, 24};
+constexpr int kNumVariants = 3;
+constexpr int kMaxL = 24;                // r0 < kMaxL: the tail a push leaves is shorter than its L
+constexpr int kMaxDevices = 64;          // devices whose kernel attributes are tracked
 
 struct filark_stream {
     int device;
@@ -36,8 +39,7 @@ struct filark_stream {
     SerialParams serial;            // the same for the serial diagnostic kernel
     float* d_state;
     size_t state_floats;
-    float* d_hist;                  // raw tail of the previous push: [n_ch][kHist] (channel-major) or
-                                    // [2][kHist][n_ch] (time-major, double-buffered by push parity)
+    float* d_hist;                  // raw tail of the previous push: [n_ch][kHist] (both layouts)
     CmCtl* d_cctl;                  // channel-major kernel: double-buffered control slots (filark_kernels.cuh)
     unsigned* d_progress;           // [n_ch] segments completed per channel (cumulative)
     // what the previous channel-major push touched: a push may overlap the one before it on the
@@ -82,20 +84,36 @@ static void registry_forget(const filark_stream* h)
         it = it->second == h ? g_last_on_stream.erase(it) : ++it;
 }
 
-// Tuning switches, read once: a push is a few microseconds of host work and short
-// pushes are bound by it.
-struct Tune { int warps; bool nopdl, small_ctas; };
+// Tuning switches: experiments only, compiled in with -DFK_TUNE (never in the product library,
+// which reads no environment variable).
+struct Tune { int warps; bool nopdl, small_ctas, all_kinds; };
 static const Tune& tune()
 {
+#ifdef FK_TUNE
     static const Tune t = [] {
         Tune v{};
         const char* w = std::getenv("FILARK_TUNE_WARPS");
         v.warps = w ? std::atoi(w) : 0;
         v.nopdl = std::getenv("FILARK_TUNE_NOPDL") != nullptr;
         v.small_ctas = std::getenv("FILARK_TUNE_SMALL_CTAS") != nullptr;
+        v.all_kinds = std::getenv("FILARK_TUNE_ALL_KINDS") != nullptr;
         return v;
     }();
+#else
+    static const Tune t{};
+#endif
     return t;
+}
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a per-device attribute of a kernel: set it once
+// per (kernel instance, device).  `done` is one word per template instance; bit d = device d.
+static cudaError_t set_smem_attr_once(std::atomic<unsigned long long>& done, int device, const void* func, size_t bytes)
+{
+    const bool tracked = device >= 0 && device < kMaxDevices;
+    if (tracked && ((done.load(std::memory_order_acquire) >> device) & 1ull)) return cudaSuccess;
+    const cudaError_t e = cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+    if (e == cudaSuccess && tracked) done.fetch_or(1ull << device, std::memory_order_release);
+    return e;
 }
 
 static filark_status_t cuda_fail(filark_stream* h, cudaError_t e)
@@ -130,7 +148,7 @@ template <int L> static void build_proto(const filark_stream* h, PushParams<L>* 
             if (nsteps == kSteps && norm1(q) < 1e-10) nsteps = d;      // this and later steps add < 1e-10
             q = mul(q, q);
         }
-        T.nsteps = std::getenv("FILARK_TUNE_NOSCAN") ? 0 : nsteps;   // timing experiments only (wrong results)
+        T.nsteps = nsteps;
         double g[2 * L];
         fixup_rows(s, L, g);
         for (int i = 0; i < L; ++i) { T.g[i][0] = (float)g[2 * i]; T.g[i][1] = (float)g[2 * i + 1]; }
@@ -165,8 +183,8 @@ static void* alloc_proto(int v, const filark_stream* h)
 {
     switch (kVariantL[v]) {
 #define FK_CASE(LL) case LL: { auto* p = (PushParams<LL>*)std::malloc(sizeof(PushParams<LL>)); if (p) build_proto<LL>(h, p); return p; }
-        FK_CASE(8) FK_CASE(16) FK_CASE(24) FK_CASE(32)
-        default: { auto* p = (PushParams<48>*)std::malloc(sizeof(PushParams<48>)); if (p) build_proto<48>(h, p); return p; }
+        FK_CASE(8) FK_CASE(16)
+        default: { auto* p = (PushParams<24>*)std::malloc(sizeof(PushParams<24>)); if (p) build_proto<24>(h, p); return p; }
 #undef FK_CASE
     }
 }
@@ -181,7 +199,6 @@ static int choose_variant(long long n_t)
     int best = 0; double best_cost = 1e300;
     for (int v = 0; v < kNumVariants; ++v) {
         const int L = kVariantL[v];
-        if (L > 24) continue;
         const long long slots = (n_t + L - 1) / L;
         const double cost = (double)((slots + 63) / 64) * (L + 10.0);
         if (cost < best_cost * (1.0 - 1e-9) || (cost <= best_cost * (1.0 + 1e-9) && L == 24)) { best_cost = cost; best = v; }
@@ -194,14 +211,31 @@ static Geom geometry_rt(int L, unsigned r0, int n_t, bool vec4)
     switch (L) {
         case 8: return make_geom<8>(r0, n_t, vec4);
         case 16: return make_geom<16>(r0, n_t, vec4);
-        case 24: return make_geom<24>(r0, n_t, vec4);
-        case 32: return make_geom<32>(r0, n_t, vec4);
-        default: return make_geom<48>(r0, n_t, vec4);
+        default: return make_geom<24>(r0, n_t, vec4);
     }
 }
 
 // CTAS CTAs per SM, W warps per CTA; fewer warps per CTA, on more SMs, when there are few
 // channels.  Every CTA of a push fits on the device at once (the segment waits rely on it).
+template <int L, int CTAS, bool kAllKinds, bool kDyn>
+static cudaError_t launch_cm_variant(const PushParams<L>& p, int device, int grid, int W, size_t smem, size_t smem_max, cudaStream_t stream)
+{
+    static std::atomic<unsigned long long> attr_done{0};
+    const cudaError_t e = set_smem_attr_once(attr_done, device, (const void*)filark_push_cm_kernel<L, CTAS, kAllKinds, false, kDyn>, smem_max);
+    if (e != cudaSuccess) return e;
+    // programmatic stream serialization: the kernel lets its dependents launch as soon as it has read
+    // its control slot, and orders itself against the previous push channel by channel
+    // (filark_kernels.cuh); p.wait_prior = 1 makes it an ordinary dependent launch
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)(W * 32));
+    cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = tune().nopdl ? 0 : 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, CTAS, kAllKinds, false, kDyn>, p);
+}
+
 template <int L, int CTAS, bool kAllKinds>
 static cudaError_t launch_cm_shape(const filark_stream* h, PushParams<L>& p, cudaStream_t stream)
 {
@@ -216,33 +250,24 @@ static cudaError_t launch_cm_shape(const filark_stream* h, PushParams<L>& p, cud
     if (tune().warps >= 1 && tune().warps <= W) W = tune().warps;       // tuning experiments only
     if (W < 1) return cudaErrorInvalidConfiguration;
     const size_t smem = (size_t)W * warp_bytes;
-    static bool attr_done = false;           // per template instance; idempotent
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(filark_push_cm_kernel<L, CTAS, kAllKinds>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                             (int)((size_t)cm_cta_warps<L, CTAS>() * warp_bytes));
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
     int grid = (p.n_ch + W - 1) / W;
     const int resident = h->n_sm * (per_sm / W < 16 ? per_sm / W : 16);
     if (grid > resident) grid = resident;
     // work items: runs of seg_tiles tiles of a channel, about 8 items per warp of the grid
+    const long long n_tiles_max = (((long long)p.n_t + kMaxL - 1 + L - 1) / L + 63) / 64;     // whatever r0 < kMaxL is
     {
         const long long n_tiles = ((long long)p.n_t + L - 1) / L / 64 + 1;          // r0 = 0 estimate, >= 1
         long long st = n_tiles * p.n_ch / (8LL * grid * W);
         p.seg_tiles = (int)(st < 1 ? 1 : (st > 0x3fffffff ? 0x3fffffff : st));
     }
-    // programmatic stream serialization: the kernel lets its dependents launch as soon as it has read
-    // its control slot, and orders itself against the previous push channel by channel
-    // (filark_kernels.cuh); p.wait_prior = 1 makes it an ordinary dependent launch
-    cudaLaunchConfig_t cfg{};
-    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)(W * 32));
-    cfg.dynamicSmemBytes = smem; cfg.stream = stream;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = tune().nopdl ? 0 : 1;
-    cfg.attrs = attr; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, CTAS, kAllKinds>, p);
+    // one segment per channel for certain: static work distribution; otherwise items are claimed
+    // (filark_kernels.cuh, "Work items").  Long pushes (CTAS = 1) always claim.
+    const size_t smem_max = (size_t)cm_cta_warps<L, CTAS>() * warp_bytes;
+    if constexpr (CTAS != 1) {
+        if (p.seg_tiles >= n_tiles_max)
+            return launch_cm_variant<L, CTAS, kAllKinds, false>(p, h->device, grid, W, smem, smem_max, stream);
+    }
+    return launch_cm_variant<L, CTAS, kAllKinds, true>(p, h->device, grid, W, smem, smem_max, stream);
 }
 
 // Launch shape (filark_kernels.cuh): one CTA per SM when every resident warp gets a long run of tiles
@@ -266,15 +291,9 @@ template <int L, bool kAllKinds>
 static cudaError_t launch_tm_kinds(const filark_stream* h, PushParams<L>& p, cudaStream_t stream)
 {
     const size_t smem = sizeof(float) * (size_t)kTmChannels * (size_t)warp_stride<L, true>();
-    static bool attr_done = false;
-    if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(filark_push_cm_kernel<L, 1, kAllKinds, true>,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        attr_done = true;
-    }
     const int n_cg = (p.n_ch + kTmChannels - 1) / kTmChannels;
     const int grid = n_cg < h->n_sm ? n_cg : h->n_sm;
+    const long long n_tiles_max = (((long long)p.n_t + kMaxL - 1 + L - 1) / L + 63) / 64;
     {
         const long long n_tiles = ((long long)p.n_t + L - 1) / L / 64 + 1;
         long long st = n_tiles * n_cg / (8LL * grid);
@@ -287,16 +306,21 @@ static cudaError_t launch_tm_kinds(const filark_stream* h, PushParams<L>& p, cud
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = tune().nopdl ? 0 : 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, 1, kAllKinds, true>, p);
+    if (p.seg_tiles >= n_tiles_max) {
+        static std::atomic<unsigned long long> attr_done{0};
+        const cudaError_t e = set_smem_attr_once(attr_done, h->device, (const void*)filark_push_cm_kernel<L, 1, kAllKinds, true, false>, smem);
+        if (e != cudaSuccess) return e;
+        return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, 1, kAllKinds, true, false>, p);
+    }
+    static std::atomic<unsigned long long> attr_done{0};
+    const cudaError_t e = set_smem_attr_once(attr_done, h->device, (const void*)filark_push_cm_kernel<L, 1, kAllKinds, true, true>, smem);
+    if (e != cudaSuccess) return e;
+    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, 1, kAllKinds, true, true>, p);
 }
 template <int L>
 static cudaError_t launch_tm(const filark_stream* h, PushParams<L>& p, cudaStream_t stream)
 {
-    if constexpr (L <= 24) {
-        return h->lean_kinds ? launch_tm_kinds<L, false>(h, p, stream) : launch_tm_kinds<L, true>(h, p, stream);
-    } else {
-        return cudaErrorInvalidConfiguration;            // (the caller maps longer variants to L = 24)
-    }
+    return h->lean_kinds ? launch_tm_kinds<L, false>(h, p, stream) : launch_tm_kinds<L, true>(h, p, stream);
 }
 
 template <int L>
@@ -354,7 +378,7 @@ static filark_status_t check_create_args(const void* out, int n_ch, const double
     if (!out || !sos || n_ch <= 0 || n_sec <= 0 || n_sec > FILARK_MAX_SECTIONS) return FILARK_ERR_INVALID_ARG;
     if (sta_len < 1 || lta_len < sta_len) return FILARK_ERR_INVALID_ARG;
     if (layout != FILARK_LAYOUT_CHANNEL_MAJOR && layout != FILARK_LAYOUT_TIME_MAJOR) return FILARK_ERR_INVALID_ARG;
-    if (flags & ~(FILARK_FLAG_SERIAL_SCAN | FILARK_FLAG_STRICT_ORDER | 0xFF00u)) return FILARK_ERR_INVALID_ARG;
+    if (flags & ~(FILARK_FLAG_SERIAL_SCAN | FILARK_FLAG_STRICT_ORDER | FILARK_FLAG_OVERLAP_PUSHES | 0xFF00u)) return FILARK_ERR_INVALID_ARG;
     if (flags & 0xFF00u) {
         bool ok = false;
         for (int v = 0; v < kNumVariants; ++v) ok = ok || kVariantL[v] == (int)((flags >> 8) & 0xFF);
@@ -373,7 +397,7 @@ filark_status_t filark_stream_create_ex(filark_stream_t** out, int n_ch, const d
     std::memset(h, 0, sizeof(*h));
     st = design_all(sos, n_sec, h->sec, &h->gain);
     if (st != FILARK_OK) { delete h; return st; }
-    h->lean_kinds = !std::getenv("FILARK_TUNE_ALL_KINDS");
+    h->lean_kinds = !tune().all_kinds;
     for (int k = 0; k < n_sec; ++k) h->lean_kinds = h->lean_kinds && (h->sec[k].kind == kKindDF2 || h->sec[k].kind == kKindDelta);
     h->n_ch = n_ch; h->n_sec = n_sec; h->sta_len = sta_len; h->lta_len = lta_len;
     h->layout = layout; h->flags = flags;
@@ -385,8 +409,8 @@ filark_status_t filark_stream_create_ex(filark_stream_t** out, int n_ch, const d
     h->smem_optin = (size_t)optin;
     if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_state, sizeof(float) * h->state_floats);
     if (e == cudaSuccess) e = cudaMemset(h->d_state, 0, sizeof(float) * h->state_floats);
-    if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_hist, sizeof(float) * 2 * (size_t)n_ch * kHist);
-    if (e == cudaSuccess) e = cudaMemset(h->d_hist, 0, sizeof(float) * 2 * (size_t)n_ch * kHist);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_hist, sizeof(float) * (size_t)n_ch * kHist);
+    if (e == cudaSuccess) e = cudaMemset(h->d_hist, 0, sizeof(float) * (size_t)n_ch * kHist);
     if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_cctl, sizeof(CmCtl));
     if (e == cudaSuccess) e = cudaMemset(h->d_cctl, 0, sizeof(CmCtl));
     if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_progress, sizeof(unsigned) * (size_t)n_ch);
@@ -420,6 +444,10 @@ filark_status_t filark_stream_destroy(filark_stream_t* h)
 {
     if (!h) return FILARK_OK;
     registry_forget(h);
+    // everything the handle owns lives on h->device, whatever device is current now
+    int cur = -1;
+    const bool have_cur = cudaGetDevice(&cur) == cudaSuccess;
+    const bool switched = have_cur && cur != h->device && cudaSetDevice(h->device) == cudaSuccess;
     cudaDeviceSynchronize();
     for (int v = 0; v < kNumVariants; ++v) std::free(h->proto[v]);
     cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_cctl); cudaFree(h->d_progress);
@@ -428,6 +456,8 @@ filark_status_t filark_stream_destroy(filark_stream_t* h)
         cudaStreamDestroy(h->s_h2d); cudaStreamDestroy(h->s_d2h);
         for (int j = 0; j < 2; ++j) { cudaEventDestroy(h->ev_h2d[j]); cudaEventDestroy(h->ev_kernel[j]); cudaEventDestroy(h->ev_d2h[j]); }
     }
+    if (switched) cudaSetDevice(cur);
+    cudaGetLastError();
     delete h;
     return FILARK_OK;
 }
@@ -454,9 +484,11 @@ static bool overlaps(const void* a, size_t na, const void* b, size_t nb)
     return a0 < b0 + nb && b0 < a0 + na;
 }
 
-filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in, long long n_t,
-                                           long long in_pitch, float* d_filt, float* d_cf,
-                                           long long out_pitch, cudaStream_t stream)
+// One push.  may_overlap: the caller of this function knows that nothing but this handle's own
+// previous push lies between that push and this one in `stream` (filark_stream.h, "Ordering").
+static filark_status_t push_impl(filark_stream_t* h, const float* d_in, long long n_t,
+                                 long long in_pitch, float* d_filt, float* d_cf,
+                                 long long out_pitch, cudaStream_t stream, bool may_overlap)
 {
     if (!h || n_t < 0) return FILARK_ERR_INVALID_ARG;
     if (n_t == 0) return FILARK_OK;
@@ -493,7 +525,6 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
     } else {
         int v = choose_variant(n_t);
         for (int i = 0; i < kNumVariants; ++i) if (kVariantL[i] == (int)((h->flags >> 8) & 0xFF)) v = i;
-        if (!cm && kVariantL[v] > 24) v = 2;             // time-major: 16 warps per CTA, L <= 24
         const uintptr_t all = (uintptr_t)d_in | (uintptr_t)d_filt | (uintptr_t)d_cf;
         // (channel-major: introspection only; time-major: output rows allow 16-byte stores)
         const int vec4 = cm ? (((all & 15u) == 0 && (in_pitch & 3) == 0 && (out_pitch & 3) == 0 && (n_t & 3) == 0) ? 1 : 0)
@@ -504,7 +535,7 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
         const uintptr_t lo[3] = {(uintptr_t)d_in, (uintptr_t)d_filt, (uintptr_t)d_cf};
         const uintptr_t hi[3] = {lo[0] + in_bytes, d_filt ? lo[1] + out_bytes : 0, d_cf ? lo[2] + out_bytes : 0};
         int wait_prior = 1;
-        if (!(h->flags & FILARK_FLAG_STRICT_ORDER) && h->prev_valid > 0 && h->prev_stream == stream &&
+        if (may_overlap && !(h->flags & FILARK_FLAG_STRICT_ORDER) && h->prev_valid > 0 && h->prev_stream == stream &&
             registry_is_last(stream, h)) {
             bool clash = false;
             for (int q = 0; q < h->prev_valid; ++q)
@@ -520,9 +551,7 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
         switch (kVariantL[v]) {
             case 8: e = push_variant<8>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, wait_prior, stream); break;
             case 16: e = push_variant<16>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, wait_prior, stream); break;
-            case 24: e = push_variant<24>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, wait_prior, stream); break;
-            case 32: e = push_variant<32>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, wait_prior, stream); break;
-            default: e = push_variant<48>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, wait_prior, stream); break;
+            default: e = push_variant<24>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, wait_prior, stream); break;
         }
         if (e == cudaSuccess) {
             const int keep = n_prev < kCmDepth - 2 ? n_prev : kCmDepth - 2;
@@ -539,12 +568,38 @@ filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in
     return FILARK_OK;
 }
 
+filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in, long long n_t,
+                                           long long in_pitch, float* d_filt, float* d_cf,
+                                           long long out_pitch, cudaStream_t stream)
+{
+    if (!h) return FILARK_ERR_INVALID_ARG;
+    return push_impl(h, d_in, n_t, in_pitch, d_filt, d_cf, out_pitch, stream, (h->flags & FILARK_FLAG_OVERLAP_PUSHES) != 0);
+}
+
 filark_status_t filark_stream_push(filark_stream_t* h, const float* d_in, long long n_t,
                                    float* d_filt, float* d_cf, cudaStream_t stream)
 {
     if (!h) return FILARK_ERR_INVALID_ARG;
     const long long pitch = h->layout == FILARK_LAYOUT_CHANNEL_MAJOR ? n_t : (long long)h->n_ch;
-    return filark_stream_push_pitched(h, d_in, n_t, pitch, d_filt, d_cf, pitch, stream);
+    return push_impl(h, d_in, n_t, pitch, d_filt, d_cf, pitch, stream, (h->flags & FILARK_FLAG_OVERLAP_PUSHES) != 0);
+}
+
+filark_status_t filark_stream_push_many(filark_stream_t* h, int n_push, const float* const* d_in,
+                                        const long long* n_t, float* const* d_filt, float* const* d_cf,
+                                        cudaStream_t stream)
+{
+    if (!h || n_push < 0 || (n_push > 0 && (!d_in || !n_t))) return FILARK_ERR_INVALID_ARG;
+    // (what lies between two pushes of this call is known: nothing)
+    bool first = true;
+    for (int i = 0; i < n_push; ++i) {
+        const long long pitch = h->layout == FILARK_LAYOUT_CHANNEL_MAJOR ? n_t[i] : (long long)h->n_ch;
+        const filark_status_t st = push_impl(h, d_in[i], n_t[i], pitch, d_filt ? d_filt[i] : nullptr,
+                                             d_cf ? d_cf[i] : nullptr, pitch, stream,
+                                             !first || (h->flags & FILARK_FLAG_OVERLAP_PUSHES) != 0);
+        if (st != FILARK_OK) return st;
+        if (n_t[i] > 0) first = false;
+    }
+    return FILARK_OK;
 }
 
 filark_status_t filark_stream_push_host(filark_stream_t* h, const float* h_in, long long n_t,
@@ -554,7 +609,11 @@ filark_status_t filark_stream_push_host(filark_stream_t* h, const float* h_in, l
     if (n_t == 0) return FILARK_OK;
     if (!h_in || (!h_filt && !h_cf)) return FILARK_ERR_INVALID_ARG;
     const size_t elems = (size_t)h->n_ch * (size_t)n_t;
-    cudaError_t e = cudaSuccess;
+    // (streams, events and staging buffers belong to the handle's device)
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(h, e);
+    if (dev != h->device) return FILARK_ERR_DEVICE_MISMATCH;
     if (!h->host_ready) {
         e = cudaStreamCreateWithFlags(&h->s_h2d, cudaStreamNonBlocking);
         if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&h->s_d2h, cudaStreamNonBlocking);
@@ -614,25 +673,6 @@ filark_status_t filark_stream_push_host(filark_stream_t* h, const float* h_in, l
     h->host_pushes += 1;
     return FILARK_OK;
 }
-
-#ifdef FK_TRACE
-int filark_trace_occupancy(int warps)
-{
-    int n = -1;
-    const size_t smem = (size_t)warps * sizeof(float) * warp_smem_floats<24>();
-    cudaFuncSetAttribute(filark_push_cm_kernel<24, 4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, filark_push_cm_kernel<24, 4, false>, warps * 32, smem);
-    return n;
-}
-int filark_trace_read(unsigned long long* out, unsigned max_words, int reset)
-{
-    const unsigned n = 16u * 4096u * 16u * 2u;
-    cudaDeviceSynchronize();
-    if (out && max_words >= n) cudaMemcpyFromSymbol(out, fk_trace_buf, sizeof(unsigned long long) * n);
-    if (reset) { void* d = nullptr; cudaGetSymbolAddress(&d, fk_trace_buf); cudaMemset(d, 0, sizeof(unsigned long long) * n); }
-    return (int)n;
-}
-#endif
 
 // ---- debug / introspection (include/filark_debug.h): host only, no CUDA calls -----------------
 int filark_debug_design(const double* sos, int n_sec, int* kinds, double* coefs, double* gain)

@@ -17,7 +17,8 @@ from .workloads import CHANNEL_MAJOR, TIME_MAJOR
 
 FLAG_NONE = 0
 FLAG_SERIAL_SCAN = 1
-FLAG_STRICT_ORDER = 2       # every push waits for all earlier work in its stream (filark_stream.h, "Ordering")
+FLAG_STRICT_ORDER = 2       # never overlap pushes, not even inside push_many (filark_stream.h, "Ordering")
+FLAG_OVERLAP_PUSHES = 4     # the caller promises that nothing foreign lies between consecutive push calls
 MAX_SECTIONS = 16
 
 STATUS_NAMES = {0: "FILARK_OK", 1: "FILARK_ERR_INVALID_ARG", 2: "FILARK_ERR_UNSTABLE",
@@ -54,6 +55,8 @@ def load_library():
     lib.filark_stream_create_ex.argtypes = [ctypes.POINTER(vp), ci, vp, ci, ci, ci, ci, cu]
     lib.filark_stream_push.restype = ci
     lib.filark_stream_push.argtypes = [vp, vp, ll, vp, vp, vp]
+    lib.filark_stream_push_many.restype = ci
+    lib.filark_stream_push_many.argtypes = [vp, ci, vp, vp, vp, vp, vp]
     lib.filark_stream_push_pitched.restype = ci
     lib.filark_stream_push_pitched.argtypes = [vp, vp, ll, ll, vp, vp, ll, vp]
     lib.filark_stream_push_host.restype = ci
@@ -90,6 +93,27 @@ def _cur_stream() -> int:
         return int(torch._C._cuda_getCurrentRawStream(torch.cuda.current_device()))
     except Exception:
         return int(torch.cuda.current_stream().cuda_stream)
+
+
+class PushBatch:
+    """The marshalled arguments of one filark_stream_push_many call (pointer and length arrays);
+    keeps the tensors alive.  Built once, enqueued any number of times."""
+
+    def __init__(self, stream_obj: "FilarkStream", ins, filts=None, cfs=None):
+        import torch
+        n = len(ins)
+        for seq in (filts, cfs):
+            if seq is not None and len(seq) != n:
+                raise ValueError("ins, filts and cfs must have the same length")
+        for t in list(ins) + list(filts or []) + list(cfs or []):
+            if t is not None and (not t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous()):
+                raise ValueError("buffers must be contiguous float32 CUDA tensors")
+        self.n = n
+        self.keep = (list(ins), list(filts) if filts is not None else None, list(cfs) if cfs is not None else None)
+        self.n_t = (ctypes.c_longlong * n)(*[stream_obj._n_t(x) for x in ins])
+        self.d_in = (ctypes.c_void_p * n)(*[_ptr(x) for x in ins])
+        self.d_filt = None if filts is None else (ctypes.c_void_p * n)(*[_ptr(x) for x in filts])
+        self.d_cf = None if cfs is None else (ctypes.c_void_p * n)(*[_ptr(x) for x in cfs])
 
 
 class FilarkStream:
@@ -138,6 +162,14 @@ class FilarkStream:
         st = self._lib.filark_stream_push(self._h, _ptr(d_in), n_t, _ptr(d_filt), _ptr(d_cf),
                                           _cur_stream() if stream is None else stream)
         self._check(st, "filark_stream_push")
+
+    def push_many(self, ins, filts=None, cfs=None, stream: Optional[int] = None):
+        """filark_stream_push_many: `ins` (and `filts`, `cfs`) are sequences of chunk tensors, or
+        `ins` is a prepared PushBatch."""
+        b = ins if isinstance(ins, PushBatch) else PushBatch(self, ins, filts, cfs)
+        st = self._lib.filark_stream_push_many(self._h, b.n, b.d_in, b.n_t, b.d_filt, b.d_cf,
+                                               _cur_stream() if stream is None else stream)
+        self._check(st, "filark_stream_push_many")
 
     def push_pitched(self, d_in, n_t: int, in_pitch: int, d_filt, d_cf, out_pitch: int,
                      in_offset: int = 0, out_offset: int = 0, stream: Optional[int] = None):

@@ -113,7 +113,7 @@ def test_cfg3_full_size_back_to_back_pushes(cuda_device):
     against the oracle, and every bit of both outputs against the same pushes under
     FILARK_FLAG_STRICT_ORDER, several times over (2,400 overlapped pushes of 6,000 channels were run
     this way without a difference while the overlap was developed)."""
-    from paper_2605_20132_b200.stream import FLAG_STRICT_ORDER, FilarkStream
+    from paper_2605_20132_b200.stream import FLAG_OVERLAP_PUSHES, FLAG_STRICT_ORDER, FilarkStream
     w = CONFIGS["cfg3"]
     sos = design_sos(w)
     x = generate(w, device=cuda_device)
@@ -130,7 +130,7 @@ def test_cfg3_full_size_back_to_back_pushes(cuda_device):
         return int(torch.stack([t.view(torch.int32).sum(dtype=torch.int64) for t in ts]).sum().item())
 
     sums = {}
-    for flags, reps in ((FLAG_STRICT_ORDER, 1), (0, 5)):
+    for flags, reps in ((FLAG_STRICT_ORDER, 1), (FLAG_OVERLAP_PUSHES, 5)):
         s = FilarkStream(w.n_ch, sos, w.sta_len, w.lta_len, CHANNEL_MAJOR, flags)
         for _ in range(reps):
             s.reset()
@@ -139,6 +139,6 @@ def test_cfg3_full_size_back_to_back_pushes(cuda_device):
             torch.cuda.synchronize()
             sums.setdefault(flags, []).append((checksum(fs), checksum(cs)))
         s.destroy()
-    assert all(v == sums[FLAG_STRICT_ORDER][0] for v in sums[0]), sums
+    assert all(v == sums[FLAG_STRICT_ORDER][0] for v in sums[FLAG_OVERLAP_PUSHES]), sums
     assert_parity(torch.cat([f[chans] for f in fs], 1).cpu().numpy(), ref_f, "back-to-back filt")
     assert_parity(torch.cat([c[chans] for c in cs], 1).cpu().numpy(), ref_c, "back-to-back cf")

@@ -92,7 +92,7 @@ def test_chunking_fuzz(cuda_device, sizes):
     s.destroy()
 
 
-@pytest.mark.parametrize("L", [8, 16, 24, 32, 48])
+@pytest.mark.parametrize("L", [8, 16, 24])
 @pytest.mark.parametrize("n_t", [13_007, 6_144, 1_500, 777])
 def test_every_kernel_variant(cuda_device, L, n_t):
     """Each compiled sub-block length on ragged and exact pushes (flags force the variant)."""
@@ -183,7 +183,7 @@ def test_error_codes(cuda_device):
     from paper_2605_20132_b200.stream import FilarkError, FilarkStream
     w = CONFIGS["cfg1"].scaled(n_ch=4, n_t=64)
     sos = design_sos(w)
-    for bad in [dict(n_ch=0), dict(sta_len=0), dict(lta_len=10, sta_len=20), dict(layout=7), dict(flags=8), dict(flags=7 << 8)]:
+    for bad in [dict(n_ch=0), dict(sta_len=0), dict(lta_len=10, sta_len=20), dict(layout=7), dict(flags=8), dict(flags=7 << 8), dict(flags=32 << 8)]:
         kw = dict(n_ch=4, sos=sos, sta_len=5, lta_len=50, layout=0, flags=0); kw.update(bad)
         with pytest.raises(FilarkError) as e:
             FilarkStream(**kw)

@@ -121,11 +121,11 @@ def test_push_geometry_covers_every_sample_once(lib):
     lens = set(range(1, 70)) | {1000, 1023, 1024, 1025, 1500, 1530, 2047, 2048, 6000, 90000, 99991, 900000}
     lens |= set(push_schedule(CONFIGS["cfg5"])[:50])
     for n_t in sorted(lens):
-        for force in (0, 8, 16, 24, 32, 48):
+        for force in (0, 8, 16, 24):
             for r0 in (0, 1, 4, 7, 23, 47):
                 g = lib.debug_push_geometry(n_t, r0, force)
                 L = g["L"]
-                assert L in (8, 16, 24, 32, 48) and (force == 0 or L == force)
+                assert L in (8, 16, 24) and (force == 0 or L == force)
                 total = r0 + n_t
                 n_full, r1 = divmod(total, L)
                 assert g["r1"] == r1 and 0 <= r1 < L
@@ -135,14 +135,14 @@ def test_push_geometry_covers_every_sample_once(lib):
                 assert g["vec4"] == (1 if r0 % 4 == 0 else 0)
     # a chunked stream: the state has moved over exactly (pushed - waiting) samples after every push
     rng = np.random.default_rng(5)
-    for force in (0, 8, 24, 48):
+    for force in (0, 8, 16, 24):
         r0, pushed, advanced = 0, 0, 0
         for n_t in rng.integers(1, 4000, size=200).tolist():
             g = lib.debug_push_geometry(n_t, r0, force)
             advanced += (64 * (g["n_tiles"] - 1) + g["q_last"]) * g["L"]
             pushed += n_t
             r0 = g["r1"]
-            assert advanced + r0 == pushed and r0 < 48
+            assert advanced + r0 == pushed and r0 < 24
     # the cheapest variant for the configs' chunk lengths puts the whole chunk in one tile
     assert lib.debug_push_geometry(1500)["L"] == 24 and lib.debug_push_geometry(1500)["n_tiles"] == 1
     assert lib.debug_push_geometry(1000)["L"] == 16 and lib.debug_push_geometry(1000)["n_tiles"] == 1
