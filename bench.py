@@ -35,7 +35,7 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
-ALG_BYTES_PER_SAMPLE = 12.0          # 4 read + 4 filt + 4 cf
+ALG_BYTES_PER_SAMPLE = 12.0          # 4 read + 4 filt + 4 cf; 8 when one output is NULL
 HBM_NOMINAL_GBS = 8000.0             # the denominator BASELINE.json north_star names
 FALLBACK_HBM_GBS = 6650.0            # B200_PROFILING.md fallback
 
@@ -50,6 +50,8 @@ def parse_args():
     ap.add_argument("--mode", default="chunked", choices=["chunked", "whole"])
     ap.add_argument("--layout", default="cm", choices=["cm", "tm"])
     ap.add_argument("--force-l", type=int, default=0, help="tuning: force the sub-block length variant")
+    ap.add_argument("--outputs", default="both", choices=["both", "filt", "cf"],
+                    help="which outputs the pushes ask for (the other pointer is NULL: 8 B/sample)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-detail", action="store_true")
@@ -225,6 +227,9 @@ def main():
 
     w = CONFIGS[args.workload]
     sos = design_sos(w)
+    global ALG_BYTES_PER_SAMPLE
+    if args.outputs != "both":
+        ALG_BYTES_PER_SAMPLE = 8.0
     layout = CHANNEL_MAJOR if args.layout == "cm" else TIME_MAJOR
     sched = push_schedule(w) if args.mode == "chunked" else [w.n_t]
 
@@ -243,8 +248,8 @@ def main():
     ins = pack(x, sched, layout)
     if len(sched) > 1:
         del x
-    filts = [torch.empty_like(t) for t in ins]
-    cfs = [torch.empty_like(t) for t in ins]
+    filts = [torch.empty_like(t) for t in ins] if args.outputs != "cf" else None
+    cfs = [torch.empty_like(t) for t in ins] if args.outputs != "filt" else None
     stream = FilarkStream(w.n_ch, sos, w.sta_len, w.lta_len, layout, flags=args.force_l << 8)
     samples_per_step = w.n_ch * w.n_t
     batch = PushBatch(stream, ins, filts, cfs)       # the step's schedule, marshalled once
@@ -384,7 +389,8 @@ def extra_runs(args, w, sos, stream, ins, filts, cfs, sched, torch):
         try:
             n_t = w.n_t
             x = torch.cat(ins, dim=1).contiguous()
-            f = torch.empty_like(x); c = torch.empty_like(x)
+            f = torch.empty_like(x) if args.outputs != "cf" else None
+            c = torch.empty_like(x) if args.outputs != "filt" else None
             for _ in range(2):
                 stream.reset(); stream.push(x, f, c)
             torch.cuda.synchronize()
@@ -396,7 +402,7 @@ def extra_runs(args, w, sos, stream, ins, filts, cfs, sched, torch):
             e1.record(); torch.cuda.synchronize()
             ms = e0.elapsed_time(e1) / reps
             extra["whole_record_push"] = {"ms": ms, "samples_per_s": w.n_ch * n_t / (ms * 1e-3),
-                                          "alg_gbytes_per_s": 12.0 * w.n_ch * n_t / (ms * 1e-3) / 1e9}
+                                          "alg_gbytes_per_s": ALG_BYTES_PER_SAMPLE * w.n_ch * n_t / (ms * 1e-3) / 1e9}
             del x, f, c
         except Exception as exc:                                  # context only
             extra["whole_record_push"] = {"error": repr(exc)}

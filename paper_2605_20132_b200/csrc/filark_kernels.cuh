@@ -80,7 +80,7 @@ static_assert(sizeof(CmSlot) == 4 * kCtlSlotWords && sizeof(CmCtl) == 128, "the 
 
 // One SOS section for sub-block length L; every member is warp-uniform and is read straight
 // from the constant bank.  Q[d] = A^(2L 2^d); g[i] = C A^i.
-template <int L> struct SecParams {
+template <int L> struct alignas(16) SecParams {
     int kind, nsteps;
     float c[5];
     float pad;
@@ -675,8 +675,13 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
         if (lane == 0 && !keep) *reinterpret_cast<float2*>(&fk_smem[wst + 2 * k]) = make_float2(n1, n2);
         // S3 fix-up: y[i] += g1[i] s1 + g2[i] s2
         const float2 Ea = make_float2(E1, o1), Eb = make_float2(E2, o2);
+        // (two rows per 16-byte uniform load: the tables are 16-byte aligned in the parameter bank)
 #pragma unroll
-        for (int i = 0; i < L; ++i) x[i] = fma2(T.g[i][0], Ea, fma2(T.g[i][1], Eb, x[i]));
+        for (int i = 0; i < L; i += 2) {
+            const float4 gg = *reinterpret_cast<const float4*>(&T.g[i][0]);
+            x[i] = fma2(gg.x, Ea, fma2(gg.y, Eb, x[i]));
+            x[i + 1] = fma2(gg.z, Ea, fma2(gg.w, Eb, x[i + 1]));
+        }
     }
 
     if (kTM && pf != nullptr) pf->finish();
@@ -797,7 +802,13 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
 // behind by 20 % and a long push ends with a tail (measured: 342 vs 377 Gsample/s on a 90,000-
 // sample push).
 constexpr int kCmCtasPerSm = 4;
-template <int L> __host__ __device__ constexpr int cm_max_warps() { return L <= 24 ? 16 : (L <= 32 ? 12 : 8); }
+#ifndef FK_MAXW16
+#define FK_MAXW16 16
+#endif
+#ifndef FK_MAXW
+#define FK_MAXW 16
+#endif
+template <int L> __host__ __device__ constexpr int cm_max_warps() { return L == 16 ? FK_MAXW16 : FK_MAXW; }
 template <int L, int CTAS> __host__ __device__ constexpr int cm_cta_warps() { return cm_max_warps<L>() / CTAS; }
 
 // Channel-major push: grid <= CTAS * SM count (every CTA of a push is resident once the

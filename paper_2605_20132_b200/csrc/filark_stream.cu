@@ -275,11 +275,11 @@ static cudaError_t launch_cm_shape(const filark_stream* h, PushParams<L>& p, cud
 template <int L>
 static cudaError_t launch_cm(const filark_stream* h, PushParams<L>& p, cudaStream_t stream)
 {
-    if constexpr (L == 24) {
+    if constexpr (L == 24 || (L == 16 && FK_MAXW16 != 16)) {
         const long long tiles = ((long long)p.n_t + kHist + Geo<L>::tile - 1) / Geo<L>::tile * p.n_ch;
         const bool long_push = tiles >= 12LL * h->n_sm * cm_max_warps<L>();
         if (long_push && !tune().small_ctas)
-            return h->lean_kinds ? launch_cm_shape<24, 1, false>(h, p, stream) : launch_cm_shape<24, 1, true>(h, p, stream);
+            return h->lean_kinds ? launch_cm_shape<L, 1, false>(h, p, stream) : launch_cm_shape<L, 1, true>(h, p, stream);
     }
     return h->lean_kinds ? launch_cm_shape<L, kCmCtasPerSm, false>(h, p, stream)
                          : launch_cm_shape<L, kCmCtasPerSm, true>(h, p, stream);
