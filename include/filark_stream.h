@@ -142,16 +142,23 @@ filark_status_t filark_stream_push(filark_stream_t *h, const float *d_in, long l
                                    float *d_filt, float *d_cf, cudaStream_t stream);
 
 /*
- * filark_stream_push_many -- enqueue a schedule of n_push consecutive dense pushes with one host
+ * filark_stream_push_many -- enqueue a schedule of n_push consecutive dense chunks with one host
  * call (the pipeline executor's chunk loop; a folder of files is one
- * stream of chunks).  Exactly the same result as calling filark_stream_push n_push times in order;
- * the pushes of one call overlap on the device where their buffers allow (see "Ordering").
+ * stream of chunks).  The same result as calling filark_stream_push n_push times in order (bit for
+ * bit when the launches use the same sub-block length L, which is chosen per launch; to fp32
+ * rounding otherwise, like any two chunkings of a record).  Chunks that share no buffer with each other are processed by COMMON launches of
+ * up to 64 chunks (and < 2^31 samples per channel): every channel runs through all chunks of a
+ * launch with its carried state held on the SM, so a chunk boundary inside a launch costs no
+ * hand-over through device memory; consecutive launches of one call overlap on the device (see
+ * "Ordering").  If an output of one chunk overlaps any buffer of another chunk, or with
+ * FILARK_FLAG_STRICT_ORDER, every chunk gets a launch of its own, in order.
  *   d_in    [host, in]  n_push DEVICE pointers, chunk i holding n_ch*n_t[i] floats.
  *   n_t     [host, in]  n_push chunk lengths (>= 0; a zero-length chunk is skipped).
  *   d_filt, d_cf  [host, in]  n_push DEVICE pointers each; either array may be NULL (that output is
  *           not wanted for any chunk) and single entries may be NULL, but every chunk needs at
  *           least one output.
- * Stops at the first failing push and returns its status (earlier pushes stay enqueued).
+ * The whole schedule is checked before anything is enqueued: on an argument error nothing has been
+ * launched.  Errors: as filark_stream_push.
  */
 filark_status_t filark_stream_push_many(filark_stream_t *h, int n_push, const float *const *d_in,
                                         const long long *n_t, float *const *d_filt,

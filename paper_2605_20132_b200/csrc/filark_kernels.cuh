@@ -104,24 +104,36 @@ struct AvgParams {
 __host__ __device__ constexpr int state_floats(int n_sec) { return (2 * n_sec + 4 + 3) & ~3; }
 constexpr unsigned kSeenMax = 0x7fffffffu;
 
-template <int L> struct PushParams {
+// One chunk of a launch.  A launch covers up to kMaxBatch consecutive chunks of the stream (one
+// for filark_stream_push, the chunks of a filark_stream_push_many schedule otherwise): every
+// channel's tiles run through all of them with the carried state staying in shared memory, so
+// that a chunk boundary inside a launch costs no hand-over through global memory at all.
+// Every member is warp-uniform and is read straight from the parameter bank.
+constexpr int kMaxBatch = 64;
+struct Chunk {
     const float* in;
     float* filt;
     float* cf;
+    long long in_pitch, out_pitch;
+    int n_t, n_base, n_rem;  // n_t = n_base L + n_rem
+    unsigned t_cum;          // samples of the launch in front of this chunk
+};
+
+template <int L> struct PushParams {
     float* state;            // [n_ch][state_floats]
     float* hist;             // [n_ch][kHist]
     CmCtl* cctl;
     unsigned* progress;      // [n_ch] segments completed per channel since create/reset (cumulative, wraps)
-    long long in_pitch, out_pitch;
-    int n_t, n_ch, n_sec, lta_len;
-    int n_base, n_rem;       // n_t = n_base L + n_rem
+    int n_ch, n_sec, lta_len;
+    int n_push;              // chunks of this launch, 1 .. kMaxBatch
     int seg_tiles;           // tiles per work item (host heuristic: about 8 items per resident warp)
-    int vec4;                // host's view of the alignment (introspection only: the kernel derives the
-                             // shift of every row itself, see "Alignment")
+    int vec4;                // host's view of the alignment (channel-major: introspection only, the kernel derives
+                             // the shift of every row itself, see "Alignment"; time-major: 16-byte stores allowed)
     int wait_prior;          // wait for everything before this launch in the stream before touching memory
     float gain, ratio, lta_thr;
     AvgParams avg;
     SecParams<L> sec[kMaxSec];
+    Chunk ck[kMaxBatch];
 };
 
 // Per-push geometry, derived on the device from the control block (host mirror: filark_debug_push_geometry).
@@ -241,11 +253,11 @@ template <int L> __device__ __forceinline__ int raw_index(int p) { return p + 4 
 // carried state into `wst`.  Tile-space position e of tile `tile` is input sample
 // t = tile 64L + e - r0; t < 0 reads hist[ch][r0 + t], t >= n_t is zero-filled.
 template <int L, bool kInterior>
-__device__ __forceinline__ void issue_tile_input(const PushParams<L>& p, const Geom& g, int ch, int tile, int buf, int lane)
+__device__ __forceinline__ void issue_tile_input(const PushParams<L>& p, const Chunk& ck, const Geom& g, int ch, int tile, int buf, int lane)
 {
     const int t0 = tile * Geo<L>::tile - g.r0;
-    const int n_t = p.n_t;
-    const float* __restrict__ src = p.in + (long long)ch * p.in_pitch;
+    const int n_t = ck.n_t;
+    const float* __restrict__ src = ck.in + (long long)ch * ck.in_pitch;
     const int s = row_shift(src, g.r0);
     if (kInterior && s == 0 && t0 >= 0 && t0 + Geo<L>::tile <= n_t) {   // aligned interior tile: no bounds
         // (only in the kernel built for long pushes: elsewhere the instruction cache is the scarcer
@@ -321,10 +333,10 @@ __device__ __forceinline__ void issue_tile_carry(const PushParams<L>& p, const G
 // S7: the lane regions of `buf` -> one output array (coalesced 16-byte stores).  Positions that
 // map to t < 0 (recomputed history) or t >= n_t (padding) are dropped.
 template <int L, bool kInterior>
-__device__ __forceinline__ void store_tile(const PushParams<L>& p, const Geom& g, float* __restrict__ dst, int buf,
+__device__ __forceinline__ void store_tile(const Chunk& ck, const Geom& g, float* __restrict__ dst, int buf,
                                            int lane, int t0, int s)
 {
-    const int n_t = p.n_t;
+    const int n_t = ck.n_t;
     if (kInterior && s == 0 && t0 >= 0 && t0 + Geo<L>::tile <= n_t) {
         float* __restrict__ dstt = dst + t0 + 4 * lane;
 #pragma unroll
@@ -463,18 +475,18 @@ template <int L> struct TmPrefetch {
     long long gstep;
     int t, n_t, left;
     bool chok, interior;
-    __device__ __forceinline__ TmPrefetch(const PushParams<L>& p, const Geom& g, int cg, int tile, int bufoff)
+    __device__ __forceinline__ TmPrefetch(const PushParams<L>& p, const Chunk& ck, const Geom& g, int cg, int tile, int bufoff)
         : w((int)(threadIdx.x & (kTmChannels - 1)) * warp_stride<L, true>() + bufoff, (int)(threadIdx.x / kTmChannels))
     {
         const int c = threadIdx.x & (kTmChannels - 1), j = threadIdx.x / kTmChannels;
         const int ch = cg * kTmChannels + c;
         const int t0 = tile * Geo<L>::tile - g.r0;
         chok = ch < p.n_ch;
-        gp = p.in + ch + (long long)(t0 + j) * p.in_pitch;
-        dummy = p.in;
-        gstep = 32LL * p.in_pitch;
-        t = t0 + j; n_t = p.n_t; left = Geo<L>::tile / 32;
-        interior = chok && t0 >= 0 && t0 + Geo<L>::tile <= p.n_t;
+        gp = ck.in + ch + (long long)(t0 + j) * ck.in_pitch;
+        dummy = ck.in;
+        gstep = 32LL * ck.in_pitch;
+        t = t0 + j; n_t = ck.n_t; left = Geo<L>::tile / 32;
+        interior = chok && t0 >= 0 && t0 + Geo<L>::tile <= ck.n_t;
     }
     __device__ __forceinline__ void issue(int n)
     {
@@ -500,9 +512,9 @@ template <int L> struct TmPrefetch {
 };
 
 template <int L>
-__device__ __forceinline__ void issue_tile_input_tm(const PushParams<L>& p, const Geom& g, int cg, int tile, int bufoff)
+__device__ __forceinline__ void issue_tile_input_tm(const PushParams<L>& p, const Chunk& ck, const Geom& g, int cg, int tile, int bufoff)
 {
-    TmPrefetch<L> pf(p, g, cg, tile, bufoff);
+    TmPrefetch<L> pf(p, ck, g, cg, tile, bufoff);
     pf.finish();
 }
 
@@ -510,15 +522,15 @@ __device__ __forceinline__ void issue_tile_input_tm(const PushParams<L>& p, cons
 // j + 128 k from four warps' buffers and writes them with one 16-byte store (8 time rows of 64 bytes
 // per warp instruction) when the rows are 16-byte aligned (p.vec4), one by one otherwise.
 template <int L>
-__device__ __forceinline__ void store_tile_tm(const PushParams<L>& p, const Geom& g, float* __restrict__ out, int cg,
+__device__ __forceinline__ void store_tile_tm(const PushParams<L>& p, const Chunk& ck, const Geom& g, float* __restrict__ out, int cg,
                                               int bufoff, int t0)
 {
     constexpr int S = warp_stride<L, true>();
     if (p.vec4 && (cg + 1) * kTmChannels <= p.n_ch) {
         const int q = threadIdx.x & 3, j = threadIdx.x >> 2;           // j = 0 .. 127
-        const int t1 = min(p.n_t - t0, Geo<L>::tile);                  // tile positions [max(0, -t0), t1) exist
-        float* gp = out + (long long)cg * kTmChannels + 4 * q + (long long)(t0 + j) * p.out_pitch;
-        const long long gstep = 128LL * p.out_pitch;
+        const int t1 = min(ck.n_t - t0, Geo<L>::tile);                 // tile positions [max(0, -t0), t1) exist
+        float* gp = out + (long long)cg * kTmChannels + 4 * q + (long long)(t0 + j) * ck.out_pitch;
+        const long long gstep = 128LL * ck.out_pitch;
         const unsigned sa0 = (unsigned)__cvta_generic_to_shared(&fk_smem[4 * q * S + bufoff]);
 #pragma unroll 2
         for (int e = j; e < Geo<L>::tile; e += 128) {
@@ -539,12 +551,12 @@ __device__ __forceinline__ void store_tile_tm(const PushParams<L>& p, const Geom
     const int ch = cg * kTmChannels + c;
     if (ch < p.n_ch) {
         TmWalk<L> w(c * S + bufoff, j);
-        float* gp = out + ch + (long long)(t0 + j) * p.out_pitch;
-        const long long gstep = 32LL * p.out_pitch;
+        float* gp = out + ch + (long long)(t0 + j) * ck.out_pitch;
+        const long long gstep = 32LL * ck.out_pitch;
         int t = t0 + j;
 #pragma unroll 2
         for (int k = 0; k < Geo<L>::tile / 32; ++k) {
-            if ((unsigned)t < (unsigned)p.n_t) {
+            if ((unsigned)t < (unsigned)ck.n_t) {
                 float v;
                 asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(w.sa));
                 st_stream(gp, v);
@@ -612,7 +624,7 @@ __device__ __forceinline__ void local_pass(float2 (&x)[L], const SecParams<L>& T
 // `bufoff` = buf relative to the warp's shared-memory area; `item_end` is false for a warp whose
 // channel does not exist)
 template <int L, bool kInterior, bool kAllKinds, bool kTM>
-__device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom& g, int buf, int wst, float2 (&x)[L],
+__device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk& ck, const Geom& g, int buf, int wst, float2 (&x)[L],
                                              int ch, int tile, int lane, unsigned long long seen,
                                              bool item_end, unsigned rel_val, int cg, int bufoff,
                                              TmPrefetch<L>* pf = nullptr)
@@ -685,18 +697,18 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
     }
 
     if (kTM && pf != nullptr) pf->finish();
-    if (p.filt) {
+    if (ck.filt) {
         if (kTM) {
             regs_to_buf<L>(x, buf, lane, 0);
             __syncthreads();
-            store_tile_tm<L>(p, g, p.filt, cg, bufoff, t0);
+            store_tile_tm<L>(p, ck, g, ck.filt, cg, bufoff, t0);
             __syncthreads();
         } else {
-            float* row = p.filt + (long long)ch * p.out_pitch;
+            float* row = ck.filt + (long long)ch * ck.out_pitch;
             const int sf = row_shift(row, g.r0);
             regs_to_buf<L>(x, buf, lane, sf);
             __syncwarp();
-            store_tile<L, kInterior>(p, g, row, buf, lane, t0, sf);
+            store_tile<L, kInterior>(ck, g, row, buf, lane, t0, sf);
             __syncwarp();
         }
     }
@@ -745,7 +757,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
         if (lane + 32 < ns) __stcg(gst + lane + 32, fk_smem[wst + lane + 32]);
     }
 
-    if (p.cf) {
+    if (ck.cf) {
         // warm-up (reading R10): samples whose index since create/reset is < lta_len give cf = 0
         // (seen = samples pushed before this push; tile position e is sample seen + t0 + e of the stream)
         const long long rem = (long long)p.lta_len - (long long)seen - t0;     // first tile position with cf != 0
@@ -776,14 +788,14 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Geom&
             regs_to_buf<L>(x, buf, lane, 0);
             __syncthreads();
             if (item_end && lane == 0) st_release(p.progress + ch, rel_val);
-            store_tile_tm<L>(p, g, p.cf, cg, bufoff, t0);
+            store_tile_tm<L>(p, ck, g, ck.cf, cg, bufoff, t0);
         } else {
-            float* row = p.cf + (long long)ch * p.out_pitch;
+            float* row = ck.cf + (long long)ch * ck.out_pitch;
             const int sc = row_shift(row, g.r0);
             regs_to_buf<L>(x, buf, lane, sc);
             __syncwarp();
             if (item_end && lane == 0) st_release(p.progress + ch, rel_val);
-            store_tile<L, kInterior>(p, g, row, buf, lane, t0, sc);
+            store_tile<L, kInterior>(ck, g, row, buf, lane, t0, sc);
         }
     } else if (item_end) {
         __syncwarp();
@@ -848,6 +860,8 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     __shared__ unsigned sh_ctl[32];
     __shared__ unsigned sh_flag;
     __shared__ unsigned sh_item;
+    __shared__ int sh_tile0[kMaxBatch + 1];          // tiles (per channel) of the launch in front of chunk k
+    __shared__ unsigned sh_geo[kMaxBatch];           // slot geometry of chunk k: r0 | r1 << 8 | q_last << 16
     if (threadIdx.x == 0) sh_flag = 0u;
 
     if (p.wait_prior) asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -868,6 +882,33 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         const unsigned ring = __shfl_sync(0xffffffffu, v, kCtlSlotWords * (e & 1u) + 7);
         const unsigned need = __shfl_sync(0xffffffffu, v, kCtlSlotWords * (e & 1u) + 4 + ring);   // slot[e & 1].cum[ring]
         unsigned ex = __shfl_sync(0xffffffffu, v, kCtlExited + ring);
+        // the chunks of this launch: chunk k starts r0_k = (r0 + samples in front of it) mod L samples
+        // into a slot, which fixes its tiles (make_geom); an exclusive scan gives every chunk's first tile
+        const unsigned R0 = __shfl_sync(0xffffffffu, v, kCtlSlotWords * (e & 1u) + 2);
+        int carry = 0;
+        for (int k0 = 0; k0 < p.n_push; k0 += 32) {
+            const int k = k0 + lane;
+            int inc = 0;
+            unsigned geo = 0;
+            if (k < p.n_push) {
+                // (chunk 0 starts behind ALL samples waiting in the handle -- there can be more than L of
+                // them after a launch with a longer L; every later chunk behind a partial slot)
+                const unsigned r0k = k == 0 ? R0 : (R0 + p.ck[k].t_cum) % (unsigned)L;
+                const Geom gk = make_geom<L>(r0k, p.ck[k].n_base, p.ck[k].n_rem, true);
+                inc = gk.n_tiles;
+                geo = r0k | ((unsigned)gk.r1 << 8) | ((unsigned)gk.q_last << 16);
+            }
+            if (p.n_push > 1) {
+#pragma unroll
+                for (int d = 1; d < 32; d <<= 1) {
+                    const int u = __shfl_up_sync(0xffffffffu, inc, d);
+                    if (lane >= d) inc += u;
+                }
+            }
+            if (k < p.n_push) { sh_tile0[k + 1] = carry + inc; sh_geo[k] = geo; }
+            carry += __shfl_sync(0xffffffffu, inc, 31);
+        }
+        if (lane == 0) sh_tile0[0] = 0;
         while ((int)(ex - need) < 0)                                   // push e - kCmDepth must have completed
             ex = __shfl_sync(0xffffffffu, ld_relaxed(&cc->exited[ring]), 0);
         sh_ctl[lane] = v;
@@ -877,28 +918,45 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     const unsigned ring = sh_ctl[kCtlSlotWords * (epoch & 1u) + 7];
     const unsigned* sl = &sh_ctl[kCtlSlotWords * (epoch & 1u)];
     const unsigned long long seen = (unsigned long long)sl[0] | ((unsigned long long)sl[1] << 32);
-    const unsigned r0 = sl[2], seq0 = sl[3];
-    const Geom g = make_geom<L>(r0, p.n_base, p.n_rem, p.vec4 != 0);
+    const unsigned seq0 = sl[3];
     const int ns = state_floats(p.n_sec);
+    const int n_tiles_all = sh_tile0[p.n_push];          // tiles of the launch, per channel
+    // chunk that holds tile gt of the launch (tiles are numbered through all chunks); warp-uniform
+    auto chunk_of = [&](int gt) -> int {
+        if (p.n_push == 1) return 0;
+        const int a = lane + 1, b = lane + 33;
+        const unsigned m0 = __ballot_sync(0xffffffffu, a < p.n_push && sh_tile0[a] <= gt);
+        const unsigned m1 = __ballot_sync(0xffffffffu, b < p.n_push && sh_tile0[b] <= gt);
+        return __shfl_sync(0xffffffffu, __popc(m0) + __popc(m1), 0);
+    };
+    auto geom_of = [&](int k) -> Geom {
+        const unsigned w = sh_geo[k];
+        Geom g;
+        g.r0 = (int)(w & 0xffu); g.r1 = (int)((w >> 8) & 0xffu); g.q_last = (int)(w >> 16);
+        g.n_tiles = sh_tile0[k + 1] - sh_tile0[k];
+        g.vec4 = false;
+        return g;
+    };
 
     // Work items (segment, channel), segment-major; a segment is seg_tiles consecutive tiles of a
-    // channel, sized for about 8 items per warp.  Segment s of a channel starts from the state its
-    // segment s - 1 left in global memory (`progress` says when), i.e. item (s, c) waits for an item
-    // of LOWER index of the same push (or, for s = 0, for the push before).
-    //  - One segment per channel (ordinary pushes, kDyn = false): no waits inside the push; warp gw takes
-    //    items gw, gw + n_warps, ... statically.  What such a warp waits for belongs to an EARLIER push,
+    // channel (counted through all chunks of the launch), sized for about 8 items per warp.  Segment
+    // s of a channel starts from the state its segment s - 1 left in global memory (`progress` says
+    // when), i.e. item (s, c) waits for an item of LOWER index of the same launch (or, for s = 0,
+    // for the launch before).
+    //  - One segment per channel (ordinary pushes, kDyn = false): no waits inside the launch; warp gw takes
+    //    items gw, gw + n_warps, ... statically.  What such a warp waits for belongs to an EARLIER launch,
     //    every CTA of which had started before this grid could launch.
-    //  - Several segments per channel (long pushes, kDyn = true): items are CLAIMED from work[ring], a counter
-    //    in the control block, in rising order.  The holder of a claimed item is therefore a
-    //    resident warp, and so is the holder of every item it waits for (lower index = claimed
-    //    earlier): the unfinished item of lowest index can always run, whether or not the other
+    //  - Several segments per channel (long pushes and schedules, kDyn = true): items are CLAIMED from
+    //    work[ring], a counter in the control block, in rising order.  The holder of a claimed item is
+    //    therefore a resident warp, and so is the holder of every item it waits for (lower index =
+    //    claimed earlier): the unfinished item of lowest index can always run, whether or not the other
     //    CTAs of the grid have been scheduled yet (two handles pushing on two streams share the SMs
-    //    in any proportion).  The counter is never reset: push e claims work[ring] - wbase[ring],
+    //    in any proportion).  The counter is never reset: launch e claims work[ring] - wbase[ring],
     //    and every warp (time-major: CTA) makes exactly two claims beyond the last item, so the
-    //    next push of this ring position starts at wbase + n_items + 2 claimers.
+    //    next launch of this ring position starts at wbase + n_items + 2 claimers.
     const int n_warps = gridDim.x * W;
-    const int seg_tiles = min(p.seg_tiles, g.n_tiles);
-    const int n_seg = seg_tiles == g.n_tiles ? 1 : (g.n_tiles + seg_tiles - 1) / seg_tiles;
+    const int seg_tiles = min(p.seg_tiles, n_tiles_all);
+    const int n_seg = seg_tiles == n_tiles_all ? 1 : (n_tiles_all + seg_tiles - 1) / seg_tiles;
     const unsigned n_units = kTM ? (unsigned)((p.n_ch + kTmChannels - 1) / kTmChannels) : (unsigned)p.n_ch;
     const unsigned n_items = (unsigned)n_seg * n_units;
     constexpr bool dyn = kDyn;          // (chosen on the host: kDyn = false only if n_seg = 1 whatever r0 is)
@@ -913,7 +971,8 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         if (kTM ? threadIdx.x == 0 : lane == 0) pend = atomicAdd(&cc->work[ring], 1u);
     };
     // (time-major: thread 0 publishes `pend` in sh_item before a CTA barrier, claim_take runs after it)
-    auto claim_take = [&](int& ch, int& tile, int& tend, int& seg, int& cg) -> bool {
+    // gt / gtend: first tile of the item and the tile behind its last, as tiles of the launch
+    auto claim_take = [&](int& ch, int& gt, int& gtend, int& seg, int& cg) -> bool {
         unsigned it;
         if (dyn) {
             it = (kTM ? sh_item : __shfl_sync(0xffffffffu, pend, 0)) - sl[8 + ring];
@@ -926,8 +985,8 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         const int u = (int)(it - (unsigned)seg * n_units);
         cg = kTM ? u : 0;
         ch = kTM ? u * kTmChannels + warp : u;
-        tile = seg * seg_tiles;
-        tend = min(g.n_tiles, tile + seg_tiles);
+        gt = seg * seg_tiles;
+        gtend = min(n_tiles_all, gt + seg_tiles);
         return true;
     };
     // (every lane polls the same word and the value goes through a shuffle, so that the loop is
@@ -938,8 +997,8 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         while ((int)(done - need) < 0) done = __shfl_sync(0xffffffffu, ld_relaxed(p.progress + ch), 0);
     };
 
-    int ch = 0, tile = 0, tend = 0, seg = 0, cg = 0, cur = 0, wcur = 0;
-    // ---- hand the control block to the next push, then let it launch.  The ticket's round trip
+    int ch = 0, gt = 0, gtend = 0, seg = 0, cg = 0, cur = 0, wcur = 0, k = 0;
+    // ---- hand the control block to the next launch, then let it start.  The ticket's round trip
     // runs while the first rows are requested; only warp 0 waits for it, the other warps look at
     // the flag when their first tile has arrived.
     unsigned tk = 0;
@@ -949,28 +1008,31 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         claim_issue();
         if (kTM) { if (threadIdx.x == 0) sh_item = pend; __syncthreads(); }
     }
-    bool have = claim_take(ch, tile, tend, seg, cg);
+    bool have = claim_take(ch, gt, gtend, seg, cg);
     if (dyn) {
         if (kTM) __syncthreads();                    // (sh_item is rewritten at the next item's end)
         claim_issue();
     }
     if (have) {
-        if (kTM) issue_tile_input_tm<L>(p, g, cg, tile, 0);
-        else issue_tile_input<L, CTAS == 1>(p, g, ch, tile, wbase, lane);
-    }
-    // the first segment of a channel needs what the previous push left (state, hist): wait before
-    // those loads are issued (a wait on an EARLIER push cannot be part of a cycle)
-    if (have && seg == 0 && ch < p.n_ch) {
-        wait_progress(ch, seq0, kDyn ? ld_relaxed(p.progress + ch) : pr0);
-        issue_tile_carry<L>(p, g, ch, whs, wst0, lane);
+        k = chunk_of(gt);
+        const Geom g = geom_of(k);
+        if (kTM) issue_tile_input_tm<L>(p, p.ck[k], g, cg, gt - sh_tile0[k], 0);
+        else issue_tile_input<L, CTAS == 1>(p, p.ck[k], g, ch, gt - sh_tile0[k], wbase, lane);
+        // the first segment of a channel needs what the previous launch left (state, hist): wait before
+        // those loads are issued (a wait on an EARLIER launch cannot be part of a cycle)
+        if (seg == 0 && ch < p.n_ch) {
+            wait_progress(ch, seq0, kDyn ? ld_relaxed(p.progress + ch) : pr0);
+            issue_tile_carry<L>(p, g, ch, whs, wst0, lane);
+        }
     }
     if (warp == 0) {
         tk = __shfl_sync(0xffffffffu, tk, 0);
         if (lane == 0) {
             if (tk == gridDim.x - 1) {                                // every CTA has read slot[e & 1]
                 CmSlot* nx = &cc->slot[(epoch + 1u) & 1u];
-                __stcg(&nx->seen, seen + (unsigned long long)p.n_t);
-                __stcg(&nx->r0, (unsigned)g.r1);
+                const Chunk& cl = p.ck[p.n_push - 1];
+                __stcg(&nx->seen, seen + (unsigned long long)cl.t_cum + (unsigned long long)cl.n_t);
+                __stcg(&nx->r0, (sh_geo[p.n_push - 1] >> 8) & 0xffu);
                 __stcg(&nx->seq0, seq0 + (unsigned)n_seg);
                 for (unsigned j = 0; j < (unsigned)kCmDepth; ++j) {
                     __stcg(&nx->cum[j], sl[4 + j] + (j == ring ? gridDim.x : 0u));
@@ -992,74 +1054,90 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     asm volatile("griddepcontrol.launch_dependents;");
 
     while (have) {
-        int nch = ch, ntile = tile + 1, ntend = tend, nseg = seg, ncg = cg;
+        k = __shfl_sync(0xffffffffu, k, 0);            // (provably warp-uniform: the chunk is read through uniform registers)
+        const Chunk& ck = p.ck[k];
+        const Geom g = geom_of(k);
+        const int tile = gt - sh_tile0[k];             // tile of the chunk
+        int nch = ch, ngt = gt + 1, ngtend = gtend, nseg = seg, ncg = cg, nk = k;
         bool nhave = true;
-        const bool item_end = ntile == tend;
+        const bool item_end = ngt == gtend;
+        const bool item_first = gt == seg * seg_tiles;
         const bool valid = !kTM || ch < p.n_ch;        // (time-major: the last group may have idle warps)
         unsigned npr = 0;
         if (item_end) {
             if (!dyn || !kTM) {
-                nhave = claim_take(nch, ntile, ntend, nseg, ncg);
+                nhave = claim_take(nch, ngt, ngtend, nseg, ncg);
                 if (dyn) claim_issue();
                 if (nhave && nseg == 0 && nch < p.n_ch) npr = ld_relaxed(p.progress + nch);      // used after the tile is in registers
             } else if (threadIdx.x == 0) {
                 sh_item = pend;
             }
+        } else if (tile == g.n_tiles - 1) {
+            nk = k + 1;                                // the item goes on in the next chunk
         }
         const int buf = wbase + cur * Geo<L>::buf_floats;
         const int wst = wst0 + wcur * kStateSmem;
         cp_async_wait_all();
         if (kTM) __syncthreads(); else __syncwarp();   // (time-major: every thread's part of the tile has landed)
         if (kTM && dyn && item_end) {
-            nhave = claim_take(nch, ntile, ntend, nseg, ncg);
+            nhave = claim_take(nch, ngt, ngtend, nseg, ncg);
             claim_issue();
             if (nhave && nseg == 0 && nch < p.n_ch) npr = ld_relaxed(p.progress + nch);
         }
-        if (valid && seg > 0 && tile == seg * seg_tiles) {
-            // first tile of a later segment: wait for the segment before it, then fetch its state
+        if (item_end && nhave) nk = chunk_of(ngt);
+        nk = __shfl_sync(0xffffffffu, nk, 0);
+        if (valid && seg > 0 && item_first) {
+            // first tile of a later segment: wait for the segment before it, then fetch its state (and,
+            // where the segment begins with a chunk, the raw samples waiting in front of that chunk)
             wait_progress(ch, seq0 + (unsigned)seg, ld_relaxed(p.progress + ch));
             const float* gst = p.state + (long long)ch * ns;
             if (lane < ns) fk_smem[wst + lane] = ld_relaxed_f32(gst + lane);
             if (lane + 32 < ns) fk_smem[wst + lane + 32] = ld_relaxed_f32(gst + lane + 32);
+            if (tile == 0 && lane < g.r0) fk_smem[whs + lane] = ld_relaxed_f32(p.hist + (long long)ch * kHist + lane);
             __syncwarp();
         }
-        const int sin = kTM ? 0 : row_shift(p.in + (long long)ch * p.in_pitch, g.r0);
+        const int sin = kTM ? 0 : row_shift(ck.in + (long long)ch * ck.in_pitch, g.r0);
         if (valid && tile == 0 && g.r0 != 0) {
-            // first tile of the channel: the waiting raw samples from the scratch to the head of the tile
+            // first tile of the chunk: the waiting raw samples from the scratch to the head of the tile
             for (int e = lane; e < g.r0; e += 32) fk_smem[buf + raw_index<L>(e + sin)] = fk_smem[whs + e];
             __syncwarp();
         }
         if (valid && tile == g.n_tiles - 1 && g.r1 != 0) {
-            // last tile of the channel: keep the raw samples of its trailing partial slot
+            // last tile of the chunk: keep the raw samples of its trailing partial slot -- in the scratch
+            // if this item goes on with the next chunk, in the handle for whoever continues the channel
             const int e0 = g.q_last * L;                              // tile-space position of that slot
-            float* hd = p.hist + (long long)ch * kHist;
-            for (int j = lane; j < g.r1; j += 32) hd[j] = fk_smem[buf + raw_index<L>(e0 + j + sin)];
+            if (item_end) {
+                float* hd = p.hist + (long long)ch * kHist;
+                for (int j = lane; j < g.r1; j += 32) hd[j] = fk_smem[buf + raw_index<L>(e0 + j + sin)];
+            } else {
+                for (int j = lane; j < g.r1; j += 32) fk_smem[whs + j] = fk_smem[buf + raw_index<L>(e0 + j + sin)];
+            }
         }
         float2 x[L];
         buf_to_regs<L>(x, buf, lane, sin, p.gain);
         __syncwarp();
         if (nhave) {
             const int nbuf = wbase + (cur ^ 1) * Geo<L>::buf_floats;
-            if (!kTM) issue_tile_input<L, CTAS == 1>(p, g, nch, ntile, nbuf, lane);
+            if (!kTM) issue_tile_input<L, CTAS == 1>(p, p.ck[nk], geom_of(nk), nch, ngt - sh_tile0[nk], nbuf, lane);
             if (item_end && nseg == 0 && nch < p.n_ch) {
                 wait_progress(nch, seq0, npr);
-                issue_tile_carry<L>(p, g, nch, whs, wst0 + (wcur ^ 1) * kStateSmem, lane);
+                issue_tile_carry<L>(p, geom_of(nk), nch, whs, wst0 + (wcur ^ 1) * kStateSmem, lane);
             }
         }
         // (a segment's end writes the carried state back and tells whoever continues the channel:
-        // the next segment of this push or the first segment of the next push)
+        // the next segment of this launch or the first segment of the next launch)
         if (kTM) {
             // (time-major: the next tile is requested in portions while this one is computed)
-            TmPrefetch<L> pf(p, g, ncg, ntile, (cur ^ 1) * Geo<L>::buf_floats);
-            process_tile<L, true, kAllKinds, true>(p, g, buf, wst, x, ch, tile, lane, seen, item_end && valid,
+            TmPrefetch<L> pf(p, p.ck[nk], geom_of(nk), ncg, ngt - sh_tile0[nk], (cur ^ 1) * Geo<L>::buf_floats);
+            process_tile<L, true, kAllKinds, true>(p, ck, g, buf, wst, x, ch, tile, lane, seen + ck.t_cum, item_end && valid,
                                                    seq0 + (unsigned)seg + 1u, cg, cur * Geo<L>::buf_floats,
                                                    nhave ? &pf : nullptr);
         } else {
-            process_tile<L, CTAS == 1, kAllKinds, false>(p, g, buf, wst, x, ch, tile, lane, seen, item_end && valid,
+            process_tile<L, CTAS == 1, kAllKinds, false>(p, ck, g, buf, wst, x, ch, tile, lane, seen + ck.t_cum, item_end && valid,
                                                          seq0 + (unsigned)seg + 1u, cg, cur * Geo<L>::buf_floats);
         }
         if (item_end) wcur ^= 1;
-        ch = nch; tile = ntile; tend = ntend; seg = nseg; cg = ncg; have = nhave; cur ^= 1;
+        ch = nch; gt = ngt; gtend = ngtend; seg = nseg; cg = ncg; have = nhave; k = nk; cur ^= 1;
     }
     // completion: count this CTA out (push e + kCmDepth waits until all of them are)
     __syncthreads();

@@ -13,7 +13,9 @@
 #include <cstring>
 #include <mutex>
 #include <new>
+#include <algorithm>
 #include <unordered_map>
+#include <vector>
 
 #include "../../include/filark_stream.h"
 #include "../../include/filark_debug.h"
@@ -236,6 +238,26 @@ static cudaError_t launch_cm_variant(const PushParams<L>& p, int device, int gri
     return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, CTAS, kAllKinds, false, kDyn>, p);
 }
 
+// Tiles per channel of a launch: the r0 = 0 estimate and the largest number whatever r0 < kMaxL the
+// first chunk finds waiting (a later chunk's r0 follows from the first one's).
+template <int L> static void launch_tiles(const PushParams<L>& p, long long* est, long long* most)
+{
+    long long e = 0, m = 0;
+    for (int k = 0; k < p.n_push; ++k) {
+        e += ((long long)p.ck[k].n_t + L - 1) / L / 64 + 1;
+        m += (((long long)p.ck[k].n_t + kMaxL - 1 + L - 1) / L + 63) / 64;
+    }
+    *est = e; *most = m;
+}
+
+// Tiles per work item: about 8 items per warp of the grid.  (Not evened out: a short last segment
+// per channel is welcome -- items are taken in rising order, so the short ones fill the end of the launch.)
+static int segment_tiles(long long n_tiles, long long units, long long workers)
+{
+    const long long st = n_tiles * units / (8LL * workers);
+    return (int)(st < 1 ? 1 : (st > 0x3fffffff ? 0x3fffffff : st));
+}
+
 template <int L, int CTAS, bool kAllKinds>
 static cudaError_t launch_cm_shape(const filark_stream* h, PushParams<L>& p, cudaStream_t stream)
 {
@@ -253,13 +275,10 @@ static cudaError_t launch_cm_shape(const filark_stream* h, PushParams<L>& p, cud
     int grid = (p.n_ch + W - 1) / W;
     const int resident = h->n_sm * (per_sm / W < 16 ? per_sm / W : 16);
     if (grid > resident) grid = resident;
-    // work items: runs of seg_tiles tiles of a channel, about 8 items per warp of the grid
-    const long long n_tiles_max = (((long long)p.n_t + kMaxL - 1 + L - 1) / L + 63) / 64;     // whatever r0 < kMaxL is
-    {
-        const long long n_tiles = ((long long)p.n_t + L - 1) / L / 64 + 1;          // r0 = 0 estimate, >= 1
-        long long st = n_tiles * p.n_ch / (8LL * grid * W);
-        p.seg_tiles = (int)(st < 1 ? 1 : (st > 0x3fffffff ? 0x3fffffff : st));
-    }
+    // work items: runs of seg_tiles tiles of a channel
+    long long n_tiles, n_tiles_max;
+    launch_tiles<L>(p, &n_tiles, &n_tiles_max);
+    p.seg_tiles = segment_tiles(n_tiles, p.n_ch, (long long)grid * W);
     // one segment per channel for certain: static work distribution; otherwise items are claimed
     // (filark_kernels.cuh, "Work items").  Long pushes (CTAS = 1) always claim.
     const size_t smem_max = (size_t)cm_cta_warps<L, CTAS>() * warp_bytes;
@@ -276,8 +295,9 @@ template <int L>
 static cudaError_t launch_cm(const filark_stream* h, PushParams<L>& p, cudaStream_t stream)
 {
     if constexpr (L == 24 || (L == 16 && FK_MAXW16 != 16)) {
-        const long long tiles = ((long long)p.n_t + kHist + Geo<L>::tile - 1) / Geo<L>::tile * p.n_ch;
-        const bool long_push = tiles >= 12LL * h->n_sm * cm_max_warps<L>();
+        long long n_tiles, n_tiles_max;
+        launch_tiles<L>(p, &n_tiles, &n_tiles_max);
+        const bool long_push = n_tiles_max * p.n_ch >= 12LL * h->n_sm * cm_max_warps<L>();
         if (long_push && !tune().small_ctas)
             return h->lean_kinds ? launch_cm_shape<L, 1, false>(h, p, stream) : launch_cm_shape<L, 1, true>(h, p, stream);
     }
@@ -293,12 +313,9 @@ static cudaError_t launch_tm_kinds(const filark_stream* h, PushParams<L>& p, cud
     const size_t smem = sizeof(float) * (size_t)kTmChannels * (size_t)warp_stride<L, true>();
     const int n_cg = (p.n_ch + kTmChannels - 1) / kTmChannels;
     const int grid = n_cg < h->n_sm ? n_cg : h->n_sm;
-    const long long n_tiles_max = (((long long)p.n_t + kMaxL - 1 + L - 1) / L + 63) / 64;
-    {
-        const long long n_tiles = ((long long)p.n_t + L - 1) / L / 64 + 1;
-        long long st = n_tiles * n_cg / (8LL * grid);
-        p.seg_tiles = (int)(st < 1 ? 1 : (st > 0x3fffffff ? 0x3fffffff : st));
-    }
+    long long n_tiles, n_tiles_max;
+    launch_tiles<L>(p, &n_tiles, &n_tiles_max);
+    p.seg_tiles = segment_tiles(n_tiles, n_cg, grid);
     cudaLaunchConfig_t cfg{};
     cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)(kTmChannels * 32));
     cfg.dynamicSmemBytes = smem; cfg.stream = stream;
@@ -323,17 +340,28 @@ static cudaError_t launch_tm(const filark_stream* h, PushParams<L>& p, cudaStrea
     return h->lean_kinds ? launch_tm_kinds<L, false>(h, p, stream) : launch_tm_kinds<L, true>(h, p, stream);
 }
 
+// One chunk as the caller describes it (all pushes end up here).
+struct ChunkArgs {
+    const float* in; long long n_t, in_pitch;
+    float* filt; float* cf; long long out_pitch;
+};
+
 template <int L>
-static cudaError_t push_variant(const filark_stream* h, int v, const float* d_in, int n_t, long long in_pitch,
-                                float* d_filt, float* d_cf, long long out_pitch, int vec4, int wait_prior,
+static cudaError_t push_variant(const filark_stream* h, int v, const ChunkArgs* c, int n, int vec4, int wait_prior,
                                 cudaStream_t stream)
 {
     PushParams<L> p = *(const PushParams<L>*)h->proto[v];
-    p.in = d_in; p.filt = d_filt; p.cf = d_cf;
     p.state = h->d_state; p.hist = h->d_hist; p.cctl = h->d_cctl; p.progress = h->d_progress;
-    p.in_pitch = in_pitch; p.out_pitch = out_pitch; p.n_t = n_t; p.vec4 = vec4;
-    p.n_base = n_t / L; p.n_rem = n_t % L;
-    p.wait_prior = wait_prior;
+    p.n_push = n; p.vec4 = vec4; p.wait_prior = wait_prior;
+    unsigned t_cum = 0;
+    for (int k = 0; k < n; ++k) {
+        Chunk& d = p.ck[k];
+        d.in = c[k].in; d.filt = c[k].filt; d.cf = c[k].cf;
+        d.in_pitch = c[k].in_pitch; d.out_pitch = c[k].out_pitch;
+        d.n_t = (int)c[k].n_t; d.n_base = (int)(c[k].n_t / L); d.n_rem = (int)(c[k].n_t % L);
+        d.t_cum = t_cum;
+        t_cum += (unsigned)c[k].n_t;
+    }
     if (h->layout == FILARK_LAYOUT_TIME_MAJOR) return launch_tm<L>(h, p, stream);
     return launch_cm<L>(h, p, stream);
 }
@@ -484,56 +512,84 @@ static bool overlaps(const void* a, size_t na, const void* b, size_t nb)
     return a0 < b0 + nb && b0 < a0 + na;
 }
 
-// One push.  may_overlap: the caller of this function knows that nothing but this handle's own
-// previous push lies between that push and this one in `stream` (filark_stream.h, "Ordering").
-static filark_status_t push_impl(filark_stream_t* h, const float* d_in, long long n_t,
-                                 long long in_pitch, float* d_filt, float* d_cf,
-                                 long long out_pitch, cudaStream_t stream, bool may_overlap)
+// Argument checks of one chunk (include/filark_stream.h, filark_stream_push); the byte extents of its buffers.
+static filark_status_t check_chunk(const filark_stream* h, const ChunkArgs& c, size_t* in_bytes, size_t* out_bytes)
 {
-    if (!h || n_t < 0) return FILARK_ERR_INVALID_ARG;
-    if (n_t == 0) return FILARK_OK;
-    if (!d_in || (!d_filt && !d_cf)) return FILARK_ERR_INVALID_ARG;
+    if (c.n_t < 1 || c.n_t > 0x7fff0000LL) return FILARK_ERR_INVALID_ARG;     // samples per channel of one chunk fit an int
+    if (!c.in || (!c.filt && !c.cf)) return FILARK_ERR_INVALID_ARG;
     const bool cm = h->layout == FILARK_LAYOUT_CHANNEL_MAJOR;
-    const long long row_len = cm ? n_t : (long long)h->n_ch;
-    const long long n_rows = cm ? (long long)h->n_ch : n_t;
-    if (in_pitch < row_len || out_pitch < row_len) return FILARK_ERR_INVALID_ARG;
-    if (((uintptr_t)d_in | (uintptr_t)d_filt | (uintptr_t)d_cf) & 3u) return FILARK_ERR_ALIGNMENT;
-    const size_t in_bytes = sizeof(float) * (size_t)((n_rows - 1) * in_pitch + row_len);
-    const size_t out_bytes = sizeof(float) * (size_t)((n_rows - 1) * out_pitch + row_len);
-    if ((d_filt && overlaps(d_in, in_bytes, d_filt, out_bytes)) ||
-        (d_cf && overlaps(d_in, in_bytes, d_cf, out_bytes)) ||
-        (d_filt && d_cf && overlaps(d_filt, out_bytes, d_cf, out_bytes)))
+    const long long row_len = cm ? c.n_t : (long long)h->n_ch;
+    const long long n_rows = cm ? (long long)h->n_ch : c.n_t;
+    if (c.in_pitch < row_len || c.out_pitch < row_len) return FILARK_ERR_INVALID_ARG;
+    if (((uintptr_t)c.in | (uintptr_t)c.filt | (uintptr_t)c.cf) & 3u) return FILARK_ERR_ALIGNMENT;
+    *in_bytes = sizeof(float) * (size_t)((n_rows - 1) * c.in_pitch + row_len);
+    *out_bytes = sizeof(float) * (size_t)((n_rows - 1) * c.out_pitch + row_len);
+    if ((c.filt && overlaps(c.in, *in_bytes, c.filt, *out_bytes)) ||
+        (c.cf && overlaps(c.in, *in_bytes, c.cf, *out_bytes)) ||
+        (c.filt && c.cf && overlaps(c.filt, *out_bytes, c.cf, *out_bytes)))
         return FILARK_ERR_INVALID_ARG;
-    int dev = -1;
-    cudaError_t e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return cuda_fail(h, e);
-    if (dev != h->device) return FILARK_ERR_DEVICE_MISMATCH;
+    return FILARK_OK;
+}
 
-    if (n_t > 0x7fff0000LL) return FILARK_ERR_INVALID_ARG;        // samples per channel of one push fit an int
+// Sub-block length for a launch: the cheapest variant over its chunks (every chunk has tiles of its own).
+static int choose_variant_chunks(const filark_stream* h, const ChunkArgs* c, int n)
+{
+    for (int i = 0; i < kNumVariants; ++i) if (kVariantL[i] == (int)((h->flags >> 8) & 0xFF)) return i;
+    if (n == 1) return choose_variant(c[0].n_t);
+    int best = kNumVariants - 1; double best_cost = 1e300;
+    for (int v = 0; v < kNumVariants; ++v) {
+        const int L = kVariantL[v];
+        double cost = 0.0;
+        for (int k = 0; k < n; ++k) cost += (double)(((c[k].n_t + L - 1) / L + 63) / 64) * (L + 10.0);
+        if (cost < best_cost * (1.0 - 1e-9) || (cost <= best_cost * (1.0 + 1e-9) && L == 24)) { best_cost = cost; best = v; }
+    }
+    return best;
+}
 
+// ONE launch over n <= kMaxBatch checked chunks (consecutive in the stream of samples).  may_overlap:
+// the caller knows that nothing but this handle's own previous launch lies between that launch and
+// this one in `stream` (filark_stream.h, "Ordering").
+static filark_status_t launch_chunks(filark_stream_t* h, const ChunkArgs* c, int n, cudaStream_t stream, bool may_overlap)
+{
+    const bool cm = h->layout == FILARK_LAYOUT_CHANNEL_MAJOR;
+    cudaError_t e = cudaSuccess;
+    long long total = 0;
+    for (int k = 0; k < n; ++k) total += c[k].n_t;
     if (h->flags & FILARK_FLAG_SERIAL_SCAN) {
-        // Serial diagnostic kernel (either layout).
+        // Serial diagnostic kernel (either layout), chunk by chunk.
         const int ns = state_floats(h->n_sec);
-        SerialParams p = h->serial;
-        p.in = d_in; p.filt = d_filt; p.cf = d_cf; p.state = h->d_state; p.n_t = n_t;
-        p.sc_in = cm ? in_pitch : 1; p.st_in = cm ? 1 : in_pitch;
-        p.sc_out = cm ? out_pitch : 1; p.st_out = cm ? 1 : out_pitch;
-        p.state_sc = cm ? ns : 1; p.state_sk = cm ? 1 : h->n_ch;
-        const int block = 128, grid = (h->n_ch + block - 1) / block;
-        filark_push_serial_kernel<<<grid, block, 0, stream>>>(p);
-        e = cudaGetLastError();
+        for (int k = 0; k < n && e == cudaSuccess; ++k) {
+            SerialParams p = h->serial;
+            p.in = c[k].in; p.filt = c[k].filt; p.cf = c[k].cf; p.state = h->d_state; p.n_t = c[k].n_t;
+            p.sc_in = cm ? c[k].in_pitch : 1; p.st_in = cm ? 1 : c[k].in_pitch;
+            p.sc_out = cm ? c[k].out_pitch : 1; p.st_out = cm ? 1 : c[k].out_pitch;
+            p.state_sc = cm ? ns : 1; p.state_sk = cm ? 1 : h->n_ch;
+            const int block = 128, grid = (h->n_ch + block - 1) / block;
+            filark_push_serial_kernel<<<grid, block, 0, stream>>>(p);
+            e = cudaGetLastError();
+            if (e == cudaSuccess) h->launches += 1;
+        }
     } else {
-        int v = choose_variant(n_t);
-        for (int i = 0; i < kNumVariants; ++i) if (kVariantL[i] == (int)((h->flags >> 8) & 0xFF)) v = i;
-        const uintptr_t all = (uintptr_t)d_in | (uintptr_t)d_filt | (uintptr_t)d_cf;
-        // (channel-major: introspection only; time-major: output rows allow 16-byte stores)
-        const int vec4 = cm ? (((all & 15u) == 0 && (in_pitch & 3) == 0 && (out_pitch & 3) == 0 && (n_t & 3) == 0) ? 1 : 0)
-                            : (((((uintptr_t)d_filt | (uintptr_t)d_cf) & 15u) == 0 && (out_pitch & 3) == 0) ? 1 : 0);
-        // May this push overlap the one before it?  Only if that was this handle's own push, directly
+        const int v = choose_variant_chunks(h, c, n);
+        // bounding ranges of what the launch reads ([0]) and writes ([1] filt, [2] cf); alignment
+        uintptr_t lo[3] = {~(uintptr_t)0, ~(uintptr_t)0, ~(uintptr_t)0}, hi[3] = {0, 0, 0};
+        int vec4 = 1;
+        for (int k = 0; k < n; ++k) {
+            size_t ib = 0, ob = 0;
+            check_chunk(h, c[k], &ib, &ob);
+            const uintptr_t l3[3] = {(uintptr_t)c[k].in, (uintptr_t)c[k].filt, (uintptr_t)c[k].cf};
+            const size_t b3[3] = {ib, ob, ob};
+            for (int i = 0; i < 3; ++i)
+                if (l3[i]) { if (l3[i] < lo[i]) lo[i] = l3[i]; if (l3[i] + b3[i] > hi[i]) hi[i] = l3[i] + b3[i]; }
+            const uintptr_t all = l3[0] | l3[1] | l3[2];
+            // (channel-major: introspection only; time-major: output rows allow 16-byte stores)
+            const bool ok = cm ? ((all & 15u) == 0 && (c[k].in_pitch & 3) == 0 && (c[k].out_pitch & 3) == 0 && (c[k].n_t & 3) == 0)
+                               : (((l3[1] | l3[2]) & 15u) == 0 && (c[k].out_pitch & 3) == 0);
+            if (!ok) vec4 = 0;
+        }
+        // May this launch overlap the one before it?  Only if that was this handle's own launch, directly
         // before it in the same stream as far as this library launched anything, and the two share no
-        // buffer (filark_stream.h, "Ordering").
-        const uintptr_t lo[3] = {(uintptr_t)d_in, (uintptr_t)d_filt, (uintptr_t)d_cf};
-        const uintptr_t hi[3] = {lo[0] + in_bytes, d_filt ? lo[1] + out_bytes : 0, d_cf ? lo[2] + out_bytes : 0};
+        // buffer (bounding ranges; filark_stream.h, "Ordering").
         int wait_prior = 1;
         if (may_overlap && !(h->flags & FILARK_FLAG_STRICT_ORDER) && h->prev_valid > 0 && h->prev_stream == stream &&
             registry_is_last(stream, h)) {
@@ -546,26 +602,49 @@ static filark_status_t push_impl(filark_stream_t* h, const float* d_in, long lon
                             clash = true;
             wait_prior = clash ? 1 : 0;
         }
-        const int n_prev = wait_prior ? 0 : h->prev_valid;       // a waiting push leaves nothing in flight behind it
+        const int n_prev = wait_prior ? 0 : h->prev_valid;       // a waiting launch leaves nothing in flight behind it
         h->prev_valid = 0;
         switch (kVariantL[v]) {
-            case 8: e = push_variant<8>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, wait_prior, stream); break;
-            case 16: e = push_variant<16>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, wait_prior, stream); break;
-            default: e = push_variant<24>(h, v, d_in, (int)n_t, in_pitch, d_filt, d_cf, out_pitch, vec4, wait_prior, stream); break;
+            case 8: e = push_variant<8>(h, v, c, n, vec4, wait_prior, stream); break;
+            case 16: e = push_variant<16>(h, v, c, n, vec4, wait_prior, stream); break;
+            default: e = push_variant<24>(h, v, c, n, vec4, wait_prior, stream); break;
         }
         if (e == cudaSuccess) {
             const int keep = n_prev < kCmDepth - 2 ? n_prev : kCmDepth - 2;
             for (int q = keep; q > 0; --q)
                 for (int i = 0; i < 3; ++i) { h->prev_lo[q][i] = h->prev_lo[q - 1][i]; h->prev_hi[q][i] = h->prev_hi[q - 1][i]; }
-            for (int i = 0; i < 3; ++i) { h->prev_lo[0][i] = lo[i]; h->prev_hi[0][i] = hi[i]; }
+            for (int i = 0; i < 3; ++i) { h->prev_lo[0][i] = hi[i] ? lo[i] : 0; h->prev_hi[0][i] = hi[i]; }
             h->prev_valid = keep + 1; h->prev_stream = stream;
+            h->launches += 1;
         }
     }
     registry_set(stream, h);
     if (e != cudaSuccess) return cuda_fail(h, e);
-    h->launches += 1;
-    h->samples += n_t;
+    h->samples += total;
     return FILARK_OK;
+}
+
+static filark_status_t check_device(filark_stream_t* h)
+{
+    int dev = -1;
+    const cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(h, e);
+    return dev != h->device ? FILARK_ERR_DEVICE_MISMATCH : FILARK_OK;
+}
+
+// One push = one launch over one chunk.
+static filark_status_t push_impl(filark_stream_t* h, const float* d_in, long long n_t,
+                                 long long in_pitch, float* d_filt, float* d_cf,
+                                 long long out_pitch, cudaStream_t stream, bool may_overlap)
+{
+    if (!h || n_t < 0) return FILARK_ERR_INVALID_ARG;
+    if (n_t == 0) return FILARK_OK;
+    const ChunkArgs c{d_in, n_t, in_pitch, d_filt, d_cf, out_pitch};
+    size_t ib = 0, ob = 0;
+    filark_status_t st = check_chunk(h, c, &ib, &ob);
+    if (st == FILARK_OK) st = check_device(h);
+    if (st != FILARK_OK) return st;
+    return launch_chunks(h, &c, 1, stream, may_overlap);
 }
 
 filark_status_t filark_stream_push_pitched(filark_stream_t* h, const float* d_in, long long n_t,
@@ -584,20 +663,69 @@ filark_status_t filark_stream_push(filark_stream_t* h, const float* d_in, long l
     return push_impl(h, d_in, n_t, pitch, d_filt, d_cf, pitch, stream, (h->flags & FILARK_FLAG_OVERLAP_PUSHES) != 0);
 }
 
+// Does any buffer written by one chunk of the schedule overlap a buffer of ANOTHER chunk?  (Then the
+// chunks cannot share a launch: inside a launch a channel's next tile is requested before the
+// outputs of the tile before it are stored.)  Sweep over the ranges sorted by start address.
+static bool schedule_aliases(const filark_stream* h, const ChunkArgs* c, int n)
+{
+    struct R { uintptr_t lo, hi; int out; };
+    std::vector<R> r;
+    r.reserve(3 * (size_t)n);
+    for (int k = 0; k < n; ++k) {
+        size_t ib = 0, ob = 0;
+        check_chunk(h, c[k], &ib, &ob);
+        r.push_back({(uintptr_t)c[k].in, (uintptr_t)c[k].in + ib, 0});
+        if (c[k].filt) r.push_back({(uintptr_t)c[k].filt, (uintptr_t)c[k].filt + ob, 1});
+        if (c[k].cf) r.push_back({(uintptr_t)c[k].cf, (uintptr_t)c[k].cf + ob, 1});
+    }
+    std::sort(r.begin(), r.end(), [](const R& a, const R& b) { return a.lo < b.lo; });
+    uintptr_t end_any = 0, end_out = 0;            // furthest end of the ranges seen so far: all / written ones
+    for (const R& x : r) {
+        if (x.out ? x.lo < end_any : x.lo < end_out) return true;
+        if (x.hi > end_any) end_any = x.hi;
+        if (x.out && x.hi > end_out) end_out = x.hi;
+    }
+    return false;
+}
+
 filark_status_t filark_stream_push_many(filark_stream_t* h, int n_push, const float* const* d_in,
                                         const long long* n_t, float* const* d_filt, float* const* d_cf,
                                         cudaStream_t stream)
 {
     if (!h || n_push < 0 || (n_push > 0 && (!d_in || !n_t))) return FILARK_ERR_INVALID_ARG;
-    // (what lies between two pushes of this call is known: nothing)
-    bool first = true;
+    // the whole schedule is checked before anything is enqueued
+    std::vector<ChunkArgs> c;
+    c.reserve((size_t)n_push);
     for (int i = 0; i < n_push; ++i) {
+        if (n_t[i] < 0) return FILARK_ERR_INVALID_ARG;
+        if (n_t[i] == 0) continue;
         const long long pitch = h->layout == FILARK_LAYOUT_CHANNEL_MAJOR ? n_t[i] : (long long)h->n_ch;
-        const filark_status_t st = push_impl(h, d_in[i], n_t[i], pitch, d_filt ? d_filt[i] : nullptr,
-                                             d_cf ? d_cf[i] : nullptr, pitch, stream,
-                                             !first || (h->flags & FILARK_FLAG_OVERLAP_PUSHES) != 0);
+        const ChunkArgs a{d_in[i], n_t[i], pitch, d_filt ? d_filt[i] : nullptr, d_cf ? d_cf[i] : nullptr, pitch};
+        size_t ib = 0, ob = 0;
+        const filark_status_t st = check_chunk(h, a, &ib, &ob);
         if (st != FILARK_OK) return st;
-        if (n_t[i] > 0) first = false;
+        c.push_back(a);
+    }
+    if (c.empty()) return FILARK_OK;
+    const filark_status_t sd = check_device(h);
+    if (sd != FILARK_OK) return sd;
+    // Chunks that share no buffer go into common launches of up to kMaxBatch chunks (and < 2^31 samples
+    // per channel): the carried state then never leaves the SM between them.  Otherwise, and with
+    // FILARK_FLAG_STRICT_ORDER, one launch per chunk.
+    const int n = (int)c.size();
+    const bool fuse = !(h->flags & (FILARK_FLAG_STRICT_ORDER | FILARK_FLAG_SERIAL_SCAN)) && n > 1 && !schedule_aliases(h, c.data(), n);
+    bool first = true;
+    for (int i = 0; i < n;) {
+        int m = 1;
+        if (fuse) {
+            long long tot = c[i].n_t;
+            while (i + m < n && m < kMaxBatch && tot + c[i + m].n_t <= 0x7fff0000LL) { tot += c[i + m].n_t; ++m; }
+        }
+        // (what lies between two launches of this call is known: nothing)
+        const filark_status_t st = launch_chunks(h, c.data() + i, m, stream, !first || (h->flags & FILARK_FLAG_OVERLAP_PUSHES) != 0);
+        if (st != FILARK_OK) return st;
+        first = false;
+        i += m;
     }
     return FILARK_OK;
 }

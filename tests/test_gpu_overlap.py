@@ -204,9 +204,10 @@ def test_graph_of_back_to_back_pushes(cuda_device):
 
 
 def test_push_many_equals_separate_pushes(cuda_device):
-    """filark_stream_push_many == the same pushes one call at a time (bit for bit), for a schedule
-    with ragged and zero-length chunks, NULL output arrays and single NULL outputs; it enqueues one
-    kernel per non-empty chunk."""
+    """filark_stream_push_many == the same pushes one call at a time, bit for bit (same sub-block
+    length L everywhere), for a schedule with ragged and zero-length chunks, NULL output arrays and
+    single NULL outputs; the chunks share no buffer, so one launch serves them all."""
+    L24 = 24 << 8
     n_ch, sizes = 2600, [1500, 1500, 64, 0, 1501, 3000, 7, 1500]
     n_t = sum(sizes)
     w = CONFIGS["cfg3"].scaled(n_ch=n_ch, n_t=n_t)
@@ -216,19 +217,19 @@ def test_push_many_equals_separate_pushes(cuda_device):
     chunks, p = [], 0
     for c in sizes:
         chunks.append(xd[:, p:p + c].contiguous()); p += c
-    ref = FilarkStream(n_ch, sos, w.sta_len, w.lta_len, CHANNEL_MAJOR, FLAG_STRICT_ORDER)
+    ref = FilarkStream(n_ch, sos, w.sta_len, w.lta_len, CHANNEL_MAJOR, FLAG_STRICT_ORDER | L24)
     rf, rc = _alloc(chunks)
     for a, f, c in zip(chunks, rf, rc):
         ref.push(a, f, c)
     torch.cuda.synchronize()
     ref.destroy()
-    for flags in (0, OV):
+    for flags in (L24, OV | L24):
         s = FilarkStream(n_ch, sos, w.sta_len, w.lta_len, CHANNEL_MAJOR, flags)
         of, oc = _alloc(chunks)
         for rep in range(2):
             s.push_many(chunks, of, oc)
             torch.cuda.synchronize()
-            assert s.launch_count == (rep + 1) * sum(1 for c in sizes if c)
+            assert s.launch_count == rep + 1
             for a, b in zip(of + oc, rf + rc):
                 assert torch.equal(a, b)
             s.reset()
