@@ -248,12 +248,40 @@ __device__ __forceinline__ int row_shift(const float* row, int r0)
 // index in a tile buffer of raw position p (padded lane regions)
 template <int L> __device__ __forceinline__ int raw_index(int p) { return p + 4 * (p / (2 * L)); }
 
+// Where chunk c = 32 m + lane of a tile (16 bytes, chunks in time order: what one warp instruction moves
+// between global and shared memory) sits in a tile buffer with padded lane regions: float offset
+// 4 c + 4 (c / C), C = chunks per lane region.  Written as (per-lane base) + (constant of m), so that the
+// unrolled copy loops address with immediates and no per-chunk arithmetic: for C | 32 the quotient
+// splits at once; for C = 12 (L = 24) c / 12 = lane / 12 + 2 m + (8 m + lane mod 12) / 12, and the last
+// term is (2 m) / 3 plus a step at lane mod 12 >= 4 (m mod 3 = 1) or >= 8 (m mod 3 = 2): three bases.
+template <int L> struct TimeOrder {
+    static constexpr int C = Geo<L>::chunks;
+    static_assert(32 % C == 0 || C == 12, "sub-block lengths 8, 16, 24 (and 32, 64)");
+    int b0, b1, b2;
+    __device__ __forceinline__ explicit TimeOrder(int lane)
+    {
+        if (C == 12) {
+            const int a = lane / 12, r = lane - 12 * a;
+            b0 = 4 * lane + 4 * a; b1 = b0 + (r >= 4 ? 4 : 0); b2 = b0 + (r >= 8 ? 4 : 0);
+        } else {
+            b0 = b1 = b2 = 4 * lane + 4 * (lane / C);
+        }
+    }
+    // (m is a compile-time constant wherever this is used: fully unrolled loops)
+    __device__ __forceinline__ int at(int m) const
+    {
+        if (C == 12) return (m % 3 == 0 ? b0 : (m % 3 == 1 ? b1 : b2)) + 136 * m + 4 * ((2 * m) / 3);
+        return b0 + 128 * m + 4 * ((32 * m) / C);
+    }
+};
+
 // S0: start the asynchronous copy of one tile of one channel into `buf` (padded lane regions:
 // tile-local sample e lives at buf[e + 4 (e / 2L)]) and, with the channel's first tile, of its
 // carried state into `wst`.  Tile-space position e of tile `tile` is input sample
 // t = tile 64L + e - r0; t < 0 reads hist[ch][r0 + t], t >= n_t is zero-filled.
 template <int L, bool kInterior>
-__device__ __forceinline__ void issue_tile_input(const PushParams<L>& p, const Chunk& ck, const Geom& g, int ch, int tile, int buf, int lane)
+__device__ __forceinline__ void issue_tile_input(const PushParams<L>& p, const Chunk& ck, const Geom& g, int ch, int tile, int buf, int lane,
+                                                 const TimeOrder<L>& to)
 {
     const int t0 = tile * Geo<L>::tile - g.r0;
     const int n_t = ck.n_t;
@@ -266,7 +294,7 @@ __device__ __forceinline__ void issue_tile_input(const PushParams<L>& p, const C
 #pragma unroll
         for (int m = 0; m < Geo<L>::chunks; ++m) {
             const int c = 32 * m + lane;
-            cp_async16(buf + 4 * c + 4 * (c / Geo<L>::chunks), srct + 128 * m, 16);
+            cp_async16(buf + to.at(m), srct + 128 * m, 16);
         }
     } else if (s == 0 && ((g.r0 | n_t) & 3) == 0) {                  // aligned rows, whole chunks only
         // chunk c = 32 m + lane exists if lo <= c < hi (before it: history; behind it: zero fill,
@@ -279,7 +307,7 @@ __device__ __forceinline__ void issue_tile_input(const PushParams<L>& p, const C
                 const int c = 32 * m + lane;
                 const int t = t0 + 4 * c;
                 const bool ok = t < n_t;
-                if (t >= 0) cp_async16(buf + 4 * c + 4 * (c / Geo<L>::chunks), ok ? src + t : src, ok ? 16 : 0);
+                if (t >= 0) cp_async16(buf + to.at(m), ok ? src + t : src, ok ? 16 : 0);
             }
         } else {
             const int lo = (-t0 >> 2) - lane, hi = ((n_t - t0) >> 2) - lane;
@@ -288,7 +316,7 @@ __device__ __forceinline__ void issue_tile_input(const PushParams<L>& p, const C
             for (int m = 0; m < Geo<L>::chunks; ++m) {
                 const int c = 32 * m + lane;
                 if (m > 0 || lo <= 0)
-                    cp_async16(buf + 4 * c + 4 * (c / Geo<L>::chunks), srct + 128 * m, 32 * m < hi ? 16 : 0);
+                    cp_async16(buf + to.at(m), srct + 128 * m, 32 * m < hi ? 16 : 0);
             }
         }
     } else {
@@ -334,7 +362,7 @@ __device__ __forceinline__ void issue_tile_carry(const PushParams<L>& p, const G
 // map to t < 0 (recomputed history) or t >= n_t (padding) are dropped.
 template <int L, bool kInterior>
 __device__ __forceinline__ void store_tile(const Chunk& ck, const Geom& g, float* __restrict__ dst, int buf,
-                                           int lane, int t0, int s)
+                                           int lane, int t0, int s, const TimeOrder<L>& to)
 {
     const int n_t = ck.n_t;
     if (kInterior && s == 0 && t0 >= 0 && t0 + Geo<L>::tile <= n_t) {
@@ -342,7 +370,7 @@ __device__ __forceinline__ void store_tile(const Chunk& ck, const Geom& g, float
 #pragma unroll
         for (int m = 0; m < Geo<L>::chunks; ++m) {
             const int c = 32 * m + lane;
-            const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + 4 * c + 4 * (c / Geo<L>::chunks)]);
+            const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + to.at(m)]);
             st_stream4(dstt + 128 * m, v);
         }
     } else if (s == 0 && ((g.r0 | n_t) & 3) == 0) {                  // aligned rows, whole chunks only
@@ -351,7 +379,7 @@ __device__ __forceinline__ void store_tile(const Chunk& ck, const Geom& g, float
 #pragma unroll
             for (int m = 0; m < Geo<L>::chunks; ++m) {
                 const int c = 32 * m + lane;
-                const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + 4 * c + 4 * (c / Geo<L>::chunks)]);
+                const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + to.at(m)]);
                 if ((unsigned)(t0 + 4 * c) < (unsigned)n_t) st_stream4(dstt + 4 * c, v);
             }
         } else {
@@ -360,7 +388,7 @@ __device__ __forceinline__ void store_tile(const Chunk& ck, const Geom& g, float
 #pragma unroll
             for (int m = 0; m < Geo<L>::chunks; ++m) {
                 const int c = 32 * m + lane;
-                const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + 4 * c + 4 * (c / Geo<L>::chunks)]);
+                const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + to.at(m)]);
                 if ((m > 0 || lo <= 0) && 32 * m < hi) st_stream4(dstt + 128 * m, v);
             }
         }
@@ -627,7 +655,7 @@ template <int L, bool kInterior, bool kAllKinds, bool kTM>
 __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk& ck, const Geom& g, int buf, int wst, float2 (&x)[L],
                                              int ch, int tile, int lane, unsigned long long seen,
                                              bool item_end, unsigned rel_val, int cg, int bufoff,
-                                             TmPrefetch<L>* pf = nullptr)
+                                             const TimeOrder<L>& to, TmPrefetch<L>* pf = nullptr)
 {
     const bool last = tile == g.n_tiles - 1;
     const int t0 = tile * Geo<L>::tile - g.r0;
@@ -708,7 +736,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
             const int sf = row_shift(row, g.r0);
             regs_to_buf<L>(x, buf, lane, sf);
             __syncwarp();
-            store_tile<L, kInterior>(ck, g, row, buf, lane, t0, sf);
+            store_tile<L, kInterior>(ck, g, row, buf, lane, t0, sf, to);
             __syncwarp();
         }
     }
@@ -795,7 +823,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
             regs_to_buf<L>(x, buf, lane, sc);
             __syncwarp();
             if (item_end && lane == 0) st_release(p.progress + ch, rel_val);
-            store_tile<L, kInterior>(ck, g, row, buf, lane, t0, sc);
+            store_tile<L, kInterior>(ck, g, row, buf, lane, t0, sc, to);
         }
     } else if (item_end) {
         __syncwarp();
@@ -855,6 +883,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     const int wbase = warp * warp_stride<L, kTM>();                   // two tile buffers, two state copies, history scratch
     const int wst0 = wbase + 2 * Geo<L>::buf_floats;
     const int whs = wst0 + 2 * kStateSmem;                            // history scratch
+    const TimeOrder<L> to(lane);
     const int gw = kTM ? (int)(blockIdx.x * kTmChannels + warp)       // (time-major: the channel of the first item)
                        : CTAS == 1 ? (int)(blockIdx.x + gridDim.x * warp) : (int)(blockIdx.x * W + warp);   // warp index in the grid
     __shared__ unsigned sh_ctl[32];
@@ -967,8 +996,11 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     // is never waited for except at the very start; every claimer ends with two claims beyond the
     // last item.  Holding an item while working on a lower one does not change the argument above.
     unsigned pend = 0;
+    // (inline PTX on purpose: with the atomicAdd intrinsic here ptxas stops treating the loops around it
+    // as warp-uniform in some instantiations and reads every table with per-lane loads, -30 %)
     auto claim_issue = [&]() {
-        if (kTM ? threadIdx.x == 0 : lane == 0) pend = atomicAdd(&cc->work[ring], 1u);
+        if (kTM ? threadIdx.x == 0 : lane == 0)
+            asm volatile("atom.global.add.u32 %0, [%1], 1;" : "=r"(pend) : "l"(&cc->work[ring]) : "memory");
     };
     // (time-major: thread 0 publishes `pend` in sh_item before a CTA barrier, claim_take runs after it)
     // gt / gtend: first tile of the item and the tile behind its last, as tiles of the launch
@@ -1017,7 +1049,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         k = chunk_of(gt);
         const Geom g = geom_of(k);
         if (kTM) issue_tile_input_tm<L>(p, p.ck[k], g, cg, gt - sh_tile0[k], 0);
-        else issue_tile_input<L, CTAS == 1>(p, p.ck[k], g, ch, gt - sh_tile0[k], wbase, lane);
+        else issue_tile_input<L, CTAS == 1>(p, p.ck[k], g, ch, gt - sh_tile0[k], wbase, lane, to);
         // the first segment of a channel needs what the previous launch left (state, hist): wait before
         // those loads are issued (a wait on an EARLIER launch cannot be part of a cycle)
         if (seg == 0 && ch < p.n_ch) {
@@ -1118,7 +1150,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         __syncwarp();
         if (nhave) {
             const int nbuf = wbase + (cur ^ 1) * Geo<L>::buf_floats;
-            if (!kTM) issue_tile_input<L, CTAS == 1>(p, p.ck[nk], geom_of(nk), nch, ngt - sh_tile0[nk], nbuf, lane);
+            if (!kTM) issue_tile_input<L, CTAS == 1>(p, p.ck[nk], geom_of(nk), nch, ngt - sh_tile0[nk], nbuf, lane, to);
             if (item_end && nseg == 0 && nch < p.n_ch) {
                 wait_progress(nch, seq0, npr);
                 issue_tile_carry<L>(p, geom_of(nk), nch, whs, wst0 + (wcur ^ 1) * kStateSmem, lane);
@@ -1130,11 +1162,11 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
             // (time-major: the next tile is requested in portions while this one is computed)
             TmPrefetch<L> pf(p, p.ck[nk], geom_of(nk), ncg, ngt - sh_tile0[nk], (cur ^ 1) * Geo<L>::buf_floats);
             process_tile<L, true, kAllKinds, true>(p, ck, g, buf, wst, x, ch, tile, lane, seen + ck.t_cum, item_end && valid,
-                                                   seq0 + (unsigned)seg + 1u, cg, cur * Geo<L>::buf_floats,
+                                                   seq0 + (unsigned)seg + 1u, cg, cur * Geo<L>::buf_floats, to,
                                                    nhave ? &pf : nullptr);
         } else {
             process_tile<L, CTAS == 1, kAllKinds, false>(p, ck, g, buf, wst, x, ch, tile, lane, seen + ck.t_cum, item_end && valid,
-                                                         seq0 + (unsigned)seg + 1u, cg, cur * Geo<L>::buf_floats);
+                                                         seq0 + (unsigned)seg + 1u, cg, cur * Geo<L>::buf_floats, to);
         }
         if (item_end) wcur ^= 1;
         ch = nch; gt = ngt; gtend = ngtend; seg = nseg; cg = ncg; have = nhave; k = nk; cur ^= 1;
