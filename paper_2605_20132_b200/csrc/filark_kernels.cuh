@@ -297,27 +297,18 @@ __device__ __forceinline__ void issue_tile_input(const PushParams<L>& p, const C
             cp_async16(buf + to.at(m), srct + 128 * m, 16);
         }
     } else if (s == 0 && ((g.r0 | n_t) & 3) == 0) {                  // aligned rows, whole chunks only
-        // chunk c = 32 m + lane exists if lo <= c < hi (before it: history; behind it: zero fill,
-        // src-size 0).  The bounds are taken relative to the lane once, so that every chunk costs a
-        // compare against a constant, a select and the copy -- this path runs for every tile of an
-        // ordinary push.  (r0 < 128: only the first 32 chunks can hold history.)
-        if (kInterior) {                  // (long-push kernel: rarely here, and its code is left as it was tuned)
+        // chunk c = 32 m + lane exists if lo <= c < hi (before it: history; behind it: nothing).  Every
+        // chunk is copied, the ones that do not exist with src-size 0 (zero fill, nothing is read): what
+        // waits in the history is put over the zeros when the tile is taken up.  The bounds are taken
+        // relative to the lane once, so that a chunk costs a compare against a constant, a select and the
+        // copy, and there is no lane-dependent branch -- this path runs for every tile of an ordinary push.
+        // (r0 < 128: only the first 32 chunks can hold history.)
+        const int lo = (-t0 >> 2) - lane, hi = ((n_t - t0) >> 2) - lane;
+        const float* __restrict__ srct = src + t0 + 4 * lane;
 #pragma unroll
-            for (int m = 0; m < Geo<L>::chunks; ++m) {
-                const int c = 32 * m + lane;
-                const int t = t0 + 4 * c;
-                const bool ok = t < n_t;
-                if (t >= 0) cp_async16(buf + to.at(m), ok ? src + t : src, ok ? 16 : 0);
-            }
-        } else {
-            const int lo = (-t0 >> 2) - lane, hi = ((n_t - t0) >> 2) - lane;
-            const float* __restrict__ srct = src + t0 + 4 * lane;
-#pragma unroll
-            for (int m = 0; m < Geo<L>::chunks; ++m) {
-                const int c = 32 * m + lane;
-                if (m > 0 || lo <= 0)
-                    cp_async16(buf + to.at(m), srct + 128 * m, 32 * m < hi ? 16 : 0);
-            }
+        for (int m = 0; m < Geo<L>::chunks; ++m) {
+            const bool ok = m == 0 ? (lo <= 0 && 0 < hi) : 32 * m < hi;
+            cp_async16(buf + to.at(m), srct + 128 * m, ok ? 16 : 0);
         }
     } else {
         // raw chunk c holds input samples tf .. tf + 3; samples before the row (t < 0) are history
@@ -374,23 +365,13 @@ __device__ __forceinline__ void store_tile(const Chunk& ck, const Geom& g, float
             st_stream4(dstt + 128 * m, v);
         }
     } else if (s == 0 && ((g.r0 | n_t) & 3) == 0) {                  // aligned rows, whole chunks only
-        if (kInterior) {
-            float* __restrict__ dstt = dst + t0;
+        const int lo = (-t0 >> 2) - lane, hi = ((n_t - t0) >> 2) - lane;       // as in issue_tile_input
+        float* __restrict__ dstt = dst + t0 + 4 * lane;
 #pragma unroll
-            for (int m = 0; m < Geo<L>::chunks; ++m) {
-                const int c = 32 * m + lane;
-                const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + to.at(m)]);
-                if ((unsigned)(t0 + 4 * c) < (unsigned)n_t) st_stream4(dstt + 4 * c, v);
-            }
-        } else {
-            const int lo = (-t0 >> 2) - lane, hi = ((n_t - t0) >> 2) - lane;       // as in issue_tile_input
-            float* __restrict__ dstt = dst + t0 + 4 * lane;
-#pragma unroll
-            for (int m = 0; m < Geo<L>::chunks; ++m) {
-                const int c = 32 * m + lane;
-                const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + to.at(m)]);
-                if ((m > 0 || lo <= 0) && 32 * m < hi) st_stream4(dstt + 128 * m, v);
-            }
+        for (int m = 0; m < Geo<L>::chunks; ++m) {
+            const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + to.at(m)]);
+            const bool ok = m == 0 ? (lo <= 0 && 0 < hi) : 32 * m < hi;
+            if (ok) st_stream4(dstt + 128 * m, v);
         }
     } else {
         // element j of raw chunk c is tile position e = 4 c + j - s: only 0 <= e < tile belongs to
