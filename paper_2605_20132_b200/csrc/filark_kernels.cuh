@@ -227,6 +227,20 @@ __device__ __forceinline__ void cp_async4(int dst_off, const float* src, int src
     asm volatile("cp.async.ca.shared.global [%0], [%1], 4, %2;" ::"r"(s), "l"(src), "r"(src_bytes) : "memory");
 }
 
+// Shared-space accesses by 32-bit address (the carried state of a section is read and written once per
+// section: through `fk_smem[...]` the compiler rebuilds the generic-to-shared window address every time)
+__device__ __forceinline__ unsigned smem_addr(int float_off) { return (unsigned)__cvta_generic_to_shared(&fk_smem[float_off]); }
+__device__ __forceinline__ float2 lds_f2(unsigned sa)
+{
+    float2 v;
+    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "r"(sa) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_f2(unsigned sa, float2 v)
+{
+    asm volatile("st.shared.v2.f32 [%0], {%1, %2};" ::"r"(sa), "f"(v.x), "f"(v.y) : "memory");
+}
+
 // Shared memory of one warp: two tile buffers (input of tile k / staging of its outputs, and the
 // prefetched input of tile k+1) and two copies of the channel state.
 constexpr int kStateSmem = 40;                     // >= state_floats(kMaxSec), multiple of 4
@@ -646,6 +660,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
     const int jl = keep ? 0 : (q - 1) >> 1;
     const bool out_hi = ((q - 1) & 1) != 0;
 
+    const unsigned wst_sa = smem_addr(wst);
     // ---- S1..S3 per section -------------------------------------------------------------------
     const int pf_part = kTM ? (Geo<L>::tile / 32 + p.n_sec - 1) / p.n_sec : 0;
     for (int k = 0; k < p.n_sec; ++k) {
@@ -668,7 +683,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
         }
         // S2: lane total W = P a + b (a, b: end states of the lo / hi slot from rest); the carried
         // state S enters lane 0's total through A^2L; inclusive scan over the lanes
-        const float2 S = *reinterpret_cast<const float2*>(&fk_smem[wst + 2 * k]);
+        const float2 S = lds_f2(wst_sa + 8u * (unsigned)k);
         const float P0 = T.P[0], P1 = T.P[1], P2 = T.P[2], P3 = T.P[3];
         float W1 = fmaf(P0, s1.x, fmaf(P1, s2.x, s1.y)), W2 = fmaf(P2, s1.x, fmaf(P3, s2.x, s2.y));
         {
@@ -693,7 +708,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
         const float o1 = fmaf(P0, E1, fmaf(P1, E2, s1.x)), o2 = fmaf(P2, E1, fmaf(P3, E2, s2.x));   // ... its hi slot
         const float n1 = __shfl_sync(0xffffffffu, out_hi ? W1 : o1, jl);
         const float n2 = __shfl_sync(0xffffffffu, out_hi ? W2 : o2, jl);
-        if (lane == 0 && !keep) *reinterpret_cast<float2*>(&fk_smem[wst + 2 * k]) = make_float2(n1, n2);
+        if (lane == 0 && !keep) sts_f2(wst_sa + 8u * (unsigned)k, make_float2(n1, n2));
         // S3 fix-up: y[i] += g1[i] s1 + g2[i] s2
         const float2 Ea = make_float2(E1, o1), Eb = make_float2(E2, o2);
         // (two rows per 16-byte uniform load: the tables are 16-byte aligned in the parameter bank)
@@ -732,7 +747,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
         sp = fma2(as, sp, e); lp = fma2(al, lp, e);
     }
     const int ks = wst + 2 * p.n_sec;
-    const float2 M = *reinterpret_cast<const float2*>(&fk_smem[ks]);           // carried (sta~, lta~)
+    const float2 M = lds_f2(wst_sa + 8u * (unsigned)p.n_sec);                  // carried (sta~, lta~)
     const float bLs = p.avg.betaL[0], bLl = p.avg.betaL[1];
     float Ws = sp.y + fmaf(-bLs, sp.x, sp.x), Wl = lp.y + fmaf(-bLl, lp.x, lp.x);        // alpha^L lo + hi
     {
@@ -750,7 +765,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
     const float Os = sp.x + fmaf(-bLs, Es, Es), Ol = lp.x + fmaf(-bLl, El, El);          // carry-in of the hi slot
     const float Ns = __shfl_sync(0xffffffffu, out_hi ? Ws : Os, jl);
     const float Nl = __shfl_sync(0xffffffffu, out_hi ? Wl : Ol, jl);
-    if (lane == 0 && !keep) *reinterpret_cast<float2*>(&fk_smem[ks]) = make_float2(Ns, Nl);
+    if (lane == 0 && !keep) sts_f2(wst_sa + 8u * (unsigned)p.n_sec, make_float2(Ns, Nl));
 
     // Last tile of a work item: the carried state is final here.  It goes back to global memory
     // now, and `progress` is released after the ratio loop below: the fence of the release waits for
