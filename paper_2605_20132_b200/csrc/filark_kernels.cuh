@@ -693,15 +693,20 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
             W2 = fmaf(T.Q[0][2], S1, fmaf(T.Q[0][3], S2, W2));
         }
         const int nsteps = T.nsteps;
+        auto scan_step = [&](int d) {
+            const float U1 = __shfl_up_sync(0xffffffffu, W1, 1 << d), U2 = __shfl_up_sync(0xffffffffu, W2, 1 << d);
+            // (predicated updates instead of zeroed operands: two selects fewer per step)
+            const float N1 = fmaf(T.Q[d][0], U1, fmaf(T.Q[d][1], U2, W1));
+            const float N2 = fmaf(T.Q[d][2], U1, fmaf(T.Q[d][3], U2, W2));
+            if (lane >= (1 << d)) { W1 = N1; W2 = N2; }
+        };
+        if (nsteps == kSteps) {                      // poles next to the unit circle: all steps, no tests
 #pragma unroll
-        for (int d = 0; d < kSteps; ++d) {
-            if (d < nsteps) {
-                const float U1 = __shfl_up_sync(0xffffffffu, W1, 1 << d), U2 = __shfl_up_sync(0xffffffffu, W2, 1 << d);
-                // (predicated updates instead of zeroed operands: two selects fewer per step)
-                const float N1 = fmaf(T.Q[d][0], U1, fmaf(T.Q[d][1], U2, W1));
-                const float N2 = fmaf(T.Q[d][2], U1, fmaf(T.Q[d][3], U2, W2));
-                if (lane >= (1 << d)) { W1 = N1; W2 = N2; }
-            }
+            for (int d = 0; d < kSteps; ++d) scan_step(d);
+        } else {
+#pragma unroll
+            for (int d = 0; d < kSteps - 1; ++d)
+                if (d < nsteps) scan_step(d);
         }
         float E1 = __shfl_up_sync(0xffffffffu, W1, 1), E2 = __shfl_up_sync(0xffffffffu, W2, 1);
         if (lane == 0) { E1 = S.x; E2 = S.y; }                      // state entering the lane's lo slot
@@ -794,8 +799,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
             for (int i = 0; i < L; ++i) {
                 Ps = fma2(as, Ps, x[i]); Pl = fma2(al, Pl, x[i]);
                 const float2 num = mul2(Ps, f2(ratio));
-                x[i].x = num.x * rcp_fast(Pl.x);
-                x[i].y = num.y * rcp_fast(Pl.y);
+                x[i] = mul2(num, make_float2(rcp_fast(Pl.x), rcp_fast(Pl.y)));
             }
         } else {
             const int wm = rem > (1 << 30) ? (1 << 30) : (rem < 0 ? 0 : (int)rem);
