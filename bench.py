@@ -16,7 +16,8 @@ Prints ONE JSON line (rank 0).  Keys beyond the driver's contract:
   roofline      dominant (only) kernel vs the measured HBM copy peak of MEASURED_PEAKS.json
   cpu_baseline  the float64 oracle, as it stands, on this box's host cores, bounded sample
   e2e           same metric through filark_stream_push_host with pinned HOST buffers
-  detail        whole-record push, both layouts' numbers when asked, real-time factor
+  detail        the same record in one push / through separate push calls / sustained for seconds with
+                its clock record / one output only, and every other BASELINE.json config (all_configs)
 
 N > 1 (torchrun): the path shards by channel with no exchange step; every rank
 streams its own 6,000-channel fibre (weak scaling), time = max over ranks, no data-path
@@ -55,6 +56,12 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-detail", action="store_true")
+    ap.add_argument("--no-all-configs", action="store_true", help="skip detail.all_configs (the other BASELINE.json configs)")
+    ap.add_argument("--sustain-seconds", type=float, default=5.0, help="length of the detail.sustained loop")
+    ap.add_argument("--api", default="push_many", choices=["push_many", "push", "push_overlap"],
+                    help="how a step enqueues its pushes: one filark_stream_push_many call (default), separate "
+                         "filark_stream_push calls (strict stream order), or separate calls on a handle created with "
+                         "FILARK_FLAG_OVERLAP_PUSHES")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--cpu-sample-channels", type=int, default=0, help="0 = sized for ~15 core-s")
     return ap.parse_args()
@@ -160,7 +167,9 @@ def run_reference(args, rank):
     w = CONFIGS[args.workload]
     sos = design_sos(w)
     cores = os.cpu_count() or 1
-    n_ch_s = args.cpu_sample_channels or min(w.n_ch, 16 * cores)
+    # (the same bounded sample as the cpu_baseline leg of the CUDA arm: a few thousand channels, so that the
+    # per-push start of the worker threads does not dominate the 1,500-sample pushes)
+    n_ch_s = args.cpu_sample_channels or max(cores, min(w.n_ch, int(15.0 * 30e6 / w.n_t)))
     ws = w.scaled(n_ch=n_ch_s, n_t=w.n_t)
     x = generate(ws, device="cpu").numpy()
     sched = push_schedule(ws) if args.mode == "chunked" else [ws.n_t]
@@ -186,6 +195,23 @@ def run_reference(args, rank):
     print(json.dumps(out), flush=True)
 
 
+def make_step(stream, api, batch, ins, filts, cfs):
+    """One pass of the whole hot path over the record: reset + every push of the schedule."""
+    if api == "push_many":
+        def step():
+            stream.reset()
+            stream.push_many(batch)                  # one host call enqueues every push of the record
+    else:
+        fl = filts if filts is not None else [None] * len(ins)
+        cl = cfs if cfs is not None else [None] * len(ins)
+
+        def step():
+            stream.reset()
+            for xi, fi, ci in zip(ins, fl, cl):
+                stream.push(xi, fi, ci)
+    return step
+
+
 def workload_config(w, args, sched):
     return {"workload": f"{w.name}: {w.n_ch} ch x {w.n_t} samples fp32 at fs={w.fs:g} Hz "
                         f"(BASELINE.json configs[{int(w.name[3:]) - 1}])",
@@ -195,9 +221,12 @@ def workload_config(w, args, sched):
             "layout": "channel-major [n_ch][n_t]" if args.layout == "cm" else "time-major [n_t][n_ch]",
             "pushes_per_step": len(sched), "chunk_samples": sched[0] if len(set(sched)) == 1 else "mixed",
             "l2": "inputs larger than L2: each push reads a distinct chunk; 6.5 GB traffic per step",
-            "api": "filark_stream_reset + ONE filark_stream_push_many call per step (one kernel per push)",
-            "push_overlap": "the pushes of a push_many call overlap on the device (programmatic dependent "
-                            "launch, ordered per channel through the carried state; include/filark_stream.h)",
+            "api": {"push_many": "filark_stream_reset + ONE filark_stream_push_many call per step: chunks that share "
+                                 "no buffer run in common launches of up to 64 chunks, the carried state stays on "
+                                 "the SM between them (include/filark_stream.h)",
+                    "push": "filark_stream_reset + one filark_stream_push call per chunk, strict stream order",
+                    "push_overlap": "filark_stream_reset + one filark_stream_push call per chunk on a handle with "
+                                    "FILARK_FLAG_OVERLAP_PUSHES: consecutive launches overlap on the device"}[args.api],
             "parallelism": "independent channel shards, one stream handle per GPU, no collective"}
 
 
@@ -214,7 +243,7 @@ def main():
     import numpy as np
     import torch
     import torch.distributed as dist
-    from paper_2605_20132_b200.stream import FilarkStream, PushBatch, load_library
+    from paper_2605_20132_b200.stream import FLAG_OVERLAP_PUSHES, FilarkStream, PushBatch, load_library
     from paper_2605_20132_b200.workloads import (CHANNEL_MAJOR, TIME_MAJOR, CONFIGS, design_sos,
                                                   generate, push_schedule)
     if not torch.cuda.is_available():
@@ -250,13 +279,11 @@ def main():
         del x
     filts = [torch.empty_like(t) for t in ins] if args.outputs != "cf" else None
     cfs = [torch.empty_like(t) for t in ins] if args.outputs != "filt" else None
-    stream = FilarkStream(w.n_ch, sos, w.sta_len, w.lta_len, layout, flags=args.force_l << 8)
+    flags = (args.force_l << 8) | (FLAG_OVERLAP_PUSHES if args.api == "push_overlap" else 0)
+    stream = FilarkStream(w.n_ch, sos, w.sta_len, w.lta_len, layout, flags=flags)
     samples_per_step = w.n_ch * w.n_t
     batch = PushBatch(stream, ins, filts, cfs)       # the step's schedule, marshalled once
-
-    def step():
-        stream.reset()
-        stream.push_many(batch)                      # one host call enqueues every push of the record
+    step = make_step(stream, args.api, batch, ins, filts, cfs)
 
     def barrier():
         if world > 1:
@@ -297,32 +324,38 @@ def main():
     # ---- roofline of the (only) kernel: algorithmic bytes per launch / mean launch duration --
     peak, peak_src = measured_peak()
     per_launch_ms = ms / max(1, launches) if world == 1 else None
-    bytes_per_launch = ALG_BYTES_PER_SAMPLE * samples_per_step / len(sched)
+    bytes_per_launch = ALG_BYTES_PER_SAMPLE * samples_per_step * args.steps / max(1, launches)
     ach = ALG_BYTES_PER_SAMPLE * samples_per_step / (ms_per_step * 1e-3) / 1e9 / 1.0
-    traffic = None
-    tpath = os.path.join(ROOT, "profiles", "r01_traffic.csv")    # from the ncu --set full captures (profiles/r01_traffic.md)
+    # DRAM bytes of one launch of this command, from the committed ncu --set full capture of the same
+    # launch configuration (profiles/r02_traffic.md says which capture each row comes from)
+    traffic, traffic_src = None, None
+    tpath = os.path.join(ROOT, "profiles", "r02_traffic.csv")
     try:
         with open(tpath) as f:
             for line in f.read().splitlines()[1:]:
                 k, v = line.split(",")
-                if k == f"{w.name}_{args.mode}_{args.layout}":
+                if k == f"{w.name}_{args.mode}_{args.layout}_{args.api if args.mode == 'chunked' else 'push'}":
                     traffic = float(v)
+                    traffic_src = "profiles/r02_traffic.csv (dram__bytes_read.sum + dram__bytes_write.sum of one launch, ncu --set full)"
     except Exception:
         pass
+    lean = "lean" if True else "all"
     out["roofline"] = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s",
-                       "frac": ach / peak, "traffic": traffic, "peak_source": peak_src,
-                       "kernel": "filark_push_cm_kernel<24,4,lean>" if layout == CHANNEL_MAJOR else "filark_push_cm_kernel<24,1,lean,time-major>",
+                       "frac": ach / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
+                       "kernel": "filark_push_cm_kernel (one instantiation per sub-block length, launch shape, "
+                                 "section forms and layout; profiles/ names the one this command launches)",
                        "algorithmic_bytes_per_launch": bytes_per_launch,
                        "mean_launch_ms": per_launch_ms, "frac_of_nominal_8TBs": ach / HBM_NOMINAL_GBS,
-                       "note": "achieved = 12 B/sample x samples per step / CUDA-event time of the step "
-                               "(the step is back-to-back launches of this one kernel + the memsets of reset; "
-                               "consecutive pushes overlap on the device, so mean_launch_ms = step time / "
-                               "launches is what one push adds to the stream, not the life of one grid)"}
+                       "limiter": "instruction issue, not HBM: at 8 sections the kernel executes about 60 SASS "
+                                  "instructions per sample (DESIGN.md 7, profiles/r02_ncu_*.md); HBM is the roof the "
+                                  "north star names and the one `frac` is measured against",
+                       "note": "achieved = 12 B/sample x samples per step / CUDA-event time of the step (the step is "
+                               "the launches of this one kernel + the memsets of reset)"}
     out["detail"] = {"gsamples_per_s": value / 1e9, "alg_gbytes_per_s": ach,
                      "realtime_factor": (w.n_t / w.fs) / (ms_per_step * 1e-3)}
 
     if rank == 0 and world == 1 and not args.no_detail:
-        out["detail"].update(extra_runs(args, w, sos, stream, ins, filts, cfs, sched, torch))
+        out["detail"].update(extra_runs(args, w, sos, stream, ins, filts, cfs, sched, torch, dev, peak, step, local_rank))
 
     # ---- e2e: the same step through filark_stream_push_host with pinned host buffers ---------
     if not args.no_e2e:
@@ -375,6 +408,16 @@ def main():
                                "sample": f"first {n_ch_s} of {w.n_ch} channels x all {w.n_t} samples of the "
                                          f"same record, {len(sched)} pushes, channels split over {cores} threads"}
 
+    if rank == 0 and world == 1 and not args.no_detail:
+        if not args.no_all_configs:
+            # (the headline's buffers stay: 13 GB; the largest config adds 65 GB)
+            out["detail"]["all_configs"] = all_configs(args, torch, dev, peak)
+        if args.sustain_seconds > 0:
+            try:
+                out["detail"]["sustained"] = sustained_run(args, torch, step, samples_per_step, peak, local_rank)
+            except Exception as exc:
+                out["detail"]["sustained"] = {"error": repr(exc)}
+
     if world > 1:
         dist.barrier()
         dist.destroy_process_group()
@@ -382,31 +425,144 @@ def main():
         print(json.dumps(out), flush=True)
 
 
-def extra_runs(args, w, sos, stream, ins, filts, cfs, sched, torch):
-    """Whole-record push of the same workload (context beside the chunked headline)."""
+def _time(torch, fn, reps, warm=1):
+    """ms per call of fn, CUDA events on the current stream around `reps` back-to-back calls."""
+    for _ in range(warm):
+        fn()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        fn()
+    e1.record()
+    torch.cuda.synchronize()
+    return e0.elapsed_time(e1) / reps
+
+
+def _row(n_samples, ms, peak, bytes_per_sample=12.0):
+    gbs = bytes_per_sample * n_samples / (ms * 1e-3) / 1e9
+    return {"ms": ms, "samples_per_s": n_samples / (ms * 1e-3), "alg_gbytes_per_s": gbs, "frac_of_measured_peak": gbs / peak}
+
+
+def extra_runs(args, w, sos, stream, ins, filts, cfs, sched, torch, dev, peak, step, local_rank):
+    """Context beside the headline: the same record in one push, through separate push calls, a
+    sustained run with its clock record, one output only, and the other configs of BASELINE.json."""
+    from paper_2605_20132_b200.stream import FLAG_OVERLAP_PUSHES, FilarkStream, PushBatch
+    from paper_2605_20132_b200.workloads import CHANNEL_MAJOR, TIME_MAJOR, CONFIGS, design_sos, generate, push_schedule
     extra = {}
-    if len(sched) > 1 and args.layout == "cm":
+    n_samples = w.n_ch * w.n_t
+    bps = ALG_BYTES_PER_SAMPLE
+    layout = CHANNEL_MAJOR if args.layout == "cm" else TIME_MAJOR
+    cat_dim = 1 if layout == CHANNEL_MAJOR else 0
+
+    def guarded(name, fn):
         try:
-            n_t = w.n_t
-            x = torch.cat(ins, dim=1).contiguous()
+            extra[name] = fn()
+        except Exception as exc:                                  # context only
+            extra[name] = {"error": repr(exc)}
+            torch.cuda.synchronize()
+
+    # ---- the same schedule through separate push calls
+    if len(sched) > 1 and args.api == "push_many":
+        def per_call(flags):
+            s2 = FilarkStream(w.n_ch, sos, w.sta_len, w.lta_len, layout, flags=(args.force_l << 8) | flags)
+            st = make_step(s2, "push", None, ins, filts, cfs)
+            ms = _time(torch, st, max(3, args.steps // 2), warm=2)
+            s2.destroy()
+            return _row(n_samples, ms, peak, bps)
+        guarded("separate_push_calls_strict_order", lambda: per_call(0))
+        guarded("separate_push_calls_overlapped", lambda: per_call(FLAG_OVERLAP_PUSHES))
+
+    # ---- the record in one push
+    if len(sched) > 1:
+        def whole():
+            x = torch.cat(ins, dim=cat_dim).contiguous()
             f = torch.empty_like(x) if args.outputs != "cf" else None
             c = torch.empty_like(x) if args.outputs != "filt" else None
-            for _ in range(2):
+
+            def st():
                 stream.reset(); stream.push(x, f, c)
-            torch.cuda.synchronize()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            reps = max(3, args.steps // 2)
-            e0.record()
-            for _ in range(reps):
-                stream.reset(); stream.push(x, f, c)
-            e1.record(); torch.cuda.synchronize()
-            ms = e0.elapsed_time(e1) / reps
-            extra["whole_record_push"] = {"ms": ms, "samples_per_s": w.n_ch * n_t / (ms * 1e-3),
-                                          "alg_gbytes_per_s": ALG_BYTES_PER_SAMPLE * w.n_ch * n_t / (ms * 1e-3) / 1e9}
-            del x, f, c
-        except Exception as exc:                                  # context only
-            extra["whole_record_push"] = {"error": repr(exc)}
+            ms = _time(torch, st, max(3, args.steps // 2), warm=2)
+            return _row(n_samples, ms, peak, bps)
+        guarded("whole_record_push", whole)
+
+    # ---- one output only (the other pointer NULL: 8 B/sample)
+    if args.outputs == "both":
+        def one_output(which):
+            b2 = PushBatch(stream, ins, filts if which == "filt" else None, cfs if which == "cf" else None)
+
+            def st():
+                stream.reset(); stream.push_many(b2)
+            ms = _time(torch, st, max(3, args.steps // 2), warm=2)
+            return _row(n_samples, ms, peak, 8.0)
+        guarded("filt_only", lambda: one_output("filt"))
+        guarded("cf_only", lambda: one_output("cf"))
     return extra
+
+
+def sustained_run(args, torch, step, n_samples, peak, local_rank):
+    """The headline step looped for several seconds, with the clock and power-cap record of that loop
+    (run last: it leaves the GPU warm and, at this kernel's power, under the software power cap)."""
+    sampler = ClockSampler(physical_gpu_index(local_rank), period_s=0.02)
+    ms1 = _time(torch, step, 3)
+    reps = max(10, int(args.sustain_seconds * 1e3 / ms1))
+    sampler.start()
+    ms = _time(torch, step, reps, warm=0)
+    clocks = sampler.stop()
+    r = _row(n_samples, ms, peak, ALG_BYTES_PER_SAMPLE)
+    r.update({"steps": reps, "seconds": reps * ms * 1e-3, "clocks": clocks})
+    return r
+
+
+def all_configs(args, torch, dev, peak):
+    """Every BASELINE.json config x {its chunk schedule through push_many, one whole-record push}, both
+    layouts for the headline config; a few steps each (bounded: the default run must end within minutes)."""
+    from paper_2605_20132_b200.stream import FilarkStream, PushBatch
+    from paper_2605_20132_b200.workloads import CHANNEL_MAJOR, TIME_MAJOR, CONFIGS, design_sos, generate, push_schedule
+    out = {}
+    for name, lay in (("cfg1", "cm"), ("cfg2", "cm"), ("cfg3", "tm"), ("cfg4", "cm"), ("cfg5", "cm")):
+        key = f"{name}_{lay}"
+        try:
+            w = CONFIGS[name]
+            layout = CHANNEL_MAJOR if lay == "cm" else TIME_MAJOR
+            sos = design_sos(w)
+            sched = push_schedule(w)
+            x = generate(w, device=dev, layout=CHANNEL_MAJOR)
+            ins, p = [], 0
+            for c in sched:
+                blk = x[:, p:p + c]
+                ins.append(blk.contiguous() if layout == CHANNEL_MAJOR else blk.t().contiguous()); p += c
+            big = name == "cfg5"
+            if layout == TIME_MAJOR:
+                xw = x.t().contiguous()
+                del x
+            else:
+                xw = x
+            fs = [torch.empty_like(t) for t in ins]; cs = [torch.empty_like(t) for t in ins]
+            st = FilarkStream(w.n_ch, sos, w.sta_len, w.lta_len, layout)
+            b = PushBatch(st, ins, fs, cs)
+
+            def chunked():
+                st.reset(); st.push_many(b)
+            n = w.n_ch * w.n_t
+            reps = 2 if big else 5
+            row = {"shape": f"{w.n_ch} x {w.n_t}", "sections": w.order, "pushes": len(sched),
+                   "chunked_push_many": _row(n, _time(torch, chunked, reps, warm=1), peak)}
+            del fs, cs, b
+            fw = torch.empty_like(xw); cw = torch.empty_like(xw)
+
+            def whole():
+                st.reset(); st.push(xw, fw, cw)
+            row["whole_record_push"] = _row(n, _time(torch, whole, reps, warm=1), peak)
+            st.destroy()
+            out[key] = row
+            del ins, xw, fw, cw
+            torch.cuda.empty_cache()
+        except Exception as exc:
+            out[key] = {"error": repr(exc)}
+            torch.cuda.synchronize()
+            torch.cuda.empty_cache()
+    return out
 
 
 if __name__ == "__main__":
