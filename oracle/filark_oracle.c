@@ -208,3 +208,71 @@ int filark_oracle_trace_f64(filark_oracle_t *o, int c, const double *x, long lon
     o->sta[c] = sta; o->lta[c] = lta;
     return 0;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Additions for the NEXT rows of SURVEY.md 8(f) (nothing above this line was changed).
+ * ------------------------------------------------------------------------------------------ */
+
+/*
+ * Steady-state initial condition ("a short transient determined
+ * by the filter order and the initial condition"): the state every channel would have if its
+ * input had been the constant x0[c] for ever.  For one transposed-direct-form-II section with
+ * constant input v the output is y = v (b0+b1+b2)/(1+a1+a2) and the state follows from the two
+ * update statements of the push loop read as fixed-point equations:
+ *     z2 = b2 v - a2 y,      z1 = b1 v - a1 y + z2.
+ * The averages start at the steady energy y_last^2, and the warm-up counter at lta_len (the
+ * averages ARE warmed up).  This is scipy's `sosfilt_zi(sos) * x0` idiom, which pins it.
+ */
+int filark_oracle_set_initial_condition(filark_oracle_t *o, const double *x0)
+{
+    if (!o || !x0) return 1;
+    for (int c = 0; c < o->n_ch; ++c) {
+        double v = x0[c];
+        double *z = o->z + (size_t)c * (size_t)o->n_sec * 2;
+        for (int k = 0; k < o->n_sec; ++k) {
+            const double *q = o->coef + 5 * k;     /* b0 b1 b2 a1 a2 */
+            const double y = v * (q[0] + q[1] + q[2]) / (1.0 + q[3] + q[4]);
+            z[2 * k + 1] = q[2] * v - q[4] * y;
+            z[2 * k]     = q[1] * v - q[3] * y + z[2 * k + 1];
+            v = y;
+        }
+        o->sta[c] = v * v;
+        o->lta[c] = v * v;
+    }
+    o->g = o->lta_len;
+    return 0;
+}
+
+/*
+ * State export / import (NEXT-2; PAPER.md:109 "maintaining correct state propagation", :169 state
+ * crosses file boundaries -- here: process boundaries).  out / in: n_ch * (2 n_sec + 2) doubles,
+ * per channel z1,z2 of every section, then sta, lta; *g the samples seen.
+ */
+long long filark_oracle_state_doubles(const filark_oracle_t *o)
+{
+    return o ? (long long)o->n_ch * (2LL * o->n_sec + 2) : -1;
+}
+int filark_oracle_get_state(const filark_oracle_t *o, double *out, long long *g)
+{
+    if (!o || !out || !g) return 1;
+    const int w = 2 * o->n_sec + 2;
+    for (int c = 0; c < o->n_ch; ++c) {
+        memcpy(out + (size_t)c * w, o->z + (size_t)c * 2 * o->n_sec, sizeof(double) * 2 * (size_t)o->n_sec);
+        out[(size_t)c * w + 2 * o->n_sec] = o->sta[c];
+        out[(size_t)c * w + 2 * o->n_sec + 1] = o->lta[c];
+    }
+    *g = o->g;
+    return 0;
+}
+int filark_oracle_set_state(filark_oracle_t *o, const double *in, long long g)
+{
+    if (!o || !in || g < 0) return 1;
+    const int w = 2 * o->n_sec + 2;
+    for (int c = 0; c < o->n_ch; ++c) {
+        memcpy(o->z + (size_t)c * 2 * o->n_sec, in + (size_t)c * w, sizeof(double) * 2 * (size_t)o->n_sec);
+        o->sta[c] = in[(size_t)c * w + 2 * o->n_sec];
+        o->lta[c] = in[(size_t)c * w + 2 * o->n_sec + 1];
+    }
+    o->g = g;
+    return 0;
+}

@@ -64,6 +64,14 @@ def _load():
     lib.filark_oracle_push.argtypes = [vp, vp, ll, ll, ll, vp, vp]
     lib.filark_oracle_trace_f64.restype = ci
     lib.filark_oracle_trace_f64.argtypes = [vp, ci, vp, ll, vp, vp, vp]
+    lib.filark_oracle_set_initial_condition.restype = ci
+    lib.filark_oracle_set_initial_condition.argtypes = [vp, vp]
+    lib.filark_oracle_state_doubles.restype = ll
+    lib.filark_oracle_state_doubles.argtypes = [vp]
+    lib.filark_oracle_get_state.restype = ci
+    lib.filark_oracle_get_state.argtypes = [vp, vp, vp]
+    lib.filark_oracle_set_state.restype = ci
+    lib.filark_oracle_set_state.argtypes = [vp, vp, ll]
     _lib = lib
     return lib
 
@@ -133,6 +141,26 @@ class Oracle:
                     raise RuntimeError("oracle push failed")
         self._lib.filark_oracle_advance(self._h, n_t)
         return filt, cf
+
+    def set_initial_condition(self, x0):
+        """Steady state for a constant input level x0[c] per channel (NEXT-2)."""
+        x0 = np.ascontiguousarray(np.broadcast_to(np.asarray(x0, dtype=np.float64), (self.n_ch,)))
+        if self._lib.filark_oracle_set_initial_condition(self._h, x0.ctypes.data):
+            raise RuntimeError("oracle set_initial_condition failed")
+
+    def get_state(self):
+        """(state [n_ch][2 n_sec + 2] float64: z1,z2 per section, sta, lta; samples seen)."""
+        out = np.empty((self.n_ch, 2 * self.n_sec + 2), dtype=np.float64)
+        g = ctypes.c_longlong(0)
+        if self._lib.filark_oracle_get_state(self._h, out.ctypes.data, ctypes.addressof(g)):
+            raise RuntimeError("oracle get_state failed")
+        return out, int(g.value)
+
+    def set_state(self, state, g: int):
+        state = np.ascontiguousarray(state, dtype=np.float64)
+        assert state.shape == (self.n_ch, 2 * self.n_sec + 2)
+        if self._lib.filark_oracle_set_state(self._h, state.ctypes.data, int(g)):
+            raise RuntimeError("oracle set_state failed")
 
     def trace_f64(self, x: np.ndarray, channel: int = 0):
         """Double-precision input, one channel: returns (y, sta, lta) as float64 (for pins).
