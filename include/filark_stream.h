@@ -197,6 +197,34 @@ filark_status_t filark_stream_push_host(filark_stream_t *h, const float *h_in, l
  */
 filark_status_t filark_stream_reset(filark_stream_t *h, cudaStream_t stream);
 
+/*
+ * State export / import and the steady-state initial condition ("maintaining correct
+ * state propagation"; :169 state survives file boundaries -- here: handles and processes;
+ * :255 "a short transient determined by the filter order and the initial condition").
+ *
+ * filark_stream_state_size -- bytes of this handle's state blob: 64 + n_ch * (2 n_sec + 2) * 8.
+ * filark_stream_get_state  -- synchronises `stream` (and the device), writes the blob to HOST memory.
+ *   Layout: 64-byte header {"FKSTATE1", int n_ch, n_sec, sta_len, lta_len, uint64 samples seen,
+ *   32 reserved bytes}, then per channel 2 n_sec + 2 doubles: the state s_k of every section k in
+ *   the coordinates filark_debug_design reports (s[n] = A s[n-1] + B x[n], y[n] = C s[n-1] + D x[n],
+ *   the cascade's gain in front of section 0) after the LAST pushed sample, then sta * sta_len and
+ *   lta * lta_len.  (Inside the handle the state stands at a sub-block boundary with up to 23 raw
+ *   samples waiting; the export runs those over it in float64, so the blob has no pending samples.)
+ * filark_stream_set_state  -- the reverse, into a handle created with the same n_ch, n_sec, sta_len,
+ *   lta_len (and, for the outputs to continue, the same sos): pushing B after importing the state
+ *   exported behind A gives the outputs of A || B to fp32 rounding.  Synchronises.
+ * filark_stream_set_initial_condition -- the state every channel would have if its input had been
+ *   the constant x0[c] (HOST array, n_ch floats) for ever: s = (I - A)^-1 B v per section, the
+ *   averages at the steady energy, the warm-up over (scipy's `zi = sosfilt_zi(sos) * x0` idiom).
+ *   create/reset give the zero state (reading R6).  Synchronises.
+ * Errors: INVALID_ARG (null, blob too small or of another handle shape, non-finite values, handle
+ * with FILARK_FLAG_SERIAL_SCAN), DEVICE_MISMATCH, CUDA.
+ */
+long long filark_stream_state_size(const filark_stream_t *h);
+filark_status_t filark_stream_get_state(filark_stream_t *h, void *blob, long long size, cudaStream_t stream);
+filark_status_t filark_stream_set_state(filark_stream_t *h, const void *blob, long long size, cudaStream_t stream);
+filark_status_t filark_stream_set_initial_condition(filark_stream_t *h, const float *x0, cudaStream_t stream);
+
 /* Free the handle and its device memory (on the handle's device, whichever device is current).
  * NULL is accepted.  Synchronises the handle's device. */
 filark_status_t filark_stream_destroy(filark_stream_t *h);

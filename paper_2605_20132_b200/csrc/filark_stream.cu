@@ -802,6 +802,141 @@ filark_status_t filark_stream_push_host(filark_stream_t* h, const float* h_in, l
     return FILARK_OK;
 }
 
+// ---- state export / import, initial condition ----------------------------
+// Documented form (include/filark_stream.h): header + per channel 2 n_sec + 2 doubles = the state s
+// of every section in the coordinates of filark_debug_design (s[n] = A s[n-1] + B x[n], the cascade's
+// gain applied in front of section 0) after the LAST pushed sample, then sta N_s and lta N_l.
+struct StateHeader {
+    char magic[8];                 // "FKSTATE1"
+    int n_ch, n_sec, sta_len, lta_len;
+    unsigned long long seen;       // samples per channel since create/reset
+    unsigned char pad[32];
+};
+static_assert(sizeof(StateHeader) == 64, "blob header");
+
+long long filark_stream_state_size(const filark_stream_t* h)
+{
+    return h ? (long long)sizeof(StateHeader) + (long long)h->n_ch * (2LL * h->n_sec + 2) * (long long)sizeof(double) : -1;
+}
+
+// (host, float64) one sample through the conditioned cascade and the averages, as the kernels run them
+static void host_step(const filark_stream* h, double* s, double x)
+{
+    double v = h->gain * x;
+    for (int k = 0; k < h->n_sec; ++k) {
+        const Section& c = h->sec[k];
+        double* q = s + 2 * k;
+        const double y = c.C[0] * q[0] + c.C[1] * q[1] + c.D * v;
+        const double n0 = c.A.a * q[0] + c.A.b * q[1] + c.B[0] * v;
+        const double n1 = c.A.c * q[0] + c.A.d * q[1] + c.B[1] * v;
+        q[0] = n0; q[1] = n1;
+        v = y;
+    }
+    const double e = v * v;
+    double* m = s + 2 * h->n_sec;
+    m[0] = m[0] - m[0] / h->sta_len + e;          // m~ = N m:  m~ <- (1 - 1/N) m~ + e
+    m[1] = m[1] - m[1] / h->lta_len + e;
+}
+
+filark_status_t filark_stream_get_state(filark_stream_t* h, void* blob, long long size, cudaStream_t stream)
+{
+    if (!h || !blob || size < filark_stream_state_size(h)) return FILARK_ERR_INVALID_ARG;
+    if (h->flags & FILARK_FLAG_SERIAL_SCAN) return FILARK_ERR_INVALID_ARG;
+    filark_status_t st = check_device(h);
+    if (st != FILARK_OK) return st;
+    const int ns = state_floats(h->n_sec), w = 2 * h->n_sec + 2;
+    std::vector<float> state((size_t)h->n_ch * ns), hist((size_t)h->n_ch * kHist);
+    CmCtl ctl;
+    cudaError_t e = cudaStreamSynchronize(stream);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();           // (pushes of this handle on other streams)
+    if (e == cudaSuccess) e = cudaMemcpy(state.data(), h->d_state, sizeof(float) * state.size(), cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(hist.data(), h->d_hist, sizeof(float) * hist.size(), cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemcpy(&ctl, h->d_cctl, sizeof(ctl), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(h, e);
+    const CmSlot& sl = ctl.slot[ctl.epoch & 1u];
+    StateHeader hd{};
+    std::memcpy(hd.magic, "FKSTATE1", 8);
+    hd.n_ch = h->n_ch; hd.n_sec = h->n_sec; hd.sta_len = h->sta_len; hd.lta_len = h->lta_len;
+    hd.seen = sl.seen;
+    std::memcpy(blob, &hd, sizeof(hd));
+    double* out = reinterpret_cast<double*>(static_cast<char*>(blob) + sizeof(hd));
+    // the device state stands at the last slot boundary: run the r0 samples waiting in `hist` over it
+    const int r0 = (int)sl.r0 < kHist ? (int)sl.r0 : kHist - 1;
+    for (int c = 0; c < h->n_ch; ++c) {
+        double* s = out + (size_t)c * w;
+        for (int i = 0; i < w; ++i) s[i] = (double)state[(size_t)c * ns + i];
+        for (int j = 0; j < r0; ++j) host_step(h, s, (double)hist[(size_t)c * kHist + j]);
+    }
+    return FILARK_OK;
+}
+
+// state words of every channel (float64, documented coordinates) -> handle, `seen` samples on the counter
+static filark_status_t install_state(filark_stream_t* h, const double* in, unsigned long long seen, cudaStream_t stream)
+{
+    const int ns = state_floats(h->n_sec), w = 2 * h->n_sec + 2;
+    std::vector<float> state((size_t)h->n_ch * ns, 0.0f);
+    for (int c = 0; c < h->n_ch; ++c)
+        for (int i = 0; i < w; ++i) state[(size_t)c * ns + i] = (float)in[(size_t)c * w + i];
+    CmCtl ctl;
+    std::memset(&ctl, 0, sizeof(ctl));
+    ctl.slot[0].seen = seen;
+    cudaError_t e = cudaStreamSynchronize(stream);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e == cudaSuccess) e = cudaMemcpy(h->d_state, state.data(), sizeof(float) * state.size(), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemset(h->d_hist, 0, sizeof(float) * (size_t)h->n_ch * kHist);
+    if (e == cudaSuccess) e = cudaMemcpy(h->d_cctl, &ctl, sizeof(ctl), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemset(h->d_progress, 0, sizeof(unsigned) * (size_t)h->n_ch);
+    if (e != cudaSuccess) return cuda_fail(h, e);
+    h->prev_valid = 0;
+    h->samples = (long long)seen;
+    return FILARK_OK;
+}
+
+filark_status_t filark_stream_set_state(filark_stream_t* h, const void* blob, long long size, cudaStream_t stream)
+{
+    if (!h || !blob || size < filark_stream_state_size(h)) return FILARK_ERR_INVALID_ARG;
+    if (h->flags & FILARK_FLAG_SERIAL_SCAN) return FILARK_ERR_INVALID_ARG;
+    StateHeader hd;
+    std::memcpy(&hd, blob, sizeof(hd));
+    if (std::memcmp(hd.magic, "FKSTATE1", 8) != 0 || hd.n_ch != h->n_ch || hd.n_sec != h->n_sec ||
+        hd.sta_len != h->sta_len || hd.lta_len != h->lta_len)
+        return FILARK_ERR_INVALID_ARG;
+    const int w = 2 * h->n_sec + 2;
+    const double* in = reinterpret_cast<const double*>(static_cast<const char*>(blob) + sizeof(hd));
+    for (long long i = 0; i < (long long)h->n_ch * w; ++i) if (!std::isfinite(in[i])) return FILARK_ERR_INVALID_ARG;
+    filark_status_t st = check_device(h);
+    if (st != FILARK_OK) return st;
+    return install_state(h, in, hd.seen, stream);
+}
+
+filark_status_t filark_stream_set_initial_condition(filark_stream_t* h, const float* x0, cudaStream_t stream)
+{
+    if (!h || !x0) return FILARK_ERR_INVALID_ARG;
+    if (h->flags & FILARK_FLAG_SERIAL_SCAN) return FILARK_ERR_INVALID_ARG;
+    for (int c = 0; c < h->n_ch; ++c) if (!std::isfinite(x0[c])) return FILARK_ERR_INVALID_ARG;
+    filark_status_t st = check_device(h);
+    if (st != FILARK_OK) return st;
+    // steady state of s = A s + B v, y = C s + D v for a constant input v: s = (I - A)^-1 B v
+    const int w = 2 * h->n_sec + 2;
+    std::vector<double> in((size_t)h->n_ch * w);
+    for (int c = 0; c < h->n_ch; ++c) {
+        double v = h->gain * (double)x0[c];
+        double* s = in.data() + (size_t)c * w;
+        for (int k = 0; k < h->n_sec; ++k) {
+            const Section& q = h->sec[k];
+            const double m00 = 1.0 - q.A.a, m01 = -q.A.b, m10 = -q.A.c, m11 = 1.0 - q.A.d;
+            const double det = m00 * m11 - m01 * m10;                 // = 1 + a1 + a2 > 0 (stable section)
+            const double b0 = q.B[0] * v, b1 = q.B[1] * v;
+            s[2 * k] = (m11 * b0 - m01 * b1) / det;
+            s[2 * k + 1] = (m00 * b1 - m10 * b0) / det;
+            v = q.C[0] * s[2 * k] + q.C[1] * s[2 * k + 1] + q.D * v;
+        }
+        s[2 * h->n_sec] = v * v * h->sta_len;
+        s[2 * h->n_sec + 1] = v * v * h->lta_len;
+    }
+    return install_state(h, in.data(), (unsigned long long)h->lta_len, stream);
+}
+
 // ---- debug / introspection (include/filark_debug.h): host only, no CUDA calls -----------------
 int filark_debug_design(const double* sos, int n_sec, int* kinds, double* coefs, double* gain)
 {

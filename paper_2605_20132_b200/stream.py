@@ -61,6 +61,14 @@ def load_library():
     lib.filark_stream_push_pitched.argtypes = [vp, vp, ll, ll, vp, vp, ll, vp]
     lib.filark_stream_push_host.restype = ci
     lib.filark_stream_push_host.argtypes = [vp, vp, ll, vp, vp, vp]
+    lib.filark_stream_state_size.restype = ll
+    lib.filark_stream_state_size.argtypes = [vp]
+    lib.filark_stream_get_state.restype = ci
+    lib.filark_stream_get_state.argtypes = [vp, vp, ll, vp]
+    lib.filark_stream_set_state.restype = ci
+    lib.filark_stream_set_state.argtypes = [vp, vp, ll, vp]
+    lib.filark_stream_set_initial_condition.restype = ci
+    lib.filark_stream_set_initial_condition.argtypes = [vp, vp, vp]
     lib.filark_stream_reset.restype = ci
     lib.filark_stream_reset.argtypes = [vp, vp]
     lib.filark_stream_destroy.restype = ci
@@ -192,6 +200,25 @@ class FilarkStream:
     def reset(self, stream: Optional[int] = None):
         self._check(self._lib.filark_stream_reset(self._h, _cur_stream() if stream is None else stream),
                     "filark_stream_reset")
+
+    def get_state(self, stream: Optional[int] = None) -> bytes:
+        """filark_stream_get_state: the documented state blob (host bytes)."""
+        n = int(self._lib.filark_stream_state_size(self._h))
+        buf = ctypes.create_string_buffer(n)
+        self._check(self._lib.filark_stream_get_state(self._h, buf, n, _cur_stream() if stream is None else stream),
+                    "filark_stream_get_state")
+        return buf.raw
+
+    def set_state(self, blob: bytes, stream: Optional[int] = None):
+        self._check(self._lib.filark_stream_set_state(self._h, blob, len(blob), _cur_stream() if stream is None else stream),
+                    "filark_stream_set_state")
+
+    def set_initial_condition(self, x0, stream: Optional[int] = None):
+        """x0: per-channel constant input level (scalar or [n_ch])."""
+        a = np.ascontiguousarray(np.broadcast_to(np.asarray(x0, dtype=np.float32), (self.n_ch,)))
+        self._check(self._lib.filark_stream_set_initial_condition(self._h, a.ctypes.data,
+                                                                  _cur_stream() if stream is None else stream),
+                    "filark_stream_set_initial_condition")
 
     def destroy(self):
         if getattr(self, "_h", None) is not None and self._h.value:
