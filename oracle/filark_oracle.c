@@ -276,3 +276,78 @@ int filark_oracle_set_state(filark_oracle_t *o, const double *in, long long g)
     o->g = g;
     return 0;
 }
+
+/*
+ * Trigger / event emission on the characteristic function ("any
+ * callable that consumes a data window and returns a list of time-channel-bounded events", :132 a
+ * threshold-based detector, :169 "must not miss events that straddle two consecutive files").
+ * The paper fixes no trigger rule; reading R24: the classic on/off trigger with
+ * hysteresis on the float32 CF the path outputs, per channel, state carried across pushes:
+ *     off -> on   at the first sample with cf >= thr_on            (t_on = its index, peak = cf)
+ *     on  -> off  at the first later sample with cf <  thr_off     (t_off = its index; event emitted)
+ *     while on: peak = max(peak, cf)          thr_off <= thr_on, both compared in float32
+ * Sample indices count from create/reset.  An event still open when the data end is not emitted
+ * (it is, by a later push, when it closes).  Events come out channel by channel in time order.
+ */
+typedef struct filark_oracle_event {
+    long long t_on, t_off;
+    int channel;
+    float peak;
+} filark_oracle_event_t;
+
+typedef struct filark_oracle_trigger {
+    int n_ch;
+    float thr_on, thr_off;
+    int *on;
+    long long *t_on;
+    float *peak;
+    long long g;
+} filark_oracle_trigger_t;
+
+filark_oracle_trigger_t *filark_oracle_trigger_create(int n_ch, float thr_on, float thr_off)
+{
+    if (n_ch <= 0 || !(thr_on > 0.0f) || !(thr_off > 0.0f) || thr_off > thr_on) return NULL;
+    filark_oracle_trigger_t *t = (filark_oracle_trigger_t *)calloc(1, sizeof(*t));
+    if (!t) return NULL;
+    t->n_ch = n_ch; t->thr_on = thr_on; t->thr_off = thr_off;
+    t->on = (int *)calloc((size_t)n_ch, sizeof(int));
+    t->t_on = (long long *)calloc((size_t)n_ch, sizeof(long long));
+    t->peak = (float *)calloc((size_t)n_ch, sizeof(float));
+    if (!t->on || !t->t_on || !t->peak) { free(t->on); free(t->t_on); free(t->peak); free(t); return NULL; }
+    return t;
+}
+
+void filark_oracle_trigger_destroy(filark_oracle_trigger_t *t)
+{
+    if (!t) return;
+    free(t->on); free(t->t_on); free(t->peak); free(t);
+}
+
+/* cf: one chunk of the CF, element (c, n) at c*stride_c + n*stride_n.  Appends at most cap events to
+ * out; returns the number of events the chunk closed (may exceed cap: the rest is dropped). */
+long long filark_oracle_trigger_push(filark_oracle_trigger_t *t, const float *cf, long long n_t,
+                                     long long stride_c, long long stride_n,
+                                     filark_oracle_event_t *out, long long cap)
+{
+    if (!t || !cf || n_t < 0) return -1;
+    long long n_ev = 0;
+    for (int c = 0; c < t->n_ch; ++c) {
+        for (long long n = 0; n < n_t; ++n) {
+            const float v = cf[(long long)c * stride_c + n * stride_n];
+            const long long g = t->g + n;
+            if (!t->on[c]) {
+                if (v >= t->thr_on) { t->on[c] = 1; t->t_on[c] = g; t->peak[c] = v; }
+            } else if (v < t->thr_off) {
+                if (out && n_ev < cap) {
+                    out[n_ev].t_on = t->t_on[c]; out[n_ev].t_off = g; out[n_ev].channel = c; out[n_ev].peak = t->peak[c];
+                }
+                n_ev += 1;
+                t->on[c] = 0;
+            } else if (v > t->peak[c]) {
+                t->peak[c] = v;
+            }
+        }
+    }
+    t->g += n_t;
+    return n_ev;
+}

@@ -72,6 +72,12 @@ def _load():
     lib.filark_oracle_get_state.argtypes = [vp, vp, vp]
     lib.filark_oracle_set_state.restype = ci
     lib.filark_oracle_set_state.argtypes = [vp, vp, ll]
+    lib.filark_oracle_trigger_create.restype = vp
+    lib.filark_oracle_trigger_create.argtypes = [ci, ctypes.c_float, ctypes.c_float]
+    lib.filark_oracle_trigger_destroy.restype = None
+    lib.filark_oracle_trigger_destroy.argtypes = [vp]
+    lib.filark_oracle_trigger_push.restype = ll
+    lib.filark_oracle_trigger_push.argtypes = [vp, vp, ll, ll, ll, vp, ll]
     _lib = lib
     return lib
 
@@ -172,3 +178,35 @@ class Oracle:
         if rc:
             raise RuntimeError("oracle trace failed")
         return y, s, l
+
+
+EVENT_DTYPE = np.dtype([("t_on", "<i8"), ("t_off", "<i8"), ("channel", "<i4"), ("peak", "<f4")])
+
+
+class OracleTrigger:
+    """On/off trigger with hysteresis on the CF, state carried across pushes (NEXT-1, reading R24)."""
+
+    def __init__(self, n_ch: int, thr_on: float, thr_off: float, layout: int = CHANNEL_MAJOR):
+        lib = _load()
+        self._lib, self.n_ch, self.layout = lib, int(n_ch), int(layout)
+        self._h = lib.filark_oracle_trigger_create(self.n_ch, float(thr_on), float(thr_off))
+        if not self._h:
+            raise ValueError("filark_oracle_trigger_create rejected its arguments")
+
+    def push(self, cf: np.ndarray, cap: int = 1 << 20) -> np.ndarray:
+        """cf: float32 chunk in the trigger's layout; returns the events this chunk closed."""
+        cf = np.ascontiguousarray(cf, dtype=np.float32)
+        n_t = cf.shape[1] if self.layout == CHANNEL_MAJOR else cf.shape[0]
+        sc, sn = (n_t, 1) if self.layout == CHANNEL_MAJOR else (1, self.n_ch)
+        out = np.zeros(cap, dtype=EVENT_DTYPE)
+        n = self._lib.filark_oracle_trigger_push(self._h, cf.ctypes.data, n_t, sc, sn, out.ctypes.data, cap)
+        if n < 0 or n > cap:
+            raise RuntimeError("oracle trigger push failed or overflowed")
+        return out[:n].copy()
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.filark_oracle_trigger_destroy(self._h)
+            self._h = None
+
+    __del__ = close
