@@ -497,6 +497,22 @@ def extra_runs(args, w, sos, stream, ins, filts, cfs, sched, torch, dev, peak, s
             return _row(n_samples, ms, peak, 8.0)
         guarded("filt_only", lambda: one_output("filt"))
         guarded("cf_only", lambda: one_output("cf"))
+
+        # ---- trigger on the CF fused behind S6 (NEXT-1): both outputs + events, and filt + events with d_cf = NULL
+        def with_trigger(want_cf):
+            stream.set_trigger(4.0, 2.0, 1 << 20)
+            b2 = PushBatch(stream, ins, filts, cfs if want_cf else None)
+
+            def st():
+                stream.reset(); stream.push_many(b2)
+            ms = _time(torch, st, max(3, args.steps // 2), warm=2)
+            ev, dropped = stream.pop_events()
+            stream.set_trigger(0.0, 0.0, 0)
+            r = _row(n_samples, ms, peak, 12.0 if want_cf else 8.0)
+            r.update({"thr_on": 4.0, "thr_off": 2.0, "events_per_step": len(ev) // (max(3, args.steps // 2) + 2), "dropped": dropped})
+            return r
+        guarded("trigger_both_outputs_and_events", lambda: with_trigger(True))
+        guarded("trigger_filt_and_events_no_cf", lambda: with_trigger(False))
     return extra
 
 

@@ -198,6 +198,40 @@ filark_status_t filark_stream_push_host(filark_stream_t *h, const float *h_in, l
 filark_status_t filark_stream_reset(filark_stream_t *h, cudaStream_t stream);
 
 /*
+ * Trigger / event emission on the characteristic function (the step behind S6: PAPER.md:130 a
+ * monitor "consumes a data window and returns a list of time-channel-bounded events", :132
+ * threshold-based detectors, :169 events may straddle chunk and file boundaries).  Classic on/off
+ * trigger with hysteresis per channel (reading R24 in DESIGN.md), decided on the float32 cf:
+ *     off -> on   at the first sample with cf >= thr_on
+ *     on  -> off  at the first later sample with cf <  thr_off      (0 < thr_off <= thr_on)
+ * An event is appended to a device list owned by the handle when it closes; the trigger state (on/off,
+ * t_on, peak so far) is part of the carried state, so events straddle pushes.  The trigger runs inside
+ * the push launches, behind the cf computation, also when d_cf is NULL (8 B/sample: input + filt, or
+ * with d_filt = d_cf = NULL rejected as before -- one output array is still required).
+ *
+ * filark_stream_set_trigger -- thresholds and the capacity of the event list (>= 1 events; events
+ *   closed while the list is full are dropped and counted).  thr_on = thr_off = 0 switches the
+ *   trigger off.  Synchronises `stream` and the device; empties the list and sets every channel off.
+ * filark_stream_pop_events  -- synchronises `stream`, copies the events closed so far to HOST memory
+ *   (in no particular order: sort by (t_on, channel)) and empties the list.  *n_out = events copied,
+ *   *n_dropped = events lost to a full list since the last pop (may be NULL).  If cap is smaller
+ *   than the number of pending events nothing is consumed, *n_out says how many there are and the
+ *   call returns INVALID_ARG.
+ * Errors: INVALID_ARG, ALLOC, DEVICE_MISMATCH, CUDA.  filark_stream_reset and _set_state switch every
+ * channel off but keep pending events.
+ */
+typedef struct filark_event {
+    long long t_on;    /* index (samples since create/reset) of the first sample with cf >= thr_on */
+    long long t_off;   /* index of the first later sample with cf < thr_off                         */
+    int channel;
+    float peak;        /* largest cf in [t_on, t_off)                                               */
+} filark_event_t;
+filark_status_t filark_stream_set_trigger(filark_stream_t *h, float thr_on, float thr_off,
+                                          long long max_events, cudaStream_t stream);
+filark_status_t filark_stream_pop_events(filark_stream_t *h, filark_event_t *out, long long cap,
+                                         long long *n_out, long long *n_dropped, cudaStream_t stream);
+
+/*
  * State export / import and the steady-state initial condition ("maintaining correct
  * state propagation"; :169 state survives file boundaries -- here: handles and processes;
  * :255 "a short transient determined by the filter order and the initial condition").

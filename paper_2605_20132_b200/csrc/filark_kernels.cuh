@@ -99,9 +99,12 @@ struct AvgParams {
 };
 
 // Carried state of one channel (floats): [0, 2 n_sec) section states, then sta~, lta~, the
-// number of samples seen (serial kernel only; uint32 bits, saturating), one pad word.
+// number of samples seen (serial kernel only; uint32 bits, saturating), then the trigger state
+// (kTrigWords words: on/off, peak, t_on as two words; see trigger_tile).
 // (padded to a multiple of four words: the state moves in 16-byte pieces)
-__host__ __device__ constexpr int state_floats(int n_sec) { return (2 * n_sec + 4 + 3) & ~3; }
+constexpr int kTrigWords = 4;
+__host__ __device__ constexpr int trig_word(int n_sec) { return 2 * n_sec + 3; }
+__host__ __device__ constexpr int state_floats(int n_sec) { return (2 * n_sec + 3 + kTrigWords + 3) & ~3; }
 constexpr unsigned kSeenMax = 0x7fffffffu;
 
 // One chunk of a launch.  A launch covers up to kMaxBatch consecutive chunks of the stream (one
@@ -119,6 +122,14 @@ struct Chunk {
     unsigned t_cum;          // samples of the launch in front of this chunk
 };
 
+// One closed event of the on/off trigger (== filark_event_t of include/filark_stream.h).
+struct Event {
+    long long t_on, t_off;   // sample indices since create/reset: first sample with cf >= thr_on, first later one with cf < thr_off
+    int channel;
+    float peak;              // largest cf in [t_on, t_off)
+};
+static_assert(sizeof(Event) == 24, "event record");
+
 template <int L> struct PushParams {
     float* state;            // [n_ch][state_floats]
     float* hist;             // [n_ch][kHist]
@@ -131,6 +142,11 @@ template <int L> struct PushParams {
                              // the shift of every row itself, see "Alignment"; time-major: 16-byte stores allowed)
     int wait_prior;          // wait for everything before this launch in the stream before touching memory
     float gain, ratio, lta_thr;
+    // trigger on the characteristic function (trigger_tile): off when thr_on <= 0
+    float thr_on, thr_off;
+    Event* events;           // [ev_cap] closed events, in no particular order
+    unsigned* n_events;      // events closed so far (may exceed ev_cap: the excess is dropped and counted)
+    unsigned ev_cap;
     AvgParams avg;
     SecParams<L> sec[kMaxSec];
     Chunk ck[kMaxBatch];
@@ -243,7 +259,7 @@ __device__ __forceinline__ void sts_f2(unsigned sa, float2 v)
 
 // Shared memory of one warp: two tile buffers (input of tile k / staging of its outputs, and the
 // prefetched input of tile k+1) and two copies of the channel state.
-constexpr int kStateSmem = 40;                     // >= state_floats(kMaxSec), multiple of 4
+constexpr int kStateSmem = 44;                     // >= state_floats(kMaxSec), multiple of 4
 constexpr int kHistSmem = 48;                      // raw history of the next item's channel (r0 < 48)
 template <int L> __host__ __device__ constexpr int warp_smem_floats() { return 2 * Geo<L>::buf_floats + 2 * kStateSmem + kHistSmem; }
 
@@ -641,6 +657,86 @@ __device__ __forceinline__ void local_pass(float2 (&x)[L], const SecParams<L>& T
     }
 }
 
+// Trigger on the characteristic function (reading R24 in DESIGN.md; PAPER.md:130
+// "returns a list of time-channel-bounded events", :169 events may straddle chunks): per channel
+//     off -> on  at the first sample with cf >= thr_on,   on -> off  at the first later one with cf < thr_off
+// (an event (t_on, t_off, channel, peak cf) is appended to p.events when it closes), state carried with
+// the channel's filter state.  Called for a tile only if it can matter (the channel is on, or some cf
+// of the tile reaches thr_on): the cf of the tile lies in `buf` (lane regions, shift s), tile positions
+// [e_lo, e_hi) are samples of this chunk, position e is sample g0 + e of the stream.  Every lane
+// summarises its 2L samples; the warp then visits, in time order, only the lanes that can change the
+// state (a lane with cf >= thr_on while off, one with cf < thr_off while on) and lets each walk its
+// samples; the lanes passed over while on only raise the peak.
+template <int L>
+__device__ __noinline__ void trigger_tile(const PushParams<L>& p, int buf, int s, int wtr, int ch, long long g0,
+                                          int e_lo, int e_hi, int lane)
+{
+    const float thr_on = p.thr_on, thr_off = p.thr_off;
+    const int eb = 2 * L * lane;
+    unsigned on = __float_as_uint(fk_smem[wtr]);
+    // Does this tile matter?  Only if the channel is on, or some cf of the tile reaches thr_on (positions
+    // outside the chunk included: that costs a needless visit at most).  Everything that belongs to the
+    // trigger lives in this function, so that the push kernel carries none of it when no trigger is set.
+    {
+        float m = 0.0f;
+        if (s == 0) {
+            const float4* r = reinterpret_cast<const float4*>(&fk_smem[buf + lane * Geo<L>::pitch]);
+#pragma unroll
+            for (int q = 0; q < L / 2; ++q) { const float4 v = r[q]; m = fmaxf(fmaxf(m, fmaxf(v.x, v.y)), fmaxf(v.z, v.w)); }
+        } else {
+            for (int e = eb; e < eb + 2 * L; ++e) m = fmaxf(m, fk_smem[buf + raw_index<L>(e + s)]);
+        }
+        if (on == 0u && !__any_sync(0xffffffffu, m >= thr_on)) return;
+    }
+    float mx = 0.0f;
+    bool has_on = false, has_off = false;
+    for (int e = max(eb, e_lo); e < min(eb + 2 * L, e_hi); ++e) {
+        const float c = fk_smem[buf + raw_index<L>(e + s)];
+        mx = fmaxf(mx, c);
+        has_on = has_on || c >= thr_on;
+        has_off = has_off || c < thr_off;
+    }
+    const unsigned b_on = __ballot_sync(0xffffffffu, has_on), b_off = __ballot_sync(0xffffffffu, has_off);
+    float peak = fk_smem[wtr + 1];
+    long long t_on = (long long)(((unsigned long long)__float_as_uint(fk_smem[wtr + 3]) << 32) | __float_as_uint(fk_smem[wtr + 2]));
+    const unsigned mxb = __float_as_uint(mx);               // (cf >= 0: the bit patterns order like the values)
+    int last = -1;                                           // last lane that walked
+    for (;;) {
+        const unsigned cand = (on ? b_off : b_on) & (last >= 31 ? 0u : ~0u << (last + 1));
+        const int l = cand ? __ffs((int)cand) - 1 : 32;
+        if (on) {                                            // lanes passed over while on
+            const bool mid = lane > last && lane < l;
+            peak = fmaxf(peak, __uint_as_float(__reduce_max_sync(0xffffffffu, mid ? mxb : 0u)));
+        }
+        if (l == 32) break;
+        if (lane == l) {
+            for (int e = max(eb, e_lo); e < min(eb + 2 * L, e_hi); ++e) {
+                const float c = fk_smem[buf + raw_index<L>(e + s)];
+                if (!on) {
+                    if (c >= thr_on) { on = 1u; t_on = g0 + e; peak = c; }
+                } else if (c < thr_off) {
+                    const unsigned idx = atomicAdd(p.n_events, 1u);
+                    if (idx < p.ev_cap) p.events[idx] = Event{t_on, g0 + e, ch, peak};
+                    on = 0u;
+                } else {
+                    peak = fmaxf(peak, c);
+                }
+            }
+        }
+        on = __shfl_sync(0xffffffffu, on, l);
+        peak = __shfl_sync(0xffffffffu, peak, l);
+        t_on = __shfl_sync(0xffffffffu, t_on, l);
+        last = l;
+    }
+    if (lane == 0) {
+        fk_smem[wtr] = __uint_as_float(on);
+        fk_smem[wtr + 1] = peak;
+        fk_smem[wtr + 2] = __uint_as_float((unsigned)((unsigned long long)t_on & 0xffffffffull));
+        fk_smem[wtr + 3] = __uint_as_float((unsigned)((unsigned long long)t_on >> 32));
+    }
+    __syncwarp();
+}
+
 // One tile of one channel, samples already in x (gain applied): S1..S7.  `buf` stages the
 // outputs.  buf / wst are float offsets into fk_smem.
 // (kTM: time-major chunk; the CTA's warps hold the channels cg kTmChannels + warp and store together;
@@ -786,7 +882,8 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
         if (lane + 32 < ns) __stcg(gst + lane + 32, fk_smem[wst + lane + 32]);
     }
 
-    if (ck.cf) {
+    const bool trig = p.thr_on > 0.0f;
+    if (ck.cf || trig) {
         // warm-up (reading R10): samples whose index since create/reset is < lta_len give cf = 0
         // (seen = samples pushed before this push; tile position e is sample seen + t0 + e of the stream)
         const long long rem = (long long)p.lta_len - (long long)seen - t0;     // first tile position with cf != 0
@@ -812,18 +909,21 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
                 x[i].y = (Pl.y > thr && base + L + i >= wm) ? qb : 0.0f;
             }
         }
-        if (kTM) {
-            regs_to_buf<L>(x, buf, lane, 0);
-            __syncthreads();
-            if (item_end && lane == 0) st_release(p.progress + ch, rel_val);
-            store_tile_tm<L>(p, ck, g, ck.cf, cg, bufoff, t0);
-        } else {
-            float* row = ck.cf + (long long)ch * ck.out_pitch;
-            const int sc = row_shift(row, g.r0);
-            regs_to_buf<L>(x, buf, lane, sc);
-            __syncwarp();
-            if (item_end && lane == 0) st_release(p.progress + ch, rel_val);
-            store_tile<L, kInterior>(ck, g, row, buf, lane, t0, sc, to);
+        const int sc = (kTM || !ck.cf) ? 0 : row_shift(ck.cf + (long long)ch * ck.out_pitch, g.r0);
+        regs_to_buf<L>(x, buf, lane, sc);
+        if (kTM) __syncthreads(); else __syncwarp();
+        if (trig && (!kTM || ch < p.n_ch)) {
+            trigger_tile<L>(p, buf, sc, wst + trig_word(p.n_sec), ch, (long long)seen + t0, max(0, -t0),
+                            min(Geo<L>::tile, ck.n_t - t0), lane);
+            if (item_end && lane == 0) {             // (the state went back before the trigger ran)
+                float* gtr = p.state + (long long)ch * state_floats(p.n_sec) + trig_word(p.n_sec);
+                for (int j = 0; j < kTrigWords; ++j) __stcg(gtr + j, fk_smem[wst + trig_word(p.n_sec) + j]);
+            }
+        }
+        if (item_end && lane == 0) st_release(p.progress + ch, rel_val);
+        if (ck.cf) {
+            if (kTM) store_tile_tm<L>(p, ck, g, ck.cf, cg, bufoff, t0);
+            else store_tile<L, kInterior>(ck, g, ck.cf + (long long)ch * ck.out_pitch, buf, lane, t0, sc, to);
         }
     } else if (item_end) {
         __syncwarp();

@@ -42,6 +42,11 @@ struct filark_stream {
     float* d_state;
     size_t state_floats;
     float* d_hist;                  // raw tail of the previous push: [n_ch][kHist] (both layouts)
+    // trigger on the characteristic function (filark_stream_set_trigger): off while thr_on <= 0
+    float thr_on, thr_off;
+    Event* d_events;
+    unsigned* d_n_events;
+    unsigned ev_cap;
     CmCtl* d_cctl;                  // channel-major kernel: double-buffered control slots (filark_kernels.cuh)
     unsigned* d_progress;           // [n_ch] segments completed per channel (cumulative)
     // what the previous channel-major push touched: a push may overlap the one before it on the
@@ -353,6 +358,7 @@ static cudaError_t push_variant(const filark_stream* h, int v, const ChunkArgs* 
     PushParams<L> p = *(const PushParams<L>*)h->proto[v];
     p.state = h->d_state; p.hist = h->d_hist; p.cctl = h->d_cctl; p.progress = h->d_progress;
     p.n_push = n; p.vec4 = vec4; p.wait_prior = wait_prior;
+    p.thr_on = h->thr_on; p.thr_off = h->thr_off; p.events = h->d_events; p.n_events = h->d_n_events; p.ev_cap = h->ev_cap;
     unsigned t_cum = 0;
     for (int k = 0; k < n; ++k) {
         Chunk& d = p.ck[k];
@@ -479,6 +485,7 @@ filark_status_t filark_stream_destroy(filark_stream_t* h)
     cudaDeviceSynchronize();
     for (int v = 0; v < kNumVariants; ++v) std::free(h->proto[v]);
     cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_cctl); cudaFree(h->d_progress);
+    cudaFree(h->d_events); cudaFree(h->d_n_events);
     for (int j = 0; j < 2; ++j) for (int i = 0; i < 3; ++i) cudaFree(h->d_stage[j][i]);
     if (h->host_ready) {
         cudaStreamDestroy(h->s_h2d); cudaStreamDestroy(h->s_d2h);
@@ -799,6 +806,66 @@ filark_status_t filark_stream_push_host(filark_stream_t* h, const float* h_in, l
     if (e != cudaSuccess) return cuda_fail(h, e);
     h->ev_pending[j] = true;
     h->host_pushes += 1;
+    return FILARK_OK;
+}
+
+// ---- trigger / event emission on the characteristic function -------------
+filark_status_t filark_stream_set_trigger(filark_stream_t* h, float thr_on, float thr_off, long long max_events,
+                                          cudaStream_t stream)
+{
+    if (!h) return FILARK_ERR_INVALID_ARG;
+    if (h->flags & FILARK_FLAG_SERIAL_SCAN) return FILARK_ERR_INVALID_ARG;
+    const bool off = thr_on == 0.0f && thr_off == 0.0f;
+    if (!off && (!(thr_on > 0.0f) || !(thr_off > 0.0f) || thr_off > thr_on || !std::isfinite(thr_on) ||
+                 max_events < 1 || max_events > 0x7fffffffLL))
+        return FILARK_ERR_INVALID_ARG;
+    filark_status_t st = check_device(h);
+    if (st != FILARK_OK) return st;
+    // everything enqueued so far runs with the old settings
+    cudaError_t e = cudaStreamSynchronize(stream);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) return cuda_fail(h, e);
+    if (!off && (unsigned)max_events != h->ev_cap) {
+        cudaFree(h->d_events); h->d_events = nullptr; h->ev_cap = 0;
+        e = cudaMalloc((void**)&h->d_events, sizeof(Event) * (size_t)max_events);
+        if (e != cudaSuccess) { cudaGetLastError(); h->last_cuda_error = (int)e; h->thr_on = h->thr_off = 0.0f; return FILARK_ERR_ALLOC; }
+        h->ev_cap = (unsigned)max_events;
+    }
+    if (!h->d_n_events) {
+        e = cudaMalloc((void**)&h->d_n_events, sizeof(unsigned));
+        if (e != cudaSuccess) { cudaGetLastError(); h->last_cuda_error = (int)e; return FILARK_ERR_ALLOC; }
+    }
+    // no event pending, every channel off
+    e = cudaMemset(h->d_n_events, 0, sizeof(unsigned));
+    const int ns = state_floats(h->n_sec);
+    if (e == cudaSuccess)
+        e = cudaMemset2D(h->d_state + trig_word(h->n_sec), sizeof(float) * (size_t)ns, 0, sizeof(float) * kTrigWords, (size_t)h->n_ch);
+    if (e != cudaSuccess) return cuda_fail(h, e);
+    h->thr_on = off ? 0.0f : thr_on; h->thr_off = off ? 0.0f : thr_off;
+    return FILARK_OK;
+}
+
+filark_status_t filark_stream_pop_events(filark_stream_t* h, filark_event_t* out, long long cap, long long* n_out,
+                                         long long* n_dropped, cudaStream_t stream)
+{
+    if (!h || !n_out || cap < 0 || (cap > 0 && !out)) return FILARK_ERR_INVALID_ARG;
+    *n_out = 0;
+    if (n_dropped) *n_dropped = 0;
+    if (!h->d_n_events) return FILARK_OK;                      // no trigger was ever set
+    filark_status_t st = check_device(h);
+    if (st != FILARK_OK) return st;
+    cudaError_t e = cudaStreamSynchronize(stream);
+    unsigned n = 0;
+    if (e == cudaSuccess) e = cudaMemcpy(&n, h->d_n_events, sizeof(n), cudaMemcpyDeviceToHost);
+    if (e != cudaSuccess) return cuda_fail(h, e);
+    const unsigned kept = n < h->ev_cap ? n : h->ev_cap;
+    *n_out = (long long)kept;
+    if (n_dropped) *n_dropped = (long long)(n - kept);
+    if ((long long)kept > cap) return FILARK_ERR_INVALID_ARG;   // nothing consumed: call again with room for *n_out events
+    static_assert(sizeof(filark_event_t) == sizeof(Event), "event record");
+    if (kept) e = cudaMemcpy(out, h->d_events, sizeof(Event) * (size_t)kept, cudaMemcpyDeviceToHost);
+    if (e == cudaSuccess) e = cudaMemset(h->d_n_events, 0, sizeof(unsigned));
+    if (e != cudaSuccess) return cuda_fail(h, e);
     return FILARK_OK;
 }
 

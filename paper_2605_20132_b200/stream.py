@@ -26,6 +26,7 @@ STATUS_NAMES = {0: "FILARK_OK", 1: "FILARK_ERR_INVALID_ARG", 2: "FILARK_ERR_UNST
                 6: "FILARK_ERR_ALIGNMENT"}
 
 _lib = None
+EVENT_DTYPE = np.dtype([("t_on", "<i8"), ("t_off", "<i8"), ("channel", "<i4"), ("peak", "<f4")])   # filark_event_t
 
 
 class FilarkError(RuntimeError):
@@ -69,6 +70,10 @@ def load_library():
     lib.filark_stream_set_state.argtypes = [vp, vp, ll, vp]
     lib.filark_stream_set_initial_condition.restype = ci
     lib.filark_stream_set_initial_condition.argtypes = [vp, vp, vp]
+    lib.filark_stream_set_trigger.restype = ci
+    lib.filark_stream_set_trigger.argtypes = [vp, ctypes.c_float, ctypes.c_float, ll, vp]
+    lib.filark_stream_pop_events.restype = ci
+    lib.filark_stream_pop_events.argtypes = [vp, vp, ll, ctypes.POINTER(ll), ctypes.POINTER(ll), vp]
     lib.filark_stream_reset.restype = ci
     lib.filark_stream_reset.argtypes = [vp, vp]
     lib.filark_stream_destroy.restype = ci
@@ -200,6 +205,22 @@ class FilarkStream:
     def reset(self, stream: Optional[int] = None):
         self._check(self._lib.filark_stream_reset(self._h, _cur_stream() if stream is None else stream),
                     "filark_stream_reset")
+
+    def set_trigger(self, thr_on: float, thr_off: float, max_events: int = 1 << 20, stream: Optional[int] = None):
+        self._check(self._lib.filark_stream_set_trigger(self._h, float(thr_on), float(thr_off), int(max_events),
+                                                        _cur_stream() if stream is None else stream),
+                    "filark_stream_set_trigger")
+        self._ev_cap = int(max_events)
+
+    def pop_events(self, stream: Optional[int] = None):
+        """(events as a numpy record array (t_on, t_off, channel, peak), number dropped)."""
+        cap = getattr(self, "_ev_cap", 0)
+        out = np.zeros(max(cap, 1), dtype=EVENT_DTYPE)
+        n, d = ctypes.c_longlong(0), ctypes.c_longlong(0)
+        self._check(self._lib.filark_stream_pop_events(self._h, out.ctypes.data, cap, ctypes.byref(n), ctypes.byref(d),
+                                                       _cur_stream() if stream is None else stream),
+                    "filark_stream_pop_events")
+        return out[:n.value].copy(), int(d.value)
 
     def get_state(self, stream: Optional[int] = None) -> bytes:
         """filark_stream_get_state: the documented state blob (host bytes)."""

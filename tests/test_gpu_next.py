@@ -122,3 +122,114 @@ def test_steady_state_initial_condition(cuda_device, name):
     assert (num <= 1e-4 * den + 5e-7 * np.abs(level) * np.sqrt(n_t)).all()
     assert_parity(c, ref_c, f"{name} cf with initial condition")
     s.destroy()
+
+
+# ---- NEXT-1: trigger / event emission on the CF ------------------------------------------------
+from oracle import OracleTrigger  # noqa: E402
+
+
+def _burst_record(n_ch, n_t, seed, n_bursts=60):
+    """cfg3-shaped noise with short strong bursts at random (time, channel): the CF rises steeply
+    through the thresholds (few ties) and falls back slowly."""
+    w = CONFIGS["cfg3"].scaled(n_ch=n_ch, n_t=n_t)
+    x = generate(w, device="cpu").numpy().copy()
+    rng = np.random.default_rng(seed)
+    for _ in range(n_bursts):
+        c = int(rng.integers(0, n_ch)); t = int(rng.integers(8000, n_t - 400)); n = int(rng.integers(40, 300))
+        x[c, t:t + n] += (rng.uniform(6.0, 15.0) * np.sin(2 * np.pi * rng.uniform(20, 120) / 1500.0 * np.arange(n))).astype(np.float32)
+    return w, x
+
+
+def _oracle_events(x, sos, w, thr_on, thr_off):
+    ref_f, ref_c = run_oracle(x, sos, w.sta_len, w.lta_len)
+    t = OracleTrigger(x.shape[0], thr_on, thr_off)
+    ev = t.push(ref_c)
+    t.close()
+    return ref_c, np.sort(ev, order=["channel", "t_on"])
+
+
+def _compare_events(got, ref, ref_cf, thr_on, thr_off, what):
+    """Bit-exact (channel, t_on, t_off) away from threshold ties.  Tie rule (R24): an event
+    boundary may differ between the two sides only where the oracle's cf is within 1e-4 (relative) of
+    the threshold it is compared with at one of the two boundary samples."""
+    got = np.sort(got, order=["channel", "t_on"])
+    key = lambda e: (int(e["channel"]), int(e["t_on"]), int(e["t_off"]))
+    gs, rs = {key(e): e for e in got}, {key(e): e for e in ref}
+    assert len(rs) >= 20, f"{what}: only {len(rs)} events in the reference: the case tests nothing"
+    same = set(gs) & set(rs)
+    for k in same:
+        assert abs(float(gs[k]["peak"]) - float(rs[k]["peak"])) <= 1e-4 * float(rs[k]["peak"]), (what, k)
+
+    def tie(c, t, thr):
+        return any(0 <= u < ref_cf.shape[1] and abs(float(ref_cf[c, u]) - thr) <= 1e-4 * thr for u in (t - 1, t, t + 1))
+    odd = (set(gs) ^ set(rs))
+    for c, a, b in odd:
+        assert tie(c, a, thr_on) or tie(c, b, thr_off), f"{what}: event {(c, a, b)} differs away from a tie"
+    assert len(odd) <= max(2, len(rs) // 10), f"{what}: {len(odd)} of {len(rs)} events differ"
+    return len(same)
+
+
+@pytest.mark.parametrize("layout", [CHANNEL_MAJOR, TIME_MAJOR])
+@pytest.mark.parametrize("sizes,many", [([60_000], False), ([1500], False), ([1500], True), ([777, 4096, 33, 2500], True)])
+def test_trigger_events_match_the_oracle(cuda_device, layout, sizes, many):
+    thr_on, thr_off = 3.0, 1.5
+    w, x = _burst_record(96, 60_000, 31)
+    sos = design_sos(w)
+    ref_cf, ref_ev = _oracle_events(x, sos, w, thr_on, thr_off)
+    xd = torch.from_numpy(x if layout == CHANNEL_MAJOR else np.ascontiguousarray(x.T)).to(cuda_device)
+    s = FilarkStream(w.n_ch, sos, w.sta_len, w.lta_len, layout)
+    s.set_trigger(thr_on, thr_off, 10_000)
+    bounds = split(w.n_t, sizes)
+    cut = (lambda a, b: xd[:, a:b].contiguous()) if layout == CHANNEL_MAJOR else (lambda a, b: xd[a:b, :].contiguous())
+    chunks = [cut(a, b) for a, b in bounds]
+    cfs = [torch.empty_like(c) for c in chunks]
+    if many:
+        s.push_many(chunks, None, cfs)
+    else:
+        for c, o in zip(chunks, cfs):
+            s.push(c, None, o)
+    got, dropped = s.pop_events()
+    assert dropped == 0
+    n_same = _compare_events(got, ref_ev, ref_cf, thr_on, thr_off, f"layout {layout} {sizes} many={many}")
+    assert n_same >= 20
+    # the list is empty now; the same record again after reset gives the same events again
+    again, _ = s.pop_events()
+    assert len(again) == 0
+    s.reset()
+    s.push_many(chunks, None, cfs)
+    got2, _ = s.pop_events()
+    assert np.array_equal(np.sort(got2, order=["channel", "t_on"]), np.sort(got, order=["channel", "t_on"]))
+    s.destroy()
+
+
+def test_trigger_without_cf_output_and_list_overflow(cuda_device):
+    """Events only (d_cf = NULL, filt kept): same events; a short list drops and counts the rest;
+    thr_on = thr_off = 0 switches the trigger off; a pop with too little room consumes nothing."""
+    thr_on, thr_off = 3.0, 1.5
+    w, x = _burst_record(64, 40_000, 41, n_bursts=40)
+    sos = design_sos(w)
+    ref_cf, ref_ev = _oracle_events(x, sos, w, thr_on, thr_off)
+    xd = torch.from_numpy(x).to(cuda_device)
+    f = torch.empty_like(xd)
+    s = FilarkStream(w.n_ch, sos, w.sta_len, w.lta_len)
+    s.set_trigger(thr_on, thr_off, 5000)
+    s.push(xd, f, None)
+    got, dropped = s.pop_events()
+    _compare_events(got, ref_ev, ref_cf, thr_on, thr_off, "events only")
+    n_all = len(got)
+    s.reset(); s.set_trigger(thr_on, thr_off, 7)
+    s.push(xd, f, None)
+    s._ev_cap = 3
+    with pytest.raises(FilarkError):
+        s.pop_events()                                       # room for 3, 7 pending: nothing consumed
+    s._ev_cap = 7
+    got, dropped = s.pop_events()
+    assert len(got) == 7 and dropped == n_all - 7
+    s.reset(); s.set_trigger(0.0, 0.0, 0)
+    s.push(xd, f, None)
+    got, dropped = s.pop_events()
+    assert len(got) == 0 and dropped == 0
+    for bad in ((2.0, 3.0, 10), (-1.0, 0.5, 10), (3.0, 1.0, 0)):
+        with pytest.raises(FilarkError):
+            s.set_trigger(*bad)
+    s.destroy()
