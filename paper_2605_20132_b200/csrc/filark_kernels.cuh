@@ -757,6 +757,11 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
     const bool out_hi = ((q - 1) & 1) != 0;
 
     const unsigned wst_sa = smem_addr(wst);
+    // (a running address for the carried state of the sections.  The section index k must not be needed in a
+    // vector register: where it was -- as k-dependent shared-memory address -- ptxas kept the loop counter
+    // in a vector register in some instantiations and then indexed every table per lane, with register
+    // operands instead of uniform ones in all FFMA2 of the section loop: -30 %)
+    unsigned sec_sa = wst_sa;
     // ---- S1..S3 per section -------------------------------------------------------------------
     const int pf_part = kTM ? (Geo<L>::tile / 32 + p.n_sec - 1) / p.n_sec : 0;
     for (int k = 0; k < p.n_sec; ++k) {
@@ -779,7 +784,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
         }
         // S2: lane total W = P a + b (a, b: end states of the lo / hi slot from rest); the carried
         // state S enters lane 0's total through A^2L; inclusive scan over the lanes
-        const float2 S = lds_f2(wst_sa + 8u * (unsigned)k);
+        const float2 S = lds_f2(sec_sa);
         const float P0 = T.P[0], P1 = T.P[1], P2 = T.P[2], P3 = T.P[3];
         float W1 = fmaf(P0, s1.x, fmaf(P1, s2.x, s1.y)), W2 = fmaf(P2, s1.x, fmaf(P3, s2.x, s2.y));
         {
@@ -809,7 +814,8 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
         const float o1 = fmaf(P0, E1, fmaf(P1, E2, s1.x)), o2 = fmaf(P2, E1, fmaf(P3, E2, s2.x));   // ... its hi slot
         const float n1 = __shfl_sync(0xffffffffu, out_hi ? W1 : o1, jl);
         const float n2 = __shfl_sync(0xffffffffu, out_hi ? W2 : o2, jl);
-        if (lane == 0 && !keep) sts_f2(wst_sa + 8u * (unsigned)k, make_float2(n1, n2));
+        if (lane == 0 && !keep) sts_f2(sec_sa, make_float2(n1, n2));
+        sec_sa += 8u;
         // S3 fix-up: y[i] += g1[i] s1 + g2[i] s2
         const float2 Ea = make_float2(E1, o1), Eb = make_float2(E2, o2);
         // (two rows per 16-byte uniform load: the tables are 16-byte aligned in the parameter bank)
@@ -848,7 +854,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
         sp = fma2(as, sp, e); lp = fma2(al, lp, e);
     }
     const int ks = wst + 2 * p.n_sec;
-    const float2 M = lds_f2(wst_sa + 8u * (unsigned)p.n_sec);                  // carried (sta~, lta~)
+    const float2 M = lds_f2(sec_sa);                                           // carried (sta~, lta~)
     const float bLs = p.avg.betaL[0], bLl = p.avg.betaL[1];
     float Ws = sp.y + fmaf(-bLs, sp.x, sp.x), Wl = lp.y + fmaf(-bLl, lp.x, lp.x);        // alpha^L lo + hi
     {
@@ -866,7 +872,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
     const float Os = sp.x + fmaf(-bLs, Es, Es), Ol = lp.x + fmaf(-bLl, El, El);          // carry-in of the hi slot
     const float Ns = __shfl_sync(0xffffffffu, out_hi ? Ws : Os, jl);
     const float Nl = __shfl_sync(0xffffffffu, out_hi ? Wl : Ol, jl);
-    if (lane == 0 && !keep) sts_f2(wst_sa + 8u * (unsigned)p.n_sec, make_float2(Ns, Nl));
+    if (lane == 0 && !keep) sts_f2(sec_sa, make_float2(Ns, Nl));
 
     // Last tile of a work item: the carried state is final here.  It goes back to global memory
     // now, and `progress` is released after the ratio loop below: the fence of the release waits for
