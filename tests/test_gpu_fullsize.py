@@ -142,3 +142,56 @@ def test_cfg3_full_size_back_to_back_pushes(cuda_device):
     assert all(v == sums[FLAG_STRICT_ORDER][0] for v in sums[FLAG_OVERLAP_PUSHES]), sums
     assert_parity(torch.cat([f[chans] for f in fs], 1).cpu().numpy(), ref_f, "back-to-back filt")
     assert_parity(torch.cat([c[chans] for c in cs], 1).cpu().numpy(), ref_c, "back-to-back cf")
+
+
+# ---- every config at its FULL shape, in the launch configuration bench.py times (push_many) ------
+# (>= 64 sampled channels against the oracle; properties that hold at any size on all channels; a
+# regression guard a decade below the north-star bound: the measured errors are about 1e-6)
+GUARD_REL_L2 = 1e-5
+
+
+def _full_shape(cuda_device, name, layout):
+    from paper_2605_20132_b200.stream import FilarkStream
+    w = CONFIGS[name]
+    sos = design_sos(w)
+    sched = push_schedule(w)
+    x = generate(w, device=cuda_device)                       # [n_ch][n_t]
+    rng = np.random.default_rng(100 + int(name[3:]))
+    chans = sorted(set([0, 1, 15, 16, 147, 148, w.n_ch // 2, w.n_ch - 2, w.n_ch - 1] + rng.integers(0, w.n_ch, 64).tolist()))
+    assert len(chans) >= 64
+    xs = x[chans].cpu().numpy()
+    ins, p = [], 0
+    for c in sched:
+        blk = x[:, p:p + c]
+        ins.append(blk.contiguous() if layout == CHANNEL_MAJOR else blk.t().contiguous()); p += c
+    del x
+    fs = [torch.empty_like(t) for t in ins]; cs = [torch.empty_like(t) for t in ins]
+    s = FilarkStream(w.n_ch, sos, w.sta_len, w.lta_len, layout)
+    s.push_many(ins, fs, cs)
+    torch.cuda.synchronize()
+    assert s.launch_count == -(-len(sched) // 64)
+    assert s.samples_pushed == w.n_t
+    if layout == CHANNEL_MAJOR:
+        f = torch.cat([t[chans] for t in fs], 1).cpu().numpy(); c = torch.cat([t[chans] for t in cs], 1).cpu().numpy()
+    else:
+        f = torch.cat([t[:, chans] for t in fs], 0).t().contiguous().cpu().numpy()
+        c = torch.cat([t[:, chans] for t in cs], 0).t().contiguous().cpu().numpy()
+    ok = all(bool(torch.isfinite(t).all()) for t in fs + cs)
+    cmax = max(float(t.max()) for t in cs); cmin = min(float(t.min()) for t in cs)
+    s.destroy()
+    del ins, fs, cs
+    torch.cuda.empty_cache()
+    ref_f, ref_c = run_oracle(xs, sos, w.sta_len, w.lta_len, threads=16)     # the WHOLE-record oracle
+    r_f = assert_parity(f, ref_f, f"{name} full-shape filt")
+    r_c = assert_parity(c, ref_c, f"{name} full-shape cf")
+    print("%s %s full shape (%d pushes): filt rel-L2 %.2e max %.2e; cf rel-L2 %.2e max %.2e" % ((name, layout, len(sched)) + r_f + r_c))
+    assert r_f[0] <= GUARD_REL_L2 and r_c[0] <= GUARD_REL_L2 * 3, (r_f, r_c)
+    assert ok and cmin >= 0.0 and cmax <= w.lta_len / w.sta_len * (1 + 1e-5)
+
+
+@pytest.mark.parametrize("name,layout", [("cfg2", CHANNEL_MAJOR), ("cfg3", CHANNEL_MAJOR), ("cfg3", TIME_MAJOR),
+                                         ("cfg4", CHANNEL_MAJOR), ("cfg5", CHANNEL_MAJOR)])
+def test_full_shape_push_many_against_whole_record_oracle(cuda_device, name, layout):
+    """BASELINE.json configs[1..4] at full size (cfg5: 6,000 x 900,000 in its 292 random-length pushes,
+    65 GB resident; "must match the whole-record oracle")."""
+    _full_shape(cuda_device, name, layout)
