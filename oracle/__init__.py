@@ -3,4 +3,5 @@
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
 legs may import this package.  It imports nothing from paper_2605_20132_b200.
 """
-from .oracle import EVENT_DTYPE, Oracle, OracleTrigger, build_oracle, oracle_lib_path  # noqa: F401
+from .oracle import (EVENT_DTYPE, Oracle, OracleEma, OracleTrigger, build_oracle, oracle_decimate,  # noqa: F401
+                     oracle_lib_path)

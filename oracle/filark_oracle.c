@@ -351,3 +351,101 @@ long long filark_oracle_trigger_push(filark_oracle_trigger_t *t, const float *cf
     t->g += n_t;
     return n_ev;
 }
+
+/*
+ * Display decimation ("logical downsampling is applied to match
+ * the display resolution ... drop mode preserves transient peaks, peak mode maintains amplitude
+ * envelopes, and linear interpolation smooths slowly varying wavefields").  The paper gives no
+ * formula; reading R25: a window of n_t samples per channel goes to `width` display
+ * columns; column j covers the input positions [a_j, a_{j+1}), a_j = floor(j n_t / width)
+ * (at least one sample: if a_{j+1} == a_j the column takes sample a_j):
+ *     mode 0 "drop":   out[j] = x[a_j]                         (plain striding)
+ *     mode 1 "peak":   out[j] = the sample of largest magnitude in the column, the first one on
+ *                      ties, with its sign
+ *     mode 2 "linear": out[j] = x at position p_j = j (n_t - 1) / (width - 1) (p_0 = 0 for width 1)
+ *                      by linear interpolation between the two neighbouring samples, in double
+ * Element (c, n) of x at c*stride_c + n*stride_n; out: element (c, j) at c*ostride_c + j*ostride_j.
+ */
+int filark_oracle_decimate(const float *x, int n_ch, long long n_t, long long stride_c, long long stride_n,
+                           int mode, int width, float *out, long long ostride_c, long long ostride_j)
+{
+    if (!x || !out || n_ch <= 0 || n_t <= 0 || width <= 0 || mode < 0 || mode > 2) return 1;
+    for (int c = 0; c < n_ch; ++c) {
+        const float *row = x + (long long)c * stride_c;
+        for (int j = 0; j < width; ++j) {
+            /* floor(j n_t / width) without overflow for the sizes used here (< 2^62) */
+            long long a = (long long)j * n_t / width, b = (long long)(j + 1) * n_t / width;
+            if (b <= a) b = a + 1;
+            if (b > n_t) b = n_t;
+            float v;
+            if (mode == 0) {
+                v = row[a * stride_n];
+            } else if (mode == 1) {
+                v = row[a * stride_n];
+                float best = v < 0.0f ? -v : v;
+                for (long long n = a + 1; n < b; ++n) {
+                    const float s = row[n * stride_n];
+                    const float m = s < 0.0f ? -s : s;
+                    if (m > best) { best = m; v = s; }
+                }
+            } else {
+                const double p = width > 1 ? (double)j * (double)(n_t - 1) / (double)(width - 1) : 0.0;
+                long long i = (long long)p;
+                if (i > n_t - 1) i = n_t - 1;
+                const double f = p - (double)i;
+                const double x0 = (double)row[i * stride_n];
+                const double x1 = (double)row[(i + 1 < n_t ? i + 1 : i) * stride_n];
+                v = (float)(x0 + (x1 - x0) * f);
+            }
+            out[(long long)c * ostride_c + (long long)j * ostride_j] = v;
+        }
+    }
+    return 0;
+}
+
+/*
+ * Streaming first-order operators ("running automatic gain control
+ * (AGC), running mean ... (all with stateful streaming variants)", :122 "gain equalisation (streaming
+ * exponential moving average, EMA variant)").  The paper gives no formula; reading R26: the
+ * exponential-average forms, state carried across pushes, zero at create/reset:
+ *     m[n] = m[n-1] + (u[n] - m[n-1]) / N
+ *     mode 0 "running mean":   u = x,    out = m                      (the EMA itself)
+ *     mode 1 "de-mean":        u = x,    out = x - m                  (running mean removed)
+ *     mode 2 "running AGC":    u = |x|,  out = x / (m + eps)          (gain from the average magnitude)
+ */
+typedef struct filark_oracle_ema {
+    int n_ch, n_len, mode;
+    double eps;
+    double *m;
+} filark_oracle_ema_t;
+
+filark_oracle_ema_t *filark_oracle_ema_create(int n_ch, int n_len, int mode, double eps)
+{
+    if (n_ch <= 0 || n_len < 1 || mode < 0 || mode > 2 || !(eps >= 0.0)) return NULL;
+    filark_oracle_ema_t *o = (filark_oracle_ema_t *)calloc(1, sizeof(*o));
+    if (!o) return NULL;
+    o->n_ch = n_ch; o->n_len = n_len; o->mode = mode; o->eps = eps;
+    o->m = (double *)calloc((size_t)n_ch, sizeof(double));
+    if (!o->m) { free(o); return NULL; }
+    return o;
+}
+void filark_oracle_ema_destroy(filark_oracle_ema_t *o) { if (o) { free(o->m); free(o); } }
+
+int filark_oracle_ema_push(filark_oracle_ema_t *o, const float *x, long long n_t, long long stride_c,
+                           long long stride_n, float *out)
+{
+    if (!o || !x || !out || n_t < 0) return 1;
+    const double len = (double)o->n_len;
+    for (int c = 0; c < o->n_ch; ++c) {
+        double m = o->m[c];
+        for (long long n = 0; n < n_t; ++n) {
+            const long long idx = (long long)c * stride_c + n * stride_n;
+            const double v = (double)x[idx];
+            const double u = o->mode == 2 ? (v < 0.0 ? -v : v) : v;
+            m = m + (u - m) / len;
+            out[idx] = (float)(o->mode == 0 ? m : (o->mode == 1 ? v - m : v / (m + o->eps)));
+        }
+        o->m[c] = m;
+    }
+    return 0;
+}

@@ -72,6 +72,14 @@ def _load():
     lib.filark_oracle_get_state.argtypes = [vp, vp, vp]
     lib.filark_oracle_set_state.restype = ci
     lib.filark_oracle_set_state.argtypes = [vp, vp, ll]
+    lib.filark_oracle_decimate.restype = ci
+    lib.filark_oracle_decimate.argtypes = [vp, ci, ll, ll, ll, ci, ci, vp, ll, ll]
+    lib.filark_oracle_ema_create.restype = vp
+    lib.filark_oracle_ema_create.argtypes = [ci, ci, ci, ctypes.c_double]
+    lib.filark_oracle_ema_destroy.restype = None
+    lib.filark_oracle_ema_destroy.argtypes = [vp]
+    lib.filark_oracle_ema_push.restype = ci
+    lib.filark_oracle_ema_push.argtypes = [vp, vp, ll, ll, ll, vp]
     lib.filark_oracle_trigger_create.restype = vp
     lib.filark_oracle_trigger_create.argtypes = [ci, ctypes.c_float, ctypes.c_float]
     lib.filark_oracle_trigger_destroy.restype = None
@@ -207,6 +215,54 @@ class OracleTrigger:
     def close(self):
         if getattr(self, "_h", None):
             self._lib.filark_oracle_trigger_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+
+DECIMATE_MODES = {"drop": 0, "peak": 1, "linear": 2}
+EMA_MODES = {"mean": 0, "demean": 1, "agc": 2}
+
+
+def oracle_decimate(x: np.ndarray, mode: str, width: int, layout: int = CHANNEL_MAJOR) -> np.ndarray:
+    """Display decimation (NEXT-4, reading R25).  x: [n_ch][n_t] or [n_t][n_ch]; returns [n_ch][width] or [width][n_ch]."""
+    lib = _load()
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    if layout == CHANNEL_MAJOR:
+        n_ch, n_t = x.shape
+        out = np.empty((n_ch, width), dtype=np.float32)
+        rc = lib.filark_oracle_decimate(x.ctypes.data, n_ch, n_t, n_t, 1, DECIMATE_MODES[mode], width, out.ctypes.data, width, 1)
+    else:
+        n_t, n_ch = x.shape
+        out = np.empty((width, n_ch), dtype=np.float32)
+        rc = lib.filark_oracle_decimate(x.ctypes.data, n_ch, n_t, 1, n_ch, DECIMATE_MODES[mode], width, out.ctypes.data, 1, n_ch)
+    if rc:
+        raise ValueError("filark_oracle_decimate rejected its arguments")
+    return out
+
+
+class OracleEma:
+    """Streaming first-order operators (NEXT-3, reading R26): running mean, de-mean, running AGC."""
+
+    def __init__(self, n_ch: int, n_len: int, mode: str, eps: float = 0.0, layout: int = CHANNEL_MAJOR):
+        lib = _load()
+        self._lib, self.n_ch, self.layout = lib, int(n_ch), int(layout)
+        self._h = lib.filark_oracle_ema_create(self.n_ch, int(n_len), EMA_MODES[mode], float(eps))
+        if not self._h:
+            raise ValueError("filark_oracle_ema_create rejected its arguments")
+
+    def push(self, x: np.ndarray) -> np.ndarray:
+        x = np.ascontiguousarray(x, dtype=np.float32)
+        n_t = x.shape[1] if self.layout == CHANNEL_MAJOR else x.shape[0]
+        sc, sn = (n_t, 1) if self.layout == CHANNEL_MAJOR else (1, self.n_ch)
+        out = np.empty_like(x)
+        if self._lib.filark_oracle_ema_push(self._h, x.ctypes.data, n_t, sc, sn, out.ctypes.data):
+            raise RuntimeError("oracle ema push failed")
+        return out
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.filark_oracle_ema_destroy(self._h)
             self._h = None
 
     __del__ = close

@@ -172,3 +172,70 @@ def test_trigger_against_brute_force_on_random_cf():
     for e, (c, a, b, pk) in zip(ev, exp):
         assert (int(e["channel"]), int(e["t_on"]), int(e["t_off"])) == (c, a, b) and e["peak"] == pk
     t.close()
+
+
+# ---- NEXT-4: display decimation (reading R25) --------------------------------------------------
+from oracle import OracleEma, oracle_decimate  # noqa: E402
+from oracle.oracle import TIME_MAJOR as _TM  # noqa: E402
+
+
+def test_decimate_small_worked_example():
+    """10 samples to 4 columns: columns [0,2) [2,5) [5,7) [7,10)."""
+    x = np.array([[1, -3, 2, 2, -2, 0.5, -0.5, 4, -9, 9]], dtype=np.float32)
+    assert oracle_decimate(x, "drop", 4).tolist() == [[1.0, 2.0, 0.5, 4.0]]
+    assert oracle_decimate(x, "peak", 4).tolist() == [[-3.0, 2.0, 0.5, -9.0]]         # first of equal magnitudes
+    lin = oracle_decimate(x, "linear", 4)[0]
+    assert np.allclose(lin, [1.0, 2.0, -0.5, 9.0])                                      # positions 0, 3, 6, 9
+    assert np.allclose(oracle_decimate(x, "linear", 3)[0], [1.0, (-2 + 0.5) / 2, 9.0])  # positions 0, 4.5, 9
+
+
+@pytest.mark.parametrize("n_t,width", [(1000, 128), (2048, 2048), (100, 300), (90_000, 2048), (7, 1)])
+def test_decimate_against_numpy(n_t, width):
+    rng = np.random.default_rng(n_t + width)
+    x = rng.standard_normal((3, n_t)).astype(np.float32)
+    a = (np.arange(width + 1, dtype=np.int64) * n_t) // width
+    lo, hi = a[:-1], np.maximum(a[1:], a[:-1] + 1)
+    assert np.array_equal(oracle_decimate(x, "drop", width), x[:, lo])
+    pk = oracle_decimate(x, "peak", width)
+    for c in range(3):
+        for j in (0, width // 3, width - 1):
+            seg = x[c, lo[j]:hi[j]]
+            assert pk[c, j] == seg[np.argmax(np.abs(seg))]
+    assert (np.abs(pk) >= np.abs(x[:, lo])).all()                       # the envelope is never below the dropped sample
+    ref = np.stack([np.interp(np.linspace(0, n_t - 1, width) if width > 1 else [0.0], np.arange(n_t), x[c].astype(np.float64)) for c in range(3)])
+    assert np.allclose(oracle_decimate(x, "linear", width), ref, rtol=1e-6, atol=1e-6)
+    # time-major input gives the transposed result
+    for mode in ("drop", "peak", "linear"):
+        assert np.array_equal(oracle_decimate(np.ascontiguousarray(x.T), mode, width, _TM).T, oracle_decimate(x, mode, width))
+
+
+# ---- NEXT-3: streaming first-order operators (reading R26) ------------------------------------
+def test_ema_operators_against_lfilter_and_closed_forms():
+    rng = np.random.default_rng(2)
+    x = (rng.standard_normal((2, 4000)) * 3.0 + 1.5).astype(np.float32)
+    N = 40
+    m = signal.lfilter([1.0 / N], [1.0, -(1.0 - 1.0 / N)], x.astype(np.float64), axis=1)
+    o = OracleEma(2, N, "mean"); assert np.allclose(o.push(x), m, rtol=1e-6, atol=1e-7); o.close()
+    o = OracleEma(2, N, "demean"); assert np.allclose(o.push(x), x - m, rtol=1e-5, atol=1e-6); o.close()
+    ma = signal.lfilter([1.0 / N], [1.0, -(1.0 - 1.0 / N)], np.abs(x.astype(np.float64)), axis=1)
+    o = OracleEma(2, N, "agc", 1e-3); assert np.allclose(o.push(x), x / (ma + 1e-3), rtol=1e-5); o.close()
+    # closed form: a constant input c gives m[n] = c (1 - (1 - 1/N)^(n+1))
+    c = np.full((1, 300), 2.5, dtype=np.float32)
+    o = OracleEma(1, N, "mean")
+    assert np.allclose(o.push(c)[0], 2.5 * (1 - (1 - 1 / N) ** (np.arange(300) + 1)), rtol=1e-6); o.close()
+    # AGC of a scaled input: the output does not change (eps = 0) once the average is non-zero
+    o1, o2 = OracleEma(2, N, "agc"), OracleEma(2, N, "agc")
+    assert np.allclose(o1.push(x), o2.push(8.0 * x), rtol=1e-6); o1.close(); o2.close()
+
+
+@pytest.mark.parametrize("mode", ["mean", "demean", "agc"])
+def test_ema_operators_are_chunk_invariant_bitwise(mode):
+    rng = np.random.default_rng(4)
+    x = rng.standard_normal((3, 2000)).astype(np.float32)
+    a = OracleEma(3, 25, mode, 1e-6); whole = a.push(x); a.close()
+    b = OracleEma(3, 25, mode, 1e-6)
+    parts, p = [], 0
+    for s in [1, 2, 3, 500, 31, 1463]:
+        parts.append(b.push(x[:, p:p + s])); p += s
+    b.close()
+    assert np.array_equal(np.concatenate(parts, 1), whole)
