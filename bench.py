@@ -513,6 +513,25 @@ def extra_runs(args, w, sos, stream, ins, filts, cfs, sched, torch, dev, peak, s
             return r
         guarded("trigger_both_outputs_and_events", lambda: with_trigger(True))
         guarded("trigger_filt_and_events_no_cf", lambda: with_trigger(False))
+
+    # ---- the two small operators beside the path (NEXT-3, NEXT-4; include/filark_ops.h): pure streaming work
+    if layout == CHANNEL_MAJOR and args.outputs == "both":
+        def small_ops():
+            from paper_2605_20132_b200.ops import FilarkEma, decimate
+            x = torch.cat(ins, dim=1).contiguous()
+            y = torch.empty_like(x)
+            out = {}
+            for mode in ("demean", "agc"):
+                h = FilarkEma(w.n_ch, w.lta_len, mode, 1e-6)
+                ms = _time(torch, lambda: h.push(x, y), 5, warm=1)
+                out[f"ema_{mode}"] = _row(n_samples, ms, peak, 8.0)
+                h.destroy()
+            for mode in ("drop", "peak", "linear"):
+                disp = torch.empty((w.n_ch, 2048), device=x.device)
+                ms = _time(torch, lambda: decimate(x, mode, 2048, CHANNEL_MAJOR, disp), 5, warm=1)
+                out[f"decimate_{mode}_to_2048"] = _row(n_samples, ms, peak, 4.0 if mode == "peak" else 4.0 * 2048 / w.n_t)
+            return out
+        guarded("small_operators", small_ops)
     return extra
 
 

@@ -11,10 +11,11 @@ import sys
 _PKG = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_PKG, "csrc")
 LIB_PATH = os.path.join(_PKG, "libfilark_stream.so")
-SOURCES = [os.path.join(_CSRC, "filark_stream.cu")]
+SOURCES = [os.path.join(_CSRC, "filark_stream.cu"), os.path.join(_CSRC, "filark_ops.cu")]
 DEPENDS = SOURCES + [os.path.join(_CSRC, "filark_kernels.cuh"), os.path.join(_CSRC, "design.hpp"),
                      os.path.join(os.path.dirname(_PKG), "include", "filark_stream.h"),
-                     os.path.join(os.path.dirname(_PKG), "include", "filark_debug.h")]
+                     os.path.join(os.path.dirname(_PKG), "include", "filark_debug.h"),
+                     os.path.join(os.path.dirname(_PKG), "include", "filark_ops.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--use_fast_math=false"]
 

@@ -1,0 +1,326 @@
+// filark_ops.cu -- the two small operators beside the stream path (include/filark_ops.h):
+// streaming first-order operators (running mean / de-mean / running AGC: SURVEY.md 8(f) NEXT-3,
+// PAPER.md:121-122, reading R26) and display decimation (NEXT-4, reading R25).
+// Both are pure streaming work: one read of the input, one write of the output.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdint>
+#include <new>
+
+#include "../../include/filark_ops.h"
+
+namespace {
+
+// ---------------------------------------------------------------------------------------------
+// NEXT-3.  m[n] = alpha m[n-1] + c u[n], alpha = 1 - 1/N, c = 1/N: the same blocked scan as the
+// STA/LTA averages of the stream kernel.  Channel-major: one warp per channel, a tile is 32 lanes x K
+// contiguous samples; zero-state pass per lane, carry over the lanes by a 5-step shuffle scan with
+// the constants alpha^(K 2^d), fix-up m[i] += alpha^(i+1) m_in.  Tiles go through shared memory both
+// ways so that global accesses are coalesced (lane regions K + 1 floats apart: no bank conflicts).
+constexpr int kEmaK = 16;
+constexpr int kEmaWarps = 8;
+struct EmaParams {
+    const float* in;
+    float* out;
+    float* state;
+    long long n_t;
+    int n_ch, mode;
+    float alpha, c, eps;
+    float apow[kEmaK];       // alpha^(i+1)
+    float aq[5];             // alpha^(K 2^d)
+};
+
+__device__ __forceinline__ float ema_out(int mode, float x, float m, float eps)
+{
+    return mode == FILARK_EMA_MEAN ? m : (mode == FILARK_EMA_DEMEAN ? x - m : __fdividef(x, m + eps));
+}
+
+__global__ void __launch_bounds__(kEmaWarps * 32) filark_ema_cm_kernel(const __grid_constant__ EmaParams p)
+{
+    constexpr int K = kEmaK, T = 32 * K;
+    __shared__ float sm[kEmaWarps][32 * (K + 1)];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    float* s = sm[warp];
+    for (int ch = blockIdx.x * kEmaWarps + warp; ch < p.n_ch; ch += gridDim.x * kEmaWarps) {
+        const float* __restrict__ row = p.in + (long long)ch * p.n_t;
+        float* __restrict__ orow = p.out + (long long)ch * p.n_t;
+        float carry = p.state[ch];
+        for (long long t0 = 0; t0 < p.n_t; t0 += T) {
+            const int n = (int)(p.n_t - t0 < T ? p.n_t - t0 : T);
+#pragma unroll
+            for (int j = 0; j < K; ++j) {
+                const int e = lane + 32 * j;
+                s[(e / K) * (K + 1) + e % K] = e < n ? row[t0 + e] : 0.0f;
+            }
+            __syncwarp();
+            float x[K], m[K];
+            float acc = 0.0f;
+#pragma unroll
+            for (int i = 0; i < K; ++i) {
+                x[i] = s[lane * (K + 1) + i];
+                const float u = p.mode == FILARK_EMA_AGC ? fabsf(x[i]) : x[i];
+                acc = fmaf(p.alpha, acc, p.c * u);
+                m[i] = acc;
+            }
+            float W = acc;
+            if (lane == 0) W = fmaf(p.aq[0], carry, W);
+#pragma unroll
+            for (int d = 0; d < 5; ++d) {
+                const float U = __shfl_up_sync(0xffffffffu, W, 1 << d);
+                if (lane >= (1 << d)) W = fmaf(p.aq[d], U, W);
+            }
+            float E = __shfl_up_sync(0xffffffffu, W, 1);
+            if (lane == 0) E = carry;
+            const int e_last = n - 1;
+            float mlast = 0.0f;
+#pragma unroll
+            for (int i = 0; i < K; ++i) {
+                m[i] = fmaf(p.apow[i], E, m[i]);
+                if (lane * K + i == e_last) mlast = m[i];
+                s[lane * (K + 1) + i] = ema_out(p.mode, x[i], m[i], p.eps);
+            }
+            carry = __shfl_sync(0xffffffffu, mlast, e_last / K);
+            __syncwarp();
+#pragma unroll
+            for (int j = 0; j < K; ++j) {
+                const int e = lane + 32 * j;
+                if (e < n) orow[t0 + e] = s[(e / K) * (K + 1) + e % K];
+            }
+            __syncwarp();
+        }
+        if (lane == 0) p.state[ch] = carry;
+    }
+}
+
+// Time-major: adjacent threads are adjacent channels (coalesced rows), each thread runs its channel
+// serially in time: no scan is needed, the recurrence is one FMA per sample.
+__global__ void __launch_bounds__(128) filark_ema_tm_kernel(const __grid_constant__ EmaParams p)
+{
+    const int ch = blockIdx.x * blockDim.x + threadIdx.x;
+    if (ch >= p.n_ch) return;
+    float m = p.state[ch];
+    for (long long t = 0; t < p.n_t; ++t) {
+        const float x = p.in[t * p.n_ch + ch];
+        const float u = p.mode == FILARK_EMA_AGC ? fabsf(x) : x;
+        m = fmaf(p.c, u - m, m);                  // (unit DC gain whatever the rounding of 1/N: the error of a
+                                                  // rounded alpha would add up over the N samples of the memory)
+        p.out[t * p.n_ch + ch] = ema_out(p.mode, x, m, p.eps);
+    }
+    p.state[ch] = m;
+}
+
+// ---------------------------------------------------------------------------------------------
+// NEXT-4.  Column j of a channel covers input samples [a_j, a_{j+1}), a_j = floor(j n_t / width).
+struct DecParams {
+    const float* in;
+    float* out;
+    long long n_t, pitch;
+    int n_ch, width, mode;
+};
+__device__ __forceinline__ long long col_start(long long j, long long n_t, int width) { return j * n_t / width; }
+
+__device__ __forceinline__ float lin_at(const float* row, long long stride, long long n_t, int j, int width)
+{
+    const double pos = width > 1 ? (double)j * (double)(n_t - 1) / (double)(width - 1) : 0.0;
+    long long i = (long long)pos;
+    if (i > n_t - 1) i = n_t - 1;
+    const float f = (float)(pos - (double)i);
+    const float x0 = row[i * stride], x1 = row[(i + 1 < n_t ? i + 1 : i) * stride];
+    return fmaf(x1 - x0, f, x0);
+}
+
+// Channel-major: grid (column groups, channels).  Narrow columns (<= 32 samples): one thread per column
+// (a warp reads 32 adjacent columns: one contiguous stretch of the row).  Wide columns: one warp per
+// column, lanes stride through it (coalesced), the largest magnitude -- the first one on ties -- by a
+// shuffle reduction on (magnitude, position).
+__global__ void __launch_bounds__(128) filark_decimate_cm_kernel(const __grid_constant__ DecParams p)
+{
+    const int ch = blockIdx.y;
+    const float* __restrict__ row = p.in + (long long)ch * p.pitch;
+    float* __restrict__ orow = p.out + (long long)ch * p.width;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const bool narrow = p.n_t <= 32LL * p.width;
+    if (p.mode != FILARK_DECIMATE_PEAK || narrow) {
+        const int j = blockIdx.x * blockDim.x + threadIdx.x;
+        if (j >= p.width) return;
+        const long long a = col_start(j, p.n_t, p.width);
+        float v;
+        if (p.mode == FILARK_DECIMATE_DROP) {
+            v = row[a];
+        } else if (p.mode == FILARK_DECIMATE_LINEAR) {
+            v = lin_at(row, 1, p.n_t, j, p.width);
+        } else {
+            long long b = col_start(j + 1, p.n_t, p.width);
+            if (b <= a) b = a + 1;
+            v = row[a];
+            float best = fabsf(v);
+            for (long long n = a + 1; n < b; ++n) {
+                const float s = row[n];
+                if (fabsf(s) > best) { best = fabsf(s); v = s; }
+            }
+        }
+        orow[j] = v;
+        return;
+    }
+    for (int j = blockIdx.x * 4 + warp; j < p.width; j += gridDim.x * 4) {
+        const long long a = col_start(j, p.n_t, p.width);
+        long long b = col_start(j + 1, p.n_t, p.width);
+        if (b <= a) b = a + 1;
+        float v = 0.0f, best = -1.0f;
+        long long at = b;
+        for (long long n = a + lane; n < b; n += 32) {
+            const float s = row[n];
+            if (fabsf(s) > best) { best = fabsf(s); v = s; at = n; }
+        }
+#pragma unroll
+        for (int d = 16; d > 0; d >>= 1) {
+            const float ob = __shfl_xor_sync(0xffffffffu, best, d), ov = __shfl_xor_sync(0xffffffffu, v, d);
+            const long long oa = __shfl_xor_sync(0xffffffffu, at, d);
+            if (ob > best || (ob == best && oa < at)) { best = ob; v = ov; at = oa; }
+        }
+        if (lane == 0) orow[j] = v;
+    }
+}
+
+// Time-major: adjacent threads are adjacent channels; a thread walks the samples of its columns in time.
+__global__ void __launch_bounds__(128) filark_decimate_tm_kernel(const __grid_constant__ DecParams p, int cols_per_block)
+{
+    const int ch = blockIdx.x * blockDim.x + threadIdx.x;
+    if (ch >= p.n_ch) return;
+    const float* __restrict__ col = p.in + ch;
+    const int j0 = blockIdx.y * cols_per_block, j1 = min(p.width, j0 + cols_per_block);
+    for (int j = j0; j < j1; ++j) {
+        const long long a = col_start(j, p.n_t, p.width);
+        float v;
+        if (p.mode == FILARK_DECIMATE_DROP) {
+            v = col[a * p.pitch];
+        } else if (p.mode == FILARK_DECIMATE_LINEAR) {
+            v = lin_at(col, p.pitch, p.n_t, j, p.width);
+        } else {
+            long long b = col_start(j + 1, p.n_t, p.width);
+            if (b <= a) b = a + 1;
+            v = col[a * p.pitch];
+            float best = fabsf(v);
+            for (long long n = a + 1; n < b; ++n) {
+                const float s = col[n * p.pitch];
+                if (fabsf(s) > best) { best = fabsf(s); v = s; }
+            }
+        }
+        p.out[(long long)j * p.n_ch + ch] = v;
+    }
+}
+
+}  // namespace
+
+struct filark_ema {
+    int device, n_ch, n_len, mode, layout;
+    float eps;
+    EmaParams proto;
+    float* d_state;
+    int n_sm;
+};
+
+extern "C" {
+
+filark_status_t filark_ema_create(filark_ema_t** out, int n_ch, int n_len, int mode, float eps, int layout)
+{
+    if (!out || n_ch <= 0 || n_len < 1 || mode < FILARK_EMA_MEAN || mode > FILARK_EMA_AGC || !(eps >= 0.0f) ||
+        !std::isfinite(eps) || (layout != FILARK_LAYOUT_CHANNEL_MAJOR && layout != FILARK_LAYOUT_TIME_MAJOR))
+        return FILARK_ERR_INVALID_ARG;
+    filark_ema* h = new (std::nothrow) filark_ema();
+    if (!h) return FILARK_ERR_ALLOC;
+    h->n_ch = n_ch; h->n_len = n_len; h->mode = mode; h->layout = layout; h->eps = eps;
+    cudaError_t e = cudaGetDevice(&h->device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device);
+    if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_state, sizeof(float) * (size_t)n_ch);
+    if (e == cudaSuccess) e = cudaMemset(h->d_state, 0, sizeof(float) * (size_t)n_ch);
+    if (e != cudaSuccess) {
+        const bool oom = e == cudaErrorMemoryAllocation;
+        cudaFree(h->d_state); delete h; cudaGetLastError();
+        return oom ? FILARK_ERR_ALLOC : FILARK_ERR_CUDA;
+    }
+    // constants in float64, rounded last: alpha^k = exp(k log1p(-1/N))
+    EmaParams& p = h->proto;
+    p = EmaParams{};
+    const double c = 1.0 / (double)n_len;
+    const double la = n_len > 1 ? std::log1p(-c) : -INFINITY;          // N = 1: alpha = 0
+    auto apow = [&](double k) { return n_len > 1 ? std::exp(k * la) : 0.0; };
+    p.n_ch = n_ch; p.mode = mode; p.eps = eps; p.alpha = (float)(1.0 - c); p.c = (float)c; p.state = h->d_state;
+    for (int i = 0; i < kEmaK; ++i) p.apow[i] = (float)apow(i + 1.0);
+    for (int d = 0; d < 5; ++d) p.aq[d] = (float)apow((double)kEmaK * (double)(1 << d));
+    *out = h;
+    return FILARK_OK;
+}
+
+filark_status_t filark_ema_push(filark_ema_t* h, const float* d_in, long long n_t, float* d_out, cudaStream_t stream)
+{
+    if (!h || n_t < 0) return FILARK_ERR_INVALID_ARG;
+    if (n_t == 0) return FILARK_OK;
+    if (!d_in || !d_out || n_t > 0x7fff0000LL) return FILARK_ERR_INVALID_ARG;
+    if (((uintptr_t)d_in | (uintptr_t)d_out) & 3u) return FILARK_ERR_ALIGNMENT;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return FILARK_ERR_CUDA;
+    if (dev != h->device) return FILARK_ERR_DEVICE_MISMATCH;
+    EmaParams p = h->proto;
+    p.in = d_in; p.out = d_out; p.n_t = n_t;
+    if (h->layout == FILARK_LAYOUT_CHANNEL_MAJOR) {
+        int grid = (h->n_ch + kEmaWarps - 1) / kEmaWarps;
+        const int cap = h->n_sm * 8;
+        if (grid > cap) grid = cap;
+        filark_ema_cm_kernel<<<grid, kEmaWarps * 32, 0, stream>>>(p);
+    } else {
+        filark_ema_tm_kernel<<<(h->n_ch + 127) / 128, 128, 0, stream>>>(p);
+    }
+    return cudaGetLastError() == cudaSuccess ? FILARK_OK : FILARK_ERR_CUDA;
+}
+
+filark_status_t filark_ema_reset(filark_ema_t* h, cudaStream_t stream)
+{
+    if (!h) return FILARK_ERR_INVALID_ARG;
+    return cudaMemsetAsync(h->d_state, 0, sizeof(float) * (size_t)h->n_ch, stream) == cudaSuccess ? FILARK_OK : FILARK_ERR_CUDA;
+}
+
+filark_status_t filark_ema_destroy(filark_ema_t* h)
+{
+    if (!h) return FILARK_OK;
+    int cur = -1;
+    const bool have_cur = cudaGetDevice(&cur) == cudaSuccess;
+    const bool switched = have_cur && cur != h->device && cudaSetDevice(h->device) == cudaSuccess;
+    cudaDeviceSynchronize();
+    cudaFree(h->d_state);
+    if (switched) cudaSetDevice(cur);
+    cudaGetLastError();
+    delete h;
+    return FILARK_OK;
+}
+
+filark_status_t filark_decimate(const float* d_in, int n_ch, long long n_t, long long pitch, int layout, int mode,
+                                int width, float* d_out, cudaStream_t stream)
+{
+    if (!d_in || !d_out || n_ch <= 0 || n_t <= 0 || width <= 0 || n_t > 0x7fff0000LL) return FILARK_ERR_INVALID_ARG;
+    if (mode < FILARK_DECIMATE_DROP || mode > FILARK_DECIMATE_LINEAR) return FILARK_ERR_INVALID_ARG;
+    const bool cm = layout == FILARK_LAYOUT_CHANNEL_MAJOR;
+    if (!cm && layout != FILARK_LAYOUT_TIME_MAJOR) return FILARK_ERR_INVALID_ARG;
+    if (pitch < (cm ? n_t : (long long)n_ch)) return FILARK_ERR_INVALID_ARG;
+    if (((uintptr_t)d_in | (uintptr_t)d_out) & 3u) return FILARK_ERR_ALIGNMENT;
+    const uintptr_t a0 = (uintptr_t)d_in, a1 = a0 + sizeof(float) * (size_t)(((cm ? n_ch : n_t) - 1) * pitch + (cm ? n_t : n_ch));
+    const uintptr_t b0 = (uintptr_t)d_out, b1 = b0 + sizeof(float) * (size_t)n_ch * (size_t)width;
+    if (a0 < b1 && b0 < a1) return FILARK_ERR_INVALID_ARG;
+    DecParams p{d_in, d_out, n_t, pitch, n_ch, width, mode};
+    if (cm) {
+        if (n_ch > 65535) return FILARK_ERR_INVALID_ARG;
+        const bool per_thread = mode != FILARK_DECIMATE_PEAK || n_t <= 32LL * width;
+        int gx = per_thread ? (width + 127) / 128 : (width + 3) / 4;
+        if (!per_thread && gx > 64) gx = 64;
+        filark_decimate_cm_kernel<<<dim3((unsigned)gx, (unsigned)n_ch), 128, 0, stream>>>(p);
+    } else {
+        int gy = (width + 31) / 32;
+        if (gy > 65535) gy = 65535;
+        const int cols = (width + gy - 1) / gy;
+        filark_decimate_tm_kernel<<<dim3((unsigned)((n_ch + 127) / 128), (unsigned)gy), 128, 0, stream>>>(p, cols);
+    }
+    return cudaGetLastError() == cudaSuccess ? FILARK_OK : FILARK_ERR_CUDA;
+}
+
+}  // extern "C"

@@ -233,3 +233,93 @@ def test_trigger_without_cf_output_and_list_overflow(cuda_device):
         with pytest.raises(FilarkError):
             s.set_trigger(*bad)
     s.destroy()
+
+
+# ---- NEXT-3: streaming first-order operators; NEXT-4: display decimation -------------------------
+from oracle import OracleEma, oracle_decimate  # noqa: E402
+from paper_2605_20132_b200.ops import FilarkEma, decimate  # noqa: E402
+
+
+@pytest.mark.parametrize("mode", ["mean", "demean", "agc"])
+@pytest.mark.parametrize("layout", [CHANNEL_MAJOR, TIME_MAJOR])
+@pytest.mark.parametrize("n_len", [1, 40, 5000])
+def test_ema_operators(cuda_device, mode, layout, n_len):
+    """Running mean / de-mean / running AGC against the oracle, pushed in ragged chunks (the state is
+    carried; tiles of 512 samples, so the chunk lengths cover several tiles and ragged tails)."""
+    n_ch, n_t = 150, 12_345
+    rng = np.random.default_rng(n_len)
+    x = (rng.standard_normal((n_ch, n_t)) * 2.0 + 0.7).astype(np.float32)
+    eps = 1e-3 if mode == "agc" else 0.0
+    o = OracleEma(n_ch, n_len, mode, eps)
+    ref = o.push(x)
+    o.close()
+    xd = torch.from_numpy(x if layout == CHANNEL_MAJOR else np.ascontiguousarray(x.T)).to(cuda_device)
+    h = FilarkEma(n_ch, n_len, mode, eps, layout)
+    outs = []
+    for a, b in split(n_t, [4096, 1, 511, 512, 513, 3000]):
+        xin = (xd[:, a:b] if layout == CHANNEL_MAJOR else xd[a:b, :]).contiguous()
+        y = torch.empty_like(xin)
+        h.push(xin, y)
+        outs.append(y)
+    got = torch.cat(outs, 1 if layout == CHANNEL_MAJOR else 0).cpu().numpy()
+    if layout == TIME_MAJOR:
+        got = got.T
+    # (north-star bounds relative to the scale of the data the operator works on: de-mean with N = 1 is
+    # identically zero in the oracle)
+    num = np.sqrt(((got - ref).astype(np.float64) ** 2).sum(1))
+    den = np.maximum(np.sqrt((ref.astype(np.float64) ** 2).sum(1)), np.sqrt((x.astype(np.float64) ** 2).sum(1)) * 1e-2)
+    assert (num <= 2e-5 * den).all(), (num / den).max()
+    assert np.abs(got - ref).max() <= 1e-3 * max(np.abs(ref).max(), 1e-2 * np.abs(x).max())
+    # reset: the same record again gives the same output bit for bit; in place is allowed
+    h.reset()
+    xin = xd.clone()
+    h.push(xin, xin)
+    again = xin.cpu().numpy()
+    if layout == TIME_MAJOR:
+        again = again.T
+    assert np.abs(again - ref).max() <= 1e-3 * max(np.abs(ref).max(), 1e-2 * np.abs(x).max())
+    h.destroy()
+
+
+@pytest.mark.parametrize("mode", ["drop", "peak", "linear"])
+@pytest.mark.parametrize("layout", [CHANNEL_MAJOR, TIME_MAJOR])
+@pytest.mark.parametrize("n_t,width", [(90_000, 2048), (1500, 2048), (2048, 2048), (100_003, 777), (33, 1)])
+def test_display_decimation(cuda_device, mode, layout, n_t, width):
+    """drop and peak are selections: bit-exact; linear within fp32 rounding of the oracle's double."""
+    n_ch = 97
+    rng = np.random.default_rng(n_t + width)
+    x = rng.standard_normal((n_ch, n_t)).astype(np.float32)
+    x[:, ::7] = np.round(x[:, ::7])                                    # equal magnitudes: the first one wins
+    xl = x if layout == CHANNEL_MAJOR else np.ascontiguousarray(x.T)
+    ref = oracle_decimate(xl, mode, width, layout)
+    got = decimate(torch.from_numpy(xl).to(cuda_device), mode, width, layout).cpu().numpy()
+    if mode == "linear":
+        assert np.abs(got - ref).max() <= 1e-5 * max(1.0, np.abs(ref).max())
+    else:
+        assert np.array_equal(got, ref)
+
+
+def test_decimation_of_the_stream_outputs_and_argument_checks(cuda_device):
+    """The step behind S7 in the viewer: the filtered tile and its CF go to a
+    2048-column display buffer; pitched input (a window of a longer record); bad arguments."""
+    w = CONFIGS["cfg3"].scaled(n_ch=64, n_t=30_000)
+    sos = design_sos(w)
+    x = generate(w, device="cpu")
+    s = FilarkStream(w.n_ch, sos, w.sta_len, w.lta_len)
+    xd = x.to(cuda_device); f = torch.empty_like(xd); c = torch.empty_like(xd)
+    s.push(xd, f, c)
+    env = decimate(f, "peak", 2048)
+    torch.cuda.synchronize()
+    assert np.array_equal(env.cpu().numpy(), oracle_decimate(f.cpu().numpy(), "peak", 2048))
+    # a window [5000, 25000) of every channel: pitch = the record's row length
+    from paper_2605_20132_b200.ops import _lib, DECIMATE_MODES
+    out = torch.empty((w.n_ch, 512), device=cuda_device)
+    st = _lib().filark_decimate(f.data_ptr() + 4 * 5000, w.n_ch, 20_000, w.n_t, 0, DECIMATE_MODES["drop"], 512, out.data_ptr(), None)
+    assert st == 0
+    torch.cuda.synchronize()
+    assert np.array_equal(out.cpu().numpy(), oracle_decimate(f[:, 5000:25_000].cpu().numpy(), "drop", 512))
+    for bad in (dict(n_t=0), dict(width=0), dict(mode=7), dict(layout=3), dict(pitch=10)):
+        a = dict(n_t=20_000, width=512, mode=0, layout=0, pitch=w.n_t); a.update(bad)
+        assert _lib().filark_decimate(f.data_ptr(), w.n_ch, a["n_t"], a["pitch"], a["layout"], a["mode"], a["width"], out.data_ptr(), None) == 1
+    assert _lib().filark_decimate(f.data_ptr(), w.n_ch, 20_000, w.n_t, 0, 0, 512, f.data_ptr() + 4096, None) == 1     # overlap
+    s.destroy()

@@ -25,7 +25,7 @@ def lib():
 
 def _declared_symbols():
     names = []
-    for hdr in ("filark_stream.h", "filark_debug.h"):
+    for hdr in ("filark_stream.h", "filark_debug.h", "filark_ops.h"):
         text = open(os.path.join(ROOT, "include", hdr)).read()
         text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
         names += re.findall(r"\b(filark_[a-z_0-9]+)\s*\(", text)
