@@ -674,20 +674,6 @@ __device__ __noinline__ void trigger_tile(const PushParams<L>& p, int buf, int s
     const float thr_on = p.thr_on, thr_off = p.thr_off;
     const int eb = 2 * L * lane;
     unsigned on = __float_as_uint(fk_smem[wtr]);
-    // Does this tile matter?  Only if the channel is on, or some cf of the tile reaches thr_on (positions
-    // outside the chunk included: that costs a needless visit at most).  Everything that belongs to the
-    // trigger lives in this function, so that the push kernel carries none of it when no trigger is set.
-    {
-        float m = 0.0f;
-        if (s == 0) {
-            const float4* r = reinterpret_cast<const float4*>(&fk_smem[buf + lane * Geo<L>::pitch]);
-#pragma unroll
-            for (int q = 0; q < L / 2; ++q) { const float4 v = r[q]; m = fmaxf(fmaxf(m, fmaxf(v.x, v.y)), fmaxf(v.z, v.w)); }
-        } else {
-            for (int e = eb; e < eb + 2 * L; ++e) m = fmaxf(m, fk_smem[buf + raw_index<L>(e + s)]);
-        }
-        if (on == 0u && !__any_sync(0xffffffffu, m >= thr_on)) return;
-    }
     float mx = 0.0f;
     bool has_on = false, has_off = false;
     for (int e = max(eb, e_lo); e < min(eb + 2 * L, e_hi); ++e) {
@@ -742,12 +728,15 @@ __device__ __noinline__ void trigger_tile(const PushParams<L>& p, int buf, int s
 // (kTM: time-major chunk; the CTA's warps hold the channels cg kTmChannels + warp and store together;
 // `bufoff` = buf relative to the warp's shared-memory area; `item_end` is false for a warp whose
 // channel does not exist)
-template <int L, bool kInterior, bool kAllKinds, bool kTM>
+// kForm: 0 = the two common section forms only, 1 = every section form, 2 = every form + the trigger
+// (filark_stream_set_trigger): a push kernel without a trigger set carries none of its code.
+template <int L, bool kInterior, int kForm, bool kTM>
 __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk& ck, const Geom& g, int buf, int wst, float2 (&x)[L],
                                              int ch, int tile, int lane, unsigned long long seen,
                                              bool item_end, unsigned rel_val, int cg, int bufoff,
                                              const TimeOrder<L>& to, TmPrefetch<L>* pf = nullptr)
 {
+    constexpr bool kAllKinds = kForm >= 1, kTrig = kForm == 2;
     const bool last = tile == g.n_tiles - 1;
     const int t0 = tile * Geo<L>::tile - g.r0;
     // the carried state moves to the end of the tile's last FULL slot (slot q - 1)
@@ -888,8 +877,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
         if (lane + 32 < ns) __stcg(gst + lane + 32, fk_smem[wst + lane + 32]);
     }
 
-    const bool trig = p.thr_on > 0.0f;
-    if (ck.cf || trig) {
+    if (ck.cf || kTrig) {
         // warm-up (reading R10): samples whose index since create/reset is < lta_len give cf = 0
         // (seen = samples pushed before this push; tile position e is sample seen + t0 + e of the stream)
         const long long rem = (long long)p.lta_len - (long long)seen - t0;     // first tile position with cf != 0
@@ -915,10 +903,21 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
                 x[i].y = (Pl.y > thr && base + L + i >= wm) ? qb : 0.0f;
             }
         }
+        // trigger: does this tile matter?  Only if the channel is on, or some cf of the tile reaches thr_on
+        // (positions outside the chunk included: that costs a needless visit at most)
+        bool visit = false;
+        if (kTrig) {
+            float mx = fmaxf(x[0].x, x[0].y);
+#pragma unroll
+            for (int i = 1; i < L; ++i) mx = fmaxf(mx, fmaxf(x[i].x, x[i].y));
+            visit = __any_sync(0xffffffffu, mx >= p.thr_on) || __float_as_uint(fk_smem[wst + trig_word(p.n_sec)]) != 0u;
+        }
         const int sc = (kTM || !ck.cf) ? 0 : row_shift(ck.cf + (long long)ch * ck.out_pitch, g.r0);
-        regs_to_buf<L>(x, buf, lane, sc);
-        if (kTM) __syncthreads(); else __syncwarp();
-        if (trig && (!kTM || ch < p.n_ch)) {
+        if (ck.cf || visit) {
+            regs_to_buf<L>(x, buf, lane, sc);
+            if (kTM) __syncthreads(); else __syncwarp();
+        }
+        if (kTrig && visit && (!kTM || ch < p.n_ch)) {
             trigger_tile<L>(p, buf, sc, wst + trig_word(p.n_sec), ch, (long long)seen + t0, max(0, -t0),
                             min(Geo<L>::tile, ck.n_t - t0), lane);
             if (item_end && lane == 0) {             // (the state went back before the trigger ran)
@@ -977,7 +976,7 @@ template <int L, int CTAS> __host__ __device__ constexpr int cm_cta_warps() { re
 // push in front of it.
 // kTM: time-major chunks through the transpose in shared memory (above): CTAS = 1, kTmChannels warps;
 // the work items are (segment, group of kTmChannels channels) and belong to the CTA as a whole.
-template <int L, int CTAS, bool kAllKinds, bool kTM, bool kDyn>
+template <int L, int CTAS, int kForm, bool kTM, bool kDyn>
 __global__ void __launch_bounds__(cm_cta_warps<L, CTAS>() * 32, CTAS)
 filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
 {
@@ -1267,11 +1266,11 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         if (kTM) {
             // (time-major: the next tile is requested in portions while this one is computed)
             TmPrefetch<L> pf(p, p.ck[nk], geom_of(nk), ncg, ngt - sh_tile0[nk], (cur ^ 1) * Geo<L>::buf_floats);
-            process_tile<L, true, kAllKinds, true>(p, ck, g, buf, wst, x, ch, tile, lane, seen + ck.t_cum, item_end && valid,
+            process_tile<L, true, kForm, true>(p, ck, g, buf, wst, x, ch, tile, lane, seen + ck.t_cum, item_end && valid,
                                                    seq0 + (unsigned)seg + 1u, cg, cur * Geo<L>::buf_floats, to,
                                                    nhave ? &pf : nullptr);
         } else {
-            process_tile<L, CTAS == 1, kAllKinds, false>(p, ck, g, buf, wst, x, ch, tile, lane, seen + ck.t_cum, item_end && valid,
+            process_tile<L, CTAS == 1, kForm, false>(p, ck, g, buf, wst, x, ch, tile, lane, seen + ck.t_cum, item_end && valid,
                                                          seq0 + (unsigned)seg + 1u, cg, cur * Geo<L>::buf_floats, to);
         }
         if (item_end) wcur ^= 1;

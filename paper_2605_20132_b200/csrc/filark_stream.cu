@@ -224,11 +224,11 @@ static Geom geometry_rt(int L, unsigned r0, int n_t, bool vec4)
 
 // CTAS CTAs per SM, W warps per CTA; fewer warps per CTA, on more SMs, when there are few
 // channels.  Every CTA of a push fits on the device at once (the segment waits rely on it).
-template <int L, int CTAS, bool kAllKinds, bool kDyn>
+template <int L, int CTAS, int kForm, bool kDyn>
 static cudaError_t launch_cm_variant(const PushParams<L>& p, int device, int grid, int W, size_t smem, size_t smem_max, cudaStream_t stream)
 {
     static std::atomic<unsigned long long> attr_done{0};
-    const cudaError_t e = set_smem_attr_once(attr_done, device, (const void*)filark_push_cm_kernel<L, CTAS, kAllKinds, false, kDyn>, smem_max);
+    const cudaError_t e = set_smem_attr_once(attr_done, device, (const void*)filark_push_cm_kernel<L, CTAS, kForm, false, kDyn>, smem_max);
     if (e != cudaSuccess) return e;
     // programmatic stream serialization: the kernel lets its dependents launch as soon as it has read
     // its control slot, and orders itself against the previous push channel by channel
@@ -240,7 +240,7 @@ static cudaError_t launch_cm_variant(const PushParams<L>& p, int device, int gri
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = tune().nopdl ? 0 : 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, CTAS, kAllKinds, false, kDyn>, p);
+    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, CTAS, kForm, false, kDyn>, p);
 }
 
 // Tiles per channel of a launch: the r0 = 0 estimate and the largest number whatever r0 < kMaxL the
@@ -263,7 +263,7 @@ static int segment_tiles(long long n_tiles, long long units, long long workers)
     return (int)(st < 1 ? 1 : (st > 0x3fffffff ? 0x3fffffff : st));
 }
 
-template <int L, int CTAS, bool kAllKinds>
+template <int L, int CTAS, int kForm>
 static cudaError_t launch_cm_shape(const filark_stream* h, PushParams<L>& p, cudaStream_t stream)
 {
     const size_t warp_bytes = sizeof(float) * (size_t)warp_smem_floats<L>();
@@ -289,30 +289,35 @@ static cudaError_t launch_cm_shape(const filark_stream* h, PushParams<L>& p, cud
     const size_t smem_max = (size_t)cm_cta_warps<L, CTAS>() * warp_bytes;
     if constexpr (CTAS != 1) {
         if (p.seg_tiles >= n_tiles_max)
-            return launch_cm_variant<L, CTAS, kAllKinds, false>(p, h->device, grid, W, smem, smem_max, stream);
+            return launch_cm_variant<L, CTAS, kForm, false>(p, h->device, grid, W, smem, smem_max, stream);
     }
-    return launch_cm_variant<L, CTAS, kAllKinds, true>(p, h->device, grid, W, smem, smem_max, stream);
+    return launch_cm_variant<L, CTAS, kForm, true>(p, h->device, grid, W, smem, smem_max, stream);
 }
+
+// Kernel form (filark_kernels.cuh, process_tile): lean section forms / all forms / all forms + trigger.
+static int kernel_form(const filark_stream* h) { return h->thr_on > 0.0f ? 2 : (h->lean_kinds ? 0 : 1); }
 
 // Launch shape (filark_kernels.cuh): one CTA per SM when every resident warp gets a long run of tiles
 // anyway, small CTAs otherwise.  (L = 24 is the only variant long pushes ever use.)
 template <int L>
 static cudaError_t launch_cm(const filark_stream* h, PushParams<L>& p, cudaStream_t stream)
 {
+    const int form = kernel_form(h);
     if constexpr (L == 24 || (L == 16 && FK_MAXW16 != 16)) {
         long long n_tiles, n_tiles_max;
         launch_tiles<L>(p, &n_tiles, &n_tiles_max);
         const bool long_push = n_tiles_max * p.n_ch >= 12LL * h->n_sm * cm_max_warps<L>();
         if (long_push && !tune().small_ctas)
-            return h->lean_kinds ? launch_cm_shape<L, 1, false>(h, p, stream) : launch_cm_shape<L, 1, true>(h, p, stream);
+            return form == 0 ? launch_cm_shape<L, 1, 0>(h, p, stream)
+                             : (form == 1 ? launch_cm_shape<L, 1, 1>(h, p, stream) : launch_cm_shape<L, 1, 2>(h, p, stream));
     }
-    return h->lean_kinds ? launch_cm_shape<L, kCmCtasPerSm, false>(h, p, stream)
-                         : launch_cm_shape<L, kCmCtasPerSm, true>(h, p, stream);
+    return form == 0 ? launch_cm_shape<L, kCmCtasPerSm, 0>(h, p, stream)
+                     : (form == 1 ? launch_cm_shape<L, kCmCtasPerSm, 1>(h, p, stream) : launch_cm_shape<L, kCmCtasPerSm, 2>(h, p, stream));
 }
 
 // Time-major chunks: the same kernel with the transpose in shared memory (filark_kernels.cuh): one CTA
 // of kTmChannels warps per SM, work items = (segment, group of kTmChannels adjacent channels).
-template <int L, bool kAllKinds>
+template <int L, int kForm>
 static cudaError_t launch_tm_kinds(const filark_stream* h, PushParams<L>& p, cudaStream_t stream)
 {
     const size_t smem = sizeof(float) * (size_t)kTmChannels * (size_t)warp_stride<L, true>();
@@ -330,19 +335,20 @@ static cudaError_t launch_tm_kinds(const filark_stream* h, PushParams<L>& p, cud
     cfg.attrs = attr; cfg.numAttrs = 1;
     if (p.seg_tiles >= n_tiles_max) {
         static std::atomic<unsigned long long> attr_done{0};
-        const cudaError_t e = set_smem_attr_once(attr_done, h->device, (const void*)filark_push_cm_kernel<L, 1, kAllKinds, true, false>, smem);
+        const cudaError_t e = set_smem_attr_once(attr_done, h->device, (const void*)filark_push_cm_kernel<L, 1, kForm, true, false>, smem);
         if (e != cudaSuccess) return e;
-        return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, 1, kAllKinds, true, false>, p);
+        return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, 1, kForm, true, false>, p);
     }
     static std::atomic<unsigned long long> attr_done{0};
-    const cudaError_t e = set_smem_attr_once(attr_done, h->device, (const void*)filark_push_cm_kernel<L, 1, kAllKinds, true, true>, smem);
+    const cudaError_t e = set_smem_attr_once(attr_done, h->device, (const void*)filark_push_cm_kernel<L, 1, kForm, true, true>, smem);
     if (e != cudaSuccess) return e;
-    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, 1, kAllKinds, true, true>, p);
+    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, 1, kForm, true, true>, p);
 }
 template <int L>
 static cudaError_t launch_tm(const filark_stream* h, PushParams<L>& p, cudaStream_t stream)
 {
-    return h->lean_kinds ? launch_tm_kinds<L, false>(h, p, stream) : launch_tm_kinds<L, true>(h, p, stream);
+    const int form = kernel_form(h);
+    return form == 0 ? launch_tm_kinds<L, 0>(h, p, stream) : (form == 1 ? launch_tm_kinds<L, 1>(h, p, stream) : launch_tm_kinds<L, 2>(h, p, stream));
 }
 
 // One chunk as the caller describes it (all pushes end up here).
