@@ -220,6 +220,26 @@ class OracleTrigger:
     __del__ = close
 
 
+def oracle_zero_phase(x: np.ndarray, sos) -> np.ndarray:
+    """Zero-phase (forward-backward) filtering of a bounded window, channel-major x [n_ch][n_t]
+    (PAPER.md:77 the display filter is "either a zero-phase or causal IIR filter ...
+    applied only to the currently visible buffer").  Reading R29: the cascade run forward from the
+    steady state of the window's first sample, the result reversed in time, run again from the steady
+    state of ITS first sample, and reversed back -- no padding.  Built from the oracle's own steps."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    n_ch = x.shape[0]
+    fwd = Oracle(n_ch, sos, 1, 1)
+    fwd.set_initial_condition(x[:, 0].astype(np.float64))
+    y, _ = fwd.push(x, want_cf=False)
+    fwd.close()
+    r = np.ascontiguousarray(y[:, ::-1])
+    bwd = Oracle(n_ch, sos, 1, 1)
+    bwd.set_initial_condition(r[:, 0].astype(np.float64))
+    z, _ = bwd.push(r, want_cf=False)
+    bwd.close()
+    return np.ascontiguousarray(z[:, ::-1])
+
+
 DECIMATE_MODES = {"drop": 0, "peak": 1, "linear": 2}
 EMA_MODES = {"mean": 0, "demean": 1, "agc": 2}
 

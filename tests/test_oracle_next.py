@@ -239,3 +239,31 @@ def test_ema_operators_are_chunk_invariant_bitwise(mode):
         parts.append(b.push(x[:, p:p + s])); p += s
     b.close()
     assert np.array_equal(np.concatenate(parts, 1), whole)
+
+
+# ---- NEXT-2: zero-phase display-filter mode (reading R29) -------------------------------------
+from oracle import oracle_zero_phase  # noqa: E402
+
+
+@pytest.mark.parametrize("name", ["low-pass", "high-pass", "cfg3 band-pass"])
+def test_zero_phase_is_scipys_sosfiltfilt_without_padding(name):
+    sos = _designs()[name]
+    rng = np.random.default_rng(12)
+    x = (rng.standard_normal((3, 4000)) + 2.0).astype(np.float32)
+    got = oracle_zero_phase(x, sos)
+    ref = signal.sosfiltfilt(sos, x.astype(np.float64), axis=1, padtype=None)
+    # (the intermediate signal is rounded to float32 once in the oracle: outputs of the path are float32)
+    assert np.abs(got - ref).max() <= 5e-6 * max(1.0, np.abs(ref).max())
+
+
+def test_zero_phase_commutes_with_time_reversal():
+    """Zero phase: filtering the time-reversed window gives the time-reversed output up to the edge
+    effects of the two initial conditions -- exactly so for a window that starts and ends at rest."""
+    sos = signal.butter(4, 0.1, "low", output="sos")
+    x = np.zeros((1, 6000), dtype=np.float32)
+    x[0, 2500:3500] = np.hanning(1000).astype(np.float32)
+    a = oracle_zero_phase(x, sos)
+    b = oracle_zero_phase(np.ascontiguousarray(x[:, ::-1]), sos)[:, ::-1]
+    assert np.abs(a - b).max() <= 1e-5
+    # no delay: the output of a symmetric pulse is symmetric about the same centre
+    assert np.abs(a[0, 2000:4000] - a[0, 2000:4000][::-1]).max() <= 1e-2 * a.max()
