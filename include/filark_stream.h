@@ -259,6 +259,20 @@ filark_status_t filark_stream_get_state(filark_stream_t *h, void *blob, long lon
 filark_status_t filark_stream_set_state(filark_stream_t *h, const void *blob, long long size, cudaStream_t stream);
 filark_status_t filark_stream_set_initial_condition(filark_stream_t *h, const float *x0, cudaStream_t stream);
 
+/*
+ * filark_stream_zero_phase -- the zero-phase mode of the display filter ("Implemented as
+ * either a zero-phase or causal IIR filter ... applied only to the currently visible buffer"): the
+ * handle's cascade run forward over a bounded window, the result reversed in time, run again, and
+ * reversed back; each pass starts from the steady state of the first sample of its input, there is no
+ * padding (reading R29: scipy's sosfiltfilt(..., padtype=None)).  d_in, d_out: dense windows of n_ch x
+ * n_t floats in the handle's layout (d_out may equal d_in).  Does NOT touch the carried state of the
+ * stream (a second stream of the same cascade and two window-sized temporaries are made on first use
+ * and grow on demand: the only allocations; a larger window synchronises).  Enqueues six kernels on
+ * `stream`.  Errors: INVALID_ARG, ALIGNMENT, ALLOC, DEVICE_MISMATCH, CUDA.
+ */
+filark_status_t filark_stream_zero_phase(filark_stream_t *h, const float *d_in, long long n_t, float *d_out,
+                                         cudaStream_t stream);
+
 /* Free the handle and its device memory (on the handle's device, whichever device is current).
  * NULL is accepted.  Synchronises the handle's device. */
 filark_status_t filark_stream_destroy(filark_stream_t *h);

@@ -54,6 +54,12 @@ struct filark_stream {
     int prev_valid;                 // how many of the entries below describe pushes that may still run
     cudaStream_t prev_stream;
     uintptr_t prev_lo[kCmDepth - 1][3], prev_hi[kCmDepth - 1][3];     // [0] = the push before, [1] = the one before that
+    // zero-phase window mode (filark_stream_zero_phase): a second stream of the same cascade and two
+    // window-sized temporaries, made on first use; the cascade as it was given
+    double sos[6 * kMaxSec];
+    filark_stream* zp;
+    float* d_zp_tmp[2];
+    size_t zp_elems;
     int n_sm;
     size_t smem_optin;
     int last_cuda_error;
@@ -441,6 +447,7 @@ filark_status_t filark_stream_create_ex(filark_stream_t** out, int n_ch, const d
     for (int k = 0; k < n_sec; ++k) h->lean_kinds = h->lean_kinds && (h->sec[k].kind == kKindDF2 || h->sec[k].kind == kKindDelta);
     h->n_ch = n_ch; h->n_sec = n_sec; h->sta_len = sta_len; h->lta_len = lta_len;
     h->layout = layout; h->flags = flags;
+    std::memcpy(h->sos, sos, sizeof(double) * 6 * (size_t)n_sec);
     h->state_floats = (size_t)n_ch * (size_t)state_floats(n_sec);
     cudaError_t e = cudaGetDevice(&h->device);
     int optin = 0;
@@ -492,6 +499,8 @@ filark_status_t filark_stream_destroy(filark_stream_t* h)
     for (int v = 0; v < kNumVariants; ++v) std::free(h->proto[v]);
     cudaFree(h->d_state); cudaFree(h->d_hist); cudaFree(h->d_cctl); cudaFree(h->d_progress);
     cudaFree(h->d_events); cudaFree(h->d_n_events);
+    cudaFree(h->d_zp_tmp[0]); cudaFree(h->d_zp_tmp[1]);
+    if (h->zp) { filark_stream* z = h->zp; h->zp = nullptr; filark_stream_destroy(z); }
     for (int j = 0; j < 2; ++j) for (int i = 0; i < 3; ++i) cudaFree(h->d_stage[j][i]);
     if (h->host_ready) {
         cudaStreamDestroy(h->s_h2d); cudaStreamDestroy(h->s_d2h);
@@ -873,6 +882,87 @@ filark_status_t filark_stream_pop_events(filark_stream_t* h, filark_event_t* out
     if (e == cudaSuccess) e = cudaMemset(h->d_n_events, 0, sizeof(unsigned));
     if (e != cudaSuccess) return cuda_fail(h, e);
     return FILARK_OK;
+}
+
+// ---- zero-phase window mode (reading R29) -----------------------
+// state[c][i] = kvec[i] * (first sample of channel c): the steady state of the cascade for that level
+struct IcParams { float kvec[2 * kMaxSec]; };
+__global__ void filark_ic_kernel(float* state, int ns, int n_state, const __grid_constant__ IcParams k,
+                                 const float* x, long long stride_c, int n_ch)
+{
+    const int c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= n_ch) return;
+    const float x0 = x[(long long)c * stride_c];
+    for (int i = 0; i < n_state; ++i) state[(long long)c * ns + i] = k.kvec[i] * x0;
+}
+// out(c, n) = in(c, n_t - 1 - n); element (c, n) at c*sc + n*sn
+__global__ void filark_reverse_kernel(const float* in, float* out, int n_ch, long long n_t, long long sc, long long sn, int fast_c)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (long long)n_ch * n_t) return;
+    // consecutive threads along the contiguous axis of the layout
+    const long long c = fast_c ? i % n_ch : i / n_t, n = fast_c ? i / n_ch : i % n_t;
+    out[c * sc + n * sn] = in[c * sc + (n_t - 1 - n) * sn];
+}
+
+filark_status_t filark_stream_zero_phase(filark_stream_t* h, const float* d_in, long long n_t, float* d_out, cudaStream_t stream)
+{
+    if (!h || n_t < 0) return FILARK_ERR_INVALID_ARG;
+    if (n_t == 0) return FILARK_OK;
+    if (!d_in || !d_out || n_t > 0x7fff0000LL || (h->flags & FILARK_FLAG_SERIAL_SCAN)) return FILARK_ERR_INVALID_ARG;
+    if (((uintptr_t)d_in | (uintptr_t)d_out) & 3u) return FILARK_ERR_ALIGNMENT;
+    filark_status_t st = check_device(h);
+    if (st != FILARK_OK) return st;
+    const size_t elems = (size_t)h->n_ch * (size_t)n_t;
+    if (!h->zp) {
+        st = filark_stream_create_ex(&h->zp, h->n_ch, h->sos, h->n_sec, 1, 1, h->layout, FILARK_FLAG_NONE);
+        if (st != FILARK_OK) { h->zp = nullptr; return st; }
+    }
+    if (elems > h->zp_elems) {
+        cudaStreamSynchronize(stream);
+        cudaDeviceSynchronize();
+        cudaFree(h->d_zp_tmp[0]); cudaFree(h->d_zp_tmp[1]);
+        h->d_zp_tmp[0] = h->d_zp_tmp[1] = nullptr; h->zp_elems = 0;
+        cudaError_t e = cudaMalloc((void**)&h->d_zp_tmp[0], sizeof(float) * elems);
+        if (e == cudaSuccess) e = cudaMalloc((void**)&h->d_zp_tmp[1], sizeof(float) * elems);
+        if (e != cudaSuccess) {
+            cudaFree(h->d_zp_tmp[0]); cudaFree(h->d_zp_tmp[1]); h->d_zp_tmp[0] = h->d_zp_tmp[1] = nullptr;
+            cudaGetLastError(); h->last_cuda_error = (int)e;
+            return e == cudaErrorMemoryAllocation ? FILARK_ERR_ALLOC : FILARK_ERR_CUDA;
+        }
+        h->zp_elems = elems;
+    }
+    // steady state of the cascade per unit input level (float64, as filark_stream_set_initial_condition)
+    filark_stream* z = h->zp;
+    IcParams k{};
+    {
+        double v = z->gain;
+        for (int j = 0; j < z->n_sec; ++j) {
+            const Section& q = z->sec[j];
+            const double m00 = 1.0 - q.A.a, m01 = -q.A.b, m10 = -q.A.c, m11 = 1.0 - q.A.d;
+            const double det = m00 * m11 - m01 * m10, b0 = q.B[0] * v, b1 = q.B[1] * v;
+            const double s0 = (m11 * b0 - m01 * b1) / det, s1 = (m00 * b1 - m10 * b0) / det;
+            k.kvec[2 * j] = (float)s0; k.kvec[2 * j + 1] = (float)s1;
+            v = q.C[0] * s0 + q.C[1] * s1 + q.D * v;
+        }
+    }
+    const bool cm = h->layout == FILARK_LAYOUT_CHANNEL_MAJOR;
+    const long long sc = cm ? n_t : 1, sn = cm ? 1 : (long long)h->n_ch;
+    const int ns = state_floats(h->n_sec);
+    const unsigned gc = (unsigned)((h->n_ch + 127) / 128), ge = (unsigned)((elems + 255) / 256);
+    const float* src = d_in;
+    for (int pass = 0; pass < 2; ++pass) {
+        st = filark_stream_reset(z, stream);
+        if (st != FILARK_OK) return st;
+        filark_ic_kernel<<<gc, 128, 0, stream>>>(z->d_state, ns, 2 * h->n_sec, k, src, sc, h->n_ch);
+        st = filark_stream_push(z, src, n_t, h->d_zp_tmp[0], nullptr, stream);
+        if (st != FILARK_OK) return st;
+        float* dst = pass == 0 ? h->d_zp_tmp[1] : d_out;
+        filark_reverse_kernel<<<ge, 256, 0, stream>>>(h->d_zp_tmp[0], dst, h->n_ch, n_t, sc, sn, cm ? 0 : 1);
+        src = h->d_zp_tmp[1];
+    }
+    const cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? FILARK_OK : cuda_fail(h, e);
 }
 
 // ---- state export / import, initial condition ----------------------------

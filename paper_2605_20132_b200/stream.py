@@ -74,6 +74,8 @@ def load_library():
     lib.filark_stream_set_trigger.argtypes = [vp, ctypes.c_float, ctypes.c_float, ll, vp]
     lib.filark_stream_pop_events.restype = ci
     lib.filark_stream_pop_events.argtypes = [vp, vp, ll, ctypes.POINTER(ll), ctypes.POINTER(ll), vp]
+    lib.filark_stream_zero_phase.restype = ci
+    lib.filark_stream_zero_phase.argtypes = [vp, vp, ll, vp, vp]
     lib.filark_stream_reset.restype = ci
     lib.filark_stream_reset.argtypes = [vp, vp]
     lib.filark_stream_destroy.restype = ci
@@ -221,6 +223,13 @@ class FilarkStream:
                                                        _cur_stream() if stream is None else stream),
                     "filark_stream_pop_events")
         return out[:n.value].copy(), int(d.value)
+
+    def zero_phase(self, d_in, d_out, stream: Optional[int] = None):
+        """filark_stream_zero_phase: forward-backward filtering of a bounded window (carried state untouched)."""
+        n_t = self._n_t(d_in)
+        self._check(self._lib.filark_stream_zero_phase(self._h, _ptr(d_in), n_t, _ptr(d_out),
+                                                       _cur_stream() if stream is None else stream),
+                    "filark_stream_zero_phase")
 
     def get_state(self, stream: Optional[int] = None) -> bytes:
         """filark_stream_get_state: the documented state blob (host bytes)."""

@@ -323,3 +323,43 @@ def test_decimation_of_the_stream_outputs_and_argument_checks(cuda_device):
         assert _lib().filark_decimate(f.data_ptr(), w.n_ch, a["n_t"], a["pitch"], a["layout"], a["mode"], a["width"], out.data_ptr(), None) == 1
     assert _lib().filark_decimate(f.data_ptr(), w.n_ch, 20_000, w.n_t, 0, 0, 512, f.data_ptr() + 4096, None) == 1     # overlap
     s.destroy()
+
+
+# ---- NEXT-2: zero-phase window mode -------------------------------------------------------------
+from oracle import oracle_zero_phase  # noqa: E402
+
+
+@pytest.mark.parametrize("name", ["lowpass4", "highpass3", "cfg3"])
+@pytest.mark.parametrize("layout", [CHANNEL_MAJOR, TIME_MAJOR])
+def test_zero_phase_window(cuda_device, name, layout):
+    """Forward-backward filtering of a visible window (PAPER.md:77) against the oracle's composition;
+    the stream's own carried state is not touched."""
+    sos = FILTERS[name] if name != "cfg3" else design_sos(CONFIGS["cfg3"])
+    n_ch, n_t = 80, 8_191
+    rng = np.random.default_rng(17)
+    x = (rng.standard_normal((n_ch, n_t)) + rng.uniform(-3, 3, (n_ch, 1))).astype(np.float32)
+    ref = oracle_zero_phase(x, sos)
+    xl = x if layout == CHANNEL_MAJOR else np.ascontiguousarray(x.T)
+    xd = torch.from_numpy(xl).to(cuda_device)
+    s = FilarkStream(n_ch, sos, 40, 900, layout)
+    f0 = torch.empty_like(xd); c0 = torch.empty_like(xd)
+    s.push(xd, f0, c0)                                    # the stream is somewhere in its record
+    out = torch.empty_like(xd)
+    s.zero_phase(xd, out)
+    s.zero_phase(xd[:5000].contiguous() if layout == TIME_MAJOR else xd[:, :5000].contiguous(),
+                 torch.empty((5000, n_ch) if layout == TIME_MAJOR else (n_ch, 5000), device=cuda_device))   # a smaller window reuses the temporaries
+    got = out.cpu().numpy()
+    got = got.T if layout == TIME_MAJOR else got
+    scale = np.maximum(np.abs(ref).max(1), 1e-2 * np.abs(x).max(1))
+    assert (np.abs(got - ref).max(1) <= 1e-3 * scale).all()
+    num = np.sqrt(((got - ref).astype(np.float64) ** 2).sum(1)); den = np.sqrt((ref.astype(np.float64) ** 2).sum(1))
+    assert (num <= 1e-4 * den + 5e-7 * np.abs(x).max(1) * np.sqrt(n_t)).all(), (num / den).max()
+    # the stream goes on as if nothing had happened
+    f1 = torch.empty_like(xd); c1 = torch.empty_like(xd)
+    s.push(xd, f1, c1)
+    s2 = FilarkStream(n_ch, sos, 40, 900, layout)
+    g0 = torch.empty_like(xd); g1 = torch.empty_like(xd); d0 = torch.empty_like(xd); d1 = torch.empty_like(xd)
+    s2.push(xd, g0, d0); s2.push(xd, g1, d1)
+    torch.cuda.synchronize()
+    assert torch.equal(f1, g1) and torch.equal(c1, d1)
+    s.destroy(); s2.destroy()
