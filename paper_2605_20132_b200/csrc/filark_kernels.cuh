@@ -305,11 +305,42 @@ template <int L> struct TimeOrder {
     }
 };
 
+// (out of line: the unrolled copies of the shifted path are long, and the kernel's aligned paths are
+// faster the smaller the kernel is -- inlined they cost the aligned headline 3 %)
+template <int L>
+__device__ __noinline__ void issue_tile_input_shifted(const float* __restrict__ src, int n_t, int t0, int s, int buf, int lane,
+                                                      const TimeOrder<L> to)
+{
+    const int tf0 = t0 + 4 * lane - s;
+    const float* __restrict__ srct = src + tf0;
+#pragma unroll
+    for (int m = 0; m <= Geo<L>::chunks; ++m) {
+        const int tf = tf0 + 128 * m;
+        const int rem = n_t - tf;
+        const int bytes = tf < 0 ? 0 : (rem >= 4 ? 16 : (rem > 0 ? 4 * rem : 0));
+        if (m == 0) {
+            if (tf <= -4 || tf >= 0) {
+                cp_async16(buf + to.at(0), srct, bytes);
+            } else {
+                for (int j = 1; j < 4; ++j) {
+                    const int t = tf + j;
+                    if (t >= 0) cp_async4(buf + to.at(0) + j, src + (t < n_t ? t : 0), t < n_t ? 4 : 0);
+                }
+            }
+        } else if (m < Geo<L>::chunks || lane == 0) {
+            cp_async16(buf + to.at(m), srct + 128 * m, bytes);
+        }
+    }
+}
+
 // S0: start the asynchronous copy of one tile of one channel into `buf` (padded lane regions:
 // tile-local sample e lives at buf[e + 4 (e / 2L)]) and, with the channel's first tile, of its
 // carried state into `wst`.  Tile-space position e of tile `tile` is input sample
 // t = tile 64L + e - r0; t < 0 reads hist[ch][r0 + t], t >= n_t is zero-filled.
-template <int L, bool kInterior>
+// kShift: built for launches with rows that are not 16-byte aligned (the host knows: p.vec4 = 0): their tiles
+// take the unrolled shifted paths; otherwise a compact loop serves the rare shifted tile (a handle whose
+// sample count is not a multiple of four when an aligned launch arrives) and the kernel stays small.
+template <int L, bool kInterior, bool kShift>
 __device__ __forceinline__ void issue_tile_input(const PushParams<L>& p, const Chunk& ck, const Geom& g, int ch, int tile, int buf, int lane,
                                                  const TimeOrder<L>& to)
 {
@@ -341,21 +372,31 @@ __device__ __forceinline__ void issue_tile_input(const PushParams<L>& p, const C
             cp_async16(buf + to.at(m), srct + 128 * m, ok ? 16 : 0);
         }
     } else {
-        // raw chunk c holds input samples tf .. tf + 3; samples before the row (t < 0) are history
-        // (issue_tile_carry), samples behind it (t >= n_t) are zero-filled; one chunk more than a
-        // tile has, because of the shift (what it loads beyond the tile is not used)
-#pragma unroll 1
-        for (int c = lane; c <= 32 * Geo<L>::chunks; c += 32) {
-            const int tf = t0 + 4 * c - s;
-            const int d = buf + 4 * c + 4 * (c / Geo<L>::chunks);
-            if (tf >= 0) {
-                const int rem = n_t - tf;
-                const int bytes = rem >= 4 ? 16 : (rem > 0 ? 4 * rem : 0);
-                cp_async16(d, bytes ? src + tf : p.hist, bytes);
-            } else if (tf > -4) {
-                for (int j = 1; j < 4; ++j) {
-                    const int t = tf + j;
-                    if (t >= 0) cp_async4(d + j, src + (t < n_t ? t : 0), t < n_t ? 4 : 0);
+        // Shifted rows.  Raw chunk c = 32 m + lane holds input samples tf .. tf + 3, tf = t0 + 4 c - s (16-byte
+        // aligned in global memory by the choice of s); one chunk more than a tile has (c = 32 chunks: lane 0
+        // only; what it loads beyond the tile is not used).  Chunks before the row (history, put over them when
+        // the tile is taken up) or behind it are zero-filled with src-size 0, the chunk that holds the row's
+        // end is copied up to there; unrolled with immediate addresses like the aligned path.  Only the chunk
+        // that straddles t = 0 (first tile of a chunk, m = 0) moves element by element.
+        if constexpr (kShift) {
+            issue_tile_input_shifted<L>(src, n_t, t0, s, buf, lane, to);
+        } else {
+            // raw chunk c holds input samples tf .. tf + 3; samples before the row (t < 0) are history
+            // (issue_tile_carry), samples behind it (t >= n_t) are zero-filled; one chunk more than a
+            // tile has, because of the shift (what it loads beyond the tile is not used)
+    #pragma unroll 1
+            for (int c = lane; c <= 32 * Geo<L>::chunks; c += 32) {
+                const int tf = t0 + 4 * c - s;
+                const int d = buf + 4 * c + 4 * (c / Geo<L>::chunks);
+                if (tf >= 0) {
+                    const int rem = n_t - tf;
+                    const int bytes = rem >= 4 ? 16 : (rem > 0 ? 4 * rem : 0);
+                    cp_async16(d, bytes ? src + tf : p.hist, bytes);
+                } else if (tf > -4) {
+                    for (int j = 1; j < 4; ++j) {
+                        const int t = tf + j;
+                        if (t >= 0) cp_async4(d + j, src + (t < n_t ? t : 0), t < n_t ? 4 : 0);
+                    }
                 }
             }
         }
@@ -379,9 +420,40 @@ __device__ __forceinline__ void issue_tile_carry(const PushParams<L>& p, const G
     cp_async_commit();
 }
 
+template <int L>
+__device__ __noinline__ void store_tile_shifted(float* __restrict__ dst, int n_t, int t0, int s, int buf, int lane, const TimeOrder<L> to)
+{
+    const int e0 = 4 * lane - s, tf0 = t0 + e0;
+    float* __restrict__ dstt = dst + tf0;
+#pragma unroll
+    for (int m = 0; m <= Geo<L>::chunks; ++m) {
+        const int e = e0 + 128 * m, tf = tf0 + 128 * m;
+        const bool full = e >= 0 && e + 4 <= Geo<L>::tile && tf >= 0 && tf + 4 <= n_t && (m < Geo<L>::chunks || lane == 0);
+        if (m < Geo<L>::chunks || lane == 0) {
+            const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + to.at(m)]);
+            if (full) st_stream4(dstt + 128 * m, v);
+        }
+    }
+    const int cand[4] = {0, 32 * Geo<L>::chunks, (s - t0) >> 2, (n_t - t0 + s) >> 2};
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const int c = cand[i];
+        if (c >= 0 && c <= 32 * Geo<L>::chunks && (c & 31) == lane) {
+            const int e = 4 * c - s, tf = t0 + e;
+            const int b = buf + 4 * c + 4 * (c / Geo<L>::chunks);
+            if (!(e >= 0 && e + 4 <= Geo<L>::tile && tf >= 0 && tf + 4 <= n_t)) {
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    if ((unsigned)(e + j) < (unsigned)Geo<L>::tile && (unsigned)(tf + j) < (unsigned)n_t)
+                        st_stream(dst + tf + j, fk_smem[b + j]);
+            }
+        }
+    }
+}
+
 // S7: the lane regions of `buf` -> one output array (coalesced 16-byte stores).  Positions that
 // map to t < 0 (recomputed history) or t >= n_t (padding) are dropped.
-template <int L, bool kInterior>
+template <int L, bool kInterior, bool kShift>
 __device__ __forceinline__ void store_tile(const Chunk& ck, const Geom& g, float* __restrict__ dst, int buf,
                                            int lane, int t0, int s, const TimeOrder<L>& to)
 {
@@ -404,22 +476,31 @@ __device__ __forceinline__ void store_tile(const Chunk& ck, const Geom& g, float
             if (ok) st_stream4(dstt + 128 * m, v);
         }
     } else {
-        // element j of raw chunk c is tile position e = 4 c + j - s: only 0 <= e < tile belongs to
-        // this tile (the first chunk starts with the previous tile's last samples, the extra chunk
-        // ends with the next tile's first ones), and only 0 <= t < n_t exists
-#pragma unroll 1
-        for (int c = lane; c <= 32 * Geo<L>::chunks; c += 32) {
-            const int e = 4 * c - s;
-            const int tf = t0 + e;
-            const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + 4 * c + 4 * (c / Geo<L>::chunks)]);
-            if (e >= 0 && e + 4 <= Geo<L>::tile && tf >= 0 && tf + 4 <= n_t) {
-                st_stream4(dst + tf, v);
-            } else {
-                const float vv[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    if ((unsigned)(e + j) < (unsigned)Geo<L>::tile && (unsigned)(tf + j) < (unsigned)n_t)
-                        st_stream(dst + tf + j, vv[j]);
+        // Shifted rows.  Element j of raw chunk c = 32 m + lane is tile position e = 4 c + j - s: only
+        // 0 <= e < tile belongs to this tile (the first chunk starts with the previous tile's last samples,
+        // the extra chunk ends with the next tile's first ones), and only 0 <= t < n_t exists.  Chunks that lie
+        // completely inside go out with one predicated 16-byte store each (unrolled, immediate addresses);
+        // the at most four chunks that cross a boundary (e = 0, e = tile, t = 0, t = n_t) follow element by element.
+        if constexpr (kShift) {
+            store_tile_shifted<L>(dst, n_t, t0, s, buf, lane, to);
+        } else {
+            // element j of raw chunk c is tile position e = 4 c + j - s: only 0 <= e < tile belongs to
+            // this tile (the first chunk starts with the previous tile's last samples, the extra chunk
+            // ends with the next tile's first ones), and only 0 <= t < n_t exists
+    #pragma unroll 1
+            for (int c = lane; c <= 32 * Geo<L>::chunks; c += 32) {
+                const int e = 4 * c - s;
+                const int tf = t0 + e;
+                const float4 v = *reinterpret_cast<const float4*>(&fk_smem[buf + 4 * c + 4 * (c / Geo<L>::chunks)]);
+                if (e >= 0 && e + 4 <= Geo<L>::tile && tf >= 0 && tf + 4 <= n_t) {
+                    st_stream4(dst + tf, v);
+                } else {
+                    const float vv[4] = {v.x, v.y, v.z, v.w};
+    #pragma unroll
+                    for (int j = 0; j < 4; ++j)
+                        if ((unsigned)(e + j) < (unsigned)Geo<L>::tile && (unsigned)(tf + j) < (unsigned)n_t)
+                            st_stream(dst + tf + j, vv[j]);
+                }
             }
         }
     }
@@ -730,7 +811,7 @@ __device__ __noinline__ void trigger_tile(const PushParams<L>& p, int buf, int s
 // channel does not exist)
 // kForm: 0 = the two common section forms only, 1 = every section form, 2 = every form + the trigger
 // (filark_stream_set_trigger): a push kernel without a trigger set carries none of its code.
-template <int L, bool kInterior, int kForm, bool kTM>
+template <int L, bool kInterior, int kForm, bool kTM, bool kShift>
 __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk& ck, const Geom& g, int buf, int wst, float2 (&x)[L],
                                              int ch, int tile, int lane, unsigned long long seen,
                                              bool item_end, unsigned rel_val, int cg, int bufoff,
@@ -828,7 +909,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
             const int sf = row_shift(row, g.r0);
             regs_to_buf<L>(x, buf, lane, sf);
             __syncwarp();
-            store_tile<L, kInterior>(ck, g, row, buf, lane, t0, sf, to);
+            store_tile<L, kInterior, kShift>(ck, g, row, buf, lane, t0, sf, to);
             __syncwarp();
         }
     }
@@ -928,7 +1009,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
         if (item_end && lane == 0) st_release(p.progress + ch, rel_val);
         if (ck.cf) {
             if (kTM) store_tile_tm<L>(p, ck, g, ck.cf, cg, bufoff, t0);
-            else store_tile<L, kInterior>(ck, g, ck.cf + (long long)ch * ck.out_pitch, buf, lane, t0, sc, to);
+            else store_tile<L, kInterior, kShift>(ck, g, ck.cf + (long long)ch * ck.out_pitch, buf, lane, t0, sc, to);
         }
     } else if (item_end) {
         __syncwarp();
@@ -976,7 +1057,7 @@ template <int L, int CTAS> __host__ __device__ constexpr int cm_cta_warps() { re
 // push in front of it.
 // kTM: time-major chunks through the transpose in shared memory (above): CTAS = 1, kTmChannels warps;
 // the work items are (segment, group of kTmChannels channels) and belong to the CTA as a whole.
-template <int L, int CTAS, int kForm, bool kTM, bool kDyn>
+template <int L, int CTAS, int kForm, bool kTM, bool kDyn, bool kShift = false>
 __global__ void __launch_bounds__(cm_cta_warps<L, CTAS>() * 32, CTAS)
 filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
 {
@@ -1154,7 +1235,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         k = chunk_of(gt);
         const Geom g = geom_of(k);
         if (kTM) issue_tile_input_tm<L>(p, p.ck[k], g, cg, gt - sh_tile0[k], 0);
-        else issue_tile_input<L, CTAS == 1>(p, p.ck[k], g, ch, gt - sh_tile0[k], wbase, lane, to);
+        else issue_tile_input<L, CTAS == 1, kShift>(p, p.ck[k], g, ch, gt - sh_tile0[k], wbase, lane, to);
         // the first segment of a channel needs what the previous launch left (state, hist): wait before
         // those loads are issued (a wait on an EARLIER launch cannot be part of a cycle)
         if (seg == 0 && ch < p.n_ch) {
@@ -1255,7 +1336,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         __syncwarp();
         if (nhave) {
             const int nbuf = wbase + (cur ^ 1) * Geo<L>::buf_floats;
-            if (!kTM) issue_tile_input<L, CTAS == 1>(p, p.ck[nk], geom_of(nk), nch, ngt - sh_tile0[nk], nbuf, lane, to);
+            if (!kTM) issue_tile_input<L, CTAS == 1, kShift>(p, p.ck[nk], geom_of(nk), nch, ngt - sh_tile0[nk], nbuf, lane, to);
             if (item_end && nseg == 0 && nch < p.n_ch) {
                 wait_progress(nch, seq0, npr);
                 issue_tile_carry<L>(p, geom_of(nk), nch, whs, wst0 + (wcur ^ 1) * kStateSmem, lane);
@@ -1266,11 +1347,11 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         if (kTM) {
             // (time-major: the next tile is requested in portions while this one is computed)
             TmPrefetch<L> pf(p, p.ck[nk], geom_of(nk), ncg, ngt - sh_tile0[nk], (cur ^ 1) * Geo<L>::buf_floats);
-            process_tile<L, true, kForm, true>(p, ck, g, buf, wst, x, ch, tile, lane, seen + ck.t_cum, item_end && valid,
+            process_tile<L, true, kForm, true, false>(p, ck, g, buf, wst, x, ch, tile, lane, seen + ck.t_cum, item_end && valid,
                                                    seq0 + (unsigned)seg + 1u, cg, cur * Geo<L>::buf_floats, to,
                                                    nhave ? &pf : nullptr);
         } else {
-            process_tile<L, CTAS == 1, kForm, false>(p, ck, g, buf, wst, x, ch, tile, lane, seen + ck.t_cum, item_end && valid,
+            process_tile<L, CTAS == 1, kForm, false, kShift>(p, ck, g, buf, wst, x, ch, tile, lane, seen + ck.t_cum, item_end && valid,
                                                          seq0 + (unsigned)seg + 1u, cg, cur * Geo<L>::buf_floats, to);
         }
         if (item_end) wcur ^= 1;

@@ -230,11 +230,11 @@ static Geom geometry_rt(int L, unsigned r0, int n_t, bool vec4)
 
 // CTAS CTAs per SM, W warps per CTA; fewer warps per CTA, on more SMs, when there are few
 // channels.  Every CTA of a push fits on the device at once (the segment waits rely on it).
-template <int L, int CTAS, int kForm, bool kDyn>
-static cudaError_t launch_cm_variant(const PushParams<L>& p, int device, int grid, int W, size_t smem, size_t smem_max, cudaStream_t stream)
+template <int L, int CTAS, int kForm, bool kDyn, bool kShift>
+static cudaError_t launch_cm_shift(const PushParams<L>& p, int device, int grid, int W, size_t smem, size_t smem_max, cudaStream_t stream)
 {
     static std::atomic<unsigned long long> attr_done{0};
-    const cudaError_t e = set_smem_attr_once(attr_done, device, (const void*)filark_push_cm_kernel<L, CTAS, kForm, false, kDyn>, smem_max);
+    const cudaError_t e = set_smem_attr_once(attr_done, device, (const void*)filark_push_cm_kernel<L, CTAS, kForm, false, kDyn, kShift>, smem_max);
     if (e != cudaSuccess) return e;
     // programmatic stream serialization: the kernel lets its dependents launch as soon as it has read
     // its control slot, and orders itself against the previous push channel by channel
@@ -246,7 +246,18 @@ static cudaError_t launch_cm_variant(const PushParams<L>& p, int device, int gri
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = tune().nopdl ? 0 : 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, CTAS, kForm, false, kDyn>, p);
+    return cudaLaunchKernelEx(&cfg, filark_push_cm_kernel<L, CTAS, kForm, false, kDyn, kShift>, p);
+}
+
+// Rows that are not 16-byte aligned (p.vec4 = 0: some pointer, pitch or chunk length is not a multiple of
+// four floats): the build of the kernel with the unrolled shifted paths (L = 24 only; filark_kernels.cuh).
+template <int L, int CTAS, int kForm, bool kDyn>
+static cudaError_t launch_cm_variant(const PushParams<L>& p, int device, int grid, int W, size_t smem, size_t smem_max, cudaStream_t stream)
+{
+    if constexpr (L == 24) {
+        if (!p.vec4) return launch_cm_shift<L, CTAS, kForm, kDyn, true>(p, device, grid, W, smem, smem_max, stream);
+    }
+    return launch_cm_shift<L, CTAS, kForm, kDyn, false>(p, device, grid, W, smem, smem_max, stream);
 }
 
 // Tiles per channel of a launch: the r0 = 0 estimate and the largest number whatever r0 < kMaxL the

@@ -92,6 +92,18 @@ def test_chunking_fuzz(cuda_device, sizes):
     s.destroy()
 
 
+def test_aligned_chunks_behind_an_odd_sample_count(cuda_device):
+    """Chunks whose rows are 16-byte aligned take the kernel build without the unrolled shifted paths; when the
+    handle's sample count is odd by then, their tiles are shifted all the same (compact loop of that build).
+    Chunks with odd lengths take the other build."""
+    w = CONFIGS["cfg3"].scaled(n_ch=11, n_t=16_000)
+    x_dev, ref_f, ref_c = _case(w, cuda_device, CHANNEL_MAJOR)
+    s = _stream(w)
+    f, c = run_gpu(s, x_dev, CHANNEL_MAJOR, split(w.n_t, [1501, 1500, 1500, 7, 1500, 3000, 2, 1536, 1537]))
+    _check(f, c, ref_f, ref_c, CHANNEL_MAJOR, "aligned chunks, odd count")
+    s.destroy()
+
+
 @pytest.mark.parametrize("L", [8, 16, 24])
 @pytest.mark.parametrize("n_t", [13_007, 6_144, 1_500, 777])
 def test_every_kernel_variant(cuda_device, L, n_t):
