@@ -55,7 +55,9 @@ typedef enum filark_status {
     FILARK_ERR_ALLOC = 3,           /* host or device allocation failed                            */
     FILARK_ERR_CUDA = 4,            /* a CUDA call failed; see filark_last_cuda_error              */
     FILARK_ERR_DEVICE_MISMATCH = 5, /* current device differs from the handle's device             */
-    FILARK_ERR_ALIGNMENT = 6        /* a device pointer is not 4-byte aligned                      */
+    FILARK_ERR_ALIGNMENT = 6,       /* a device pointer is not 4-byte aligned                      */
+    FILARK_ERR_TOO_LARGE = 7        /* filark_stream_once_noalloc: more channels than its fixed
+                                       device scratch holds (FILARK_NOALLOC_MAX_CHANNELS)          */
 } filark_status_t;
 
 /* Memory order of a chunk (reading R14/R15 in DESIGN.md). */
@@ -272,6 +274,39 @@ filark_status_t filark_stream_set_initial_condition(filark_stream_t *h, const fl
  */
 filark_status_t filark_stream_zero_phase(filark_stream_t *h, const float *d_in, long long n_t, float *d_out,
                                          cudaStream_t stream);
+
+/*
+ * filark_stream_once_noalloc -- the whole path S0..S7 over ONE dense record from rest, without a handle and
+ * WITHOUT ANY ALLOCATION: for callers that cannot call cudaMalloc (a CUDA graph being captured, a tight
+ * serving loop, a harness that forbids it).  The result is what filark_stream_create_ex + one
+ * filark_stream_push of the same record give (the same kernel runs), e.g. the characteristic function of
+ * a window of channels x samples.
+ *
+ * What a handle keeps in device memory of its own -- the carried state, the raw-history rows, the
+ * per-channel progress words and the control block of the push kernel -- lives here in ONE fixed array in
+ * the library's device image (`static __device__`, FILARK_NOALLOC_SCRATCH_BYTES = 6.6 MiB, held by every
+ * GPU that loads the library until the process exits), sized for FILARK_NOALLOC_MAX_CHANNELS channels.
+ * More channels are refused with FILARK_ERR_TOO_LARGE (shard the channels over several calls, or use a
+ * handle).  The call enqueues, on `stream`: three memsets that put the part of the array it uses back to
+ * zero (the array keeps what the previous call left), then one launch of the push kernel.  The cascade is
+ * designed on the host in the call (float64, about 0.1 ms for eight sections); no cudaMalloc, cudaFree or
+ * other allocating CUDA routine is called, nothing is synchronised.
+ *
+ * EVERY call on a device shares that array.  Calls in one stream follow one another and are safe; calls
+ * that can overlap on the GPU (different streams without an ordering between them, several host threads)
+ * RACE on it and give wrong results: order them yourself.  Handles do not use the array.
+ *
+ *   sos, n_sec, sta_len, lta_len, layout   as filark_stream_create_ex (flags: none)
+ *   d_in    n_ch x n_t floats, dense, in `layout`; d_filt / d_cf: the same shape, either may be NULL (not
+ *           both); none may overlap another.  n_t >= 0 (0: no-op).
+ *   cuda_error   may be NULL; receives the cudaError_t (as int) of a failing CUDA call.
+ * Errors: INVALID_ARG, UNSTABLE, ALIGNMENT, TOO_LARGE, CUDA.
+ */
+#define FILARK_NOALLOC_MAX_CHANNELS 16384
+#define FILARK_NOALLOC_SCRATCH_BYTES (FILARK_NOALLOC_MAX_CHANNELS * 420 + 256)
+filark_status_t filark_stream_once_noalloc(const double *sos, int n_sec, int sta_len, int lta_len, int layout,
+                                           const float *d_in, int n_ch, long long n_t, float *d_filt,
+                                           float *d_cf, cudaStream_t stream, int *cuda_error);
 
 /* Free the handle and its device memory (on the handle's device, whichever device is current).
  * NULL is accepted.  Synchronises the handle's device. */

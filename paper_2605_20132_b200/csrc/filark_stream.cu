@@ -407,6 +407,7 @@ const char* filark_status_string(filark_status_t s)
         case FILARK_ERR_CUDA: return "CUDA error";
         case FILARK_ERR_DEVICE_MISMATCH: return "current device differs from the handle's device";
         case FILARK_ERR_ALIGNMENT: return "device pointer not 4-byte aligned";
+        case FILARK_ERR_TOO_LARGE: return "more channels than the fixed device scratch of filark_stream_once_noalloc holds";
     }
     return "unknown status";
 }
@@ -1156,3 +1157,113 @@ int filark_debug_block_power(const double* sos6, long long e, double* out4)
 }
 
 }  // extern "C"
+
+// ---------------------------------------------------------------------------------------------------
+// filark_stream_once_noalloc (include/filark_stream.h): the push kernel over one record from rest, with
+// the device memory a handle would own -- carried state, raw-history rows, progress words, control block --
+// in ONE fixed array of the library's device image instead of cudaMalloc'ed buffers.
+//
+// In host code the NAME of a __device__ array is a host-side stand-in, not a device address: the address
+// the kernel gets comes from cudaGetSymbolAddress, asked once per device with that device current.
+namespace {
+
+constexpr int kNaMaxCh = FILARK_NOALLOC_MAX_CHANNELS;
+constexpr size_t kNaStateBytes = sizeof(float) * (size_t)kNaMaxCh * (size_t)state_floats(kMaxSec);
+constexpr size_t kNaHistBytes = sizeof(float) * (size_t)kNaMaxCh * (size_t)kHist;
+constexpr size_t kNaProgressBytes = sizeof(unsigned) * (size_t)kNaMaxCh;
+constexpr size_t kNaHistOff = kNaStateBytes, kNaProgressOff = kNaHistOff + kNaHistBytes, kNaCtlOff = kNaProgressOff + kNaProgressBytes;
+constexpr size_t kNaBytes = kNaCtlOff + 256;
+static_assert(kNaBytes == (size_t)FILARK_NOALLOC_SCRATCH_BYTES, "the header states the size of the array");
+static_assert(kNaHistOff % 256 == 0 && kNaProgressOff % 256 == 0 && kNaCtlOff % 256 == 0 && sizeof(CmCtl) <= 256, "aligned parts");
+
+static __device__ __align__(256) unsigned char fk_noalloc_scratch[kNaBytes];
+
+std::mutex g_na_mutex;
+unsigned char* g_na_ptr[kMaxDevices];       // device address of fk_noalloc_scratch, by device
+
+// Device address of the array on the CURRENT device (`device`).
+cudaError_t noalloc_scratch(int device, unsigned char** out)
+{
+    const bool tracked = device >= 0 && device < kMaxDevices;
+    std::lock_guard<std::mutex> lock(g_na_mutex);
+    if (tracked && g_na_ptr[device]) { *out = g_na_ptr[device]; return cudaSuccess; }
+    void* ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&ptr, fk_noalloc_scratch);
+    if (e != cudaSuccess) return e;
+    if (!ptr) return cudaErrorInvalidSymbol;
+    if (tracked) g_na_ptr[device] = (unsigned char*)ptr;
+    *out = (unsigned char*)ptr;
+    return cudaSuccess;
+}
+
+// "the last launch on this stream was not yours", for every handle (registry_is_last): a handle that pushes
+// behind this call in the same stream must not let its push start early
+const filark_stream* const kNaForeign = reinterpret_cast<const filark_stream*>(&g_na_mutex);
+
+}  // namespace
+
+extern "C" filark_status_t filark_stream_once_noalloc(const double* sos, int n_sec, int sta_len, int lta_len, int layout,
+                                                      const float* d_in, int n_ch, long long n_t, float* d_filt,
+                                                      float* d_cf, cudaStream_t stream, int* cuda_error)
+{
+    if (cuda_error) *cuda_error = 0;
+    auto fail = [&](cudaError_t e) { if (cuda_error) *cuda_error = (int)e; cudaGetLastError(); return FILARK_ERR_CUDA; };
+    filark_status_t st = check_create_args(&st, n_ch, sos, n_sec, sta_len, lta_len, layout, FILARK_FLAG_NONE);
+    if (st != FILARK_OK) return st;
+    if (n_t < 0) return FILARK_ERR_INVALID_ARG;
+    if (n_ch > kNaMaxCh) return FILARK_ERR_TOO_LARGE;
+    if (n_t == 0) return FILARK_OK;
+
+    // a handle on the stack: the design of the cascade and what the launch code reads of a handle
+    filark_stream h;
+    std::memset(&h, 0, sizeof(h));
+    st = design_all(sos, n_sec, h.sec, &h.gain);
+    if (st != FILARK_OK) return st;
+    h.lean_kinds = !tune().all_kinds;
+    for (int k = 0; k < n_sec; ++k) h.lean_kinds = h.lean_kinds && (h.sec[k].kind == kKindDF2 || h.sec[k].kind == kKindDelta);
+    h.n_ch = n_ch; h.n_sec = n_sec; h.sta_len = sta_len; h.lta_len = lta_len; h.layout = layout; h.flags = FILARK_FLAG_NONE;
+    h.state_floats = (size_t)n_ch * (size_t)state_floats(n_sec);
+
+    const long long pitch = layout == FILARK_LAYOUT_CHANNEL_MAJOR ? n_t : (long long)n_ch;
+    const ChunkArgs c{d_in, n_t, pitch, d_filt, d_cf, pitch};
+    size_t ib = 0, ob = 0;
+    st = check_chunk(&h, c, &ib, &ob);
+    if (st != FILARK_OK) return st;
+
+    cudaError_t e = cudaGetDevice(&h.device);
+    int optin = 0;
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&h.n_sm, cudaDevAttrMultiProcessorCount, h.device);
+    if (e == cudaSuccess) e = cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, h.device);
+    h.smem_optin = (size_t)optin;
+    unsigned char* base = nullptr;
+    if (e == cudaSuccess) e = noalloc_scratch(h.device, &base);
+    if (e != cudaSuccess) return fail(e);
+    h.d_state = reinterpret_cast<float*>(base);
+    h.d_hist = reinterpret_cast<float*>(base + kNaHistOff);
+    h.d_progress = reinterpret_cast<unsigned*>(base + kNaProgressOff);
+    h.d_cctl = reinterpret_cast<CmCtl*>(base + kNaCtlOff);
+
+    // the array keeps what the last call left: from rest means state, progress and control block at zero
+    // (the history rows are read only as far as the control block says, i.e. not at all)
+    e = cudaMemsetAsync(h.d_state, 0, sizeof(float) * h.state_floats, stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(h.d_progress, 0, sizeof(unsigned) * (size_t)n_ch, stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(h.d_cctl, 0, sizeof(CmCtl), stream);
+    if (e != cudaSuccess) return fail(e);
+
+    // tables of the one variant this record takes, on the stack
+    const int v = choose_variant(n_t);
+    alignas(16) unsigned char proto[sizeof(PushParams<24>)];
+    static_assert(sizeof(PushParams<24>) >= sizeof(PushParams<16>) && sizeof(PushParams<24>) >= sizeof(PushParams<8>), "largest variant");
+    h.proto[v] = proto;
+    const bool cm = layout == FILARK_LAYOUT_CHANNEL_MAJOR;
+    const uintptr_t all = (uintptr_t)d_in | (uintptr_t)d_filt | (uintptr_t)d_cf;
+    const int vec4 = cm ? ((all & 15u) == 0 && (n_t & 3) == 0) : ((((uintptr_t)d_filt | (uintptr_t)d_cf) & 15u) == 0 && (n_ch & 3) == 0);
+    switch (kVariantL[v]) {
+        case 8: build_proto<8>(&h, reinterpret_cast<PushParams<8>*>(proto)); e = push_variant<8>(&h, v, &c, 1, vec4, 1, stream); break;
+        case 16: build_proto<16>(&h, reinterpret_cast<PushParams<16>*>(proto)); e = push_variant<16>(&h, v, &c, 1, vec4, 1, stream); break;
+        default: build_proto<24>(&h, reinterpret_cast<PushParams<24>*>(proto)); e = push_variant<24>(&h, v, &c, 1, vec4, 1, stream); break;
+    }
+    registry_set(stream, kNaForeign);
+    if (e != cudaSuccess) return fail(e);
+    return FILARK_OK;
+}

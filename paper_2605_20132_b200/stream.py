@@ -23,7 +23,7 @@ MAX_SECTIONS = 16
 
 STATUS_NAMES = {0: "FILARK_OK", 1: "FILARK_ERR_INVALID_ARG", 2: "FILARK_ERR_UNSTABLE",
                 3: "FILARK_ERR_ALLOC", 4: "FILARK_ERR_CUDA", 5: "FILARK_ERR_DEVICE_MISMATCH",
-                6: "FILARK_ERR_ALIGNMENT"}
+                6: "FILARK_ERR_ALIGNMENT", 7: "FILARK_ERR_TOO_LARGE"}
 
 _lib = None
 EVENT_DTYPE = np.dtype([("t_on", "<i8"), ("t_off", "<i8"), ("channel", "<i4"), ("peak", "<f4")])   # filark_event_t
@@ -76,6 +76,8 @@ def load_library():
     lib.filark_stream_pop_events.argtypes = [vp, vp, ll, ctypes.POINTER(ll), ctypes.POINTER(ll), vp]
     lib.filark_stream_zero_phase.restype = ci
     lib.filark_stream_zero_phase.argtypes = [vp, vp, ll, vp, vp]
+    lib.filark_stream_once_noalloc.restype = ci
+    lib.filark_stream_once_noalloc.argtypes = [vp, ci, ci, ci, ci, vp, ci, ll, vp, vp, vp, ctypes.POINTER(ci)]
     lib.filark_stream_reset.restype = ci
     lib.filark_stream_reset.argtypes = [vp, vp]
     lib.filark_stream_destroy.restype = ci
@@ -108,6 +110,31 @@ def _cur_stream() -> int:
         return int(torch._C._cuda_getCurrentRawStream(torch.cuda.current_device()))
     except Exception:
         return int(torch.cuda.current_stream().cuda_stream)
+
+
+NOALLOC_MAX_CHANNELS = 16384      # FILARK_NOALLOC_MAX_CHANNELS
+
+
+def once_noalloc(sos, sta_len: int, lta_len: int, d_in, d_filt=None, d_cf=None, layout: int = CHANNEL_MAJOR,
+                 stream: Optional[int] = None):
+    """filark_stream_once_noalloc: the whole path over one dense record from rest, no handle, no allocation
+    (fixed scratch in the library's device image; at most NOALLOC_MAX_CHANNELS channels; calls that overlap
+    on the GPU race on that scratch)."""
+    import torch
+    lib = load_library()
+    sos = np.ascontiguousarray(np.asarray(sos, dtype=np.float64))
+    if sos.ndim != 2 or sos.shape[1] != 6:
+        raise ValueError("sos must be [n_sec][6]")
+    for t in (d_in, d_filt, d_cf):
+        if t is not None and (not t.is_cuda or t.dtype != torch.float32 or not t.is_contiguous() or t.dim() != 2):
+            raise ValueError("buffers must be contiguous 2-D float32 CUDA tensors")
+    n_ch, n_t = (d_in.shape[0], d_in.shape[1]) if layout == CHANNEL_MAJOR else (d_in.shape[1], d_in.shape[0])
+    err = ctypes.c_int(0)
+    st = lib.filark_stream_once_noalloc(sos.ctypes.data, int(sos.shape[0]), int(sta_len), int(lta_len), int(layout),
+                                        _ptr(d_in), int(n_ch), int(n_t), _ptr(d_filt), _ptr(d_cf),
+                                        _cur_stream() if stream is None else stream, ctypes.byref(err))
+    if st != 0:
+        raise FilarkError(st, "filark_stream_once_noalloc", f"(cudaError {err.value})" if st == 4 else "")
 
 
 class PushBatch:

@@ -42,7 +42,7 @@ def test_library_exports_every_declared_symbol(lib):
 
 def test_status_strings(lib):
     l = lib.load_library()
-    for code in range(7):
+    for code in range(8):
         assert l.filark_status_string(code)
 
 
