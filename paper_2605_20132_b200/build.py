@@ -4,6 +4,7 @@
 """
 from __future__ import annotations
 
+import glob
 import os
 import subprocess
 import sys
@@ -12,10 +13,8 @@ _PKG = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_PKG, "csrc")
 LIB_PATH = os.path.join(_PKG, "libfilark_stream.so")
 SOURCES = [os.path.join(_CSRC, "filark_stream.cu"), os.path.join(_CSRC, "filark_ops.cu")]
-DEPENDS = SOURCES + [os.path.join(_CSRC, "filark_kernels.cuh"), os.path.join(_CSRC, "design.hpp"),
-                     os.path.join(os.path.dirname(_PKG), "include", "filark_stream.h"),
-                     os.path.join(os.path.dirname(_PKG), "include", "filark_debug.h"),
-                     os.path.join(os.path.dirname(_PKG), "include", "filark_ops.h")]
+# every file under csrc/ and include/ (kernels and tables live in headers)
+DEPENDS = sorted(glob.glob(os.path.join(_CSRC, "*")) + glob.glob(os.path.join(os.path.dirname(_PKG), "include", "*.h")))
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--use_fast_math=false"]
 

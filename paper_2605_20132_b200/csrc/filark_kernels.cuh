@@ -193,10 +193,12 @@ __device__ __forceinline__ unsigned ld_acquire(const unsigned* p)
     asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
-// Polls of `progress` and of the control block are relaxed loads at gpu scope (served by L2, no
-// fence behind them, so that they can be issued early and consumed late).  Everything they guard
-// (state, hist, control slots) was written before a release at gpu scope and is only ever read
-// with loads that bypass L1 (cp.async.cg, ld.global.cg) issued after the poll has returned.
+// `progress`: the FIRST look at a word (asked for early, where the warp has other latency to sit out) is an
+// acquire load at gpu scope; if its value already suffices -- the usual case -- nothing more is needed.
+// Otherwise the warp polls with relaxed loads (served by L2, no fence behind them) and ends with one more
+// acquire load.  Everything these guard (state, hist) was written before a release at gpu scope and is read
+// with loads that bypass L1 (cp.async.cg, ld.relaxed.gpu) issued after the acquire has returned.  The
+// control block is read with relaxed loads: its slots are complete before the grid can launch (below).
 __device__ __forceinline__ unsigned ld_relaxed(const unsigned* p)
 {
     unsigned v;
@@ -1084,7 +1086,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     // the answer is there when the control slot says what to compare it with
     // (static work distribution only: a claimed first item can be any channel)
     unsigned pr0 = 0;
-    if (!kDyn && gw < p.n_ch) pr0 = ld_relaxed(p.progress + gw);
+    if (!kDyn && gw < p.n_ch) pr0 = ld_acquire(p.progress + gw);
 
     // ---- control slot of this push.  Nothing changes epoch or slot[epoch & 1] between the launch of
     // this grid (after every CTA of the previous push had taken its ticket and the last of them
@@ -1212,7 +1214,10 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
     // path for everything after it)
     auto wait_progress = [&](int ch, unsigned need, unsigned have_val) {
         unsigned done = __shfl_sync(0xffffffffu, have_val, 0);
-        while ((int)(done - need) < 0) done = __shfl_sync(0xffffffffu, ld_relaxed(p.progress + ch), 0);
+        if ((int)(done - need) < 0) {
+            do done = __shfl_sync(0xffffffffu, ld_relaxed(p.progress + ch), 0); while ((int)(done - need) < 0);
+            (void)ld_acquire(p.progress + ch);       // (the acquire that goes with the release of the value the polls saw)
+        }
     };
 
     int ch = 0, gt = 0, gtend = 0, seg = 0, cg = 0, cur = 0, wcur = 0, k = 0;
@@ -1239,7 +1244,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         // the first segment of a channel needs what the previous launch left (state, hist): wait before
         // those loads are issued (a wait on an EARLIER launch cannot be part of a cycle)
         if (seg == 0 && ch < p.n_ch) {
-            wait_progress(ch, seq0, kDyn ? ld_relaxed(p.progress + ch) : pr0);
+            wait_progress(ch, seq0, kDyn ? ld_acquire(p.progress + ch) : pr0);
             issue_tile_carry<L>(p, g, ch, whs, wst0, lane);
         }
     }
@@ -1286,7 +1291,7 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
             if (!dyn || !kTM) {
                 nhave = claim_take(nch, ngt, ngtend, nseg, ncg);
                 if (dyn) claim_issue();
-                if (nhave && nseg == 0 && nch < p.n_ch) npr = ld_relaxed(p.progress + nch);      // used after the tile is in registers
+                if (nhave && nseg == 0 && nch < p.n_ch) npr = ld_acquire(p.progress + nch);      // used after the tile is in registers
             } else if (threadIdx.x == 0) {
                 sh_item = pend;
             }
@@ -1300,14 +1305,14 @@ filark_push_cm_kernel(const __grid_constant__ PushParams<L> p)
         if (kTM && dyn && item_end) {
             nhave = claim_take(nch, ngt, ngtend, nseg, ncg);
             claim_issue();
-            if (nhave && nseg == 0 && nch < p.n_ch) npr = ld_relaxed(p.progress + nch);
+            if (nhave && nseg == 0 && nch < p.n_ch) npr = ld_acquire(p.progress + nch);
         }
         if (item_end && nhave) nk = chunk_of(ngt);
         nk = __shfl_sync(0xffffffffu, nk, 0);
         if (valid && seg > 0 && item_first) {
             // first tile of a later segment: wait for the segment before it, then fetch its state (and,
             // where the segment begins with a chunk, the raw samples waiting in front of that chunk)
-            wait_progress(ch, seq0 + (unsigned)seg, ld_relaxed(p.progress + ch));
+            wait_progress(ch, seq0 + (unsigned)seg, ld_acquire(p.progress + ch));
             const float* gst = p.state + (long long)ch * ns;
             if (lane < ns) fk_smem[wst + lane] = ld_relaxed_f32(gst + lane);
             if (lane + 32 < ns) fk_smem[wst + lane + 32] = ld_relaxed_f32(gst + lane + 32);
