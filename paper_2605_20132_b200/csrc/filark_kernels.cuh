@@ -811,7 +811,7 @@ __device__ __noinline__ void trigger_tile(const PushParams<L>& p, int buf, int s
 // (kTM: time-major chunk; the CTA's warps hold the channels cg kTmChannels + warp and store together;
 // `bufoff` = buf relative to the warp's shared-memory area; `item_end` is false for a warp whose
 // channel does not exist)
-// kForm: 0 = the two common section forms only, 1 = every section form, 2 = every form + the trigger
+// kForm: 0 = the two common section forms only, 1 = every section form, 2 / 3 = the same two + the trigger
 // (filark_stream_set_trigger): a push kernel without a trigger set carries none of its code.
 template <int L, bool kInterior, int kForm, bool kTM, bool kShift>
 __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk& ck, const Geom& g, int buf, int wst, float2 (&x)[L],
@@ -819,7 +819,7 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
                                              bool item_end, unsigned rel_val, int cg, int bufoff,
                                              const TimeOrder<L>& to, TmPrefetch<L>* pf = nullptr)
 {
-    constexpr bool kAllKinds = kForm >= 1, kTrig = kForm == 2;
+    constexpr bool kAllKinds = (kForm & 1) != 0, kTrig = kForm >= 2;
     const bool last = tile == g.n_tiles - 1;
     const int t0 = tile * Geo<L>::tile - g.r0;
     // the carried state moves to the end of the tile's last FULL slot (slot q - 1)

@@ -311,8 +311,9 @@ static cudaError_t launch_cm_shape(const filark_stream* h, PushParams<L>& p, cud
     return launch_cm_variant<L, CTAS, kForm, true>(p, h->device, grid, W, smem, smem_max, stream);
 }
 
-// Kernel form (filark_kernels.cuh, process_tile): lean section forms / all forms / all forms + trigger.
-static int kernel_form(const filark_stream* h) { return h->thr_on > 0.0f ? 2 : (h->lean_kinds ? 0 : 1); }
+// Kernel form (filark_kernels.cuh, process_tile): bit 0 = every section form (not only the two a Butterworth
+// band-pass gives), bit 1 = the trigger.
+static int kernel_form(const filark_stream* h) { return (h->thr_on > 0.0f ? 2 : 0) + (h->lean_kinds ? 0 : 1); }
 
 // Launch shape (filark_kernels.cuh): one CTA per SM when every resident warp gets a long run of tiles
 // anyway, small CTAs otherwise.  (L = 24 is the only variant long pushes ever use.)
@@ -326,10 +327,12 @@ static cudaError_t launch_cm(const filark_stream* h, PushParams<L>& p, cudaStrea
         const bool long_push = n_tiles_max * p.n_ch >= 12LL * h->n_sm * cm_max_warps<L>();
         if (long_push && !tune().small_ctas)
             return form == 0 ? launch_cm_shape<L, 1, 0>(h, p, stream)
-                             : (form == 1 ? launch_cm_shape<L, 1, 1>(h, p, stream) : launch_cm_shape<L, 1, 2>(h, p, stream));
+                             : (form == 1 ? launch_cm_shape<L, 1, 1>(h, p, stream)
+                                          : (form == 2 ? launch_cm_shape<L, 1, 2>(h, p, stream) : launch_cm_shape<L, 1, 3>(h, p, stream)));
     }
     return form == 0 ? launch_cm_shape<L, kCmCtasPerSm, 0>(h, p, stream)
-                     : (form == 1 ? launch_cm_shape<L, kCmCtasPerSm, 1>(h, p, stream) : launch_cm_shape<L, kCmCtasPerSm, 2>(h, p, stream));
+                     : (form == 1 ? launch_cm_shape<L, kCmCtasPerSm, 1>(h, p, stream)
+                                  : (form == 2 ? launch_cm_shape<L, kCmCtasPerSm, 2>(h, p, stream) : launch_cm_shape<L, kCmCtasPerSm, 3>(h, p, stream)));
 }
 
 // Time-major chunks: the same kernel with the transpose in shared memory (filark_kernels.cuh): one CTA
@@ -365,7 +368,9 @@ template <int L>
 static cudaError_t launch_tm(const filark_stream* h, PushParams<L>& p, cudaStream_t stream)
 {
     const int form = kernel_form(h);
-    return form == 0 ? launch_tm_kinds<L, 0>(h, p, stream) : (form == 1 ? launch_tm_kinds<L, 1>(h, p, stream) : launch_tm_kinds<L, 2>(h, p, stream));
+    return form == 0 ? launch_tm_kinds<L, 0>(h, p, stream)
+                     : (form == 1 ? launch_tm_kinds<L, 1>(h, p, stream)
+                                  : (form == 2 ? launch_tm_kinds<L, 2>(h, p, stream) : launch_tm_kinds<L, 3>(h, p, stream)));
 }
 
 // One chunk as the caller describes it (all pushes end up here).
