@@ -131,11 +131,19 @@ __device__ __forceinline__ float lin_at(const float* row, long long stride, long
 }
 
 // Channel-major: grid (column groups, channels).  Narrow columns (<= 32 samples): one thread per column
-// (a warp reads 32 adjacent columns: one contiguous stretch of the row).  Wide columns: one warp per
-// column, lanes stride through it (coalesced), the largest magnitude -- the first one on ties -- by a
-// shuffle reduction on (magnitude, position).
+// (a warp reads 32 adjacent columns: one contiguous stretch of the row).  Wide columns, peak mode: a warp
+// takes 32 adjacent columns at a time, copies their stretch of the row into its slice of shared memory with
+// coalesced loads (one read of every sample) and every lane then walks its own column there; stretches
+// longer than the slice (columns of more than 64 samples) go column by column, the lanes striding through a
+// column and the largest magnitude -- the first one on ties -- found by a shuffle reduction on
+// (magnitude, position).
+constexpr int kDecSlice = 2048;                                   // samples of a warp's slice
+constexpr size_t kDecSmemBytes = sizeof(float) * 4 * (kDecSlice + kDecSlice / 32 + 1);
+__device__ __forceinline__ int dec_at(int i) { return i + (i >> 5); }   // (one pad per 32: the lanes' columns start in different banks)
+
 __global__ void __launch_bounds__(128) filark_decimate_cm_kernel(const __grid_constant__ DecParams p)
 {
+    extern __shared__ float dec_slices[];            // wide columns in peak mode only: 4 slices (kDecSmemBytes)
     const int ch = blockIdx.y;
     const float* __restrict__ row = p.in + (long long)ch * p.pitch;
     float* __restrict__ orow = p.out + (long long)ch * p.width;
@@ -163,23 +171,50 @@ __global__ void __launch_bounds__(128) filark_decimate_cm_kernel(const __grid_co
         orow[j] = v;
         return;
     }
-    for (int j = blockIdx.x * 4 + warp; j < p.width; j += gridDim.x * 4) {
-        const long long a = col_start(j, p.n_t, p.width);
-        long long b = col_start(j + 1, p.n_t, p.width);
-        if (b <= a) b = a + 1;
-        float v = 0.0f, best = -1.0f;
-        long long at = b;
-        for (long long n = a + lane; n < b; n += 32) {
-            const float s = row[n];
-            if (fabsf(s) > best) { best = fabsf(s); v = s; at = n; }
-        }
+    float* s = dec_slices + warp * (kDecSlice + kDecSlice / 32 + 1);
+    for (int j0 = (blockIdx.x * 4 + warp) * 32; j0 < p.width; j0 += gridDim.x * 4 * 32) {
+        const int j1 = min(p.width, j0 + 32);
+        const long long a0 = col_start(j0, p.n_t, p.width), a1 = col_start(j1, p.n_t, p.width);
+        if (a1 - a0 <= kDecSlice) {
+            const int len = (int)(a1 - a0);
+            // (eight loads in flight per lane: the copy is the part that waits for memory)
+            for (int i0 = lane; i0 < len; i0 += 256) {
+                float v[8];
 #pragma unroll
-        for (int d = 16; d > 0; d >>= 1) {
-            const float ob = __shfl_xor_sync(0xffffffffu, best, d), ov = __shfl_xor_sync(0xffffffffu, v, d);
-            const long long oa = __shfl_xor_sync(0xffffffffu, at, d);
-            if (ob > best || (ob == best && oa < at)) { best = ob; v = ov; at = oa; }
+                for (int u = 0; u < 8; ++u) v[u] = i0 + 32 * u < len ? __ldcs(row + a0 + i0 + 32 * u) : 0.0f;
+#pragma unroll
+                for (int u = 0; u < 8; ++u) if (i0 + 32 * u < len) s[dec_at(i0 + 32 * u)] = v[u];
+            }
+            __syncwarp();
+            const int j = j0 + lane;
+            if (j < j1) {
+                const int a = (int)(col_start(j, p.n_t, p.width) - a0), b = (int)(col_start(j + 1, p.n_t, p.width) - a0);
+                float v = s[dec_at(a)], best = fabsf(v);
+                for (int n = a + 1; n < b; ++n) {
+                    const float x = s[dec_at(n)];
+                    if (fabsf(x) > best) { best = fabsf(x); v = x; }
+                }
+                orow[j] = v;
+            }
+            __syncwarp();
+            continue;
         }
-        if (lane == 0) orow[j] = v;
+        for (int j = j0; j < j1; ++j) {
+            const long long a = col_start(j, p.n_t, p.width), b = col_start(j + 1, p.n_t, p.width);
+            float v = 0.0f, best = -1.0f;
+            long long at = b;
+            for (long long n = a + lane; n < b; n += 32) {
+                const float x = row[n];
+                if (fabsf(x) > best) { best = fabsf(x); v = x; at = n; }
+            }
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) {
+                const float ob = __shfl_xor_sync(0xffffffffu, best, d), ov = __shfl_xor_sync(0xffffffffu, v, d);
+                const long long oa = __shfl_xor_sync(0xffffffffu, at, d);
+                if (ob > best || (ob == best && oa < at)) { best = ob; v = ov; at = oa; }
+            }
+            if (lane == 0) orow[j] = v;
+        }
     }
 }
 
@@ -311,9 +346,9 @@ filark_status_t filark_decimate(const float* d_in, int n_ch, long long n_t, long
     if (cm) {
         if (n_ch > 65535) return FILARK_ERR_INVALID_ARG;
         const bool per_thread = mode != FILARK_DECIMATE_PEAK || n_t <= 32LL * width;
-        int gx = per_thread ? (width + 127) / 128 : (width + 3) / 4;
+        int gx = (width + 127) / 128;                 // 128 columns per block either way (wide: 32 per warp)
         if (!per_thread && gx > 64) gx = 64;
-        filark_decimate_cm_kernel<<<dim3((unsigned)gx, (unsigned)n_ch), 128, 0, stream>>>(p);
+        filark_decimate_cm_kernel<<<dim3((unsigned)gx, (unsigned)n_ch), 128, per_thread ? 0 : kDecSmemBytes, stream>>>(p);
     } else {
         int gy = (width + 31) / 32;
         if (gy > 65535) gy = 65535;
