@@ -220,6 +220,42 @@ class OracleTrigger:
     __del__ = close
 
 
+BOX_DTYPE = np.dtype([("t_on", "<i8"), ("t_off", "<i8"), ("ch_lo", "<i4"), ("ch_hi", "<i4"), ("peak", "<f4"),
+                      ("n_events", "<i4")])
+
+
+def oracle_associate(events: np.ndarray, ch_gap: int, t_gap: int) -> np.ndarray:
+    """Per-channel trigger events -> time-channel-bounded events ("(t_on, t_off, channel
+    range, peak cf) -- the monitor contract's actual output"; "a list of time-channel-bounded
+    events", :132 "each described by a time and channel extent").  The paper gives no rule; reading R30 in
+    DESIGN.md, written out as it is defined:
+
+      two events are LINKED if their channels differ by at most ch_gap and their half-open intervals
+      [t_on, t_off) come within t_gap samples of each other:  t_on1 < t_off2 + t_gap  and  t_on2 < t_off1 + t_gap
+      (t_gap = 0: they overlap);
+      a BOX is a connected component of the link graph: t_on = the smallest t_on, t_off = the largest t_off,
+      [ch_lo, ch_hi] = the channel extent, peak = the largest peak, n_events = its size;
+      boxes are listed in rising (t_on, ch_lo, t_off, ch_hi).
+
+    The link matrix is built by comparing every pair; the components come from scipy's
+    connected_components (a library primitive as one step)."""
+    from scipy.sparse import csr_matrix
+    from scipy.sparse.csgraph import connected_components
+    ev = np.asarray(events, dtype=EVENT_DTYPE)
+    n = ev.shape[0]
+    if n == 0:
+        return np.zeros(0, dtype=BOX_DTYPE)
+    ch = ev["channel"].astype(np.int64); t0 = ev["t_on"].astype(np.int64); t1 = ev["t_off"].astype(np.int64)
+    link = (np.abs(ch[:, None] - ch[None, :]) <= int(ch_gap)) & (t0[:, None] < t1[None, :] + int(t_gap)) & \
+           (t0[None, :] < t1[:, None] + int(t_gap))
+    n_box, label = connected_components(csr_matrix(link), directed=False)
+    out = np.zeros(n_box, dtype=BOX_DTYPE)
+    for b in range(n_box):
+        m = ev[label == b]
+        out[b] = (m["t_on"].min(), m["t_off"].max(), m["channel"].min(), m["channel"].max(), m["peak"].max(), m.shape[0])
+    return out[np.lexsort((out["ch_hi"], out["t_off"], out["ch_lo"], out["t_on"]))]
+
+
 def oracle_zero_phase(x: np.ndarray, sos) -> np.ndarray:
     """Zero-phase (forward-backward) filtering of a bounded window, channel-major x [n_ch][n_t]
     (PAPER.md:77 the display filter is "either a zero-phase or causal IIR filter ...

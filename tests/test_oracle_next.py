@@ -267,3 +267,104 @@ def test_zero_phase_commutes_with_time_reversal():
     assert np.abs(a - b).max() <= 1e-5
     # no delay: the output of a symmetric pulse is symmetric about the same centre
     assert np.abs(a[0, 2000:4000] - a[0, 2000:4000][::-1]).max() <= 1e-2 * a.max()
+
+
+# ---- NEXT-1, second half: per-channel events -> time-channel boxes (reading R30) ----------------------
+import os  # noqa: E402
+
+from oracle import BOX_DTYPE, EVENT_DTYPE, oracle_associate  # noqa: E402
+
+
+def _read_associate_golden():
+    ev, boxes = [], {"B": [], "C": [], "D": []}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "associate_small.txt")):
+        f = line.split()
+        if not f or f[0] == "#":
+            continue
+        if f[0] == "E":
+            ev.append((int(f[1]), int(f[2]), int(f[3]), float(f[4])))
+        else:
+            boxes[f[0]].append((int(f[1]), int(f[2]), int(f[3]), int(f[4]), float(f[5]), int(f[6])))
+    return np.array(ev, dtype=EVENT_DTYPE), {k: np.array(v, dtype=BOX_DTYPE) for k, v in boxes.items()}
+
+
+def test_associate_worked_example():
+    """The hand-derived fixture (tests/golden/associate_small.txt), three settings of the two gaps."""
+    ev, want = _read_associate_golden()
+    for key, (cg, tg) in {"B": (1, 0), "C": (2, 0), "D": (1, 60)}.items():
+        got = oracle_associate(ev, cg, tg)
+        assert got.tolist() == want[key].tolist(), key
+        # the order of the input does not matter
+        assert oracle_associate(ev[::-1], cg, tg).tolist() == want[key].tolist()
+
+
+def _associate_brute(ev, ch_gap, t_gap):
+    """Union-find in plain Python loops over every pair (tiny inputs only)."""
+    n = len(ev)
+    parent = list(range(n))
+
+    def find(i):
+        while parent[i] != i:
+            i = parent[i]
+        return i
+    for i in range(n):
+        for j in range(i):
+            a, b = ev[i], ev[j]
+            if abs(int(a["channel"]) - int(b["channel"])) <= ch_gap and a["t_on"] < b["t_off"] + t_gap and b["t_on"] < a["t_off"] + t_gap:
+                parent[find(i)] = find(j)
+    groups = {}
+    for i in range(n):
+        groups.setdefault(find(i), []).append(i)
+    out = []
+    for idx in groups.values():
+        m = ev[idx]
+        out.append((int(m["t_on"].min()), int(m["t_off"].max()), int(m["channel"].min()), int(m["channel"].max()),
+                    float(m["peak"].max()), len(idx)))
+    return sorted(out, key=lambda b: (b[0], b[2], b[1], b[3]))
+
+
+def _random_events(rng, n, n_ch, t_max, dur):
+    t_on = rng.integers(0, t_max, n)
+    ev = np.zeros(n, dtype=EVENT_DTYPE)
+    ev["t_on"] = t_on; ev["t_off"] = t_on + rng.integers(1, dur, n)
+    ev["channel"] = rng.integers(0, n_ch, n); ev["peak"] = rng.random(n).astype(np.float32) * 10
+    return ev
+
+
+@pytest.mark.parametrize("seed", range(6))
+def test_associate_equals_pairwise_union_find(seed):
+    rng = np.random.default_rng(seed)
+    ev = _random_events(rng, 60, 12, 400, 60)
+    for cg, tg in ((0, 0), (1, 0), (1, 25), (3, 5)):
+        got = oracle_associate(ev, cg, tg)
+        assert [tuple(b) for b in got.tolist()] == _associate_brute(ev, cg, tg)
+
+
+def test_associate_invariants_and_special_cases():
+    rng = np.random.default_rng(42)
+    ev = _random_events(rng, 500, 40, 5000, 80)
+    boxes = oracle_associate(ev, 1, 0)
+    assert boxes["n_events"].sum() == ev.shape[0]                       # every event in exactly one box
+    assert np.all(boxes["t_on"] < boxes["t_off"]) and np.all(boxes["ch_lo"] <= boxes["ch_hi"])
+    for e in ev:                                                        # ... and inside some box of at least its peak
+        inside = (boxes["t_on"] <= e["t_on"]) & (e["t_off"] <= boxes["t_off"]) & (boxes["ch_lo"] <= e["channel"]) & \
+                 (e["channel"] <= boxes["ch_hi"]) & (boxes["peak"] >= e["peak"])
+        assert inside.any()
+    # gaps so large that everything is linked: one box, the bounding box of all events
+    one = oracle_associate(ev, 1000, 10**9)
+    assert one.shape[0] == 1 and one[0]["n_events"] == 500
+    assert (one[0]["t_on"], one[0]["t_off"], one[0]["ch_lo"], one[0]["ch_hi"]) == \
+           (ev["t_on"].min(), ev["t_off"].max(), ev["channel"].min(), ev["channel"].max())
+    assert one[0]["peak"] == ev["peak"].max()
+    # larger gaps only merge: the number of boxes never grows
+    assert oracle_associate(ev, 2, 0).shape[0] <= boxes.shape[0] and oracle_associate(ev, 1, 50).shape[0] <= boxes.shape[0]
+    # events that cannot be linked (one per channel, channels two apart): the identity
+    lone = np.zeros(5, dtype=EVENT_DTYPE)
+    lone["t_on"] = 10; lone["t_off"] = 20; lone["channel"] = np.arange(5) * 2; lone["peak"] = 1.0
+    b = oracle_associate(lone, 1, 0)
+    assert b.shape[0] == 5 and np.all(b["n_events"] == 1) and b["ch_lo"].tolist() == [0, 2, 4, 6, 8]
+    # touching intervals do not overlap (half-open): [10, 20) and [20, 30) on adjacent channels
+    two = np.zeros(2, dtype=EVENT_DTYPE)
+    two["t_on"] = [10, 20]; two["t_off"] = [20, 30]; two["channel"] = [3, 4]; two["peak"] = 1.0
+    assert oracle_associate(two, 1, 0).shape[0] == 2 and oracle_associate(two, 1, 1).shape[0] == 1
+    assert oracle_associate(np.zeros(0, dtype=EVENT_DTYPE), 1, 0).shape[0] == 0
