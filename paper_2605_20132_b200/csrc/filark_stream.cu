@@ -14,6 +14,7 @@
 #include <mutex>
 #include <new>
 #include <algorithm>
+#include <map>
 #include <unordered_map>
 #include <vector>
 
@@ -1270,5 +1271,71 @@ extern "C" filark_status_t filark_stream_once_noalloc(const double* sos, int n_s
     }
     registry_set(stream, kNaForeign);
     if (e != cudaSuccess) return fail(e);
+    return FILARK_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------
+// filark_events_associate (include/filark_stream.h; reading R30): host work on a host list.
+extern "C" filark_status_t filark_events_associate(const filark_event_t* ev, long long n, int ch_gap, long long t_gap,
+                                                   filark_box_t* boxes, long long cap, long long* n_boxes)
+{
+    if (!n_boxes || n < 0 || cap < 0 || ch_gap < 0 || t_gap < 0 || (n > 0 && !ev) || (cap > 0 && !boxes) || n > 0x7fffffffLL)
+        return FILARK_ERR_INVALID_ARG;
+    *n_boxes = 0;
+    if (n == 0) return FILARK_OK;
+    try {
+        const int m = (int)n;
+        std::vector<int> order(m), parent(m);
+        for (int i = 0; i < m; ++i) order[i] = parent[i] = i;
+        std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return ev[a].t_on < ev[b].t_on; });
+        auto find = [&](int i) { while (parent[i] != i) { parent[i] = parent[parent[i]]; i = parent[i]; } return i; };
+        // events still within reach of a later one, by channel.  In rising t_on an event j is out of reach
+        // for good once t_off[j] + t_gap <= t_on of the event at hand.
+        std::map<int, std::vector<int>> active;
+        for (int oi = 0; oi < m; ++oi) {
+            const int i = order[oi];
+            const filark_event_t& e = ev[i];
+            const long long lo = (long long)e.channel - ch_gap, hi = (long long)e.channel + ch_gap;
+            for (auto it = active.lower_bound((int)std::max(lo, (long long)INT32_MIN)); it != active.end() && it->first <= hi;) {
+                std::vector<int>& v = it->second;
+                size_t keep = 0;
+                for (size_t q = 0; q < v.size(); ++q) {
+                    const filark_event_t& o = ev[v[q]];
+                    if (o.t_off + t_gap <= e.t_on) continue;                     // out of reach for good
+                    v[keep++] = v[q];
+                    if (o.t_on < e.t_off + t_gap) { const int a = find(i), b = find(v[q]); if (a != b) parent[a] = b; }
+                }
+                v.resize(keep);
+                if (v.empty()) it = active.erase(it); else ++it;
+            }
+            active[e.channel].push_back(i);
+        }
+        std::vector<int> box_of(m, -1);
+        std::vector<filark_box_t> out;
+        for (int i = 0; i < m; ++i) {
+            const int r = find(i);
+            const filark_event_t& e = ev[i];
+            if (box_of[r] < 0) {
+                box_of[r] = (int)out.size();
+                out.push_back(filark_box_t{e.t_on, e.t_off, e.channel, e.channel, e.peak, 1});
+            } else {
+                filark_box_t& b = out[(size_t)box_of[r]];
+                b.t_on = std::min(b.t_on, e.t_on); b.t_off = std::max(b.t_off, e.t_off);
+                b.ch_lo = std::min(b.ch_lo, e.channel); b.ch_hi = std::max(b.ch_hi, e.channel);
+                b.peak = std::max(b.peak, e.peak); b.n_events += 1;
+            }
+        }
+        std::stable_sort(out.begin(), out.end(), [](const filark_box_t& a, const filark_box_t& b) {
+            if (a.t_on != b.t_on) return a.t_on < b.t_on;
+            if (a.ch_lo != b.ch_lo) return a.ch_lo < b.ch_lo;
+            if (a.t_off != b.t_off) return a.t_off < b.t_off;
+            return a.ch_hi < b.ch_hi;
+        });
+        *n_boxes = (long long)out.size();
+        const size_t w = std::min((size_t)cap, out.size());
+        for (size_t i = 0; i < w; ++i) boxes[i] = out[i];
+    } catch (const std::bad_alloc&) {
+        return FILARK_ERR_ALLOC;
+    }
     return FILARK_OK;
 }

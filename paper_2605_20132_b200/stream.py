@@ -76,6 +76,8 @@ def load_library():
     lib.filark_stream_pop_events.argtypes = [vp, vp, ll, ctypes.POINTER(ll), ctypes.POINTER(ll), vp]
     lib.filark_stream_zero_phase.restype = ci
     lib.filark_stream_zero_phase.argtypes = [vp, vp, ll, vp, vp]
+    lib.filark_events_associate.restype = ci
+    lib.filark_events_associate.argtypes = [vp, ll, ci, ll, vp, ll, ctypes.POINTER(ll)]
     lib.filark_stream_once_noalloc.restype = ci
     lib.filark_stream_once_noalloc.argtypes = [vp, ci, ci, ci, ci, vp, ci, ll, vp, vp, vp, ctypes.POINTER(ci)]
     lib.filark_stream_reset.restype = ci
@@ -110,6 +112,25 @@ def _cur_stream() -> int:
         return int(torch._C._cuda_getCurrentRawStream(torch.cuda.current_device()))
     except Exception:
         return int(torch.cuda.current_stream().cuda_stream)
+
+
+BOX_DTYPE = np.dtype([("t_on", "<i8"), ("t_off", "<i8"), ("ch_lo", "<i4"), ("ch_hi", "<i4"), ("peak", "<f4"),
+                      ("n_events", "<i4")])   # filark_box_t
+
+
+def associate_events(events, ch_gap: int = 1, t_gap: int = 0, cap: Optional[int] = None):
+    """filark_events_associate: per-channel events (EVENT_DTYPE, as pop_events returns them) -> time-channel
+    boxes (BOX_DTYPE); a host function.  Returns (boxes, number of boxes found)."""
+    lib = load_library()
+    ev = np.ascontiguousarray(events, dtype=EVENT_DTYPE)
+    cap = ev.shape[0] if cap is None else int(cap)
+    out = np.zeros(max(cap, 1), dtype=BOX_DTYPE)
+    n = ctypes.c_longlong(0)
+    st = lib.filark_events_associate(ev.ctypes.data if ev.shape[0] else None, ev.shape[0], int(ch_gap), int(t_gap),
+                                     out.ctypes.data, cap, ctypes.byref(n))
+    if st != 0:
+        raise FilarkError(st, "filark_events_associate")
+    return out[:min(cap, n.value)].copy(), int(n.value)
 
 
 NOALLOC_MAX_CHANNELS = 16384      # FILARK_NOALLOC_MAX_CHANNELS

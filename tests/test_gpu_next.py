@@ -202,6 +202,29 @@ def test_trigger_events_match_the_oracle(cuda_device, layout, sizes, many):
     s.destroy()
 
 
+def test_events_to_time_channel_boxes(cuda_device):
+    """NEXT-1's output form: the events the trigger emitted on the GPU, associated into time-channel boxes by
+    filark_events_associate, against the oracle's association of the same list (reading R30); and the boxes
+    of the cfg3 recipe's moving sources do span channel ranges."""
+    from oracle import oracle_associate
+    from paper_2605_20132_b200.stream import associate_events
+    w = CONFIGS["cfg3"].scaled(n_ch=400, n_t=45_000)
+    sos = design_sos(w)
+    xd = generate(w, device="cpu").to(cuda_device)
+    s = FilarkStream(w.n_ch, sos, w.sta_len, w.lta_len)
+    s.set_trigger(4.0, 2.0, 1 << 18)
+    s.push(xd, None, torch.empty_like(xd))
+    ev, dropped = s.pop_events()
+    s.destroy()
+    assert dropped == 0 and len(ev) > 50
+    for ch_gap, t_gap in ((1, 0), (2, 75)):
+        boxes, total = associate_events(ev, ch_gap, t_gap)
+        ref = oracle_associate(ev, ch_gap, t_gap)
+        assert total == ref.shape[0] and sorted(map(tuple, boxes.tolist())) == sorted(map(tuple, ref.tolist()))
+        assert boxes["n_events"].sum() == len(ev)
+    assert total < len(ev) and (boxes["ch_hi"] - boxes["ch_lo"]).max() >= 3       # arrivals seen on neighbouring channels merge
+
+
 def test_trigger_without_cf_output_and_list_overflow(cuda_device):
     """Events only (d_cf = NULL, filt kept): same events; a short list drops and counts the rest;
     thr_on = thr_off = 0 switches the trigger off; a pop with too little room consumes nothing."""
