@@ -117,6 +117,7 @@ struct DecParams {
     float* out;
     long long n_t, pitch;
     int n_ch, width, mode;
+    int slice;               // channel-major peak mode: samples a warp can stage (0: column by column)
 };
 __device__ __forceinline__ long long col_start(long long j, long long n_t, int width) { return j * n_t / width; }
 
@@ -138,7 +139,7 @@ __device__ __forceinline__ float lin_at(const float* row, long long stride, long
 // column and the largest magnitude -- the first one on ties -- found by a shuffle reduction on
 // (magnitude, position).
 constexpr int kDecSlice = 2048;                                   // samples of a warp's slice
-constexpr size_t kDecSmemBytes = sizeof(float) * 4 * (kDecSlice + kDecSlice / 32 + 1);
+// (a launch asks for the slice its columns need: 32 columns of ceil(n_t / width) samples, at most kDecSlice)
 __device__ __forceinline__ int dec_at(int i) { return i + (i >> 5); }   // (one pad per 32: the lanes' columns start in different banks)
 
 __global__ void __launch_bounds__(128) filark_decimate_cm_kernel(const __grid_constant__ DecParams p)
@@ -171,11 +172,11 @@ __global__ void __launch_bounds__(128) filark_decimate_cm_kernel(const __grid_co
         orow[j] = v;
         return;
     }
-    float* s = dec_slices + warp * (kDecSlice + kDecSlice / 32 + 1);
+    float* s = dec_slices + warp * (p.slice + p.slice / 32 + 1);
     for (int j0 = (blockIdx.x * 4 + warp) * 32; j0 < p.width; j0 += gridDim.x * 4 * 32) {
         const int j1 = min(p.width, j0 + 32);
         const long long a0 = col_start(j0, p.n_t, p.width), a1 = col_start(j1, p.n_t, p.width);
-        if (a1 - a0 <= kDecSlice) {
+        if (a1 - a0 <= p.slice) {
             const int len = (int)(a1 - a0);
             // (eight loads in flight per lane: the copy is the part that waits for memory)
             for (int i0 = lane; i0 < len; i0 += 256) {
@@ -190,7 +191,15 @@ __global__ void __launch_bounds__(128) filark_decimate_cm_kernel(const __grid_co
             if (j < j1) {
                 const int a = (int)(col_start(j, p.n_t, p.width) - a0), b = (int)(col_start(j + 1, p.n_t, p.width) - a0);
                 float v = s[dec_at(a)], best = fabsf(v);
-                for (int n = a + 1; n < b; ++n) {
+                int n = a + 1;
+                for (; n + 4 <= b; n += 4) {                  // (four loads in flight; the comparisons stay in time order)
+                    const float x0 = s[dec_at(n)], x1 = s[dec_at(n + 1)], x2 = s[dec_at(n + 2)], x3 = s[dec_at(n + 3)];
+                    if (fabsf(x0) > best) { best = fabsf(x0); v = x0; }
+                    if (fabsf(x1) > best) { best = fabsf(x1); v = x1; }
+                    if (fabsf(x2) > best) { best = fabsf(x2); v = x2; }
+                    if (fabsf(x3) > best) { best = fabsf(x3); v = x3; }
+                }
+                for (; n < b; ++n) {
                     const float x = s[dec_at(n)];
                     if (fabsf(x) > best) { best = fabsf(x); v = x; }
                 }
@@ -342,13 +351,19 @@ filark_status_t filark_decimate(const float* d_in, int n_ch, long long n_t, long
     const uintptr_t a0 = (uintptr_t)d_in, a1 = a0 + sizeof(float) * (size_t)(((cm ? n_ch : n_t) - 1) * pitch + (cm ? n_t : n_ch));
     const uintptr_t b0 = (uintptr_t)d_out, b1 = b0 + sizeof(float) * (size_t)n_ch * (size_t)width;
     if (a0 < b1 && b0 < a1) return FILARK_ERR_INVALID_ARG;
-    DecParams p{d_in, d_out, n_t, pitch, n_ch, width, mode};
+    DecParams p{d_in, d_out, n_t, pitch, n_ch, width, mode, 0};
     if (cm) {
         if (n_ch > 65535) return FILARK_ERR_INVALID_ARG;
         const bool per_thread = mode != FILARK_DECIMATE_PEAK || n_t <= 32LL * width;
         int gx = (width + 127) / 128;                 // 128 columns per block either way (wide: 32 per warp)
         if (!per_thread && gx > 64) gx = 64;
-        filark_decimate_cm_kernel<<<dim3((unsigned)gx, (unsigned)n_ch), 128, per_thread ? 0 : kDecSmemBytes, stream>>>(p);
+        size_t smem = 0;
+        if (!per_thread) {
+            const long long need = 32 * ((n_t + width - 1) / width) + 32;
+            p.slice = need <= kDecSlice ? (int)need : 0;      // wider columns: column by column, no staging
+            smem = sizeof(float) * 4 * (size_t)(p.slice + p.slice / 32 + 1);
+        }
+        filark_decimate_cm_kernel<<<dim3((unsigned)gx, (unsigned)n_ch), 128, smem, stream>>>(p);
     } else {
         int gy = (width + 31) / 32;
         if (gy > 65535) gy = 65535;
