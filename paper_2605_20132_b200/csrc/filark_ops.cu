@@ -129,21 +129,131 @@ __global__ void __launch_bounds__(kEmaWarps * 32) filark_ema_cm_kernel(const __g
     }
 }
 
-// Time-major: adjacent threads are adjacent channels (coalesced rows), each thread runs its channel
-// serially in time: no scan is needed, the recurrence is one FMA per sample.
-__global__ void __launch_bounds__(128) filark_ema_tm_kernel(const __grid_constant__ EmaParams p)
+// Time-major: a block owns 32 adjacent channels (one per lane: a warp reads 128 contiguous bytes of a time
+// row) and walks the time axis in tiles of 32 x R rows; warp w is the time slice of rows [w R, (w + 1) R) of
+// the tile.  The same blocked scan with the roles turned: every thread runs its R rows from rest, warp 0
+// chains the 32 slices of every channel through shared memory (exact powers alpha^k for the carry, as in
+// the channel-major kernel), every thread then adds alpha^(i+1) x its carry-in.  (One thread per channel
+// running serially in time -- the first version -- kept 188 warps busy: 13 Gsample/s.)
+constexpr int kEmaTmR = 8;
+static_assert(kEmaTmR <= kEmaK, "apow[] holds alpha^1 .. alpha^K");
+// kStaged: rows are 16-byte aligned (pointer, n_ch a multiple of four): the tiles arrive through a ring of
+// kEmaTmStages shared-memory buffers filled by 16-byte cp.async two tiles ahead, so that about 64 KB per
+// block are in flight all the time (with plain loads a block has one tile in flight during its load phase
+// and nothing during the chain and the stores: 2.4 TB/s); otherwise every thread loads its own rows.
+constexpr int kEmaTmStages = 3;
+constexpr size_t kEmaTmStageBytes = sizeof(float) * kEmaTmStages * 32 * kEmaTmR * 32;
+extern __shared__ __align__(16) float ema_stage[];
+template <int kMode, bool kStaged>
+__global__ void __launch_bounds__(1024, 2) filark_ema_tm_kernel(const __grid_constant__ EmaParams p)
 {
-    const int ch = blockIdx.x * blockDim.x + threadIdx.x;
-    if (ch >= p.n_ch) return;
-    float m = p.state[ch];
-    for (long long t = 0; t < p.n_t; ++t) {
-        const float x = p.in[t * p.n_ch + ch];
-        const float u = p.mode == FILARK_EMA_AGC ? fabsf(x) : x;
-        m = fmaf(p.c, u - m, m);                  // (unit DC gain whatever the rounding of 1/N: the error of a
-                                                  // rounded alpha would add up over the N samples of the memory)
-        p.out[t * p.n_ch + ch] = ema_out(p.mode, x, m, p.eps);
+    constexpr int R = kEmaTmR, T = 32 * R;
+    __shared__ float sw[32][32];                 // [slice][channel]: end value from rest, then the slice's carry-in
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const int n_cb = (p.n_ch + 31) / 32;
+    for (int cb = blockIdx.x; cb < n_cb; cb += gridDim.x) {
+        const int ch = cb * 32 + lane;
+        const bool ok = ch < p.n_ch;
+        float carry = (w == 0 && ok) ? p.state[ch] : 0.0f;
+        // one tile = 256 rows of 128 bytes: thread (q, j) = (tid mod 8, tid / 8) copies 16 bytes of rows j and j + 128;
+        // what lies outside the record or the channels is zero-filled; every call commits one group
+        auto stage_tile = [&](long long t0, int stage) {
+            if (t0 < p.n_t) {
+                const int q = threadIdx.x & 7, j = threadIdx.x >> 3;
+                const bool chok = cb * 32 + 4 * q < p.n_ch;
+#pragma unroll
+                for (int h = 0; h < 2; ++h) {
+                    const long long t = t0 + j + 128 * h;
+                    const unsigned dst = (unsigned)__cvta_generic_to_shared(ema_stage + (size_t)stage * T * 32 + (j + 128 * h) * 32 + 4 * q);
+                    const float* src = p.in + (chok && t < p.n_t ? t * p.n_ch + cb * 32 + 4 * q : 0);
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;" ::"r"(dst), "l"(src), "r"(chok && t < p.n_t ? 16 : 0) : "memory");
+                }
+            }
+            asm volatile("cp.async.commit_group;" ::: "memory");
+        };
+        if (kStaged) {
+            __syncthreads();                     // (the ring is free: the channel block before is done with it)
+            for (int k = 0; k < kEmaTmStages - 1; ++k) stage_tile((long long)k * T, k);
+        }
+        const bool all_ch = (cb + 1) * 32 <= p.n_ch;
+        const long long stride = p.n_ch;
+        for (long long t0 = 0; t0 < p.n_t; t0 += T) {
+            const int nt = (int)(p.n_t - t0 < T ? p.n_t - t0 : T);          // rows of this tile
+            const int nv = min(max(nt - w * R, 0), R);                       // ... of this slice
+            const bool full = nt == T && all_ch;                             // (block-uniform: no tests per row)
+            const long long base = (t0 + (long long)w * R) * stride + ch;
+            float x[R], m[R];
+            if (kStaged) {
+                // tile k + kEmaTmStages - 1 is asked for, tile k has landed
+                const int k = (int)(t0 / T);
+                stage_tile(t0 + (long long)(kEmaTmStages - 1) * T, (k + kEmaTmStages - 1) % kEmaTmStages);
+                asm volatile("cp.async.wait_group %0;" ::"n"(kEmaTmStages - 1) : "memory");
+                __syncthreads();
+                const float* st = ema_stage + (size_t)(k % kEmaTmStages) * T * 32 + (w * R) * 32 + lane;
+#pragma unroll
+                for (int i = 0; i < R; ++i) x[i] = st[i * 32];
+            } else {
+                const float* ip = p.in + base;
+#pragma unroll
+                for (int i = 0; i < R; ++i) { x[i] = (full || (ok && i < nv)) ? __ldcs(ip) : 0.0f; ip += stride; }
+            }
+            // (rows that do not exist were zero-filled: they move nothing as long as the recurrence is not run over them)
+            float acc = 0.0f;
+            if (full) {
+#pragma unroll
+                for (int i = 0; i < R; ++i) {
+                    const float u = kMode == FILARK_EMA_AGC ? fabsf(x[i]) : x[i];
+                    acc = fmaf(p.alpha, acc, p.c * u);
+                    m[i] = acc;
+                }
+            } else {
+#pragma unroll
+                for (int i = 0; i < R; ++i) {
+                    const float u = kMode == FILARK_EMA_AGC ? fabsf(x[i]) : x[i];
+                    if (i < nv) acc = fmaf(p.alpha, acc, p.c * u);
+                    m[i] = acc;
+                }
+            }
+            sw[w][lane] = acc;
+            __syncthreads();
+            if (w == 0) {
+                float cin = carry;
+                if (nt == T) {
+                    const float aR = p.apow[R - 1];
+#pragma unroll 8
+                    for (int s = 0; s < 32; ++s) {
+                        const float end = sw[s][lane];
+                        sw[s][lane] = cin;
+                        cin = fmaf(aR, cin, end);
+                    }
+                } else {
+#pragma unroll 4
+                    for (int s = 0; s < 32; ++s) {
+                        const int nvs = min(max(nt - s * R, 0), R);
+                        const float end = sw[s][lane];
+                        sw[s][lane] = cin;
+                        if (nvs > 0) cin = fmaf(p.apow[nvs - 1], cin, end);
+                    }
+                }
+                carry = cin;
+            }
+            __syncthreads();
+            const float E = sw[w][lane];
+            float* op = p.out + base;
+            if (full) {
+#pragma unroll
+                for (int i = 0; i < R; ++i) { __stcs(op, ema_out(kMode, x[i], fmaf(p.apow[i], E, m[i]), p.eps)); op += stride; }
+            } else {
+#pragma unroll
+                for (int i = 0; i < R; ++i) {
+                    if (ok && i < nv) __stcs(op, ema_out(kMode, x[i], fmaf(p.apow[i], E, m[i]), p.eps));
+                    op += stride;
+                }
+            }
+            __syncthreads();
+        }
+        if (w == 0 && ok) p.state[ch] = carry;
     }
-    p.state[ch] = m;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -293,6 +403,13 @@ __global__ void __launch_bounds__(128) filark_decimate_tm_kernel(const __grid_co
 
 }  // namespace
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is per device: set it on every launch of a staged kernel (a
+// cheap host call; the streaming operators are not launch-rate bound).
+static cudaError_t ema_smem_attr_once(int, const void* func, size_t bytes)
+{
+    return cudaFuncSetAttribute(func, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+}
+
 struct filark_ema {
     int device, n_ch, n_len, mode, layout;
     float eps;
@@ -362,7 +479,22 @@ filark_status_t filark_ema_push(filark_ema_t* h, const float* d_in, long long n_
         }
 #undef FK_EMA_LAUNCH
     } else {
-        filark_ema_tm_kernel<<<(h->n_ch + 127) / 128, 128, 0, stream>>>(p);
+        int grid = (h->n_ch + 31) / 32;
+        if (grid > 2 * h->n_sm) grid = 2 * h->n_sm;
+        const bool staged = ((uintptr_t)d_in & 15u) == 0 && (h->n_ch & 3) == 0;
+        cudaError_t e = cudaSuccess;
+#define FK_EMA_TM(M)                                                                                              \
+        if (staged) {                                                                                             \
+            e = ema_smem_attr_once(h->device, (const void*)filark_ema_tm_kernel<M, true>, kEmaTmStageBytes);      \
+            if (e == cudaSuccess) filark_ema_tm_kernel<M, true><<<grid, 1024, kEmaTmStageBytes, stream>>>(p);     \
+        } else {                                                                                                  \
+            filark_ema_tm_kernel<M, false><<<grid, 1024, 0, stream>>>(p);                                         \
+        }
+        if (h->mode == FILARK_EMA_MEAN) { FK_EMA_TM(FILARK_EMA_MEAN) }
+        else if (h->mode == FILARK_EMA_DEMEAN) { FK_EMA_TM(FILARK_EMA_DEMEAN) }
+        else { FK_EMA_TM(FILARK_EMA_AGC) }
+#undef FK_EMA_TM
+        if (e != cudaSuccess) return FILARK_ERR_CUDA;
     }
     return cudaGetLastError() == cudaSuccess ? FILARK_OK : FILARK_ERR_CUDA;
 }

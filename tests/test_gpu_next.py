@@ -304,6 +304,35 @@ def test_ema_operators(cuda_device, mode, layout, n_len):
     h.destroy()
 
 
+@pytest.mark.parametrize("mode", ["mean", "demean", "agc"])
+@pytest.mark.parametrize("n_ch", [100, 64, 4])
+def test_ema_time_major_aligned_rows(cuda_device, mode, n_ch):
+    """Time-major with a channel count that is a multiple of four: the rows arrive through the cp.async ring
+    (n_ch = 100: the last block of 32 channels is partial; 64: complete blocks; 4: one 16-byte piece per row);
+    chunk lengths around the tile of 256 rows, one chunk in place."""
+    n_t, n_len = 3_000, 300
+    rng = np.random.default_rng(n_ch)
+    x = (rng.standard_normal((n_ch, n_t)) * 2.0 + 0.7).astype(np.float32)
+    eps = 1e-3 if mode == "agc" else 0.0
+    o = OracleEma(n_ch, n_len, mode, eps)
+    ref = o.push(x)
+    o.close()
+    xd = torch.from_numpy(np.ascontiguousarray(x.T)).to(cuda_device)
+    h = FilarkEma(n_ch, n_len, mode, eps, TIME_MAJOR)
+    outs = []
+    for i, (a, b) in enumerate(split(n_t, [256, 255, 257, 1, 768, 513, 950])):
+        xin = xd[a:b, :].contiguous()
+        y = xin if i == 4 else torch.empty_like(xin)
+        h.push(xin, y)
+        outs.append(y)
+    got = torch.cat(outs, 0).cpu().numpy().T
+    num = np.sqrt(((got - ref).astype(np.float64) ** 2).sum(1))
+    den = np.maximum(np.sqrt((ref.astype(np.float64) ** 2).sum(1)), np.sqrt((x.astype(np.float64) ** 2).sum(1)) * 1e-2)
+    assert (num <= 2e-5 * den).all(), (num / den).max()
+    assert np.abs(got - ref).max() <= 1e-3 * max(np.abs(ref).max(), 1e-2 * np.abs(x).max())
+    h.destroy()
+
+
 @pytest.mark.parametrize("mode", ["drop", "peak", "linear"])
 @pytest.mark.parametrize("layout", [CHANNEL_MAJOR, TIME_MAJOR])
 @pytest.mark.parametrize("n_t,width", [(90_000, 2048), (1500, 2048), (2048, 2048), (100_003, 777), (33, 1)])
