@@ -78,6 +78,10 @@ typedef enum filark_status {
                                        output buffers: consecutive push calls may then overlap on
                                        the device (see "Ordering" at filark_stream_push)         */
 
+#define FILARK_FLAG_TM_TRANSPOSE 8u  /* tuning/testing, time-major chunks: always the kernel that transposes a
+                                       tile through shared memory (one channel per warp), also where the
+                                       kernel with one channel per lane would serve                    */
+
 #define FILARK_FLAG_FORCE_L(L) ((unsigned)(L) << 8)  /* tuning/testing: use the kernel variant with
                                        sub-block length L (8, 16 or 24) for every push instead of
                                        the one chosen from n_t                                   */

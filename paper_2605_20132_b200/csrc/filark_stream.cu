@@ -22,6 +22,7 @@
 #include "../../include/filark_debug.h"
 #include "design.hpp"
 #include "filark_kernels.cuh"
+#include "filark_kernels_tr.cuh"
 
 using namespace filark;
 
@@ -374,6 +375,33 @@ static cudaError_t launch_tm(const filark_stream* h, PushParams<L>& p, cudaStrea
                                   : (form == 2 ? launch_tm_kinds<L, 2>(h, p, stream) : launch_tm_kinds<L, 3>(h, p, stream)));
 }
 
+// Time-major chunks with one channel per LANE (filark_kernels_tr.cuh): one CTA of 16 warps per SM, work items =
+// (segment, block of 32 channels), always claimed.
+template <int kForm>
+static cudaError_t launch_tr_kinds(const filark_stream* h, PushParams<kTrL>& p, cudaStream_t stream)
+{
+    const int n_cb = (p.n_ch + kTrCh - 1) / kTrCh;
+    const int grid = n_cb < h->n_sm ? n_cb : h->n_sm;
+    long long n_tiles = 0;
+    for (int k = 0; k < p.n_push; ++k) n_tiles += ((long long)p.ck[k].n_t + kTrL - 1) / kTrL / 32 + 1;
+    p.seg_tiles = segment_tiles(n_tiles, n_cb, grid);
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)(kTrWarps * 32));
+    cfg.dynamicSmemBytes = kTrSmemBytes; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = tune().nopdl ? 0 : 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    static std::atomic<unsigned long long> attr_done{0};
+    const cudaError_t e = set_smem_attr_once(attr_done, h->device, (const void*)filark_push_tr_kernel<kForm>, kTrSmemBytes);
+    if (e != cudaSuccess) return e;
+    return cudaLaunchKernelEx(&cfg, filark_push_tr_kernel<kForm>, p);
+}
+static cudaError_t launch_tr(const filark_stream* h, PushParams<kTrL>& p, cudaStream_t stream)
+{
+    return kernel_form(h) == 0 ? launch_tr_kinds<0>(h, p, stream) : launch_tr_kinds<1>(h, p, stream);
+}
+
 // One chunk as the caller describes it (all pushes end up here).
 struct ChunkArgs {
     const float* in; long long n_t, in_pitch;
@@ -382,7 +410,7 @@ struct ChunkArgs {
 
 template <int L>
 static cudaError_t push_variant(const filark_stream* h, int v, const ChunkArgs* c, int n, int vec4, int wait_prior,
-                                cudaStream_t stream)
+                                cudaStream_t stream, bool lanes = false)
 {
     PushParams<L> p = *(const PushParams<L>*)h->proto[v];
     p.state = h->d_state; p.hist = h->d_hist; p.cctl = h->d_cctl; p.progress = h->d_progress;
@@ -396,6 +424,9 @@ static cudaError_t push_variant(const filark_stream* h, int v, const ChunkArgs* 
         d.n_t = (int)c[k].n_t; d.n_base = (int)(c[k].n_t / L); d.n_rem = (int)(c[k].n_t % L);
         d.t_cum = t_cum;
         t_cum += (unsigned)c[k].n_t;
+    }
+    if constexpr (L == kTrL) {
+        if (lanes) return launch_tr(h, p, stream);
     }
     if (h->layout == FILARK_LAYOUT_TIME_MAJOR) return launch_tm<L>(h, p, stream);
     return launch_cm<L>(h, p, stream);
@@ -442,7 +473,7 @@ static filark_status_t check_create_args(const void* out, int n_ch, const double
     if (!out || !sos || n_ch <= 0 || n_sec <= 0 || n_sec > FILARK_MAX_SECTIONS) return FILARK_ERR_INVALID_ARG;
     if (sta_len < 1 || lta_len < sta_len) return FILARK_ERR_INVALID_ARG;
     if (layout != FILARK_LAYOUT_CHANNEL_MAJOR && layout != FILARK_LAYOUT_TIME_MAJOR) return FILARK_ERR_INVALID_ARG;
-    if (flags & ~(FILARK_FLAG_SERIAL_SCAN | FILARK_FLAG_STRICT_ORDER | FILARK_FLAG_OVERLAP_PUSHES | 0xFF00u)) return FILARK_ERR_INVALID_ARG;
+    if (flags & ~(FILARK_FLAG_SERIAL_SCAN | FILARK_FLAG_STRICT_ORDER | FILARK_FLAG_OVERLAP_PUSHES | FILARK_FLAG_TM_TRANSPOSE | 0xFF00u)) return FILARK_ERR_INVALID_ARG;
     if (flags & 0xFF00u) {
         bool ok = false;
         for (int v = 0; v < kNumVariants; ++v) ok = ok || kVariantL[v] == (int)((flags >> 8) & 0xFF);
@@ -610,7 +641,13 @@ static filark_status_t launch_chunks(filark_stream_t* h, const ChunkArgs* c, int
             if (e == cudaSuccess) h->launches += 1;
         }
     } else {
-        const int v = choose_variant_chunks(h, c, n);
+        int v = choose_variant_chunks(h, c, n);
+        // time-major: the kernel with one channel per lane (filark_kernels_tr.cuh) unless a trigger is set, another
+        // sub-block length is forced, or a pitch is too long for its 32-bit row offsets
+        const unsigned force_L = (h->flags >> 8) & 0xFFu;
+        bool lanes = !cm && kernel_form(h) < 2 && !(h->flags & FILARK_FLAG_TM_TRANSPOSE) && (force_L == 0 || force_L == (unsigned)kTrL);
+        for (int k = 0; k < n && lanes; ++k) lanes = c[k].in_pitch < (1LL << 25) && c[k].out_pitch < (1LL << 25);
+        if (lanes) for (int i = 0; i < kNumVariants; ++i) if (kVariantL[i] == kTrL) v = i;
         // bounding ranges of what the launch reads ([0]) and writes ([1] filt, [2] cf); alignment
         uintptr_t lo[3] = {~(uintptr_t)0, ~(uintptr_t)0, ~(uintptr_t)0}, hi[3] = {0, 0, 0};
         int vec4 = 1;
@@ -647,7 +684,7 @@ static filark_status_t launch_chunks(filark_stream_t* h, const ChunkArgs* c, int
         switch (kVariantL[v]) {
             case 8: e = push_variant<8>(h, v, c, n, vec4, wait_prior, stream); break;
             case 16: e = push_variant<16>(h, v, c, n, vec4, wait_prior, stream); break;
-            default: e = push_variant<24>(h, v, c, n, vec4, wait_prior, stream); break;
+            default: e = push_variant<24>(h, v, c, n, vec4, wait_prior, stream, lanes); break;
         }
         if (e == cudaSuccess) {
             const int keep = n_prev < kCmDepth - 2 ? n_prev : kCmDepth - 2;
@@ -1257,17 +1294,20 @@ extern "C" filark_status_t filark_stream_once_noalloc(const double* sos, int n_s
     if (e != cudaSuccess) return fail(e);
 
     // tables of the one variant this record takes, on the stack
-    const int v = choose_variant(n_t);
+    // (time-major: the kernel with one channel per lane, as a handle without a trigger takes it)
+    const bool cm = layout == FILARK_LAYOUT_CHANNEL_MAJOR;
+    const bool lanes = !cm && pitch < (1LL << 25);
+    int v = choose_variant(n_t);
+    if (lanes) for (int i = 0; i < kNumVariants; ++i) if (kVariantL[i] == kTrL) v = i;
     alignas(16) unsigned char proto[sizeof(PushParams<24>)];
     static_assert(sizeof(PushParams<24>) >= sizeof(PushParams<16>) && sizeof(PushParams<24>) >= sizeof(PushParams<8>), "largest variant");
     h.proto[v] = proto;
-    const bool cm = layout == FILARK_LAYOUT_CHANNEL_MAJOR;
     const uintptr_t all = (uintptr_t)d_in | (uintptr_t)d_filt | (uintptr_t)d_cf;
     const int vec4 = cm ? ((all & 15u) == 0 && (n_t & 3) == 0) : ((((uintptr_t)d_filt | (uintptr_t)d_cf) & 15u) == 0 && (n_ch & 3) == 0);
     switch (kVariantL[v]) {
         case 8: build_proto<8>(&h, reinterpret_cast<PushParams<8>*>(proto)); e = push_variant<8>(&h, v, &c, 1, vec4, 1, stream); break;
         case 16: build_proto<16>(&h, reinterpret_cast<PushParams<16>*>(proto)); e = push_variant<16>(&h, v, &c, 1, vec4, 1, stream); break;
-        default: build_proto<24>(&h, reinterpret_cast<PushParams<24>*>(proto)); e = push_variant<24>(&h, v, &c, 1, vec4, 1, stream); break;
+        default: build_proto<24>(&h, reinterpret_cast<PushParams<24>*>(proto)); e = push_variant<24>(&h, v, &c, 1, vec4, 1, stream, lanes); break;
     }
     registry_set(stream, kNaForeign);
     if (e != cudaSuccess) return fail(e);

@@ -19,6 +19,7 @@ FLAG_NONE = 0
 FLAG_SERIAL_SCAN = 1
 FLAG_STRICT_ORDER = 2       # never overlap pushes, not even inside push_many (filark_stream.h, "Ordering")
 FLAG_OVERLAP_PUSHES = 4     # the caller promises that nothing foreign lies between consecutive push calls
+FLAG_TM_TRANSPOSE = 8       # time-major: always the transposing kernel (testing)
 MAX_SECTIONS = 16
 
 STATUS_NAMES = {0: "FILARK_OK", 1: "FILARK_ERR_INVALID_ARG", 2: "FILARK_ERR_UNSTABLE",

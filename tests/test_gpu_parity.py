@@ -65,13 +65,19 @@ def test_scaled_configs_channel_major(cuda_device, name, n_ch, n_t):
     s.destroy()
 
 
-@pytest.mark.parametrize("name,n_ch,n_t", [("cfg3", 48, 30_000), ("cfg5", 33, 60_000)])
-def test_scaled_configs_time_major(cuda_device, name, n_ch, n_t):
+@pytest.mark.parametrize("flags", [0, 8], ids=["lanes", "transpose"])
+@pytest.mark.parametrize("name,n_ch,n_t", [("cfg3", 48, 30_000), ("cfg5", 33, 60_000), ("cfg3", 100, 9_000)])
+def test_scaled_configs_time_major(cuda_device, name, n_ch, n_t, flags):
+    """Both time-major kernels: one channel per lane (filark_kernels_tr.cuh, the default) and the transposing
+    one (FILARK_FLAG_TM_TRANSPOSE = 8; what a handle with a trigger set runs)."""
     w = CONFIGS[name].scaled(n_ch=n_ch, n_t=n_t)
     x_dev, ref_f, ref_c = _case(w, cuda_device, TIME_MAJOR)
-    s = _stream(w, TIME_MAJOR)
+    s = _stream(w, TIME_MAJOR, flags)
     f, c = run_gpu(s, x_dev, TIME_MAJOR, split(n_t, push_schedule(w)))
     _check(f, c, ref_f, ref_c, TIME_MAJOR, f"{name} time-major")
+    s.reset()
+    f, c = run_gpu(s, x_dev, TIME_MAJOR, [(0, n_t)])
+    _check(f, c, ref_f, ref_c, TIME_MAJOR, f"{name} time-major whole")
     s.destroy()
 
 
@@ -195,7 +201,7 @@ def test_error_codes(cuda_device):
     from paper_2605_20132_b200.stream import FilarkError, FilarkStream
     w = CONFIGS["cfg1"].scaled(n_ch=4, n_t=64)
     sos = design_sos(w)
-    for bad in [dict(n_ch=0), dict(sta_len=0), dict(lta_len=10, sta_len=20), dict(layout=7), dict(flags=8), dict(flags=7 << 8), dict(flags=32 << 8)]:
+    for bad in [dict(n_ch=0), dict(sta_len=0), dict(lta_len=10, sta_len=20), dict(layout=7), dict(flags=16), dict(flags=7 << 8), dict(flags=32 << 8)]:
         kw = dict(n_ch=4, sos=sos, sta_len=5, lta_len=50, layout=0, flags=0); kw.update(bad)
         with pytest.raises(FilarkError) as e:
             FilarkStream(**kw)

@@ -28,11 +28,13 @@ def kernels():
         name = f.split("\n")[0]
         # filark_push_cm_kernel<L, CTAS, kForm, kTM, kDyn, kShift>
         m = re.search(r"filark_push_cm_kernelILi(\d+)ELi(\d)ELi(\d)ELb(\d)ELb(\d)ELb(\d)", name)
-        if not m:
+        mt = re.search(r"filark_push_tr_kernelILi(\d)", name)       # time-major, one channel per lane: <kForm>
+        if not m and not mt:
             continue
         ffma2 = [ln for ln in f.split("\n") if "FFMA2" in ln]
         ops = collections.Counter(mm.group(1).split(".")[0] for mm in re.finditer(r"\*/\s+(?:@!?U?P\d+\s+)?([A-Z0-9_.]+)", f))
-        out[tuple(int(g) for g in m.groups())] = dict(ffma2=len(ffma2), uniform=sum("UR" in ln for ln in ffma2),
+        key = tuple(int(g) for g in m.groups()) if m else ("tr", int(mt.group(1)))
+        out[key] = dict(ffma2=len(ffma2), uniform=sum("UR" in ln for ln in ffma2),
                                                       spills=ops["STL"] + ops["LDL"])
     return out
 
@@ -48,6 +50,7 @@ def test_headline_kernels_keep_uniform_operands_and_do_not_spill(kernels):
 
 
 def test_every_form_at_24_samples_is_uniform_too(kernels):
+    assert ("tr", 0) in kernels and ("tr", 1) in kernels
     for key, v in kernels.items():
-        if key[0] == 24:
+        if key[0] in (24, "tr"):
             assert v["uniform"] == v["ffma2"] and v["spills"] == 0, key
