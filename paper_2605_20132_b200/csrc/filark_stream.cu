@@ -647,6 +647,9 @@ static filark_status_t launch_chunks(filark_stream_t* h, const ChunkArgs* c, int
         const unsigned force_L = (h->flags >> 8) & 0xFFu;
         bool lanes = !cm && kernel_form(h) < 2 && !(h->flags & FILARK_FLAG_TM_TRANSPOSE) && (force_L == 0 || force_L == (unsigned)kTrL);
         for (int k = 0; k < n && lanes; ++k) lanes = c[k].in_pitch < (1LL << 25) && c[k].out_pitch < (1LL << 25);
+        // (a launch of fewer than four of its tiles per channel is over before its warps have fallen into step:
+        // measured on separate 1,500-sample pushes, 171 against 190 Gsample/s for the transposing kernel)
+        if (total < 4LL * kTrRows) lanes = false;
         if (lanes) for (int i = 0; i < kNumVariants; ++i) if (kVariantL[i] == kTrL) v = i;
         // bounding ranges of what the launch reads ([0]) and writes ([1] filt, [2] cf); alignment
         uintptr_t lo[3] = {~(uintptr_t)0, ~(uintptr_t)0, ~(uintptr_t)0}, hi[3] = {0, 0, 0};
@@ -1296,7 +1299,7 @@ extern "C" filark_status_t filark_stream_once_noalloc(const double* sos, int n_s
     // tables of the one variant this record takes, on the stack
     // (time-major: the kernel with one channel per lane, as a handle without a trigger takes it)
     const bool cm = layout == FILARK_LAYOUT_CHANNEL_MAJOR;
-    const bool lanes = !cm && pitch < (1LL << 25);
+    const bool lanes = !cm && pitch < (1LL << 25) && n_t >= 4LL * kTrRows;
     int v = choose_variant(n_t);
     if (lanes) for (int i = 0; i < kNumVariants; ++i) if (kVariantL[i] == kTrL) v = i;
     alignas(16) unsigned char proto[sizeof(PushParams<24>)];
