@@ -248,8 +248,11 @@ filark_push_tr_kernel(const __grid_constant__ PushParams<kTrL> p)
                 const float* ip = ck.in + (long long)ta * ck.in_pitch + chl;
                 const int pitch = (int)ck.in_pitch;
                 if (inside) {
+                    // (two running row pointers: one 64-bit multiply-add per access instead of an address built per row)
+                    const float* plo = ip;
+                    const float* phi = ip + L * pitch;
 #pragma unroll
-                    for (int i = 0; i < L; ++i) x[i] = make_float2(__ldcs(ip + i * pitch), __ldcs(ip + (L + i) * pitch));
+                    for (int i = 0; i < L; ++i) { x[i] = make_float2(__ldcs(plo), __ldcs(phi)); plo += pitch; phi += pitch; }
                 } else {
                     // an edge of the chunk: rows in front of it are the samples that waited for it, rows behind it are zero
 #pragma unroll
@@ -333,8 +336,10 @@ filark_push_tr_kernel(const __grid_constant__ PushParams<kTrL> p)
                 float* fp = ck.filt + (long long)ta * ck.out_pitch + ch;
                 const int pitch = (int)ck.out_pitch;
                 if (inside && ok) {
+                    float* plo = fp;
+                    float* phi = fp + L * pitch;
 #pragma unroll
-                    for (int i = 0; i < L; ++i) { __stcs(fp + i * pitch, x[i].x); __stcs(fp + (L + i) * pitch, x[i].y); }
+                    for (int i = 0; i < L; ++i) { __stcs(plo, x[i].x); __stcs(phi, x[i].y); plo += pitch; phi += pitch; }
                 } else if (ok) {
 #pragma unroll
                     for (int i = 0; i < L; ++i) {
@@ -398,8 +403,10 @@ filark_push_tr_kernel(const __grid_constant__ PushParams<kTrL> p)
                 float* cp = ck.cf + (long long)ta * ck.out_pitch + ch;
                 const int pitch = (int)ck.out_pitch;
                 if (inside && ok) {
+                    float* plo = cp;
+                    float* phi = cp + L * pitch;
 #pragma unroll
-                    for (int i = 0; i < L; ++i) { __stcs(cp + i * pitch, x[i].x); __stcs(cp + (L + i) * pitch, x[i].y); }
+                    for (int i = 0; i < L; ++i) { __stcs(plo, x[i].x); __stcs(phi, x[i].y); plo += pitch; phi += pitch; }
                 } else if (ok) {
 #pragma unroll
                     for (int i = 0; i < L; ++i) {
