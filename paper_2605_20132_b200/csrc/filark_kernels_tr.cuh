@@ -255,15 +255,18 @@ filark_push_tr_kernel(const __grid_constant__ PushParams<kTrL> p)
                     for (int i = 0; i < L; ++i) { x[i] = make_float2(__ldcs(plo), __ldcs(phi)); plo += pitch; phi += pitch; }
                 } else {
                     // an edge of the chunk: rows in front of it are the samples that waited for it, rows behind it are zero
+                    const float* plo = ip;
+                    const float* phi = ip + L * pitch;
 #pragma unroll
                     for (int i = 0; i < L; ++i) {
                         const int tl = ta + i, th = ta + L + i;
                         float a = 0.0f, b = 0.0f;
                         if (tl < 0) { if (tl + g.r0 >= 0) a = hs_rd[(tl + g.r0) * 32 + lane]; }
-                        else if (tl < n_t) a = __ldcs(ip + (long long)i * ck.in_pitch);
+                        else if (tl < n_t) a = __ldcs(plo);
                         if (th < 0) { if (th + g.r0 >= 0) b = hs_rd[(th + g.r0) * 32 + lane]; }
-                        else if (th < n_t) b = __ldcs(ip + (long long)(L + i) * ck.in_pitch);
+                        else if (th < n_t) b = __ldcs(phi);
                         x[i] = make_float2(a, b);
+                        plo += pitch; phi += pitch;
                     }
                 }
             }
@@ -343,8 +346,8 @@ filark_push_tr_kernel(const __grid_constant__ PushParams<kTrL> p)
                 } else if (ok) {
 #pragma unroll
                     for (int i = 0; i < L; ++i) {
-                        if ((unsigned)(ta + i) < (unsigned)n_t) __stcs(fp + (long long)i * ck.out_pitch, x[i].x);
-                        if ((unsigned)(ta + L + i) < (unsigned)n_t) __stcs(fp + (long long)(L + i) * ck.out_pitch, x[i].y);
+                        if ((unsigned)(ta + i) < (unsigned)n_t) __stcs(fp + i * pitch, x[i].x);
+                        if ((unsigned)(ta + L + i) < (unsigned)n_t) __stcs(fp + (L + i) * pitch, x[i].y);
                     }
                 }
             }
@@ -410,8 +413,8 @@ filark_push_tr_kernel(const __grid_constant__ PushParams<kTrL> p)
                 } else if (ok) {
 #pragma unroll
                     for (int i = 0; i < L; ++i) {
-                        if ((unsigned)(ta + i) < (unsigned)n_t) __stcs(cp + (long long)i * ck.out_pitch, x[i].x);
-                        if ((unsigned)(ta + L + i) < (unsigned)n_t) __stcs(cp + (long long)(L + i) * ck.out_pitch, x[i].y);
+                        if ((unsigned)(ta + i) < (unsigned)n_t) __stcs(cp + i * pitch, x[i].x);
+                        if ((unsigned)(ta + L + i) < (unsigned)n_t) __stcs(cp + (L + i) * pitch, x[i].y);
                     }
                 }
             }
