@@ -342,11 +342,13 @@ def main():
     lean = "lean" if True else "all"
     out["roofline"] = {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s",
                        "frac": ach / peak, "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
-                       "kernel": "filark_push_cm_kernel (one instantiation per sub-block length, launch shape, "
-                                 "section forms and layout; profiles/ names the one this command launches)",
+                       "kernel": ("filark_push_tr_kernel (time-major: one channel per lane, the warps of a CTA are time slices; "
+                                  "short launches and handles with a trigger: filark_push_cm_kernel<.., kTM>)" if args.layout == "tm" else
+                                  "filark_push_cm_kernel (one instantiation per sub-block length, launch shape, "
+                                  "section forms and layout; profiles/ names the one this command launches)"),
                        "algorithmic_bytes_per_launch": bytes_per_launch,
                        "mean_launch_ms": per_launch_ms, "frac_of_nominal_8TBs": ach / HBM_NOMINAL_GBS,
-                       "limiter": "instruction issue, not HBM: at 8 sections the kernel executes about 60 SASS "
+                       "limiter": "instruction issue, not HBM: at 8 sections the kernel executes about 60 (time-major: 75-85) SASS "
                                   "instructions per sample (DESIGN.md 7, profiles/r02_ncu_*.md); HBM is the roof the "
                                   "north star names and the one `frac` is measured against",
                        "note": "achieved = 12 B/sample x samples per step / CUDA-event time of the step (the step is "

@@ -998,7 +998,9 @@ __device__ __forceinline__ void process_tile(const PushParams<L>& p, const Chunk
         const int sc = (kTM || !ck.cf) ? 0 : row_shift(ck.cf + (long long)ch * ck.out_pitch, g.r0);
         if (ck.cf || visit) {
             regs_to_buf<L>(x, buf, lane, sc);
-            if (kTM) __syncthreads(); else __syncwarp();
+            // (time-major: the CTA stores the cf together -- every warp is here; without a cf output only the warps
+            // whose tile matters to the trigger are, each for its own buffer: a CTA barrier would never complete)
+            if (kTM && ck.cf) __syncthreads(); else __syncwarp();
         }
         if (kTrig && visit && (!kTM || ch < p.n_ch)) {
             trigger_tile<L>(p, buf, sc, wst + trig_word(p.n_sec), ch, (long long)seen + t0, max(0, -t0),

@@ -202,6 +202,31 @@ def test_trigger_events_match_the_oracle(cuda_device, layout, sizes, many):
     s.destroy()
 
 
+def test_trigger_time_major_without_cf_output(cuda_device):
+    """Time-major, events only (d_cf = NULL): only the warps whose tile matters to the trigger stage their cf --
+    this used to wait at a CTA barrier for the others (found by `bench.py --layout tm`); watchdog by timeout."""
+    thr_on, thr_off = 3.0, 1.5
+    w, x = _burst_record(80, 30_000, 51, n_bursts=30)
+    sos = design_sos(w)
+    ref_cf, ref_ev = _oracle_events(x, sos, w, thr_on, thr_off)
+    xd = torch.from_numpy(np.ascontiguousarray(x.T)).to(cuda_device)
+    f = torch.empty_like(xd)
+    s = FilarkStream(w.n_ch, sos, w.sta_len, w.lta_len, TIME_MAJOR)
+    s.set_trigger(thr_on, thr_off, 10_000)
+    chunks = [xd[a:b, :].contiguous() for a, b in split(w.n_t, [1500, 700, 4096])]
+    s.push_many(chunks, [f[a:b, :] for a, b in split(w.n_t, [1500, 700, 4096])], None)
+    done = torch.cuda.Event(); done.record()
+    import time
+    t0 = time.time()
+    while not done.query():
+        assert time.time() - t0 < 60.0, "the launch does not complete"
+        time.sleep(0.01)
+    got, dropped = s.pop_events()
+    assert dropped == 0
+    assert _compare_events(got, ref_ev, ref_cf, thr_on, thr_off, "time-major, no cf output") >= 10
+    s.destroy()
+
+
 def test_events_to_time_channel_boxes(cuda_device):
     """NEXT-1's output form: the events the trigger emitted on the GPU, associated into time-channel boxes by
     filark_events_associate, against the oracle's association of the same list (reading R30); and the boxes
