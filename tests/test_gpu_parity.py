@@ -86,6 +86,33 @@ FUZZ = [[1], [2, 3], [31, 32, 33], [1, 2, 3, 31, 32, 33, 97, 499, 1021, 1024, 10
         [7919], [1023, 1], [4096, 5], "random"]
 
 
+@pytest.mark.parametrize("n_ch", [1, 31, 33, 70])
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_time_major_schedules_fuzz(cuda_device, n_ch, seed):
+    """The time-major kernel with one channel per lane on schedules of odd chunk lengths through push_many (one
+    launch: samples that do not fill a slot wait for the next chunk in shared memory; tiles of 768 rows; chunks
+    shorter than a slot; a block of channels that is not full), then a second schedule on the same handle."""
+    rng = np.random.default_rng(100 * n_ch + seed)
+    pool = [1, 5, 23, 24, 25, 47, 700, 767, 768, 769, 1500, 3000]
+    sizes = rng.choice(pool, size=40).tolist()
+    n_t = 12_000
+    w = CONFIGS["cfg3"].scaled(n_ch=n_ch, n_t=n_t)
+    x_dev, ref_f, ref_c = _case(w, cuda_device, TIME_MAJOR)
+    s = _stream(w, TIME_MAJOR)
+    bounds = split(n_t, sizes)
+    half = len(bounds) // 2
+    f, c = torch.empty_like(x_dev), torch.empty_like(x_dev)
+    for part in (bounds[:half], bounds[half:]):
+        ins = [x_dev[a:b, :].contiguous() for a, b in part]
+        fo, co = [torch.empty_like(t) for t in ins], [torch.empty_like(t) for t in ins]
+        s.push_many(ins, fo, co)
+        for (a, b), tf, tc in zip(part, fo, co):
+            f[a:b, :] = tf; c[a:b, :] = tc
+    torch.cuda.synchronize()
+    _check(f, c, ref_f, ref_c, TIME_MAJOR, f"time-major fuzz n_ch={n_ch} {sizes[:8]}")
+    s.destroy()
+
+
 @pytest.mark.parametrize("sizes", FUZZ, ids=[str(s) for s in FUZZ])
 def test_chunking_fuzz(cuda_device, sizes):
     w = CONFIGS["cfg3"].scaled(n_ch=9, n_t=13_007 if sizes != [1] else 700)
